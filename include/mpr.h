@@ -1,0 +1,169 @@
+/* include/mpr.h -- C ABI of libmpr.so: the conditional hybrid Monte-Carlo hot path of the
+ * modified planar rotator (MPR) prediction method, hand-written CUDA for sm_100a (B200).
+ *
+ * What the library computes (arxiv/paper_1910_08448; PAPER.md:N = line N of the paper text,
+ * DESIGN.md section 3 lists the readings R1..R17 where the paper is silent):
+ *   - H = -J sum_<ij> cos[q (phi_i - phi_j)], phi in [0, 2pi], q = 1/2, J = 1
+ *                                                        PAPER.md:27-29 (Eq. 2)
+ *   - "maps the measured data onto spins"                PAPER.md:13 (sec. 1), R1
+ *   - "the temperature ... needs to be inferred from the incomplete data"
+ *                                                        PAPER.md:31 (sec. 2), R6
+ *   - "a conditional Monte Carlo simulation, in which only the spins at the prediction
+ *     locations are allowed to change their states ... hybrid algorithm"
+ *                                                        PAPER.md:31 (sec. 2), R4/R5/R7
+ *   - "averaging over multiple configurations in equilibrium" -> prediction
+ *                                                        PAPER.md:31 (sec. 2), R15
+ *   - specific energy e = <H>/L^2                        PAPER.md:35 (sec. 2), R3
+ *   - precision settings (spins, energy, functions)      PAPER.md:35 (sec. 2), R12/R13
+ *
+ * Conventions for every call
+ *   - Pointers named d_* are DEVICE pointers, h_* / plain scalars are HOST memory.
+ *   - Grids are row-major, site index s = y*L + x, 0 <= x,y < L.
+ *   - Ownership: the caller owns every buffer (inputs, outputs, workspace); the library
+ *     allocates no device memory and creates no stream.  It borrows d_values, d_mask and
+ *     the workspace for the life of the context and never writes d_values / d_mask.
+ *   - Errors: every call returns 0 (MPR_OK) or a negative mpr_status.  Nothing is thrown,
+ *     printed or aborted.  mpr_last_error() gives a text for the last failure of a context.
+ *   - Ordering: all device work is enqueued on the context's stream.  Calls that return
+ *     host scalars (create, estimate_temperature, run, get_counters, get_energy_series,
+ *     get_launch_stats) synchronise that stream before returning; the others are asynchronous.
+ *   - Determinism: for fixed (inputs, seed, mode, T) the spin state after any number of
+ *     sweeps is bit-identical for every kernel path, tile size and fused depth.
+ *   - There is no CPU fallback: without a CUDA device every compute call returns MPR_ERR_CUDA.
+ */
+#ifndef MPR_H_
+#define MPR_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct mpr_ctx mpr_ctx; /* opaque, host-side */
+
+typedef enum {
+  MPR_OK = 0,
+  MPR_ERR_INVALID_ARG = -1,      /* L < 2, null pointer, bad mode, negative count, T <= 0   */
+  MPR_ERR_NO_MEASURED = -2,      /* no measured site, or no measured nearest-neighbour pair */
+  MPR_ERR_DEGENERATE_RANGE = -3, /* z_max == z_min over the measured sample                 */
+  MPR_ERR_NONFINITE = -4,        /* NaN/Inf at a measured site                              */
+  MPR_ERR_WORKSPACE = -5,        /* workspace null, misaligned (256 B) or too small         */
+  MPR_ERR_NOT_READY = -6,        /* run before a temperature was set or estimated           */
+  MPR_ERR_NO_ROOT = -7,          /* e_sample outside the reachable e(T) range, R6           */
+  MPR_ERR_CUDA = -8              /* a CUDA call failed (no device, launch error, ...)       */
+} mpr_status;
+
+/* Precision modes (triple = spins / energy / functions; R12):
+ *   MPR_DP            DDD  double storage, double arithmetic and functions
+ *   MPR_SP            SSD  float storage of the spins, double arithmetic and functions
+ *   MPR_SP_PRECISE    float storage and arithmetic, sinf/cosf/expf (not in the paper)
+ *   MPR_SP_INTRINSIC  SSS  float storage and arithmetic, __sinf/__cosf/__expf
+ * Energy sums are accumulated in double in every mode (R13).                              */
+typedef enum { MPR_DP = 0, MPR_SP = 1, MPR_SP_PRECISE = 2, MPR_SP_INTRINSIC = 3 } mpr_precision;
+
+/* Kernel paths.  Both give bit-identical spin states (determinism contract).
+ *   MPR_PATH_TILED   one launch per hybrid sweep group: TMA stages a tile + halo of both colour
+ *                    planes in shared memory, all 4*k colour passes of k sweeps run there.
+ *   MPR_PATH_PLAIN   one launch per colour pass on the global colour planes (reference path
+ *                    for the self-consistency tests; also used for the R8 quench passes).  */
+typedef enum { MPR_PATH_TILED = 0, MPR_PATH_PLAIN = 1 } mpr_path;
+
+/* Bytes of workspace mpr_create needs for an L x L grid (any mode).  HOST out pointer.     */
+int mpr_workspace_bytes(int L, size_t* bytes);
+
+/* The paper's problem statement: an L x L grid, values at the measured
+ * sites, a set of prediction sites.
+ *   d_values  f64[L*L]  value at measured sites; never read where d_mask == 1 (may be NaN)
+ *   d_mask    u8 [L*L]  1 = prediction ("free") site, 0 = measured site
+ *   d_workspace         >= mpr_workspace_bytes(L) bytes, 256-byte aligned
+ *   cuda_stream         a cudaStream_t (0 = default stream)
+ * Does R1 (z_min, z_max over the measured sample, phi = 2pi (z - z_min)/(z_max - z_min)),
+ * the sample energy of R6 (e_s over measured nearest-neighbour pairs), packs the mask into
+ * per-colour bitmaps, selects MPR_DP, seed 0, and resets the chain (R8).
+ * Fails with INVALID_ARG, WORKSPACE, NO_MEASURED, DEGENERATE_RANGE, NONFINITE or CUDA;
+ * *out is null on failure.                                                                 */
+int mpr_create(mpr_ctx** out, int L, const double* d_values, const uint8_t* d_mask,
+               void* d_workspace, size_t workspace_bytes, void* cuda_stream);
+void mpr_destroy(mpr_ctx* ctx); /* frees the host struct only */
+
+/* Re-encodes the spins for `mode` and resets the chain (trial 0).                          */
+int mpr_set_precision(mpr_ctx* ctx, mpr_precision mode);
+/* Philox key (R9).  Resets the chain.                                                      */
+int mpr_set_seed(mpr_ctx* ctx, uint64_t seed);
+/* Reduced temperature T > 0, bypassing the estimate.  Does not touch the chain.            */
+int mpr_set_temperature(mpr_ctx* ctx, double T);
+/* Number of quench double-passes of the R8 initialisation (default 32).  Resets the chain. */
+int mpr_set_quench(mpr_ctx* ctx, int n);
+/* Kernel path (default MPR_PATH_TILED) and temporal-blocking depth k >= 1 (hybrid sweeps
+ * fused per launch of the tiled kernel, default 1).  Results do not depend on either.      */
+int mpr_set_path(mpr_ctx* ctx, mpr_path path);
+int mpr_set_fused_sweeps(mpr_ctx* ctx, int k);
+/* R8: free spins i.i.d. uniform from Philox (pass INIT, `trial` in counter word 3), then the
+ * quench passes; sweep counter, move counters and the prediction accumulator are cleared.  */
+int mpr_reset_chain(mpr_ctx* ctx, uint32_t trial);
+
+/* R6: conditional energy matching.  Finds T with e_cond(T) = e_sample by bracketing on
+ * [1e-4, 1] (expanded by decades within [1e-6, 1e2]) and Illinois regula falsi; each trial
+ * is a fresh chain of 200 + 50 hybrid sweeps.  HOST outs (each may be null).  Sets T and
+ * resets the chain (trial 0).  Fails with NO_MEASURED (no measured pair) or NO_ROOT.       */
+int mpr_estimate_temperature(mpr_ctx* ctx, double* T_hat, double* e_sample, int* n_trials);
+
+/* Continues the chain: n_eq hybrid sweeps (R4: Metropolis colour 0, 1, over-relaxation
+ * colour 0, 1), then n_meas sweeps each followed by the energy sample e_n = 2H/N_b (R3) and
+ * phi added to the per-site accumulator.
+ *   d_pred    f64[L*L] or null: measured sites get their input value back bit-exact,
+ *             prediction sites z_min + (z_max - z_min) * mean(phi) / 2pi over all measurement
+ *             sweeps since the last chain reset (NaN if there were none).
+ *   e_mean, e_stderr   HOST, may be null: mean of this call's e_n and its binned standard
+ *             error (R16); NaN / 0 when n_meas == 0.                                       */
+int mpr_run(mpr_ctx* ctx, int n_eq, int n_meas, double* d_pred, double* e_mean, double* e_stderr);
+
+/* n hybrid sweeps without measurement (asynchronous).                                      */
+int mpr_sweep(mpr_ctx* ctx, int n);
+/* Single colour passes on the plain path, for tests: kind 0 = Metropolis (uses the Philox
+ * stream of sweep number `sweep`), 1 = over-relaxation, 2 = quench.                        */
+int mpr_pass(mpr_ctx* ctx, int kind, int colour, uint64_t sweep);
+
+/* Spins as angles, d_phi f64[L*L] row-major (parity tests, checkpoint).                    */
+int mpr_get_state(mpr_ctx* ctx, double* d_phi);
+/* Overwrites the spins at the prediction sites from d_phi (measured sites keep R1's map). */
+int mpr_set_state(mpr_ctx* ctx, const double* d_phi);
+/* Energy of the current state: H (Eq. 2) and e = 2H/N_b.  HOST outs.                       */
+int mpr_energy(mpr_ctx* ctx, double* H, double* e);
+/* Sample energy of R6 and the number of measured pairs.  HOST outs.                        */
+int mpr_sample_energy(mpr_ctx* ctx, double* e_sample, int64_t* n_pairs);
+/* Accepted / attempted Metropolis moves and hybrid sweeps since the last chain reset.      */
+int mpr_get_counters(mpr_ctx* ctx, uint64_t* accepted, uint64_t* attempted, uint64_t* sweeps);
+/* e_n of the last mpr_run, copied to HOST out[0..cap); returns their number (>= 0).        */
+int64_t mpr_get_energy_series(mpr_ctx* ctx, double* out, int64_t cap);
+/* z_min, z_max of the measured sample and the number of prediction sites.  HOST outs.      */
+int mpr_get_info(mpr_ctx* ctx, double* z_min, double* z_max, int64_t* n_free, double* T);
+/* Kernel launches enqueued by this context so far (for bench.py's gpu_launches).           */
+int mpr_get_launch_stats(mpr_ctx* ctx, uint64_t* launches);
+
+/* End-to-end call on HOST buffers (bench.py's e2e leg): copies h_values / h_mask to a staging
+ * area at the end of the workspace, creates a context, selects mode and seed, takes T (or
+ * estimates it when T <= 0), runs n_eq + n_meas sweeps and copies the prediction back.
+ *   h_values f64[L*L], h_mask u8[L*L], h_pred f64[L*L]: HOST (pinned memory makes the copies
+ *   asynchronous); d_workspace >= mpr_workspace_bytes_host(L) bytes; outs HOST, may be null. */
+int mpr_workspace_bytes_host(int L, size_t* bytes);
+int mpr_predict_host(int L, const double* h_values, const uint8_t* h_mask, mpr_precision mode,
+                     uint64_t seed, double T, int n_eq, int n_meas, void* d_workspace,
+                     size_t workspace_bytes, void* cuda_stream, double* h_pred, double* e_mean,
+                     double* e_stderr, double* T_used, uint64_t* launches);
+
+/* The Philox4x32-10 block function and the uniform the kernels use, evaluated on the DEVICE
+ * for n counters (tests pin the in-kernel generator against the CUDA toolkit's own).
+ *   d_ctr u32[4n], key[2] HOST, d_out u32[4n]                                              */
+int mpr_debug_philox(const uint32_t* d_ctr, const uint32_t key[2], uint32_t* d_out, int64_t n,
+                     void* cuda_stream);
+
+const char* mpr_last_error(const mpr_ctx* ctx);
+const char* mpr_status_string(int status);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* MPR_H_ */

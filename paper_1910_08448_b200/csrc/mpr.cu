@@ -1,0 +1,729 @@
+// mpr.cu -- host side of libmpr.so: the C ABI declared in include/mpr.h, workspace carving,
+// launch logic of both kernel paths, the temperature-matching loop (R6) and the binned error
+// (R16).  No torch types, no device allocation, no CPU fallback.
+#include "../../include/mpr.h"
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <limits>
+#include <new>
+#include <string>
+#include <vector>
+
+#include <cuda.h>
+#include <cuda_runtime.h>
+
+#include "mpr_device.cuh"
+#include "mpr_plain.cuh"
+#include "mpr_tiled.cuh"
+
+using namespace mpr;
+
+namespace {
+
+constexpr double kQ = 0.5;   // PAPER.md:27; north_star fixes q = 1/2
+constexpr double kJ = 1.0;
+constexpr int kMaxL = 32768;
+constexpr int kPartials = 1 << 18;       // doubles
+constexpr int kSeriesCap = 1 << 16;      // energy samples per mpr_run
+constexpr int kAcceptSlots = 1024;
+constexpr int kTrialEq = 200, kTrialMeas = 50, kMaxIllinois = 20;   // R6
+
+size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+struct Layout {
+  Geom g;
+  size_t off_state[2], off_acc, off_bits, off_part, off_series, off_slots, off_scal, total;
+};
+
+Layout make_layout(int L) {
+  Layout lo;
+  lo.g.L = L;
+  lo.g.Wp = static_cast<int>(align_up(static_cast<size_t>((L + 1) / 2), 16));
+  lo.g.Wm = (lo.g.Wp + 31) / 32;
+  lo.g.plane = static_cast<size_t>(L) * lo.g.Wp;
+  size_t o = 0;
+  const size_t state_bytes = 2 * lo.g.plane * sizeof(double2);
+  lo.off_state[0] = o; o = align_up(o + state_bytes, 256);
+  lo.off_state[1] = o; o = align_up(o + state_bytes, 256);
+  lo.off_acc = o;      o = align_up(o + 2 * lo.g.plane * sizeof(double), 256);
+  lo.off_bits = o;     o = align_up(o + static_cast<size_t>(2) * L * lo.g.Wm * sizeof(uint32_t), 256);
+  lo.off_part = o;     o = align_up(o + kPartials * sizeof(double), 256);
+  lo.off_series = o;   o = align_up(o + kSeriesCap * sizeof(double), 256);
+  lo.off_slots = o;    o = align_up(o + kAcceptSlots * sizeof(unsigned long long), 256);
+  lo.off_scal = o;     o = align_up(o + 64 * sizeof(double), 256);
+  lo.total = o;
+  return lo;
+}
+
+}  // namespace
+
+struct mpr_ctx {
+  Layout lo;
+  const double* d_values = nullptr;
+  const uint8_t* d_mask = nullptr;
+  char* ws = nullptr;
+  cudaStream_t stream = nullptr;
+  int mode = MPR_DP;
+  int path = MPR_PATH_TILED;
+  int fused = 1;
+  int n_quench = 32;
+  uint64_t seed = 0;
+  uint32_t trial = 0;
+  uint64_t sweep = 0;
+  uint64_t attempted = 0;
+  long long n_acc = 0;
+  int cur = 0;                 // which state buffer holds the chain
+  double T = -1.0;
+  double zmin = 0.0, zmax = 0.0;
+  double e_sample = 0.0;
+  long long n_pairs = 0;
+  long long n_free = 0;
+  uint64_t launches = 0;
+  std::vector<double> series;
+  std::string err;
+  TiledPlan tiled;
+
+  void* state(int b) const { return ws + lo.off_state[b]; }
+  double* acc() const { return reinterpret_cast<double*>(ws + lo.off_acc); }
+  uint32_t* bits() const { return reinterpret_cast<uint32_t*>(ws + lo.off_bits); }
+  double* part() const { return reinterpret_cast<double*>(ws + lo.off_part); }
+  double* dseries() const { return reinterpret_cast<double*>(ws + lo.off_series); }
+  unsigned long long* slots() const { return reinterpret_cast<unsigned long long*>(ws + lo.off_slots); }
+  double* scal() const { return reinterpret_cast<double*>(ws + lo.off_scal); }
+};
+
+namespace {
+
+int fail(mpr_ctx* c, int code, const std::string& msg) {
+  if (c) c->err = msg;
+  return code;
+}
+#define CUDA_OK(ctx, expr)                                                                         \
+  do {                                                                                             \
+    cudaError_t e_ = (expr);                                                                       \
+    if (e_ != cudaSuccess)                                                                         \
+      return fail(ctx, MPR_ERR_CUDA, std::string(#expr) + ": " + cudaGetErrorString(e_));          \
+  } while (0)
+#define LAUNCH_OK(ctx)                                                                             \
+  do {                                                                                             \
+    (ctx)->launches += 1;                                                                          \
+    cudaError_t e_ = cudaGetLastError();                                                           \
+    if (e_ != cudaSuccess) return fail(ctx, MPR_ERR_CUDA, std::string("launch: ") + cudaGetErrorString(e_)); \
+  } while (0)
+#define TRY(expr)                                                                                  \
+  do {                                                                                             \
+    int st_ = (expr);                                                                              \
+    if (st_ != MPR_OK) return st_;                                                                 \
+  } while (0)
+
+// R7: proposal half-width delta = min(pi, 4 sqrt(T / (4 J q^2))).
+double proposal_width(double T) {
+  const double d = 4.0 * std::sqrt(T / (4.0 * kJ * kQ * kQ));
+  const double pi = 3.14159265358979323846264338327950288;
+  return d < pi ? d : pi;
+}
+
+template <typename R>
+ChainConst<R> chain_const(const mpr_ctx* c) {
+  ChainConst<R> k;
+  const double T = c->T > 0.0 ? c->T : 1.0;
+  k.delta = static_cast<R>(proposal_width(T));
+  k.inv_T = static_cast<R>(1.0 / T);
+  k.k0 = static_cast<uint32_t>(c->seed);
+  k.k1 = static_cast<uint32_t>(c->seed >> 32);
+  k.trial = c->trial;
+  return k;
+}
+
+// Mean and binned standard error (R16): 10 equal bins if n >= 20, else bins of one sample;
+// unbiased variance of the bin means over the number of bins.
+void mean_stderr(const std::vector<double>& v, double* mean, double* se) {
+  const size_t n = v.size();
+  double m = 0.0;
+  for (double x : v) m += x;
+  m = n ? m / static_cast<double>(n) : std::numeric_limits<double>::quiet_NaN();
+  double s = 0.0;
+  if (n >= 2) {
+    const size_t nb = n >= 20 ? 10 : n;
+    const size_t len = n / nb;
+    std::vector<double> bm(nb, 0.0);
+    double bmean = 0.0;
+    for (size_t b = 0; b < nb; ++b) {
+      for (size_t k = 0; k < len; ++k) bm[b] += v[b * len + k];
+      bm[b] /= static_cast<double>(len);
+      bmean += bm[b];
+    }
+    bmean /= static_cast<double>(nb);
+    double var = 0.0;
+    for (size_t b = 0; b < nb; ++b) var += (bm[b] - bmean) * (bm[b] - bmean);
+    var /= static_cast<double>(nb - 1);
+    s = std::sqrt(var / static_cast<double>(nb));
+  }
+  if (mean) *mean = m;
+  if (se) *se = s;
+}
+
+// ---- mode dispatch ---------------------------------------------------------------------------
+template <int MODE> int plain_pass(mpr_ctx* c, int kind, int col, uint64_t sweep) {
+  using R = typename Traits<MODE>::real;
+  using V = typename Traits<MODE>::vec;
+  const Geom& g = c->lo.g;
+  dim3 block(128), grid((g.Wp + 127) / 128, g.L);
+  V* st = static_cast<V*>(c->state(c->cur));
+  const ChainConst<R> k = chain_const<R>(c);
+  const uint32_t sw = static_cast<uint32_t>(sweep);
+  if (kind == KIND_MET)
+    plain_pass_kernel<MODE, KIND_MET><<<grid, block, 0, c->stream>>>(st, c->bits(), g, col, sw, k, c->slots());
+  else if (kind == KIND_OR)
+    plain_pass_kernel<MODE, KIND_OR><<<grid, block, 0, c->stream>>>(st, c->bits(), g, col, sw, k, c->slots());
+  else
+    plain_pass_kernel<MODE, KIND_QUENCH><<<grid, block, 0, c->stream>>>(st, c->bits(), g, col, sw, k, c->slots());
+  LAUNCH_OK(c);
+  return MPR_OK;
+}
+
+template <int MODE> int init_chain(mpr_ctx* c) {
+  using V = typename Traits<MODE>::vec;
+  const Geom& g = c->lo.g;
+  dim3 block(128), grid((g.Wp + 127) / 128, g.L, 2);
+  init_chain_kernel<MODE><<<grid, block, 0, c->stream>>>(c->d_values, c->d_mask, g, c->zmin, c->zmax,
+                                                         static_cast<uint32_t>(c->seed),
+                                                         static_cast<uint32_t>(c->seed >> 32), c->trial,
+                                                         static_cast<V*>(c->state(c->cur)));
+  LAUNCH_OK(c);
+  return MPR_OK;
+}
+
+// Energy of the current state into d_out[0] (e = 2H/N_b when `as_e`, else H).
+template <int MODE> int plain_energy(mpr_ctx* c, double* d_out, bool as_e) {
+  using V = typename Traits<MODE>::vec;
+  const Geom& g = c->lo.g;
+  const int nblk = g.L < 2048 ? g.L : 2048;
+  plain_energy_kernel<MODE><<<nblk, 256, 0, c->stream>>>(static_cast<const V*>(c->state(c->cur)), g, c->part());
+  LAUNCH_OK(c);
+  const double nb = 2.0 * g.L * (g.L - 1.0);
+  final_sum_kernel<<<1, 1024, 0, c->stream>>>(c->part(), nblk, as_e ? -kJ * 2.0 / nb : -kJ, d_out);
+  LAUNCH_OK(c);
+  return MPR_OK;
+}
+
+template <int MODE> int plain_accumulate(mpr_ctx* c) {
+  using V = typename Traits<MODE>::vec;
+  const Geom& g = c->lo.g;
+  dim3 block(128), grid((g.Wp + 127) / 128, g.L, 2);
+  plain_accumulate_kernel<MODE><<<grid, block, 0, c->stream>>>(static_cast<const V*>(c->state(c->cur)), c->bits(),
+                                                               g, c->acc());
+  LAUNCH_OK(c);
+  return MPR_OK;
+}
+
+template <int MODE> int get_state(mpr_ctx* c, double* d_phi) {
+  using V = typename Traits<MODE>::vec;
+  const Geom& g = c->lo.g;
+  dim3 block(128), grid((g.L + 127) / 128, g.L);
+  get_state_kernel<MODE><<<grid, block, 0, c->stream>>>(static_cast<const V*>(c->state(c->cur)), g, d_phi);
+  LAUNCH_OK(c);
+  return MPR_OK;
+}
+
+template <int MODE> int set_state(mpr_ctx* c, const double* d_phi) {
+  using V = typename Traits<MODE>::vec;
+  const Geom& g = c->lo.g;
+  dim3 block(128), grid((g.Wp + 127) / 128, g.L, 2);
+  set_state_kernel<MODE><<<grid, block, 0, c->stream>>>(d_phi, g, c->bits(), static_cast<V*>(c->state(c->cur)));
+  LAUNCH_OK(c);
+  return MPR_OK;
+}
+
+// k hybrid sweeps of the tiled path (k <= fused depth), with the energy sample and the
+// accumulation of phi after the last one when `measure`; d_e receives e_n.
+template <int MODE> int tiled_sweeps(mpr_ctx* c, int k, bool measure, double* d_e) {
+  using R = typename Traits<MODE>::real;
+  const Geom& g = c->lo.g;
+  int ntiles = 0;
+  const int st = tiled_launch<MODE>(c->tiled, g, c->state(c->cur), c->state(1 - c->cur), c->bits(), c->acc(),
+                                    c->part(), c->slots(), chain_const<R>(c), static_cast<uint32_t>(c->sweep + 1), k,
+                                    measure, c->stream, &ntiles);
+  if (st != 0) return fail(c, MPR_ERR_CUDA, std::string("tiled launch: ") + tiled_error(st));
+  c->launches += 1;
+  c->cur = 1 - c->cur;
+  if (measure) {
+    const double nb = 2.0 * g.L * (g.L - 1.0);
+    final_sum_kernel<<<1, 1024, 0, c->stream>>>(c->part(), ntiles, -kJ * 2.0 / nb, d_e);
+    LAUNCH_OK(c);
+  }
+  return MPR_OK;
+}
+
+#define DISPATCH(c, call)                                                     \
+  ((c)->mode == MPR_DP           ? call<MODE_DP>                              \
+   : (c)->mode == MPR_SP         ? call<MODE_SP>                              \
+   : (c)->mode == MPR_SP_PRECISE ? call<MODE_SP_PRECISE>                      \
+                                 : call<MODE_SP_INTRINSIC>)
+
+int do_pass(mpr_ctx* c, int kind, int col, uint64_t sweep) {
+  switch (c->mode) {
+    case MPR_DP: return plain_pass<MODE_DP>(c, kind, col, sweep);
+    case MPR_SP: return plain_pass<MODE_SP>(c, kind, col, sweep);
+    case MPR_SP_PRECISE: return plain_pass<MODE_SP_PRECISE>(c, kind, col, sweep);
+    default: return plain_pass<MODE_SP_INTRINSIC>(c, kind, col, sweep);
+  }
+}
+int do_init(mpr_ctx* c) {
+  switch (c->mode) {
+    case MPR_DP: return init_chain<MODE_DP>(c);
+    case MPR_SP: return init_chain<MODE_SP>(c);
+    case MPR_SP_PRECISE: return init_chain<MODE_SP_PRECISE>(c);
+    default: return init_chain<MODE_SP_INTRINSIC>(c);
+  }
+}
+int do_energy(mpr_ctx* c, double* d_out, bool as_e) {
+  switch (c->mode) {
+    case MPR_DP: return plain_energy<MODE_DP>(c, d_out, as_e);
+    case MPR_SP: return plain_energy<MODE_SP>(c, d_out, as_e);
+    case MPR_SP_PRECISE: return plain_energy<MODE_SP_PRECISE>(c, d_out, as_e);
+    default: return plain_energy<MODE_SP_INTRINSIC>(c, d_out, as_e);
+  }
+}
+int do_accumulate(mpr_ctx* c) {
+  switch (c->mode) {
+    case MPR_DP: return plain_accumulate<MODE_DP>(c);
+    case MPR_SP: return plain_accumulate<MODE_SP>(c);
+    case MPR_SP_PRECISE: return plain_accumulate<MODE_SP_PRECISE>(c);
+    default: return plain_accumulate<MODE_SP_INTRINSIC>(c);
+  }
+}
+int do_tiled(mpr_ctx* c, int k, bool measure, double* d_e) {
+  switch (c->mode) {
+    case MPR_DP: return tiled_sweeps<MODE_DP>(c, k, measure, d_e);
+    case MPR_SP: return tiled_sweeps<MODE_SP>(c, k, measure, d_e);
+    case MPR_SP_PRECISE: return tiled_sweeps<MODE_SP_PRECISE>(c, k, measure, d_e);
+    default: return tiled_sweeps<MODE_SP_INTRINSIC>(c, k, measure, d_e);
+  }
+}
+
+// R8: uniform initial spins, then n_quench x (quench colour 0, quench colour 1); everything
+// that belongs to the chain is cleared.
+int reset_chain(mpr_ctx* c, uint32_t trial) {
+  c->trial = trial;
+  c->sweep = 0;
+  c->attempted = 0;
+  c->n_acc = 0;
+  c->series.clear();
+  TRY(do_init(c));
+  for (int k = 0; k < c->n_quench; ++k) {
+    TRY(do_pass(c, KIND_QUENCH, 0, 0));
+    TRY(do_pass(c, KIND_QUENCH, 1, 0));
+  }
+  CUDA_OK(c, cudaMemsetAsync(c->slots(), 0, kAcceptSlots * sizeof(unsigned long long), c->stream));
+  const size_t n = 2 * c->lo.g.plane;
+  clear_acc_kernel<<<1184, 256, 0, c->stream>>>(c->acc(), n);
+  LAUNCH_OK(c);
+  return MPR_OK;
+}
+
+// n hybrid sweeps (R4); with `measure`, each is followed by the energy sample into
+// dseries[first_slot + i] and the accumulation of phi.
+int hybrid_sweeps(mpr_ctx* c, int n, bool measure, int first_slot) {
+  if (n <= 0) return MPR_OK;
+  if (!(c->T > 0.0)) return fail(c, MPR_ERR_NOT_READY, "temperature not set");
+  if (c->path == MPR_PATH_PLAIN) {
+    for (int i = 0; i < n; ++i) {
+      const uint64_t sw = c->sweep + 1;
+      TRY(do_pass(c, KIND_MET, 0, sw));
+      TRY(do_pass(c, KIND_MET, 1, sw));
+      TRY(do_pass(c, KIND_OR, 0, sw));
+      TRY(do_pass(c, KIND_OR, 1, sw));
+      c->sweep = sw;
+      c->attempted += static_cast<uint64_t>(c->n_free);
+      if (measure) {
+        TRY(do_energy(c, c->dseries() + first_slot + i, true));
+        TRY(do_accumulate(c));
+        c->n_acc += 1;
+      }
+    }
+    return MPR_OK;
+  }
+  int done = 0;
+  while (done < n) {
+    // measurement needs the state after every sweep: one sweep per launch there
+    const int k = measure ? 1 : (n - done < c->fused ? n - done : c->fused);
+    TRY(do_tiled(c, k, measure, measure ? c->dseries() + first_slot + done : nullptr));
+    c->sweep += static_cast<uint64_t>(k);
+    c->attempted += static_cast<uint64_t>(k) * static_cast<uint64_t>(c->n_free);
+    if (measure) c->n_acc += 1;
+    done += k;
+  }
+  return MPR_OK;
+}
+
+int fetch_series(mpr_ctx* c, int n) {
+  c->series.assign(static_cast<size_t>(n), 0.0);
+  if (n > 0)
+    CUDA_OK(c, cudaMemcpyAsync(c->series.data(), c->dseries(), n * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+  CUDA_OK(c, cudaStreamSynchronize(c->stream));
+  return MPR_OK;
+}
+
+// One temperature trial of R6: fresh chain with the trial index in the Philox counter.
+int trial_energy(mpr_ctx* c, int* est_trials, double T, double* e, double* se) {
+  *est_trials += 1;
+  c->T = T;
+  TRY(reset_chain(c, static_cast<uint32_t>(*est_trials)));
+  TRY(hybrid_sweeps(c, kTrialEq, false, 0));
+  TRY(hybrid_sweeps(c, kTrialMeas, true, 0));
+  TRY(fetch_series(c, kTrialMeas));
+  mean_stderr(c->series, e, se);
+  return MPR_OK;
+}
+
+int setup(mpr_ctx* c) {
+  const Geom& g = c->lo.g;
+  const size_t N = static_cast<size_t>(g.L) * g.L;
+  // R1: range of the measured sample
+  const int nblk = 1024;
+  sample_range_kernel<<<nblk, 256, 0, c->stream>>>(c->d_values, c->d_mask, N, c->part());
+  LAUNCH_OK(c);
+  sample_range_final_kernel<<<1, 32, 0, c->stream>>>(c->part(), nblk, c->scal());
+  LAUNCH_OK(c);
+  double h[4];
+  CUDA_OK(c, cudaMemcpyAsync(h, c->scal(), sizeof(h), cudaMemcpyDeviceToHost, c->stream));
+  CUDA_OK(c, cudaStreamSynchronize(c->stream));
+  if (h[2] == 0.0) return fail(c, MPR_ERR_NO_MEASURED, "no measured site");
+  if (h[3] != 0.0) return fail(c, MPR_ERR_NONFINITE, "non-finite value at a measured site");
+  if (!(h[1] > h[0])) return fail(c, MPR_ERR_DEGENERATE_RANGE, "z_max == z_min over the measured sample");
+  c->zmin = h[0];
+  c->zmax = h[1];
+  // R6: sample energy
+  sample_energy_kernel<<<nblk, 256, 0, c->stream>>>(c->d_values, c->d_mask, g.L, c->zmin, c->zmax, c->part());
+  LAUNCH_OK(c);
+  pair_final_kernel<<<1, 32, 0, c->stream>>>(c->part(), nblk, c->scal());
+  LAUNCH_OK(c);
+  // mask bitmaps and the number of prediction sites
+  const size_t nwords = static_cast<size_t>(2) * g.L * g.Wm;
+  const int mblk = static_cast<int>((nwords + 255) / 256);
+  if (mblk > kPartials) return fail(c, MPR_ERR_INVALID_ARG, "grid too large");
+  double* cnt_part = c->part() + 2 * nblk;
+  pack_mask_kernel<<<mblk, 256, 0, c->stream>>>(c->d_mask, g, c->bits(), cnt_part);
+  LAUNCH_OK(c);
+  final_sum_kernel<<<1, 1024, 0, c->stream>>>(cnt_part, mblk, 1.0, c->scal() + 2);
+  LAUNCH_OK(c);
+  double h2[3];
+  CUDA_OK(c, cudaMemcpyAsync(h2, c->scal(), sizeof(h2), cudaMemcpyDeviceToHost, c->stream));
+  CUDA_OK(c, cudaStreamSynchronize(c->stream));
+  c->n_pairs = static_cast<long long>(h2[1]);
+  c->e_sample = c->n_pairs > 0 ? -2.0 * kJ * h2[0] / h2[1] : std::numeric_limits<double>::quiet_NaN();
+  c->n_free = static_cast<long long>(h2[2]);
+  return MPR_OK;
+}
+
+}  // namespace
+
+// =============================================================================================
+extern "C" {
+
+const char* mpr_status_string(int status) {
+  switch (status) {
+    case MPR_OK: return "ok";
+    case MPR_ERR_INVALID_ARG: return "invalid argument";
+    case MPR_ERR_NO_MEASURED: return "no measured site / pair";
+    case MPR_ERR_DEGENERATE_RANGE: return "degenerate value range";
+    case MPR_ERR_NONFINITE: return "non-finite measured value";
+    case MPR_ERR_WORKSPACE: return "workspace null, misaligned or too small";
+    case MPR_ERR_NOT_READY: return "temperature not set";
+    case MPR_ERR_NO_ROOT: return "sample energy not bracketed by e(T)";
+    case MPR_ERR_CUDA: return "CUDA error";
+    default: return "unknown status";
+  }
+}
+
+const char* mpr_last_error(const mpr_ctx* ctx) { return ctx ? ctx->err.c_str() : ""; }
+
+int mpr_workspace_bytes(int L, size_t* bytes) {
+  if (L < 2 || L > kMaxL || !bytes) return MPR_ERR_INVALID_ARG;
+  *bytes = make_layout(L).total;
+  return MPR_OK;
+}
+
+int mpr_create(mpr_ctx** out, int L, const double* d_values, const uint8_t* d_mask, void* d_workspace,
+               size_t workspace_bytes, void* cuda_stream) {
+  if (!out) return MPR_ERR_INVALID_ARG;
+  *out = nullptr;
+  if (L < 2 || L > kMaxL || !d_values || !d_mask) return MPR_ERR_INVALID_ARG;
+  const Layout lo = make_layout(L);
+  if (!d_workspace || (reinterpret_cast<uintptr_t>(d_workspace) & 255u) || workspace_bytes < lo.total)
+    return MPR_ERR_WORKSPACE;
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) return MPR_ERR_CUDA;
+  mpr_ctx* c = new (std::nothrow) mpr_ctx;
+  if (!c) return MPR_ERR_INVALID_ARG;
+  c->lo = lo;
+  c->d_values = d_values;
+  c->d_mask = d_mask;
+  c->ws = static_cast<char*>(d_workspace);
+  c->stream = static_cast<cudaStream_t>(cuda_stream);
+  int st = setup(c);
+  if (st == MPR_OK) {
+    const int ts = tiled_plan_init(&c->tiled, c->lo.g);
+    if (ts != 0) st = fail(c, MPR_ERR_CUDA, std::string("tiled plan: ") + tiled_error(ts));
+  }
+  if (st == MPR_OK) st = reset_chain(c, 0);
+  if (st != MPR_OK) { delete c; return st; }
+  *out = c;
+  return MPR_OK;
+}
+
+void mpr_destroy(mpr_ctx* ctx) { delete ctx; }
+
+int mpr_set_precision(mpr_ctx* c, mpr_precision mode) {
+  if (!c || mode < MPR_DP || mode > MPR_SP_INTRINSIC) return fail(c, MPR_ERR_INVALID_ARG, "bad mode");
+  c->mode = mode;
+  return reset_chain(c, 0);
+}
+int mpr_set_seed(mpr_ctx* c, uint64_t seed) {
+  if (!c) return MPR_ERR_INVALID_ARG;
+  c->seed = seed;
+  return reset_chain(c, 0);
+}
+int mpr_set_temperature(mpr_ctx* c, double T) {
+  if (!c || !(T > 0.0) || !std::isfinite(T)) return fail(c, MPR_ERR_INVALID_ARG, "T must be finite and > 0");
+  c->T = T;
+  return MPR_OK;
+}
+int mpr_set_quench(mpr_ctx* c, int n) {
+  if (!c || n < 0) return fail(c, MPR_ERR_INVALID_ARG, "n_quench < 0");
+  c->n_quench = n;
+  return reset_chain(c, 0);
+}
+int mpr_set_path(mpr_ctx* c, mpr_path path) {
+  if (!c || (path != MPR_PATH_TILED && path != MPR_PATH_PLAIN)) return fail(c, MPR_ERR_INVALID_ARG, "bad path");
+  c->path = path;
+  return MPR_OK;
+}
+int mpr_set_fused_sweeps(mpr_ctx* c, int k) {
+  if (!c || k < 1 || k > tiled_max_fused()) return fail(c, MPR_ERR_INVALID_ARG, "fused depth out of range");
+  c->fused = k;
+  return MPR_OK;
+}
+int mpr_reset_chain(mpr_ctx* c, uint32_t trial) {
+  if (!c) return MPR_ERR_INVALID_ARG;
+  return reset_chain(c, trial);
+}
+
+int mpr_estimate_temperature(mpr_ctx* c, double* T_hat, double* e_sample, int* n_trials) {
+  if (!c) return MPR_ERR_INVALID_ARG;
+  if (c->n_pairs == 0) return fail(c, MPR_ERR_NO_MEASURED, "no measured nearest-neighbour pair");
+  const double es = c->e_sample;
+  if (e_sample) *e_sample = es;
+  int trials = 0;
+  double T_lo = 1e-4, T_hi = 1.0, g_lo = 0.0, g_hi = 0.0, e = 0.0, se = 0.0;
+  bool have_hi = false;
+  auto done = [&](int st) { if (n_trials) *n_trials = trials; return st; };
+  TRY(trial_energy(c, &trials, T_lo, &e, &se));
+  g_lo = e - es;
+  while (g_lo > 0.0) {
+    if (T_lo <= 1.5e-6) return done(fail(c, MPR_ERR_NO_ROOT, "e_sample below e(T) for every T >= 1e-6"));
+    T_hi = T_lo; g_hi = g_lo; have_hi = true;
+    T_lo /= 10.0;
+    TRY(trial_energy(c, &trials, T_lo, &e, &se));
+    g_lo = e - es;
+  }
+  if (!have_hi) {
+    TRY(trial_energy(c, &trials, T_hi, &e, &se));
+    g_hi = e - es;
+    while (g_hi < 0.0) {
+      if (T_hi >= 0.99e2) return done(fail(c, MPR_ERR_NO_ROOT, "e_sample above e(T) for every T <= 1e2"));
+      T_lo = T_hi; g_lo = g_hi;
+      T_hi *= 10.0;
+      TRY(trial_energy(c, &trials, T_hi, &e, &se));
+      g_hi = e - es;
+    }
+  }
+  double T_new = T_hi, T_prev = T_hi;
+  int last_side = 0;
+  for (int it = 0; it < kMaxIllinois; ++it) {
+    T_new = T_hi - g_hi * (T_hi - T_lo) / (g_hi - g_lo);
+    if (!(T_new > T_lo && T_new < T_hi)) T_new = 0.5 * (T_lo + T_hi);
+    TRY(trial_energy(c, &trials, T_new, &e, &se));
+    const double g = e - es;
+    if (std::fabs(g) <= 2.0 * se) break;
+    if (g < 0.0) {
+      T_lo = T_new; g_lo = g;
+      if (last_side == -1) g_hi *= 0.5;
+      last_side = -1;
+    } else {
+      T_hi = T_new; g_hi = g;
+      if (last_side == +1) g_lo *= 0.5;
+      last_side = +1;
+    }
+    if (it > 0 && std::fabs(T_new - T_prev) / T_new < 0.01) break;
+    T_prev = T_new;
+  }
+  c->T = T_new;
+  TRY(reset_chain(c, 0));
+  if (T_hat) *T_hat = T_new;
+  return done(MPR_OK);
+}
+
+int mpr_sweep(mpr_ctx* c, int n) {
+  if (!c || n < 0) return fail(c, MPR_ERR_INVALID_ARG, "n < 0");
+  return hybrid_sweeps(c, n, false, 0);
+}
+
+int mpr_pass(mpr_ctx* c, int kind, int colour, uint64_t sweep) {
+  if (!c || kind < 0 || kind > 2) return fail(c, MPR_ERR_INVALID_ARG, "bad pass kind");
+  if (kind == KIND_MET && !(c->T > 0.0)) return fail(c, MPR_ERR_NOT_READY, "temperature not set");
+  return do_pass(c, kind, colour & 1, sweep);
+}
+
+int mpr_run(mpr_ctx* c, int n_eq, int n_meas, double* d_pred, double* e_mean, double* e_stderr) {
+  if (!c || n_eq < 0 || n_meas < 0 || n_meas > kSeriesCap) return fail(c, MPR_ERR_INVALID_ARG, "bad sweep counts");
+  if (!(c->T > 0.0)) return fail(c, MPR_ERR_NOT_READY, "temperature not set");
+  TRY(hybrid_sweeps(c, n_eq, false, 0));
+  TRY(hybrid_sweeps(c, n_meas, true, 0));
+  if (d_pred) {
+    const Geom& g = c->lo.g;
+    dim3 block(128), grid((g.L + 127) / 128, g.L);
+    predict_kernel<<<grid, block, 0, c->stream>>>(c->d_values, c->d_mask, g, c->acc(), c->zmin, c->zmax, c->n_acc,
+                                                  d_pred);
+    LAUNCH_OK(c);
+  }
+  TRY(fetch_series(c, n_meas));
+  mean_stderr(c->series, e_mean, e_stderr);
+  return MPR_OK;
+}
+
+int mpr_get_state(mpr_ctx* c, double* d_phi) {
+  if (!c || !d_phi) return fail(c, MPR_ERR_INVALID_ARG, "null pointer");
+  switch (c->mode) {
+    case MPR_DP: return get_state<MODE_DP>(c, d_phi);
+    case MPR_SP: return get_state<MODE_SP>(c, d_phi);
+    case MPR_SP_PRECISE: return get_state<MODE_SP_PRECISE>(c, d_phi);
+    default: return get_state<MODE_SP_INTRINSIC>(c, d_phi);
+  }
+}
+int mpr_set_state(mpr_ctx* c, const double* d_phi) {
+  if (!c || !d_phi) return fail(c, MPR_ERR_INVALID_ARG, "null pointer");
+  switch (c->mode) {
+    case MPR_DP: return set_state<MODE_DP>(c, d_phi);
+    case MPR_SP: return set_state<MODE_SP>(c, d_phi);
+    case MPR_SP_PRECISE: return set_state<MODE_SP_PRECISE>(c, d_phi);
+    default: return set_state<MODE_SP_INTRINSIC>(c, d_phi);
+  }
+}
+
+int mpr_energy(mpr_ctx* c, double* H, double* e) {
+  if (!c) return MPR_ERR_INVALID_ARG;
+  TRY(do_energy(c, c->scal() + 8, false));
+  double h = 0.0;
+  CUDA_OK(c, cudaMemcpyAsync(&h, c->scal() + 8, sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+  CUDA_OK(c, cudaStreamSynchronize(c->stream));
+  const double nb = 2.0 * c->lo.g.L * (c->lo.g.L - 1.0);
+  if (H) *H = h;
+  if (e) *e = 2.0 * h / nb;
+  return MPR_OK;
+}
+
+int mpr_sample_energy(mpr_ctx* c, double* e_sample, int64_t* n_pairs) {
+  if (!c) return MPR_ERR_INVALID_ARG;
+  if (n_pairs) *n_pairs = c->n_pairs;
+  if (c->n_pairs == 0) return fail(c, MPR_ERR_NO_MEASURED, "no measured nearest-neighbour pair");
+  if (e_sample) *e_sample = c->e_sample;
+  return MPR_OK;
+}
+
+int mpr_get_counters(mpr_ctx* c, uint64_t* accepted, uint64_t* attempted, uint64_t* sweeps) {
+  if (!c) return MPR_ERR_INVALID_ARG;
+  unsigned long long h[kAcceptSlots];
+  CUDA_OK(c, cudaMemcpyAsync(h, c->slots(), sizeof(h), cudaMemcpyDeviceToHost, c->stream));
+  CUDA_OK(c, cudaStreamSynchronize(c->stream));
+  unsigned long long a = 0;
+  for (int i = 0; i < kAcceptSlots; ++i) a += h[i];
+  if (accepted) *accepted = a;
+  if (attempted) *attempted = c->attempted;
+  if (sweeps) *sweeps = c->sweep;
+  return MPR_OK;
+}
+
+int64_t mpr_get_energy_series(mpr_ctx* c, double* out, int64_t cap) {
+  if (!c) return MPR_ERR_INVALID_ARG;
+  const int64_t n = static_cast<int64_t>(c->series.size());
+  for (int64_t k = 0; out && k < n && k < cap; ++k) out[k] = c->series[k];
+  return n;
+}
+
+int mpr_get_info(mpr_ctx* c, double* z_min, double* z_max, int64_t* n_free, double* T) {
+  if (!c) return MPR_ERR_INVALID_ARG;
+  if (z_min) *z_min = c->zmin;
+  if (z_max) *z_max = c->zmax;
+  if (n_free) *n_free = c->n_free;
+  if (T) *T = c->T;
+  return MPR_OK;
+}
+
+int mpr_get_launch_stats(mpr_ctx* c, uint64_t* launches) {
+  if (!c || !launches) return MPR_ERR_INVALID_ARG;
+  *launches = c->launches;
+  return MPR_OK;
+}
+
+int mpr_workspace_bytes_host(int L, size_t* bytes) {
+  size_t b = 0;
+  const int st = mpr_workspace_bytes(L, &b);
+  if (st != MPR_OK) return st;
+  const size_t N = static_cast<size_t>(L) * L;
+  *bytes = b + align_up(N * sizeof(double), 256) * 2 + align_up(N, 256);
+  return MPR_OK;
+}
+
+int mpr_predict_host(int L, const double* h_values, const uint8_t* h_mask, mpr_precision mode, uint64_t seed, double T,
+                     int n_eq, int n_meas, void* d_workspace, size_t workspace_bytes, void* cuda_stream,
+                     double* h_pred, double* e_mean, double* e_stderr, double* T_used, uint64_t* launches) {
+  size_t need = 0, core = 0;
+  if (mpr_workspace_bytes_host(L, &need) != MPR_OK || !h_values || !h_mask) return MPR_ERR_INVALID_ARG;
+  mpr_workspace_bytes(L, &core);
+  if (!d_workspace || (reinterpret_cast<uintptr_t>(d_workspace) & 255u) || workspace_bytes < need)
+    return MPR_ERR_WORKSPACE;
+  const size_t N = static_cast<size_t>(L) * L;
+  char* base = static_cast<char*>(d_workspace) + core;
+  double* d_values = reinterpret_cast<double*>(base);
+  double* d_pred = reinterpret_cast<double*>(base + align_up(N * sizeof(double), 256));
+  uint8_t* d_mask = reinterpret_cast<uint8_t*>(base + 2 * align_up(N * sizeof(double), 256));
+  cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
+  if (cudaMemcpyAsync(d_values, h_values, N * sizeof(double), cudaMemcpyHostToDevice, s) != cudaSuccess ||
+      cudaMemcpyAsync(d_mask, h_mask, N, cudaMemcpyHostToDevice, s) != cudaSuccess)
+    return MPR_ERR_CUDA;
+  mpr_ctx* c = nullptr;
+  int st = mpr_create(&c, L, d_values, d_mask, d_workspace, core, cuda_stream);
+  if (st != MPR_OK) return st;
+  c->mode = mode;
+  c->seed = seed;
+  if (T > 0.0) {
+    c->T = T;
+    st = reset_chain(c, 0);
+  } else {
+    st = mpr_estimate_temperature(c, nullptr, nullptr, nullptr);
+  }
+  if (st == MPR_OK) st = mpr_run(c, n_eq, n_meas, h_pred ? d_pred : nullptr, e_mean, e_stderr);
+  if (st == MPR_OK && h_pred) {
+    if (cudaMemcpyAsync(h_pred, d_pred, N * sizeof(double), cudaMemcpyDeviceToHost, s) != cudaSuccess ||
+        cudaStreamSynchronize(s) != cudaSuccess)
+      st = MPR_ERR_CUDA;
+  }
+  if (T_used) *T_used = c->T;
+  if (launches) *launches = c->launches;
+  mpr_destroy(c);
+  return st;
+}
+
+int mpr_debug_philox(const uint32_t* d_ctr, const uint32_t key[2], uint32_t* d_out, int64_t n, void* cuda_stream) {
+  if (!d_ctr || !key || !d_out || n < 0) return MPR_ERR_INVALID_ARG;
+  if (n == 0) return MPR_OK;
+  philox_debug_kernel<<<static_cast<unsigned>((n + 255) / 256), 256, 0, static_cast<cudaStream_t>(cuda_stream)>>>(
+      d_ctr, key[0], key[1], d_out, n);
+  return cudaGetLastError() == cudaSuccess ? MPR_OK : MPR_ERR_CUDA;
+}
+
+}  // extern "C"

@@ -1,0 +1,330 @@
+// mpr_plain.cuh -- kernels that work directly on the global colour planes: set-up (R1 map,
+// mask bitmaps, sample energy), chain initialisation (R8), one-launch-per-colour-pass updates
+// (the PLAIN path, also the quench passes of R8), energy (R3), accumulation and back-map (R15).
+//
+// Layout.  Site (x, y) has colour (x + y) & 1 and lives in colour plane `col`
+// at row y, column j = x >> 1; a plane is L rows of Wp columns (Wp = ceil(L/2) rounded up to 16),
+// one vec (c, s) per site.  mask bit j of row y of plane col is 1 iff the site exists and is a
+// prediction site; Wm 32-bit words per row.
+#pragma once
+#include "mpr_device.cuh"
+
+namespace mpr {
+
+struct Geom {
+  int L, Wp, Wm;
+  size_t plane;          // elements per colour plane = L * Wp
+};
+
+__device__ __forceinline__ bool mask_bit(const uint32_t* __restrict__ bits, const Geom& g, int col, int y, int j) {
+  return (bits[(static_cast<size_t>(col) * g.L + y) * g.Wm + (j >> 5)] >> (j & 31)) & 1u;
+}
+
+// ---- block reduction helpers (deterministic order) -------------------------------------
+__device__ __forceinline__ double warp_sum(double v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+  return v;
+}
+__device__ __forceinline__ double block_sum(double v, double* sh /* >= 32 */) {
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, nw = (blockDim.x + 31) >> 5;
+  v = warp_sum(v);
+  __syncthreads();
+  if (lane == 0) sh[w] = v;
+  __syncthreads();
+  double r = 0.0;
+  if (w == 0) {
+    r = lane < nw ? sh[lane] : 0.0;
+    r = warp_sum(r);
+  }
+  return r;  // valid in thread 0
+}
+
+// out[0] = scale * sum(partials[0..n)), fixed order; one block.
+__global__ void final_sum_kernel(const double* __restrict__ partials, int n, double scale, double* out) {
+  __shared__ double sh[32];
+  double v = 0.0;
+  for (int i = threadIdx.x; i < n; i += blockDim.x) v += partials[i];
+  v = block_sum(v, sh);
+  if (threadIdx.x == 0) out[0] = scale * v;
+}
+
+// ---- set-up ---------------------------------------------------------------------------------
+// Per-block partials of the measured sample: [0] min, [1] max, [2] count, [3] non-finite count.
+__global__ void sample_range_kernel(const double* __restrict__ z, const uint8_t* __restrict__ mask, size_t N,
+                                    double* __restrict__ part /* 4 per block */) {
+  double mn = INFINITY, mx = -INFINITY, cnt = 0.0, bad = 0.0;
+  for (size_t i = blockIdx.x * static_cast<size_t>(blockDim.x) + threadIdx.x; i < N;
+       i += static_cast<size_t>(gridDim.x) * blockDim.x) {
+    if (mask[i]) continue;
+    const double v = z[i];
+    cnt += 1.0;
+    if (!isfinite(v)) { bad += 1.0; continue; }
+    mn = fmin(mn, v); mx = fmax(mx, v);
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    mn = fmin(mn, __shfl_down_sync(0xffffffffu, mn, o));
+    mx = fmax(mx, __shfl_down_sync(0xffffffffu, mx, o));
+    cnt += __shfl_down_sync(0xffffffffu, cnt, o);
+    bad += __shfl_down_sync(0xffffffffu, bad, o);
+  }
+  __shared__ double sh[4][32];
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, nw = blockDim.x >> 5;
+  if (lane == 0) { sh[0][w] = mn; sh[1][w] = mx; sh[2][w] = cnt; sh[3][w] = bad; }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    for (int k = 1; k < nw; ++k) {
+      mn = fmin(mn, sh[0][k]); mx = fmax(mx, sh[1][k]); cnt += sh[2][k]; bad += sh[3][k];
+    }
+    double* p = part + 4 * static_cast<size_t>(blockIdx.x);
+    p[0] = mn; p[1] = mx; p[2] = cnt; p[3] = bad;
+  }
+}
+__global__ void sample_range_final_kernel(const double* __restrict__ part, int nblocks, double* out /* 4 */) {
+  if (threadIdx.x != 0 || blockIdx.x != 0) return;
+  double mn = INFINITY, mx = -INFINITY, cnt = 0.0, bad = 0.0;
+  for (int b = 0; b < nblocks; ++b) {
+    mn = fmin(mn, part[4 * b]); mx = fmax(mx, part[4 * b + 1]); cnt += part[4 * b + 2]; bad += part[4 * b + 3];
+  }
+  out[0] = mn; out[1] = mx; out[2] = cnt; out[3] = bad;
+}
+
+// R1: phi = 2pi (z - zmin)/(zmax - zmin)
+__device__ __forceinline__ double map_to_phi(double z, double zmin, double zmax) {
+  return 6.283185307179586476925286766559 * ((z - zmin) / (zmax - zmin));
+}
+
+// R6 first half: e_s = -2J mean over measured nearest-neighbour pairs of cos[q(phi_s - phi_t)].
+// Per-block partials: [0] sum of cos, [1] pair count.
+__global__ void sample_energy_kernel(const double* __restrict__ z, const uint8_t* __restrict__ mask, int L,
+                                     double zmin, double zmax, double* __restrict__ part /* 2 per block */) {
+  __shared__ double sh[32];
+  double sum = 0.0, cnt = 0.0;
+  const size_t N = static_cast<size_t>(L) * L;
+  for (size_t i = blockIdx.x * static_cast<size_t>(blockDim.x) + threadIdx.x; i < N;
+       i += static_cast<size_t>(gridDim.x) * blockDim.x) {
+    if (mask[i]) continue;
+    const int x = static_cast<int>(i % L), y = static_cast<int>(i / L);
+    const double p = map_to_phi(z[i], zmin, zmax);
+    if (x < L - 1 && !mask[i + 1]) { sum += cos(0.5 * (p - map_to_phi(z[i + 1], zmin, zmax))); cnt += 1.0; }
+    if (y < L - 1 && !mask[i + L]) { sum += cos(0.5 * (p - map_to_phi(z[i + L], zmin, zmax))); cnt += 1.0; }
+  }
+  const double s = block_sum(sum, sh);
+  const double c = block_sum(cnt, sh);
+  if (threadIdx.x == 0) { part[2 * blockIdx.x] = s; part[2 * blockIdx.x + 1] = c; }
+}
+__global__ void pair_final_kernel(const double* __restrict__ part, int nblocks, double* out /* 2 */) {
+  if (threadIdx.x != 0 || blockIdx.x != 0) return;
+  double s = 0.0, c = 0.0;
+  for (int b = 0; b < nblocks; ++b) { s += part[2 * b]; c += part[2 * b + 1]; }
+  out[0] = s; out[1] = c;
+}
+
+// Mask bitmaps: one thread per 32-bit word; per-block partial = number of set bits.
+__global__ void pack_mask_kernel(const uint8_t* __restrict__ mask, Geom g, uint32_t* __restrict__ bits,
+                                 double* __restrict__ part) {
+  __shared__ double sh[32];
+  const size_t nwords = static_cast<size_t>(2) * g.L * g.Wm;
+  const size_t w = blockIdx.x * static_cast<size_t>(blockDim.x) + threadIdx.x;
+  double cnt = 0.0;
+  if (w < nwords) {
+    const int wi = static_cast<int>(w % g.Wm);
+    const size_t row = w / g.Wm;
+    const int y = static_cast<int>(row % g.L), col = static_cast<int>(row / g.L);
+    const int par = x_parity(y, col);
+    uint32_t word = 0;
+    for (int b = 0; b < 32; ++b) {
+      const int x = 2 * (32 * wi + b) + par;
+      if (x < g.L && mask[static_cast<size_t>(y) * g.L + x]) word |= (1u << b);
+    }
+    bits[w] = word;
+    cnt = static_cast<double>(__popc(word));
+  }
+  const double s = block_sum(cnt, sh);
+  if (threadIdx.x == 0) part[blockIdx.x] = s;
+}
+
+// ---- chain initialisation (R1 for the measured sites, R8 first half for the free ones) ------
+template <int MODE>
+__global__ void init_chain_kernel(const double* __restrict__ z, const uint8_t* __restrict__ mask, Geom g,
+                                  double zmin, double zmax, uint32_t k0, uint32_t k1, uint32_t trial,
+                                  typename Traits<MODE>::vec* __restrict__ state) {
+  using V = typename Traits<MODE>::vec;
+  const int y = blockIdx.y, col = blockIdx.z;
+  const int j = blockIdx.x * blockDim.x + threadIdx.x;
+  if (j >= g.Wp) return;
+  const int x = 2 * j + x_parity(y, col);
+  V v;
+  v.x = 1; v.y = 0;
+  if (x < g.L) {
+    const size_t s = static_cast<size_t>(y) * g.L + x;
+    double phi;
+    if (mask[s]) {
+      const uint4 r = philox4x32_10(static_cast<uint32_t>(s), 0u, PASS_INIT, trial, k0, k1);
+      phi = 6.283185307179586476925286766559 * u53(r.x, r.y);
+    } else {
+      phi = map_to_phi(z[s], zmin, zmax);
+    }
+    double sn, cs;
+    sincos(0.5 * phi, &sn, &cs);
+    if (sn < 0.0) sn = 0.0;
+    v.x = static_cast<decltype(v.x)>(cs);
+    v.y = static_cast<decltype(v.y)>(sn);
+  }
+  state[static_cast<size_t>(col) * g.plane + static_cast<size_t>(y) * g.Wp + j] = v;
+}
+
+// Overwrite the free spins from angles (tests, checkpoint restore).
+template <int MODE>
+__global__ void set_state_kernel(const double* __restrict__ phi, Geom g, const uint32_t* __restrict__ bits,
+                                 typename Traits<MODE>::vec* __restrict__ state) {
+  using V = typename Traits<MODE>::vec;
+  const int y = blockIdx.y, col = blockIdx.z;
+  const int j = blockIdx.x * blockDim.x + threadIdx.x;
+  if (j >= g.Wp) return;
+  if (!mask_bit(bits, g, col, y, j)) return;
+  const int x = 2 * j + x_parity(y, col);
+  double sn, cs;
+  sincos(0.5 * phi[static_cast<size_t>(y) * g.L + x], &sn, &cs);
+  if (sn < 0.0) sn = 0.0;
+  V v;
+  v.x = static_cast<decltype(v.x)>(cs);
+  v.y = static_cast<decltype(v.y)>(sn);
+  state[static_cast<size_t>(col) * g.plane + static_cast<size_t>(y) * g.Wp + j] = v;
+}
+
+template <int MODE>
+__global__ void get_state_kernel(const typename Traits<MODE>::vec* __restrict__ state, Geom g,
+                                 double* __restrict__ phi) {
+  const int y = blockIdx.y;
+  const int x = blockIdx.x * blockDim.x + threadIdx.x;
+  if (x >= g.L) return;
+  const int col = (x + y) & 1, j = x >> 1;
+  const auto v = state[static_cast<size_t>(col) * g.plane + static_cast<size_t>(y) * g.Wp + j];
+  phi[static_cast<size_t>(y) * g.L + x] = 2.0 * atan2(static_cast<double>(v.y), static_cast<double>(v.x));
+}
+
+// ---- one colour pass on the global planes -------------------------------------------------
+template <int MODE, int KIND>
+__global__ void __launch_bounds__(128)
+plain_pass_kernel(typename Traits<MODE>::vec* __restrict__ state, const uint32_t* __restrict__ bits, Geom g,
+                  int col, uint32_t sweep, ChainConst<typename Traits<MODE>::real> k,
+                  unsigned long long* __restrict__ accept_slots) {
+  using R = typename Traits<MODE>::real;
+  using V = typename Traits<MODE>::vec;
+  const int y = blockIdx.y;
+  const int j = blockIdx.x * blockDim.x + threadIdx.x;
+  bool accepted = false;
+  if (j < g.Wp && mask_bit(bits, g, col, y, j)) {
+    const int par = x_parity(y, col);
+    const int x = 2 * j + par;
+    V* own = state + static_cast<size_t>(col) * g.plane + static_cast<size_t>(y) * g.Wp;
+    const V* oth = state + static_cast<size_t>(1 - col) * g.plane + static_cast<size_t>(y) * g.Wp;
+    const bool hl = x > 0, hr = x < g.L - 1, hu = y > 0, hd = y < g.L - 1;
+    const int jl = j - 1 + par, jr = j + par;
+    V zero; zero.x = 0; zero.y = 0;
+    const V l = hl ? oth[jl] : zero;
+    const V r = hr ? oth[jr] : zero;
+    const V u = hu ? oth[j - g.Wp] : zero;
+    const V d = hd ? oth[j + g.Wp] : zero;
+    R A, B;
+    local_field<R>(R(l.x), R(l.y), R(r.x), R(r.y), R(u.x), R(u.y), R(d.x), R(d.y), hl, hr, hu, hd, &A, &B);
+    const V me = own[j];
+    R c = R(me.x), s = R(me.y);
+    if constexpr (KIND == KIND_MET) {
+      accepted = met_update<MODE>(&c, &s, A, B, static_cast<uint32_t>(y) * static_cast<uint32_t>(g.L) + x, sweep, k);
+    } else if constexpr (KIND == KIND_OR) {
+      or_update<MODE>(&c, &s, A, B);
+    } else {
+      quench_update<MODE>(&c, &s, A, B);
+    }
+    V out;
+    out.x = static_cast<decltype(out.x)>(c);
+    out.y = static_cast<decltype(out.y)>(s);
+    own[j] = out;
+  }
+  if constexpr (KIND == KIND_MET) {
+    const int n = __syncthreads_count(accepted);
+    if (threadIdx.x == 0 && n)
+      atomicAdd(accept_slots + ((blockIdx.y * gridDim.x + blockIdx.x) & 1023u), static_cast<unsigned long long>(n));
+  }
+}
+
+// ---- energy (R3): every bond has exactly one colour-1 end, so H = -J sum over colour-1
+// sites of u_s . F_s.  Terms in the mode's arithmetic, sums in double (R13).
+template <int MODE>
+__global__ void __launch_bounds__(256)
+plain_energy_kernel(const typename Traits<MODE>::vec* __restrict__ state, Geom g, double* __restrict__ part) {
+  using R = typename Traits<MODE>::real;
+  using V = typename Traits<MODE>::vec;
+  __shared__ double sh[32];
+  double sum = 0.0;
+  const int col = 1;
+  for (int y = blockIdx.x; y < g.L; y += gridDim.x) {
+    const int par = x_parity(y, col);
+    const V* own = state + static_cast<size_t>(col) * g.plane + static_cast<size_t>(y) * g.Wp;
+    const V* oth = state + static_cast<size_t>(1 - col) * g.plane + static_cast<size_t>(y) * g.Wp;
+    for (int j = threadIdx.x; j < g.Wp; j += blockDim.x) {
+      const int x = 2 * j + par;
+      if (x >= g.L) continue;
+      const bool hl = x > 0, hr = x < g.L - 1, hu = y > 0, hd = y < g.L - 1;
+      V zero; zero.x = 0; zero.y = 0;
+      const V l = hl ? oth[j - 1 + par] : zero;
+      const V r = hr ? oth[j + par] : zero;
+      const V u = hu ? oth[j - g.Wp] : zero;
+      const V d = hd ? oth[j + g.Wp] : zero;
+      R A, B;
+      local_field<R>(R(l.x), R(l.y), R(r.x), R(r.y), R(u.x), R(u.y), R(d.x), R(d.y), hl, hr, hu, hd, &A, &B);
+      const V me = own[j];
+      sum += static_cast<double>(fma_(R(me.x), A, R(me.y) * B));
+    }
+  }
+  const double s = block_sum(sum, sh);
+  if (threadIdx.x == 0) part[blockIdx.x] = s;
+}
+
+// ---- accumulation of phi at the free sites (R15) and the back-map --------------------------
+template <int MODE>
+__global__ void plain_accumulate_kernel(const typename Traits<MODE>::vec* __restrict__ state,
+                                        const uint32_t* __restrict__ bits, Geom g, double* __restrict__ acc) {
+  using R = typename Traits<MODE>::real;
+  const int y = blockIdx.y, col = blockIdx.z;
+  const int j = blockIdx.x * blockDim.x + threadIdx.x;
+  if (j >= g.Wp || !mask_bit(bits, g, col, y, j)) return;
+  const size_t i = static_cast<size_t>(col) * g.plane + static_cast<size_t>(y) * g.Wp + j;
+  const auto v = state[i];
+  acc[i] += spin_angle<MODE>(R(v.x), R(v.y));
+}
+
+__global__ void clear_acc_kernel(double* __restrict__ acc, size_t n) {
+  for (size_t i = blockIdx.x * static_cast<size_t>(blockDim.x) + threadIdx.x; i < n;
+       i += static_cast<size_t>(gridDim.x) * blockDim.x)
+    acc[i] = 0.0;
+}
+
+// pred = zmin + (zmax - zmin) * acc / (2pi n_acc) at prediction sites, the input value elsewhere.
+__global__ void predict_kernel(const double* __restrict__ z, const uint8_t* __restrict__ mask, Geom g,
+                               const double* __restrict__ acc, double zmin, double zmax, long long n_acc,
+                               double* __restrict__ pred) {
+  const int y = blockIdx.y;
+  const int x = blockIdx.x * blockDim.x + threadIdx.x;
+  if (x >= g.L) return;
+  const size_t s = static_cast<size_t>(y) * g.L + x;
+  if (!mask[s]) { pred[s] = z[s]; return; }
+  if (n_acc == 0) { pred[s] = __longlong_as_double(0x7ff8000000000000LL); return; }
+  const int col = (x + y) & 1, j = x >> 1;
+  const double a = acc[static_cast<size_t>(col) * g.plane + static_cast<size_t>(y) * g.Wp + j];
+  const double frac = a / (6.283185307179586476925286766559 * static_cast<double>(n_acc));
+  pred[s] = zmin + (zmax - zmin) * frac;
+}
+
+__global__ void philox_debug_kernel(const uint32_t* __restrict__ ctr, uint32_t k0, uint32_t k1,
+                                    uint32_t* __restrict__ out, long long n) {
+  const long long i = blockIdx.x * static_cast<long long>(blockDim.x) + threadIdx.x;
+  if (i >= n) return;
+  const uint4 r = philox4x32_10(ctr[4 * i], ctr[4 * i + 1], ctr[4 * i + 2], ctr[4 * i + 3], k0, k1);
+  out[4 * i] = r.x; out[4 * i + 1] = r.y; out[4 * i + 2] = r.z; out[4 * i + 3] = r.w;
+}
+
+}  // namespace mpr
