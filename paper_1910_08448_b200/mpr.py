@@ -1,0 +1,289 @@
+"""Thin ctypes binding of libmpr.so (include/mpr.h): argument marshalling only.
+
+Every step of the path runs in the CUDA kernels of the library; torch is used for device
+memory and streams.  There is no CPU fallback: importing works without a GPU (so that the
+symbol table can be checked), every compute call needs one and fails loudly otherwise.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libmpr.so")
+
+MPR_OK = 0
+ERR_INVALID_ARG, ERR_NO_MEASURED, ERR_DEGENERATE_RANGE, ERR_NONFINITE = -1, -2, -3, -4
+ERR_WORKSPACE, ERR_NOT_READY, ERR_NO_ROOT, ERR_CUDA = -5, -6, -7, -8
+
+MODES = {"DP": 0, "SP": 1, "SP_PRECISE": 2, "SP_INTRINSIC": 3}
+PATHS = {"TILED": 0, "PLAIN": 1}
+PASS_KINDS = {"MET": 0, "OR": 1, "QUENCH": 2}
+
+# every symbol include/mpr.h declares
+SYMBOLS = [
+    "mpr_workspace_bytes", "mpr_create", "mpr_destroy", "mpr_set_precision", "mpr_set_seed",
+    "mpr_set_temperature", "mpr_set_quench", "mpr_set_path", "mpr_set_fused_sweeps", "mpr_reset_chain",
+    "mpr_estimate_temperature", "mpr_run", "mpr_sweep", "mpr_pass", "mpr_get_state", "mpr_set_state",
+    "mpr_energy", "mpr_sample_energy", "mpr_get_counters", "mpr_get_energy_series", "mpr_get_info",
+    "mpr_get_launch_stats", "mpr_workspace_bytes_host", "mpr_predict_host", "mpr_debug_philox",
+    "mpr_last_error", "mpr_status_string",
+]
+
+_lib = None
+
+
+class MprError(RuntimeError):
+    def __init__(self, code, msg=""):
+        super().__init__("libmpr status %d (%s) %s" % (code, _status_string(code), msg))
+        self.code = code
+
+
+def _status_string(code):
+    try:
+        return lib().mpr_status_string(int(code)).decode()
+    except Exception:
+        return "?"
+
+
+def lib():
+    """Loads libmpr.so (building it first if the sources are newer).  Raises if it is missing."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        from . import build as _build
+        _build.build()
+    L = C.CDLL(LIB_PATH)
+    vp, dp, i64 = C.c_void_p, C.POINTER(C.c_double), C.c_int64
+    u64p, i64p = C.POINTER(C.c_uint64), C.POINTER(C.c_int64)
+    sig = {
+        "mpr_workspace_bytes": (C.c_int, [C.c_int, C.POINTER(C.c_size_t)]),
+        "mpr_create": (C.c_int, [C.POINTER(vp), C.c_int, vp, vp, vp, C.c_size_t, vp]),
+        "mpr_destroy": (None, [vp]),
+        "mpr_set_precision": (C.c_int, [vp, C.c_int]),
+        "mpr_set_seed": (C.c_int, [vp, C.c_uint64]),
+        "mpr_set_temperature": (C.c_int, [vp, C.c_double]),
+        "mpr_set_quench": (C.c_int, [vp, C.c_int]),
+        "mpr_set_path": (C.c_int, [vp, C.c_int]),
+        "mpr_set_fused_sweeps": (C.c_int, [vp, C.c_int]),
+        "mpr_reset_chain": (C.c_int, [vp, C.c_uint32]),
+        "mpr_estimate_temperature": (C.c_int, [vp, dp, dp, C.POINTER(C.c_int)]),
+        "mpr_run": (C.c_int, [vp, C.c_int, C.c_int, vp, dp, dp]),
+        "mpr_sweep": (C.c_int, [vp, C.c_int]),
+        "mpr_pass": (C.c_int, [vp, C.c_int, C.c_int, C.c_uint64]),
+        "mpr_get_state": (C.c_int, [vp, vp]),
+        "mpr_set_state": (C.c_int, [vp, vp]),
+        "mpr_energy": (C.c_int, [vp, dp, dp]),
+        "mpr_sample_energy": (C.c_int, [vp, dp, i64p]),
+        "mpr_get_counters": (C.c_int, [vp, u64p, u64p, u64p]),
+        "mpr_get_energy_series": (i64, [vp, dp, i64]),
+        "mpr_get_info": (C.c_int, [vp, dp, dp, i64p, dp]),
+        "mpr_get_launch_stats": (C.c_int, [vp, u64p]),
+        "mpr_workspace_bytes_host": (C.c_int, [C.c_int, C.POINTER(C.c_size_t)]),
+        "mpr_predict_host": (C.c_int, [C.c_int, vp, vp, C.c_int, C.c_uint64, C.c_double, C.c_int, C.c_int, vp,
+                                       C.c_size_t, vp, vp, dp, dp, dp, u64p]),
+        "mpr_debug_philox": (C.c_int, [vp, C.POINTER(C.c_uint32), vp, i64, vp]),
+        "mpr_last_error": (C.c_char_p, [vp]),
+        "mpr_status_string": (C.c_char_p, [C.c_int]),
+    }
+    for name, (res, args) in sig.items():
+        fn = getattr(L, name)
+        fn.restype, fn.argtypes = res, args
+    _lib = L
+    return L
+
+
+def workspace_bytes(L: int, host: bool = False) -> int:
+    n = C.c_size_t()
+    fn = lib().mpr_workspace_bytes_host if host else lib().mpr_workspace_bytes
+    st = fn(int(L), C.byref(n))
+    if st != MPR_OK:
+        raise MprError(st)
+    return n.value
+
+
+def _torch():
+    import torch
+    if not torch.cuda.is_available():
+        raise RuntimeError("paper_1910_08448_b200 needs a CUDA device: there is no CPU fallback")
+    return torch
+
+
+class Mpr:
+    """One MPR prediction problem on the GPU.  Mirrors the C calls of include/mpr.h by name.
+
+    values: float64 [L, L] (torch CUDA tensor or numpy array; NaN allowed at prediction sites)
+    mask:   uint8   [L, L], 1 = prediction site
+    """
+
+    def __init__(self, values, mask, mode="DP", seed=None, device="cuda:0", stream=None):
+        torch = _torch()
+        self._torch = torch
+        dev = torch.device(device)
+        self.values = torch.as_tensor(values, dtype=torch.float64).to(dev).contiguous()
+        self.mask = torch.as_tensor(mask, dtype=torch.uint8).to(dev).contiguous()
+        self.L = int(self.mask.shape[0])
+        assert self.mask.shape == (self.L, self.L) and self.values.shape == (self.L, self.L)
+        self.device = dev
+        self.ws = torch.empty(workspace_bytes(self.L) + 256, dtype=torch.uint8, device=dev)
+        off = (-self.ws.data_ptr()) % 256
+        self._ws_ptr = self.ws.data_ptr() + off
+        self._stream = stream
+        sptr = stream.cuda_stream if stream is not None else torch.cuda.current_stream(dev).cuda_stream
+        self.h = C.c_void_p()
+        with torch.cuda.device(dev):
+            st = lib().mpr_create(C.byref(self.h), self.L, self.values.data_ptr(), self.mask.data_ptr(),
+                                  self._ws_ptr, self.ws.numel() - off, sptr)
+        if st != MPR_OK:
+            self.h = C.c_void_p()
+            raise MprError(st)
+        if mode != "DP":
+            self.set_precision(mode)
+        if seed is not None:
+            self.set_seed(seed)
+
+    def close(self):
+        if getattr(self, "h", None) and self.h.value:
+            lib().mpr_destroy(self.h)
+            self.h = C.c_void_p()
+
+    __del__ = close
+
+    def _chk(self, st):
+        if st != MPR_OK:
+            raise MprError(st, lib().mpr_last_error(self.h).decode())
+
+    def _call(self, fn, *args):
+        with self._torch.cuda.device(self.device):
+            self._chk(fn(self.h, *args))
+
+    # -- setters -------------------------------------------------------------------------
+    def set_precision(self, mode):
+        self._call(lib().mpr_set_precision, MODES[mode] if isinstance(mode, str) else int(mode))
+
+    def set_seed(self, seed):
+        self._call(lib().mpr_set_seed, int(seed))
+
+    def set_temperature(self, T):
+        self._call(lib().mpr_set_temperature, float(T))
+
+    def set_quench(self, n):
+        self._call(lib().mpr_set_quench, int(n))
+
+    def set_path(self, path):
+        self._call(lib().mpr_set_path, PATHS[path] if isinstance(path, str) else int(path))
+
+    def set_fused_sweeps(self, k):
+        self._call(lib().mpr_set_fused_sweeps, int(k))
+
+    def reset_chain(self, trial=0):
+        self._call(lib().mpr_reset_chain, int(trial))
+
+    # -- the path ------------------------------------------------------------------------
+    def estimate_temperature(self):
+        T, es, nt = C.c_double(), C.c_double(), C.c_int()
+        self._call(lib().mpr_estimate_temperature, C.byref(T), C.byref(es), C.byref(nt))
+        return T.value, es.value, nt.value
+
+    def run(self, n_eq, n_meas, want_pred=True):
+        """Returns (pred CUDA tensor [L, L] or None, e_mean, e_stderr)."""
+        pred = self._torch.empty((self.L, self.L), dtype=self._torch.float64, device=self.device) if want_pred else None
+        m, s = C.c_double(), C.c_double()
+        self._call(lib().mpr_run, int(n_eq), int(n_meas), pred.data_ptr() if want_pred else None,
+                   C.byref(m), C.byref(s))
+        return pred, m.value, s.value
+
+    def sweep(self, n=1):
+        self._call(lib().mpr_sweep, int(n))
+
+    def pass_(self, kind, colour, sweep=0):
+        self._call(lib().mpr_pass, PASS_KINDS[kind] if isinstance(kind, str) else int(kind), int(colour), int(sweep))
+
+    # -- inspection ----------------------------------------------------------------------
+    def get_state(self):
+        phi = self._torch.empty((self.L, self.L), dtype=self._torch.float64, device=self.device)
+        self._call(lib().mpr_get_state, phi.data_ptr())
+        return phi
+
+    def set_state(self, phi):
+        phi = self._torch.as_tensor(phi, dtype=self._torch.float64).to(self.device).contiguous()
+        assert phi.shape == (self.L, self.L)
+        self._call(lib().mpr_set_state, phi.data_ptr())
+        self._torch.cuda.synchronize(self.device)
+
+    def energy(self):
+        H, e = C.c_double(), C.c_double()
+        self._call(lib().mpr_energy, C.byref(H), C.byref(e))
+        return H.value, e.value
+
+    def sample_energy(self):
+        es, n = C.c_double(), C.c_int64()
+        self._call(lib().mpr_sample_energy, C.byref(es), C.byref(n))
+        return es.value, n.value
+
+    def counters(self):
+        a, b, c = C.c_uint64(), C.c_uint64(), C.c_uint64()
+        self._call(lib().mpr_get_counters, C.byref(a), C.byref(b), C.byref(c))
+        return a.value, b.value, c.value
+
+    def series(self):
+        n = lib().mpr_get_energy_series(self.h, None, 0)
+        out = np.empty(max(int(n), 0), dtype=np.float64)
+        if n > 0:
+            lib().mpr_get_energy_series(self.h, out.ctypes.data_as(C.POINTER(C.c_double)), n)
+        return out
+
+    def info(self):
+        a, b, n, T = C.c_double(), C.c_double(), C.c_int64(), C.c_double()
+        self._call(lib().mpr_get_info, C.byref(a), C.byref(b), C.byref(n), C.byref(T))
+        return {"z_min": a.value, "z_max": b.value, "n_free": n.value, "T": T.value}
+
+    def launches(self):
+        n = C.c_uint64()
+        self._call(lib().mpr_get_launch_stats, C.byref(n))
+        return n.value
+
+
+def predict_host(values, mask, mode="DP", seed=0, T=-1.0, n_eq=100, n_meas=100, workspace=None, pred_out=None,
+                 device="cuda:0"):
+    """End-to-end call on HOST arrays (mpr_predict_host): host->device copies, create, (estimate T,)
+    run, device->host copy of the prediction.  Returns (pred numpy [L, L], e_mean, e_stderr, T, launches)."""
+    torch = _torch()
+    values = np.ascontiguousarray(values, dtype=np.float64)
+    mask = np.ascontiguousarray(mask, dtype=np.uint8)
+    L = int(mask.shape[0])
+    dev = torch.device(device)
+    if workspace is None:
+        workspace = torch.empty(workspace_bytes(L, host=True) + 256, dtype=torch.uint8, device=dev)
+    off = (-workspace.data_ptr()) % 256
+    if pred_out is None:
+        pred_out = np.empty((L, L), dtype=np.float64)
+    m, s, Tu, nl = C.c_double(), C.c_double(), C.c_double(), C.c_uint64()
+    with torch.cuda.device(dev):
+        st = lib().mpr_predict_host(L, values.ctypes.data, mask.ctypes.data, MODES[mode], int(seed), float(T),
+                                    int(n_eq), int(n_meas), workspace.data_ptr() + off, workspace.numel() - off,
+                                    torch.cuda.current_stream(dev).cuda_stream, pred_out.ctypes.data,
+                                    C.byref(m), C.byref(s), C.byref(Tu), C.byref(nl))
+    if st != MPR_OK:
+        raise MprError(st)
+    return pred_out, m.value, s.value, Tu.value, nl.value
+
+
+def debug_philox(ctr, key, device="cuda:0"):
+    """Philox4x32-10 as the kernels evaluate it, for n counters: ctr uint32 [n, 4], key (k0, k1)."""
+    torch = _torch()
+    dev = torch.device(device)
+    ctr = np.ascontiguousarray(ctr, dtype=np.uint32).reshape(-1, 4)
+    d_ctr = torch.from_numpy(ctr.view(np.int32)).to(dev)
+    d_out = torch.empty_like(d_ctr)
+    k = (C.c_uint32 * 2)(int(key[0]) & 0xFFFFFFFF, int(key[1]) & 0xFFFFFFFF)
+    with torch.cuda.device(dev):
+        st = lib().mpr_debug_philox(d_ctr.data_ptr(), k, d_out.data_ptr(), ctr.shape[0],
+                                    torch.cuda.current_stream(dev).cuda_stream)
+    if st != MPR_OK:
+        raise MprError(st)
+    torch.cuda.synchronize(dev)
+    return d_out.cpu().numpy().view(np.uint32)

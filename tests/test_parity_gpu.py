@@ -1,0 +1,281 @@
+"""Parity of the CUDA path (through the C ABI, paper_1910_08448_b200.mpr) with the CPU oracle on the
+same seeded inputs.  Gates (BASELINE.json north_star): DP makes identical accept/reject decisions
+and |dphi| <= 1e-9 per site after 10 sweeps; integer counters bit-exact; both kernel paths and
+every fused depth give bit-identical spins; SP modes are judged statistically."""
+import math
+
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+TWO_PI = 2.0 * math.pi
+PHI_TOL = 1e-9      # north_star: per-site |dphi| <= 1e-9 after 10 sweeps (DP)
+
+
+@pytest.fixture(scope="module")
+def mpr():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    from paper_1910_08448_b200 import build, mpr as m
+    build.build()
+    m.lib()
+    return m
+
+
+@pytest.fixture(scope="module")
+def inputs():
+    from paper_1910_08448_b200 import inputs as i
+    return i
+
+
+def phi_diff(a, b):
+    return float(np.max(np.abs(np.asarray(a) - np.asarray(b))))
+
+
+def make(inputs, L, xi, seed, f, lognormal=False):
+    return inputs.make_problem(L, xi, seed, f, lognormal)
+
+
+# --------------------------------------------------------------------------- generator
+def test_device_philox_matches_oracle(mpr, oracle_mod):
+    rng = np.random.default_rng(7)
+    ctr = rng.integers(0, 2 ** 32, (4096, 4), dtype=np.uint64).astype(np.uint32)
+    ctr[0] = 0
+    ctr[1] = 0xFFFFFFFF
+    key = (0x12345678, 0x9ABCDEF0)
+    out = mpr.debug_philox(ctr, key)
+    for i in range(0, 4096, 37):
+        assert list(out[i]) == oracle_mod.philox4x32_10(list(ctr[i]), key), i
+
+
+# --------------------------------------------------------------------------- set-up (R1, R6)
+@pytest.mark.parametrize("L,xi,f", [(64, 8.0, 0.33), (100, 10.0, 0.66), (131, 9.0, 0.9)])
+def test_setup_matches_oracle(mpr, oracle_mod, inputs, L, xi, f):
+    values, mask, _ = make(inputs, L, xi, 5, f)
+    g = mpr.Mpr(values, mask, seed=11)
+    o = oracle_mod.Oracle(values=values, mask=mask, seed=11)
+    info = g.info()
+    assert (info["z_min"], info["z_max"]) == o.zrange()
+    assert info["n_free"] == int(mask.sum())
+    es_g, n_g = g.sample_energy()
+    es_o, n_o = o.sample_energy()
+    assert n_g == n_o
+    assert abs(es_g - es_o) <= 1e-12 * abs(es_o)
+    # R8 initial state: uniform spins + 32 quench double passes
+    assert phi_diff(g.get_state().cpu().numpy(), o.get_state()) <= PHI_TOL
+    H_g, e_g = g.energy()
+    H_o, e_o = o.energy()
+    assert abs(H_g - H_o) <= 1e-11 * abs(H_o)
+    assert abs(e_g - e_o) <= 1e-12 * abs(e_o)
+
+
+def test_error_paths(mpr, inputs):
+    L = 16
+    rng = np.random.default_rng(1)
+    z = rng.normal(50, 10, (L, L))
+    mask = (rng.uniform(size=(L, L)) < 0.5).astype(np.uint8)
+    for vals, msk, code in [
+        (z, np.ones((L, L), dtype=np.uint8), mpr.ERR_NO_MEASURED),
+        (np.full((L, L), 3.0), np.zeros((L, L), dtype=np.uint8), mpr.ERR_DEGENERATE_RANGE),
+        (np.where(mask == 1, 1.0, np.inf), mask, mpr.ERR_NONFINITE),
+    ]:
+        with pytest.raises(mpr.MprError) as ei:
+            mpr.Mpr(vals, msk)
+        assert ei.value.code == code
+    vals = z.copy()
+    vals[mask == 1] = np.nan                     # values at prediction sites are never read
+    g = mpr.Mpr(vals, mask)
+    with pytest.raises(mpr.MprError) as ei:
+        g.run(1, 1)
+    assert ei.value.code == mpr.ERR_NOT_READY
+    with pytest.raises(mpr.MprError) as ei:
+        g.set_temperature(0.0)
+    assert ei.value.code == mpr.ERR_INVALID_ARG
+    with pytest.raises(mpr.MprError):
+        g.set_fused_sweeps(0)
+
+
+# --------------------------------------------------------------------------- DP parity, pass by pass
+@pytest.mark.parametrize("path", ["PLAIN", "TILED"])
+@pytest.mark.parametrize("L,xi,f,T", [(64, 8.0, 0.33, 0.07), (97, 8.0, 0.9, 0.02), (250, 16.0, 0.66, 0.3)])
+def test_dp_ten_sweeps_match_oracle(mpr, oracle_mod, inputs, L, xi, f, T, path):
+    values, mask, _ = make(inputs, L, xi, 3, f)
+    g = mpr.Mpr(values, mask, seed=1000)
+    o = oracle_mod.Oracle(values=values, mask=mask, seed=1000)
+    g.set_temperature(T)
+    o.set_temperature(T)
+    g.set_path(path)
+    g.sweep(10)
+    o.hybrid_sweeps(10)
+    sg, so = g.get_state().cpu().numpy(), o.get_state()
+    assert phi_diff(sg, so) <= PHI_TOL
+    acc_g, att_g, sw_g = g.counters()
+    acc_o, att_o, sw_o = o.counters()
+    assert (acc_g, att_g, sw_g) == (acc_o, att_o, sw_o)      # identical accept/reject decisions
+    assert sg.min() >= 0.0 and sg.max() <= TWO_PI + 1e-15
+    # measured spins never move
+    m0 = mask == 0
+    assert np.array_equal(sg[m0], g.get_state().cpu().numpy()[m0])
+    assert phi_diff(sg[m0], so[m0]) <= 1e-12
+
+
+def test_dp_single_passes_match_oracle(mpr, oracle_mod, inputs):
+    """Each kind of colour pass alone, including edge and corner sites (open boundaries, R2)."""
+    L = 33
+    values, mask, _ = make(inputs, L, 5.0, 9, 0.8)
+    g = mpr.Mpr(values, mask, seed=5)
+    o = oracle_mod.Oracle(values=values, mask=mask, seed=5)
+    g.set_quench(0)
+    o.set_quench(0)
+    g.set_temperature(0.5)
+    o.set_temperature(0.5)
+    assert phi_diff(g.get_state().cpu().numpy(), o.get_state()) <= 1e-12      # uniform init (R8)
+    for step, (kind, c) in enumerate([("MET", 0), ("MET", 1), ("OR", 0), ("OR", 1), ("QUENCH", 1), ("QUENCH", 0),
+                                      ("MET", 1), ("OR", 0)]):
+        g.pass_(kind, c, sweep=step + 1)
+        if kind == "MET":
+            o.met_pass(c, step + 1)
+        elif kind == "OR":
+            o.or_pass(c)
+        else:
+            o.quench_pass(c)
+        assert phi_diff(g.get_state().cpu().numpy(), o.get_state()) <= PHI_TOL, (step, kind, c)
+    assert g.counters()[0] == o.counters()[0]
+
+
+@pytest.mark.parametrize("L", [2, 3, 5, 16])
+def test_tiny_grids(mpr, oracle_mod, L):
+    rng = np.random.default_rng(L)
+    z = rng.normal(50, 10, (L, L))
+    mask = np.zeros((L, L), dtype=np.uint8)
+    mask.flat[rng.choice(L * L, size=max(1, L * L // 2), replace=False)] = 1
+    mask[0, 0] = 0
+    mask[-1, -1] = 0
+    g = mpr.Mpr(z, mask, seed=3)
+    o = oracle_mod.Oracle(values=z, mask=mask, seed=3)
+    for path in ("PLAIN", "TILED"):
+        g.set_path(path)
+        g.set_seed(3)
+        o.set_seed(3)
+        g.set_temperature(0.2)
+        o.set_temperature(0.2)
+        g.sweep(10)
+        o.hybrid_sweeps(10)
+        assert phi_diff(g.get_state().cpu().numpy(), o.get_state()) <= PHI_TOL
+        assert g.counters() == o.counters()
+
+
+# --------------------------------------------------------------------------- whole run (R15, R3)
+def test_dp_run_matches_oracle_config1(mpr, oracle_mod, inputs):
+    """BASELINE.json configs[0]: L = 64, 33 % masked, 100 + 100 sweeps, DP."""
+    c, values, mask, truth = inputs.make_config(1)
+    g = mpr.Mpr(values, mask, seed=c.mpr_seed)
+    o = oracle_mod.Oracle(values=values, mask=mask, seed=c.mpr_seed)
+    g.set_temperature(0.07)
+    o.set_temperature(0.07)
+    pred_g, e_g, se_g = g.run(c.n_eq, c.n_meas)
+    pred_o, e_o, se_o = o.run(c.n_eq, c.n_meas)
+    pred_g = pred_g.cpu().numpy()
+    m1 = mask == 1
+    assert np.array_equal(pred_g[~m1], values[~m1])                 # measured sites bit-exact
+    zmin, zmax = o.zrange()
+    assert np.max(np.abs(pred_g[m1] - pred_o[m1])) <= 1e-8 * (zmax - zmin)
+    assert abs(e_g - e_o) <= 1e-11 and abs(se_g - se_o) <= 1e-11
+    np.testing.assert_allclose(g.series(), o.series(), rtol=0, atol=1e-11)
+    assert g.counters() == o.counters()
+    mae_g, rmse_g = inputs.prediction_errors(pred_g, truth, mask)
+    mae_o, rmse_o = inputs.prediction_errors(pred_o, truth, mask)
+    assert abs(mae_g - mae_o) <= 1e-8 and abs(rmse_g - rmse_o) <= 1e-8
+    # chain continuation: a second run averages over all 200 measurement sweeps
+    pred_g2, _, _ = g.run(0, c.n_meas)
+    pred_o2, _, _ = o.run(0, c.n_meas)
+    assert np.max(np.abs(pred_g2.cpu().numpy()[m1] - pred_o2[m1])) <= 1e-8 * (zmax - zmin)
+
+
+def test_temperature_estimate_matches_oracle(mpr, oracle_mod, inputs):
+    c, values, mask, _ = inputs.make_config(1)
+    g = mpr.Mpr(values, mask, seed=c.mpr_seed)
+    o = oracle_mod.Oracle(values=values, mask=mask, seed=c.mpr_seed)
+    T_g, es_g, n_g = g.estimate_temperature()
+    T_o, es_o, n_o = o.estimate_temperature()
+    assert abs(es_g - es_o) <= 1e-12
+    assert n_g == n_o
+    assert abs(T_g - T_o) <= 1e-9 * T_o
+    # the chain was reset (trial 0) with T set: the next sweeps agree as well
+    g.sweep(3)
+    o.hybrid_sweeps(3)
+    assert phi_diff(g.get_state().cpu().numpy(), o.get_state()) <= PHI_TOL
+
+
+def test_no_root_is_reported(mpr):
+    L = 12
+    z = np.where(np.arange(L)[None, :] < 6, 10.0, 20.0) * np.ones((L, 1))
+    rng = np.random.default_rng(0)
+    mask = np.zeros((L, L), dtype=np.uint8)
+    mask[:, 5:7] = 1
+    mask[rng.integers(0, L, 20), rng.integers(0, 4, 20)] = 1
+    g = mpr.Mpr(z, mask, seed=2)
+    assert g.sample_energy()[0] == -2.0
+    with pytest.raises(mpr.MprError) as ei:
+        g.estimate_temperature()
+    assert ei.value.code == mpr.ERR_NO_ROOT
+
+
+# --------------------------------------------------------------------------- determinism contract
+@pytest.mark.parametrize("mode", ["DP", "SP", "SP_PRECISE", "SP_INTRINSIC"])
+def test_paths_and_fused_depths_are_bit_identical(mpr, inputs, mode):
+    L = 300                                  # several tiles in x and y, ragged in both
+    values, mask, _ = make(inputs, L, 12.0, 4, 0.66)
+    g = mpr.Mpr(values, mask, mode=mode, seed=77)
+    g.set_temperature(0.05)
+    ref = None
+    for path, k in [("PLAIN", 1), ("TILED", 1), ("TILED", 2), ("TILED", 3), ("TILED", 4)]:
+        g.set_path(path)
+        g.set_fused_sweeps(k)
+        g.reset_chain(0)
+        g.sweep(9)                            # 9 is not a multiple of 2 or 4: ragged last launch
+        st = g.get_state().cpu().numpy()
+        cnt = g.counters()
+        if ref is None:
+            ref = (st, cnt)
+        else:
+            assert np.array_equal(st, ref[0]), (path, k)
+            assert cnt == ref[1], (path, k)
+    # measurement launches: energies and accumulators agree between the paths
+    out = []
+    for path in ("PLAIN", "TILED"):
+        g.set_path(path)
+        g.reset_chain(0)
+        pred, e, se = g.run(5, 7)
+        out.append((pred.cpu().numpy(), g.series()))
+    assert np.array_equal(out[0][0], out[1][0])
+    np.testing.assert_allclose(out[0][1], out[1][1], rtol=0, atol=1e-13)
+
+
+# --------------------------------------------------------------------------- SP modes: statistics
+def test_sp_modes_statistics_config2_shape(mpr, oracle_mod, inputs):
+    """e within 3 standard errors of the DP value; MAE / RMSE within 1 % of the DP oracle's."""
+    L = 256
+    values, mask, truth = make(inputs, L, 16.0, 1, 0.66)
+    T = 0.03
+    o = oracle_mod.Oracle(values=values, mask=mask, seed=1001, threads=oracle_mod.threads_available())
+    o.set_temperature(T)
+    pred_o, e_o, se_o = o.run(300, 200)
+    mae_o, rmse_o = inputs.prediction_errors(pred_o, truth, mask)
+    for mode in ("DP", "SP", "SP_PRECISE", "SP_INTRINSIC"):
+        es, maes = [], []
+        for seed in (1001, 2002, 3003, 4004):
+            g = mpr.Mpr(values, mask, mode=mode, seed=seed)
+            g.set_temperature(T)
+            pred, e, se = g.run(300, 200)
+            es.append(e)
+            mae, rmse = inputs.prediction_errors(pred.cpu().numpy(), truth, mask)
+            maes.append((mae, rmse))
+        e_mean = float(np.mean(es))
+        e_se = float(np.std(es, ddof=1) / math.sqrt(len(es)))
+        assert abs(e_mean - e_o) <= 3.0 * math.hypot(e_se, se_o) + 1e-6, (mode, e_mean, e_o, e_se, se_o)
+        mae = float(np.mean([m for m, _ in maes]))
+        rmse = float(np.mean([r for _, r in maes]))
+        assert abs(mae / mae_o - 1.0) <= 0.01, (mode, mae, mae_o)
+        assert abs(rmse / rmse_o - 1.0) <= 0.01, (mode, rmse, rmse_o)
