@@ -47,6 +47,8 @@ def parse():
     ap.add_argument("--n-eq", type=int, default=None)
     ap.add_argument("--n-meas", type=int, default=None)
     ap.add_argument("--fused", type=int, default=1)
+    ap.add_argument("--temperature", type=float, default=None,
+                    help="profiling only: fix T and skip the temperature estimate (not the benchmark step)")
     ap.add_argument("--skip-cpu-baseline", action="store_true")
     ap.add_argument("--skip-modes", action="store_true")
     ap.add_argument("--skip-e2e", action="store_true")
@@ -180,7 +182,11 @@ def run_ours(args, rank, world, local_rank):
     def step():
         g = mpr.Mpr(d_values, d_mask, mode=mode, seed=seed, device=dev)
         g.set_fused_sweeps(args.fused)
-        T, es, nt = g.estimate_temperature()
+        if args.temperature is not None:
+            g.set_temperature(args.temperature)
+            T, es, nt = args.temperature, None, 0
+        else:
+            T, es, nt = g.estimate_temperature()
         pred, e, se = g.run(n_eq, n_meas)
         state["launches"] += g.launches()
         sw = nt * 250 + n_eq + n_meas
@@ -283,7 +289,8 @@ def run_ours(args, rank, world, local_rank):
         sweeps_e2e = 0
 
         def e2e_step():
-            _, e, se, T, nl = mpr.predict_host(h_values.numpy(), h_mask.numpy(), mode=mode, seed=seed, T=-1.0,
+            _, e, se, T, nl = mpr.predict_host(h_values.numpy(), h_mask.numpy(), mode=mode, seed=seed,
+                                               T=-1.0 if args.temperature is None else args.temperature,
                                                n_eq=n_eq, n_meas=n_meas, workspace=ws, pred_out=h_pred.numpy(),
                                                device=dev)
             return nl
