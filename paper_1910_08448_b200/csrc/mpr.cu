@@ -131,6 +131,8 @@ ChainConst<R> chain_const(const mpr_ctx* c) {
   const double T = c->T > 0.0 ? c->T : 1.0;
   k.delta = static_cast<R>(proposal_width(T));
   k.inv_T = static_cast<R>(1.0 / T);
+  k.hscale = static_cast<R>(0.25 * proposal_width(T) / 2147483648.0);
+  k.xscale = static_cast<R>(-1.4426950408889634074 / T);
   k.k0 = static_cast<uint32_t>(c->seed);
   k.k1 = static_cast<uint32_t>(c->seed >> 32);
   k.trial = c->trial;

@@ -37,8 +37,10 @@ __device__ __forceinline__ uint4 philox4x32_10(uint32_t c0, uint32_t c1, uint32_
   constexpr uint32_t M0 = 0xD2511F53u, M1 = 0xCD9E8D57u, W0 = 0x9E3779B9u, W1 = 0xBB67AE85u;
 #pragma unroll
   for (int r = 0; r < 10; ++r) {
-    const uint32_t hi0 = __umulhi(M0, c0), lo0 = M0 * c0;
-    const uint32_t hi1 = __umulhi(M1, c2), lo1 = M1 * c2;
+    const uint64_t p0 = static_cast<uint64_t>(M0) * c0;   // one IMAD.WIDE.U32 gives hi and lo
+    const uint64_t p1 = static_cast<uint64_t>(M1) * c2;
+    const uint32_t hi0 = static_cast<uint32_t>(p0 >> 32), lo0 = static_cast<uint32_t>(p0);
+    const uint32_t hi1 = static_cast<uint32_t>(p1 >> 32), lo1 = static_cast<uint32_t>(p1);
     const uint32_t n0 = hi1 ^ c1 ^ k0;
     const uint32_t n2 = hi0 ^ c3 ^ k1;
     c0 = n0; c1 = lo1; c2 = n2; c3 = lo0;
@@ -53,10 +55,12 @@ __device__ __forceinline__ double u53(uint32_t a, uint32_t b) {
   const double lo = static_cast<double>(b >> 6);
   return (hi * 67108864.0 + lo) * (1.0 / 9007199254740992.0);
 }
-// 24-bit uniform in (0,1), bin centres (float modes; judged statistically).
-__device__ __forceinline__ float u24(uint32_t a) {
-  return (static_cast<float>(a >> 8) + 0.5f) * (1.0f / 16777216.0f);
-}
+// Float modes (R9, judged statistically): the proposal offset is the word read as a signed integer,
+// converted with round-to-nearest (24-bit mantissa) -- a symmetric uniform on [-2^31, 2^31] whose
+// scale 2^-31 is folded into ChainConst::hscale; the acceptance uniform is the word converted as
+// an unsigned integer, u2 = float(w) 2^-32 in [0, 1].  One conversion instruction each.
+__device__ __forceinline__ float sym_word(uint32_t a) { return static_cast<float>(static_cast<int32_t>(a)); }
+__device__ __forceinline__ float pos_word(uint32_t a) { return static_cast<float>(a); }
 
 // ---- function-precision policies (X_F) -----------------------------------
 template <int MODE> struct Fn;
@@ -80,6 +84,12 @@ template <> struct Fn<MODE_SP_INTRINSIC> {
     *s = __sinf(x); *c = __cosf(x);
   }
   static __device__ __forceinline__ float exp_(float x) { return __expf(x); }
+  // the MUFU.EX2 that __expf(x) = ex2(x log2 e) ends in, with the scale folded by the caller
+  static __device__ __forceinline__ float ex2_(float x) {
+    float y;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+  }
   static __device__ __forceinline__ float div_(float a, float b) { return __fdividef(a, b); }
   static __device__ __forceinline__ float rsqrt_(float x) { return rsqrtf(x); }
   static __device__ __forceinline__ float atan2_(float y, float x) { return atan2f(y, x); }
@@ -92,6 +102,8 @@ __device__ __forceinline__ float fma_(float a, float b, float c) { return fmaf(a
 template <typename R> struct ChainConst {
   R delta;     // R7 proposal half-width min(pi, 4 sqrt(T/(4 J q^2)))
   R inv_T;     // 1/T
+  R hscale;    // float modes: q Delta / 2 = hscale * float(int32 word) = (delta / 4) 2^-31 word
+  R xscale;    // SP_INTRINSIC: -log2(e) / T, so that exp(-dE / T) 2^32 = ex2(dE * xscale + 32)
   uint32_t k0, k1, trial;
 };
 
@@ -108,55 +120,89 @@ __device__ __forceinline__ void local_field(R lc, R ls, R rc, R rs, R uc, R us, 
   *A = a; *B = b;
 }
 
-// Metropolis move of one free site (R7, R10).  Returns true when accepted.
+// Random words of the Metropolis move at a site (R9).  Double-arithmetic modes (DP, SP): one
+// Philox block per site, counter word 0 = the site's row-major index; all four words are used
+// (two 53-bit uniforms), exactly as in the oracle.  Float-arithmetic modes: one block per PAIR of
+// sites of the same colour and row whose plane columns are (2m, 2m + 1); counter word 0 = the index
+// of the first site of the pair (pair_site); that site takes words (0, 2), the other one (1, 3).
+struct MetWords { uint32_t p, q, a, b; };   // proposal (p [, q]) and acceptance (a [, b]) words
+
+template <int MODE>
+__device__ __forceinline__ void met_words_pair(uint32_t pair_site, uint32_t sweep,
+                                               const ChainConst<typename Traits<MODE>::real>& k,
+                                               MetWords* w0, MetWords* w1) {
+  if constexpr (sizeof(typename Traits<MODE>::real) == 8) {
+    const uint4 r0 = philox4x32_10(pair_site, sweep, PASS_MET, k.trial, k.k0, k.k1);
+    const uint4 r1 = philox4x32_10(pair_site + 2u, sweep, PASS_MET, k.trial, k.k0, k.k1);
+    *w0 = MetWords{r0.x, r0.y, r0.z, r0.w};
+    *w1 = MetWords{r1.x, r1.y, r1.z, r1.w};
+  } else {
+    const uint4 r = philox4x32_10(pair_site, sweep, PASS_MET, k.trial, k.k0, k.k1);
+    *w0 = MetWords{r.x, 0u, r.z, 0u};
+    *w1 = MetWords{r.y, 0u, r.w, 0u};
+  }
+}
+
+// Metropolis move of one site (R7, R10), written without branches: the new spin is kept iff the
+// site is free, the proposal stays in range (s' >= 0) and the acceptance test passes.  Returns
+// true when the move was accepted.
 template <int MODE>
 __device__ __forceinline__ bool met_update(typename Traits<MODE>::real* c, typename Traits<MODE>::real* s,
                                            typename Traits<MODE>::real A, typename Traits<MODE>::real B,
-                                           uint32_t site, uint32_t sweep,
+                                           const MetWords& w, bool is_free,
                                            const ChainConst<typename Traits<MODE>::real>& k) {
   using R = typename Traits<MODE>::real;
-  const uint4 r = philox4x32_10(site, sweep, PASS_MET, k.trial, k.k0, k.k1);
-  R t, u2;
+  R h;                                           // q Delta / 2
   if constexpr (sizeof(R) == 8) {
-    t = fma_(R(2), R(u53(r.x, r.y)), R(-1));     // 2 u1 - 1 (exact)
-    u2 = R(u53(r.z, r.w));
+    const R t = fma_(R(2), R(u53(w.p, w.q)), R(-1));   // 2 u1 - 1 (exact)
+    h = R(0.25) * (k.delta * t);
   } else {
-    t = fma_(R(2), R(u24(r.x)), R(-1));
-    u2 = R(u24(r.z));
+    h = k.hscale * sym_word(w.p);
   }
-  const R h = R(0.25) * (k.delta * t);           // q Delta / 2
   R sd, cd;
   Fn<MODE>::sincos_(h, &sd, &cd);
-  const R s2 = R(2) * (sd * cd);                 // sin(q Delta)
-  const R c2m1 = R(-2) * (sd * sd);              // cos(q Delta) - 1
+  const R ts = sd + sd;
+  const R s2 = ts * cd;                          // sin(q Delta)
+  const R c2m1 = -(ts * sd);                     // cos(q Delta) - 1
   const R c0 = *c, s0 = *s;
-  const R cn = fma_(c0, c2m1, c0) - s0 * s2;     // c cos - s sin
-  const R sn = fma_(s0, c2m1, s0) + c0 * s2;     // s cos + c sin
+  const R cn = fma_(-s0, s2, fma_(c0, c2m1, c0));   // c cos - s sin
+  const R sn = fma_(c0, s2, fma_(s0, c2m1, s0));    // s cos + c sin
   const R P = fma_(c0, A, s0 * B);               // u.F
   const R Q = fma_(c0, B, -(s0 * A));            // c B - s A
-  const R dE = (R(2) * sd) * fma_(sd, P, -(cd * Q));
-  const bool ok = (sn >= R(0)) && (u2 < Fn<MODE>::exp_(-(dE * k.inv_T)));
-  if (ok) { *c = cn; *s = sn; }
+  const R dE = ts * fma_(sd, P, -(cd * Q));
+  bool acc;
+  if constexpr (sizeof(R) == 8) {
+    acc = R(u53(w.a, w.b)) < Fn<MODE>::exp_(-(dE * k.inv_T));
+  } else if constexpr (MODE == MODE_SP_INTRINSIC) {
+    acc = pos_word(w.a) < Fn<MODE>::ex2_(fma_(dE, k.xscale, R(32)));   // = __expf(-dE/T) 2^32: one FFMA + MUFU.EX2
+  } else {
+    acc = pos_word(w.a) * R(2.3283064365386963e-10) < Fn<MODE>::exp_(-(dE * k.inv_T));
+  }
+  const bool ok = is_free && (sn >= R(0)) && acc;
+  *c = ok ? cn : c0;
+  *s = ok ? sn : s0;
   return ok;
 }
 
-// Over-relaxation move (R5): reflect u about the local field; keep it iff it stays on the
-// upper half circle.  One Newton step towards |u| = 1 stops the rounding drift of the norm.
+// Over-relaxation move (R5): reflect u about the local field; keep it iff the site is free, F != 0
+// and u' stays on the upper half circle.  One Newton step towards |u| = 1 stops the rounding
+// drift of the norm.  Branch-free.
 template <int MODE>
 __device__ __forceinline__ void or_update(typename Traits<MODE>::real* c, typename Traits<MODE>::real* s,
-                                          typename Traits<MODE>::real A, typename Traits<MODE>::real B) {
+                                          typename Traits<MODE>::real A, typename Traits<MODE>::real B,
+                                          bool is_free) {
   using R = typename Traits<MODE>::real;
   const R R2 = fma_(A, A, B * B);
-  if (R2 == R(0)) return;
   const R c0 = *c, s0 = *s;
   const R P = fma_(c0, A, s0 * B);
-  const R t = Fn<MODE>::div_(R(2) * P, R2);
+  const R t = Fn<MODE>::div_(P + P, R2);
   R cn = fma_(t, A, -c0);
   R sn = fma_(t, B, -s0);
-  if (!(sn >= R(0))) return;
+  const bool ok = is_free && (R2 != R(0)) && (sn >= R(0));
   const R f = fma_(R(-0.5), fma_(cn, cn, sn * sn), R(1.5));
   cn = cn * f; sn = sn * f;
-  *c = cn; *s = sn;
+  *c = ok ? cn : c0;
+  *s = ok ? sn : s0;
 }
 
 // Quench move (R8): the minimiser of the local energy, u = F/|F|.

@@ -156,7 +156,7 @@ __global__ void init_chain_kernel(const double* __restrict__ z, const uint8_t* _
   if (j >= g.Wp) return;
   const int x = 2 * j + x_parity(y, col);
   V v;
-  v.x = 1; v.y = 0;
+  v.x = 0; v.y = 0;   // columns past the grid hold the zero vector: they add nothing to a local field
   if (x < g.L) {
     const size_t s = static_cast<size_t>(y) * g.L + x;
     double phi;
@@ -233,9 +233,14 @@ plain_pass_kernel(typename Traits<MODE>::vec* __restrict__ state, const uint32_t
     const V me = own[j];
     R c = R(me.x), s = R(me.y);
     if constexpr (KIND == KIND_MET) {
-      accepted = met_update<MODE>(&c, &s, A, B, static_cast<uint32_t>(y) * static_cast<uint32_t>(g.L) + x, sweep, k);
+      // R9: the pair (2m, 2m + 1) of plane columns shares one Philox block in the float modes
+      const uint32_t pair_site = static_cast<uint32_t>(y) * static_cast<uint32_t>(g.L) +
+                                 static_cast<uint32_t>(2 * (j & ~1) + par);
+      MetWords w0, w1;
+      met_words_pair<MODE>(pair_site, sweep, k, &w0, &w1);
+      accepted = met_update<MODE>(&c, &s, A, B, (j & 1) ? w1 : w0, true, k);
     } else if constexpr (KIND == KIND_OR) {
-      or_update<MODE>(&c, &s, A, B);
+      or_update<MODE>(&c, &s, A, B, true);
     } else {
       quench_update<MODE>(&c, &s, A, B);
     }

@@ -7,8 +7,19 @@
 // by both tiles with the same Philox counters (logical site index) and the same instruction
 // sequence, so the result is bit-identical to the PLAIN path for every k.
 //
-// Staged region: TH rows x 64 plane columns (= 128 sites wide) x 2 planes, dense [plane][row][col],
-// so a warp reads 32 consecutive vec's of one row: conflict-free shared-memory wavefronts.
+// Staged region: TH rows x 64 plane columns (= 128 sites wide) x 2 planes, dense [plane][row][col].
+// Work item = one row of one colour: a warp covers its 64 columns, every thread a PAIR of adjacent
+// columns (2 lane, 2 lane + 1), read and written as one 16-byte (float modes) or two 16-byte (DP)
+// shared-memory accesses.  Warp w owns the rows w, w + NW, w + 2 NW, ... for the whole launch, so
+//  * the x-parity of its rows in a colour pass is a per-warp constant (NW is even): the left/right
+//    neighbour selection is compiled in (template PAR), no per-site selects;
+//  * the mask bits of a thread's sites (RPW rows x 2 colours x 2 sites) are read once from the
+//    global bitmaps into one 64-bit register -- no mask staging in shared memory;
+//  * all grid-boundary handling is done by zero vectors: TMA zero-fills what lies outside the
+//    tensor and the plane columns past the grid hold (0, 0), so a missing neighbour adds nothing to
+//    the local field (same sum, same order as the PLAIN path's selects: bit-identical).
+// Moves are branch-free (mpr_device.cuh); every lane computes, a site keeps its new spin iff it is
+// free and the move is accepted.
 #pragma once
 #include <cuda.h>
 #include "mpr_device.cuh"
@@ -90,8 +101,88 @@ __device__ __forceinline__ void tma_load_3d(void* dst, const CUtensorMap* map, u
 
 template <int MODE> constexpr size_t tile_smem_bytes() {
   return sizeof(typename Traits<MODE>::vec) * 2 * TileCfg<MODE>::TH * kTileCols   // spins
-         + sizeof(uint32_t) * 2 * TileCfg<MODE>::TH * 2                             // mask words
-         + 64;                                                                      // mbarrier + reduction scratch pad
+         + 64;                                                                      // mbarrier
+}
+
+// Two adjacent plane columns of one row: one 128-bit access in the float-storage modes, two in DP.
+template <typename V> struct alignas(2 * sizeof(V)) Pair { V a, b; };
+
+template <int MODE> struct TileView {
+  using V = typename Traits<MODE>::vec;
+  static constexpr int TH = TileCfg<MODE>::TH;
+  V* base;   // [2][TH][kTileCols]
+  __device__ __forceinline__ V* at(int pl, int r, int j) const { return base + (pl * TH + r) * kTileCols + j; }
+  __device__ __forceinline__ Pair<V> pair(int pl, int r, int j) const {
+    return *reinterpret_cast<const Pair<V>*>(at(pl, r, j));
+  }
+};
+
+// Local fields of the two sites (columns jj, jj + 1) of a pair in row r of colour `col`.
+// PAR = x-parity of the row for this colour: the left/right neighbours of column j are the
+// other plane's columns (j - 1 + PAR, j + PAR).  jx = clamped column of the one neighbour that
+// lies outside the aligned pair (jj - 1 for PAR = 0, jj + 2 for PAR = 1).  Sum order l, r, u, d.
+template <int MODE, int PAR>
+__device__ __forceinline__ void pair_fields(const TileView<MODE>& t, int col, int r, int jj, int jx,
+                                            typename Traits<MODE>::real* Aa, typename Traits<MODE>::real* Ba,
+                                            typename Traits<MODE>::real* Ab, typename Traits<MODE>::real* Bb) {
+  using R = typename Traits<MODE>::real;
+  using V = typename Traits<MODE>::vec;
+  const Pair<V> mid = t.pair(1 - col, r, jj);
+  const Pair<V> up = t.pair(1 - col, r - 1, jj);
+  const Pair<V> dn = t.pair(1 - col, r + 1, jj);
+  const V ex = *t.at(1 - col, r, jx);
+  R aa, ba, ab, bb;
+  if constexpr (PAR == 0) {         // a: l = ex, r = mid.a     b: l = mid.a, r = mid.b
+    aa = R(ex.x) + R(mid.a.x);    ba = R(ex.y) + R(mid.a.y);
+    ab = R(mid.a.x) + R(mid.b.x); bb = R(mid.a.y) + R(mid.b.y);
+  } else {                          // a: l = mid.a, r = mid.b  b: l = mid.b, r = ex
+    aa = R(mid.a.x) + R(mid.b.x); ba = R(mid.a.y) + R(mid.b.y);
+    ab = R(mid.b.x) + R(ex.x);    bb = R(mid.b.y) + R(ex.y);
+  }
+  aa = aa + R(up.a.x); ba = ba + R(up.a.y); ab = ab + R(up.b.x); bb = bb + R(up.b.y);
+  aa = aa + R(dn.a.x); ba = ba + R(dn.a.y); ab = ab + R(dn.b.x); bb = bb + R(dn.b.y);
+  *Aa = aa; *Ba = ba; *Ab = ab; *Bb = bb;
+}
+
+// One colour pass (p-th pass of the launch, 1-based) over the rows of this warp.  Returns the
+// number of accepted Metropolis moves at sites this CTA owns (its interior).
+template <int MODE, int KIND, int PAR>
+__device__ __forceinline__ int pass_rows(const TileView<MODE>& t, int col, int p, int h, uint64_t mbits,
+                                         bool col_interior, uint32_t site_row0, uint32_t L, uint32_t sweep,
+                                         const ChainConst<typename Traits<MODE>::real>& kc) {
+  using R = typename Traits<MODE>::real;
+  using V = typename Traits<MODE>::vec;
+  constexpr int TH = TileCfg<MODE>::TH, NW = TileCfg<MODE>::NT / 32, RPW = TH / NW;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int jj = 2 * lane;
+  const int jx = PAR ? (jj + 2 > kTileCols - 1 ? kTileCols - 1 : jj + 2) : (jj - 1 < 0 ? 0 : jj - 1);
+  int n_acc = 0;
+#pragma unroll 1
+  for (int i = 0; i < RPW; ++i) {
+    const int r = warp + NW * i;
+    if (r < p || r >= TH - p) continue;            // stale rim of the staged region (warp-uniform)
+    const uint32_t mm = static_cast<uint32_t>(mbits >> (4 * i + 2 * col));
+    const bool fa = mm & 1u, fb = mm & 2u;
+    R Aa, Ba, Ab, Bb;
+    pair_fields<MODE, PAR>(t, col, r, jj, jx, &Aa, &Ba, &Ab, &Bb);
+    const Pair<V> me = t.pair(col, r, jj);
+    R ca = R(me.a.x), sa = R(me.a.y), cb = R(me.b.x), sb = R(me.b.y);
+    if constexpr (KIND == KIND_MET) {
+      MetWords w0, w1;
+      met_words_pair<MODE>(site_row0 + static_cast<uint32_t>(r) * L + static_cast<uint32_t>(PAR), sweep, kc, &w0, &w1);
+      const bool oka = met_update<MODE>(&ca, &sa, Aa, Ba, w0, fa, kc);
+      const bool okb = met_update<MODE>(&cb, &sb, Ab, Bb, w1, fb, kc);
+      if (col_interior && r >= h && r < TH - h) n_acc += static_cast<int>(oka) + static_cast<int>(okb);
+    } else {
+      or_update<MODE>(&ca, &sa, Aa, Ba, fa);
+      or_update<MODE>(&cb, &sb, Ab, Bb, fb);
+    }
+    Pair<V> out;
+    out.a.x = static_cast<decltype(out.a.x)>(ca); out.a.y = static_cast<decltype(out.a.y)>(sa);
+    out.b.x = static_cast<decltype(out.b.x)>(cb); out.b.y = static_cast<decltype(out.b.y)>(sb);
+    *reinterpret_cast<Pair<V>*>(t.at(col, r, jj)) = out;
+  }
+  return n_acc;
 }
 
 template <int MODE, bool MEASURE>
@@ -102,40 +193,48 @@ tiled_sweep_kernel(const __grid_constant__ CUtensorMap tmap, typename Traits<MOD
                    ChainConst<typename Traits<MODE>::real> kc, uint32_t first_sweep, int nsweeps, int tiles_x) {
   using R = typename Traits<MODE>::real;
   using V = typename Traits<MODE>::vec;
-  constexpr int TH = TileCfg<MODE>::TH, NT = TileCfg<MODE>::NT, NW = NT / 32;
+  constexpr int TH = TileCfg<MODE>::TH, NT = TileCfg<MODE>::NT, NW = NT / 32, RPW = TH / NW;
+  static_assert(TH % NW == 0 && NW % 2 == 0 && RPW * 4 <= 64, "row ownership / mask register layout");
   extern __shared__ __align__(128) unsigned char smem_raw[];
-  V (*tile)[TH][kTileCols] = reinterpret_cast<V (*)[TH][kTileCols]>(smem_raw);
-  uint32_t (*mb)[TH][2] = reinterpret_cast<uint32_t (*)[TH][2]>(smem_raw + sizeof(V) * 2 * TH * kTileCols);
-  uint64_t* bar = reinterpret_cast<uint64_t*>(smem_raw + sizeof(V) * 2 * TH * kTileCols + sizeof(uint32_t) * 2 * TH * 2);
+  TileView<MODE> t{reinterpret_cast<V*>(smem_raw)};
+  uint64_t* bar = reinterpret_cast<uint64_t*>(smem_raw + sizeof(V) * 2 * TH * kTileCols);
   __shared__ double red[32];
 
   const int h = 4 * nsweeps, hc = 2 * nsweeps;
   const int IC = kTileCols - 2 * hc, IR = TH - 2 * h;
   const int tx = blockIdx.x % tiles_x, ty = blockIdx.x / tiles_x;
-  const int j0 = tx * IC - hc, y0 = ty * IR - h;
+  const int j0 = tx * IC - hc, y0 = ty * IR - h;    // j0 is even: pairs are aligned in the global planes too
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int jj = 2 * lane;
 
   if (threadIdx.x == 0) {
     mbar_init(bar, 1);
     mbar_expect_tx(bar, static_cast<uint32_t>(sizeof(V) * 2 * TH * kTileCols));
-    tma_load_3d(&tile[0][0][0], &tmap, bar, 2 * j0, y0, 0);
+    tma_load_3d(t.base, &tmap, bar, 2 * j0, y0, 0);
   }
-  // mask words of the staged region, re-aligned to the tile's first column
-  for (int i = threadIdx.x; i < 2 * TH * 2; i += NT) {
-    const int w = i & 1, r = (i >> 1) % TH, p = (i >> 1) / TH;
-    const int y = y0 + r;
-    uint32_t word = 0;
-    if (y >= 0 && y < g.L) {
-      const uint32_t* row = bits + (static_cast<size_t>(p) * g.L + y) * g.Wm;
-      const int jb = j0 + 32 * w;
-      const int wi = jb >> 5, sh = jb & 31;   // arithmetic shift: floor for negative jb
-      const uint32_t lo = (wi >= 0 && wi < g.Wm) ? row[wi] : 0u;
-      const uint32_t hi = (wi + 1 >= 0 && wi + 1 < g.Wm) ? row[wi + 1] : 0u;
-      word = __funnelshift_r(lo, hi, sh);
+  // mask bits of this thread's sites: bit 4 i + 2 col + {0, 1} = site (row warp + NW i, colour col,
+  // column jj + {0, 1}) is a prediction site.  (j0 + jj) is even, so both bits sit in one word.
+  uint64_t mbits = 0;
+  {
+    const int j = j0 + jj;
+    const int wi = j >> 5, sh = j & 31;
+#pragma unroll
+    for (int i = 0; i < RPW; ++i) {
+      const int y = y0 + warp + NW * i;
+      if (y >= 0 && y < g.L && wi >= 0 && wi < g.Wm) {
+#pragma unroll
+        for (int col = 0; col < 2; ++col) {
+          const uint32_t w = __ldg(bits + (static_cast<size_t>(col) * g.L + y) * g.Wm + wi);
+          mbits |= static_cast<uint64_t>((w >> sh) & 3u) << (4 * i + 2 * col);
+        }
+      }
     }
-    mb[p][r][w] = word;
   }
-  __syncthreads();
+  const bool col_interior = jj >= hc && jj < kTileCols - hc;
+  // Philox counter word 0 of the first site of this thread's pair in tile row 0, without the parity
+  const uint32_t site_row0 = static_cast<uint32_t>(y0) * static_cast<uint32_t>(g.L) + static_cast<uint32_t>(2 * (j0 + jj));
+  const uint32_t Lu = static_cast<uint32_t>(g.L);
+  __syncthreads();          // mbarrier initialised before anyone polls it
   mbar_wait(bar, 0);
 
   int n_acc = 0;
@@ -145,38 +244,13 @@ tiled_sweep_kernel(const __grid_constant__ CUtensorMap tmap, typename Traits<MOD
     for (int pass = 0; pass < 4; ++pass) {
       const int col = pass & 1;
       const int p = 4 * sw + pass + 1;
-      const int nitems = (TH - 2 * p) * 2;
-      for (int item = warp; item < nitems; item += NW) {
-        const int r = p + (item >> 1), half = item & 1;
-        const int y = y0 + r;
-        if (y < 0 || y >= g.L) continue;
-        const int jj = half * 32 + lane;
-        if (!((mb[col][r][half] >> lane) & 1u)) continue;
-        const int par = x_parity(y, col);
-        const int x = 2 * (j0 + jj) + par;
-        const bool hl = x > 0, hr = x < g.L - 1, hu = y > 0, hd = y < g.L - 1;
-        int jl = jj - 1 + par, jr = jj + par;
-        jl = jl < 0 ? 0 : jl;
-        jr = jr > kTileCols - 1 ? kTileCols - 1 : jr;
-        const V l = tile[1 - col][r][jl];
-        const V rr = tile[1 - col][r][jr];
-        const V u = tile[1 - col][r - 1][jj];
-        const V d = tile[1 - col][r + 1][jj];
-        R A, B;
-        local_field<R>(R(l.x), R(l.y), R(rr.x), R(rr.y), R(u.x), R(u.y), R(d.x), R(d.y), hl, hr, hu, hd, &A, &B);
-        const V me = tile[col][r][jj];
-        R c = R(me.x), s = R(me.y);
-        if (pass < 2) {
-          const bool ok = met_update<MODE>(&c, &s, A, B, static_cast<uint32_t>(y) * static_cast<uint32_t>(g.L) + x,
-                                           sweep, kc);
-          if (ok && r >= h && r < TH - h && jj >= hc && jj < kTileCols - hc) n_acc += 1;
-        } else {
-          or_update<MODE>(&c, &s, A, B);
-        }
-        V out;
-        out.x = static_cast<decltype(out.x)>(c);
-        out.y = static_cast<decltype(out.y)>(s);
-        tile[col][r][jj] = out;
+      const int par = (y0 + warp + col) & 1;       // same for all rows of this warp (NW even)
+      if (pass < 2) {
+        n_acc += par ? pass_rows<MODE, KIND_MET, 1>(t, col, p, h, mbits, col_interior, site_row0, Lu, sweep, kc)
+                     : pass_rows<MODE, KIND_MET, 0>(t, col, p, h, mbits, col_interior, site_row0, Lu, sweep, kc);
+      } else {
+        if (par) pass_rows<MODE, KIND_OR, 1>(t, col, p, h, mbits, col_interior, site_row0, Lu, sweep, kc);
+        else     pass_rows<MODE, KIND_OR, 0>(t, col, p, h, mbits, col_interior, site_row0, Lu, sweep, kc);
       }
       __syncthreads();
     }
@@ -184,31 +258,36 @@ tiled_sweep_kernel(const __grid_constant__ CUtensorMap tmap, typename Traits<MOD
 
   // interior -> other state buffer (+ energy sample and accumulation of phi when measuring)
   double esum = 0.0;
-  const int nint = IR * 2 * 2;   // rows x planes x halves
-  for (int item = warp; item < nint; item += NW) {
-    const int half = item & 1, pl = (item >> 1) & 1, r = h + (item >> 2);
-    const int y = y0 + r;
-    if (y >= g.L) continue;
-    const int jj = half * 32 + lane;
-    const int j = j0 + jj;
-    if (jj < hc || jj >= kTileCols - hc || j >= g.Wp) continue;
-    const V me = tile[pl][r][jj];
-    const size_t gi = static_cast<size_t>(pl) * g.plane + static_cast<size_t>(y) * g.Wp + j;
-    dst[gi] = me;
-    if constexpr (MEASURE) {
-      const int par = x_parity(y, pl);
-      const int x = 2 * j + par;
-      if (pl == 1 && x < g.L) {
-        const bool hl = x > 0, hr = x < g.L - 1, hu = y > 0, hd = y < g.L - 1;
-        const V l = tile[0][r][jj - 1 + par];
-        const V rr = tile[0][r][jj + par];
-        const V u = tile[0][r - 1][jj];
-        const V d = tile[0][r + 1][jj];
-        R A, B;
-        local_field<R>(R(l.x), R(l.y), R(rr.x), R(rr.y), R(u.x), R(u.y), R(d.x), R(d.y), hl, hr, hu, hd, &A, &B);
-        esum += static_cast<double>(fma_(R(me.x), A, R(me.y) * B));
+  const int j = j0 + jj;
+  if (col_interior && j < g.Wp) {
+#pragma unroll 1
+    for (int i = 0; i < RPW; ++i) {
+      const int r = warp + NW * i;
+      const int y = y0 + r;
+      if (r < h || r >= TH - h || y >= g.L) continue;
+#pragma unroll
+      for (int pl = 0; pl < 2; ++pl) {
+        const Pair<V> me = t.pair(pl, r, jj);
+        const size_t gi = static_cast<size_t>(pl) * g.plane + static_cast<size_t>(y) * g.Wp + j;
+        *reinterpret_cast<Pair<V>*>(dst + gi) = me;
+        if constexpr (MEASURE) {
+          if (pl == 1) {   // every bond has exactly one colour-1 end: H = -J sum over colour-1 sites of u.F
+            R Aa, Ba, Ab, Bb;
+            const int jl = jj - 1, jr = jj + 2;   // interior columns: both in the staged region
+            if ((y + 1) & 1) pair_fields<MODE, 1>(t, 1, r, jj, jr, &Aa, &Ba, &Ab, &Bb);
+            else             pair_fields<MODE, 0>(t, 1, r, jj, jl, &Aa, &Ba, &Ab, &Bb);
+            esum += static_cast<double>(fma_(R(me.a.x), Aa, R(me.a.y) * Ba));
+            esum += static_cast<double>(fma_(R(me.b.x), Ab, R(me.b.y) * Bb));
+          }
+          const uint32_t mm = static_cast<uint32_t>(mbits >> (4 * i + 2 * pl)) & 3u;
+          if (mm) {
+            double2 a2 = *reinterpret_cast<const double2*>(acc + gi);
+            if (mm & 1u) a2.x += spin_angle<MODE>(R(me.a.x), R(me.a.y));
+            if (mm & 2u) a2.y += spin_angle<MODE>(R(me.b.x), R(me.b.y));
+            *reinterpret_cast<double2*>(acc + gi) = a2;
+          }
+        }
       }
-      if ((mb[pl][r][half] >> lane) & 1u) acc[gi] += spin_angle<MODE>(R(me.x), R(me.y));
     }
   }
   if constexpr (MEASURE) {
