@@ -90,7 +90,13 @@ template <> struct Fn<MODE_SP_INTRINSIC> {
     asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
     return y;
   }
-  static __device__ __forceinline__ float div_(float a, float b) { return __fdividef(a, b); }
+  // a * rcp.approx(b): the MUFU.RCP at the heart of __fdividef, without its rescaling of huge / tiny
+  // divisors (|F|^2 lies in {0} U [~1e-14, 16]; F = 0 is rejected by the caller)
+  static __device__ __forceinline__ float div_(float a, float b) {
+    float r;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(b));
+    return a * r;
+  }
   static __device__ __forceinline__ float rsqrt_(float x) { return rsqrtf(x); }
   static __device__ __forceinline__ float atan2_(float y, float x) { return atan2f(y, x); }
 };
@@ -120,6 +126,49 @@ __device__ __forceinline__ void local_field(R lc, R ls, R rc, R rs, R uc, R us, 
   *A = a; *B = b;
 }
 
+// ---- two-lane arithmetic -----------------------------------------------------------------
+// Every move is written once, for TWO sites at a time (lanes a, b).  In the float modes the two
+// lanes are the halves of one 64-bit register and every add / mul / fma is ONE packed sm_100
+// instruction (add/mul/fma.rn.f32x2 -> SASS FADD2 / FMUL2 / FFMA2: half the issue slots of the
+// scalar form, same IEEE round-to-nearest result per lane).  In the double modes a lane is a
+// double and the ops are the scalar ones.  The PLAIN path calls the same functions with its one
+// site in both lanes, which is what keeps PLAIN and TILED bit-identical.
+template <typename R> struct Two;
+template <> struct Two<double> { double a, b; };
+template <> struct Two<float>  { unsigned long long v; };
+
+__device__ __forceinline__ Two<double> mk2(double a, double b) { return Two<double>{a, b}; }
+__device__ __forceinline__ Two<float> mk2(float a, float b) {
+  Two<float> r;
+  asm("mov.b64 %0, {%1, %2};" : "=l"(r.v) : "f"(a), "f"(b));
+  return r;
+}
+__device__ __forceinline__ void un2(const Two<double>& x, double* a, double* b) { *a = x.a; *b = x.b; }
+__device__ __forceinline__ void un2(const Two<float>& x, float* a, float* b) {
+  asm("mov.b64 {%0, %1}, %2;" : "=f"(*a), "=f"(*b) : "l"(x.v));
+}
+__device__ __forceinline__ Two<double> add2(const Two<double>& x, const Two<double>& y) { return {x.a + y.a, x.b + y.b}; }
+__device__ __forceinline__ Two<double> mul2(const Two<double>& x, const Two<double>& y) { return {x.a * y.a, x.b * y.b}; }
+__device__ __forceinline__ Two<double> fma2(const Two<double>& x, const Two<double>& y, const Two<double>& z) {
+  return {fma(x.a, y.a, z.a), fma(x.b, y.b, z.b)};
+}
+__device__ __forceinline__ Two<float> add2(const Two<float>& x, const Two<float>& y) {
+  Two<float> r;
+  asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r.v) : "l"(x.v), "l"(y.v));
+  return r;
+}
+__device__ __forceinline__ Two<float> mul2(const Two<float>& x, const Two<float>& y) {
+  Two<float> r;
+  asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r.v) : "l"(x.v), "l"(y.v));
+  return r;
+}
+__device__ __forceinline__ Two<float> fma2(const Two<float>& x, const Two<float>& y, const Two<float>& z) {
+  Two<float> r;
+  asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r.v) : "l"(x.v), "l"(y.v), "l"(z.v));
+  return r;
+}
+template <typename R> __device__ __forceinline__ Two<R> bc2(R k) { return mk2(k, k); }
+
 // Random words of the Metropolis move at a site (R9).  Double-arithmetic modes (DP, SP): one
 // Philox block per site, counter word 0 = the site's row-major index; all four words are used
 // (two 53-bit uniforms), exactly as in the oracle.  Float-arithmetic modes: one block per PAIR of
@@ -143,66 +192,94 @@ __device__ __forceinline__ void met_words_pair(uint32_t pair_site, uint32_t swee
   }
 }
 
-// Metropolis move of one site (R7, R10), written without branches: the new spin is kept iff the
-// site is free, the proposal stays in range (s' >= 0) and the acceptance test passes.  Returns
-// true when the move was accepted.
+// Metropolis move (R7, R10) of two sites at once, branch-free.  Lane x keeps its new spin iff the
+// site is free, the proposal stays in range (s' >= 0) and the acceptance test passes; ok[x] tells.
+//   sd = sin(q Delta/2), cd = cos(q Delta/2);  sin(q Delta) = 2 sd cd,  cos(q Delta) - 1 = -2 sd^2
+//   u' = rot(q Delta) u;  P = u.F;  -Q = s A - c B;  dE = 2 sd (sd P - cd Q)
 template <int MODE>
-__device__ __forceinline__ bool met_update(typename Traits<MODE>::real* c, typename Traits<MODE>::real* s,
-                                           typename Traits<MODE>::real A, typename Traits<MODE>::real B,
-                                           const MetWords& w, bool is_free,
-                                           const ChainConst<typename Traits<MODE>::real>& k) {
+__device__ __forceinline__ void met_update2(Two<typename Traits<MODE>::real> c, Two<typename Traits<MODE>::real> s,
+                                            Two<typename Traits<MODE>::real> A, Two<typename Traits<MODE>::real> B,
+                                            const MetWords& wa, const MetWords& wb, bool free_a, bool free_b,
+                                            const ChainConst<typename Traits<MODE>::real>& k,
+                                            typename Traits<MODE>::real out[4] /* ca, cb, sa, sb */, bool ok[2]) {
   using R = typename Traits<MODE>::real;
-  R h;                                           // q Delta / 2
+  Two<R> h;                                      // q Delta / 2
   if constexpr (sizeof(R) == 8) {
-    const R t = fma_(R(2), R(u53(w.p, w.q)), R(-1));   // 2 u1 - 1 (exact)
-    h = R(0.25) * (k.delta * t);
+    const R ta = fma_(R(2), R(u53(wa.p, wa.q)), R(-1));   // 2 u1 - 1 (exact)
+    const R tb = fma_(R(2), R(u53(wb.p, wb.q)), R(-1));
+    h = mul2(bc2(R(0.25)), mul2(bc2(k.delta), mk2(ta, tb)));
   } else {
-    h = k.hscale * sym_word(w.p);
+    h = mul2(bc2(k.hscale), mk2(sym_word(wa.p), sym_word(wb.p)));
   }
-  R sd, cd;
-  Fn<MODE>::sincos_(h, &sd, &cd);
-  const R ts = sd + sd;
-  const R s2 = ts * cd;                          // sin(q Delta)
-  const R c2m1 = -(ts * sd);                     // cos(q Delta) - 1
-  const R c0 = *c, s0 = *s;
-  const R cn = fma_(-s0, s2, fma_(c0, c2m1, c0));   // c cos - s sin
-  const R sn = fma_(c0, s2, fma_(s0, c2m1, s0));    // s cos + c sin
-  const R P = fma_(c0, A, s0 * B);               // u.F
-  const R Q = fma_(c0, B, -(s0 * A));            // c B - s A
-  const R dE = ts * fma_(sd, P, -(cd * Q));
-  bool acc;
+  R ha, hb, sda, cda, sdb, cdb;
+  un2(h, &ha, &hb);
+  Fn<MODE>::sincos_(ha, &sda, &cda);
+  Fn<MODE>::sincos_(hb, &sdb, &cdb);
+  const Two<R> sd = mk2(sda, sdb), cd = mk2(cda, cdb);
+  const Two<R> ts = add2(sd, sd);                // 2 sd
+  const Two<R> nts = mul2(sd, bc2(R(-2)));       // -2 sd
+  const Two<R> s2 = mul2(ts, cd);                // sin(q Delta)
+  const Two<R> ns2 = mul2(nts, cd);              // -sin(q Delta)
+  const Two<R> c2m1 = mul2(nts, sd);             // cos(q Delta) - 1
+  const Two<R> cn = fma2(s, ns2, fma2(c, c2m1, c));   // c cos - s sin
+  const Two<R> sn = fma2(c, s2, fma2(s, c2m1, s));    // s cos + c sin
+  const Two<R> P = fma2(c, A, mul2(s, B));            // u.F
+  const Two<R> nQ = fma2(s, A, mul2(mul2(c, bc2(R(-1))), B));   // s A - c B
+  const Two<R> dE = mul2(ts, fma2(sd, P, mul2(cd, nQ)));
+  R c0a, c0b, s0a, s0b, cna, cnb, sna, snb;
+  un2(c, &c0a, &c0b); un2(s, &s0a, &s0b); un2(cn, &cna, &cnb); un2(sn, &sna, &snb);
+  bool acc_a, acc_b;
   if constexpr (sizeof(R) == 8) {
-    acc = R(u53(w.a, w.b)) < Fn<MODE>::exp_(-(dE * k.inv_T));
+    R xa, xb;
+    un2(mul2(dE, bc2(k.inv_T)), &xa, &xb);
+    acc_a = R(u53(wa.a, wa.b)) < Fn<MODE>::exp_(-xa);
+    acc_b = R(u53(wb.a, wb.b)) < Fn<MODE>::exp_(-xb);
   } else if constexpr (MODE == MODE_SP_INTRINSIC) {
-    acc = pos_word(w.a) < Fn<MODE>::ex2_(fma_(dE, k.xscale, R(32)));   // = __expf(-dE/T) 2^32: one FFMA + MUFU.EX2
+    R xa, xb;                                    // exp(-dE/T) 2^32 = ex2(dE xscale + 32): one FFMA2 + 2 MUFU.EX2
+    un2(fma2(dE, bc2(k.xscale), bc2(R(32))), &xa, &xb);
+    acc_a = pos_word(wa.a) < Fn<MODE>::ex2_(xa);
+    acc_b = pos_word(wb.a) < Fn<MODE>::ex2_(xb);
   } else {
-    acc = pos_word(w.a) * R(2.3283064365386963e-10) < Fn<MODE>::exp_(-(dE * k.inv_T));
+    R xa, xb, ua, ub;
+    un2(mul2(dE, bc2(k.inv_T)), &xa, &xb);
+    un2(mul2(mk2(pos_word(wa.a), pos_word(wb.a)), bc2(R(2.3283064365386963e-10))), &ua, &ub);
+    acc_a = ua < Fn<MODE>::exp_(-xa);
+    acc_b = ub < Fn<MODE>::exp_(-xb);
   }
-  const bool ok = is_free && (sn >= R(0)) && acc;
-  *c = ok ? cn : c0;
-  *s = ok ? sn : s0;
-  return ok;
+  const bool oka = free_a && (sna >= R(0)) && acc_a;
+  const bool okb = free_b && (snb >= R(0)) && acc_b;
+  out[0] = oka ? cna : c0a; out[2] = oka ? sna : s0a;
+  out[1] = okb ? cnb : c0b; out[3] = okb ? snb : s0b;
+  ok[0] = oka; ok[1] = okb;
 }
 
-// Over-relaxation move (R5): reflect u about the local field; keep it iff the site is free, F != 0
-// and u' stays on the upper half circle.  One Newton step towards |u| = 1 stops the rounding
-// drift of the norm.  Branch-free.
+// Over-relaxation move (R5) of two sites at once: reflect u about the local field, u' = t F - u,
+// t = 2 (u.F)/|F|^2; keep it iff the site is free, F != 0 and u' stays on the upper half circle.
+// One Newton step towards |u'| = 1 stops the rounding drift of the norm.  Computed as
+// m = u - t F = -u' and -f, so that no negation is needed: u' f = m (-f).
 template <int MODE>
-__device__ __forceinline__ void or_update(typename Traits<MODE>::real* c, typename Traits<MODE>::real* s,
-                                          typename Traits<MODE>::real A, typename Traits<MODE>::real B,
-                                          bool is_free) {
+__device__ __forceinline__ void or_update2(Two<typename Traits<MODE>::real> c, Two<typename Traits<MODE>::real> s,
+                                           Two<typename Traits<MODE>::real> A, Two<typename Traits<MODE>::real> B,
+                                           bool free_a, bool free_b,
+                                           typename Traits<MODE>::real out[4] /* ca, cb, sa, sb */) {
   using R = typename Traits<MODE>::real;
-  const R R2 = fma_(A, A, B * B);
-  const R c0 = *c, s0 = *s;
-  const R P = fma_(c0, A, s0 * B);
-  const R t = Fn<MODE>::div_(P + P, R2);
-  R cn = fma_(t, A, -c0);
-  R sn = fma_(t, B, -s0);
-  const bool ok = is_free && (R2 != R(0)) && (sn >= R(0));
-  const R f = fma_(R(-0.5), fma_(cn, cn, sn * sn), R(1.5));
-  cn = cn * f; sn = sn * f;
-  *c = ok ? cn : c0;
-  *s = ok ? sn : s0;
+  const Two<R> F2 = fma2(A, A, mul2(B, B));
+  const Two<R> P = fma2(c, A, mul2(s, B));
+  const Two<R> nPP = mul2(P, bc2(R(-2)));
+  R f2a, f2b, na, nb;
+  un2(F2, &f2a, &f2b);
+  un2(nPP, &na, &nb);
+  const Two<R> nt = mk2(Fn<MODE>::div_(na, f2a), Fn<MODE>::div_(nb, f2b));   // -t
+  const Two<R> mc = fma2(nt, A, c);              // -c'
+  const Two<R> ms = fma2(nt, B, s);              // -s'
+  const Two<R> nf = fma2(bc2(R(0.5)), fma2(mc, mc, mul2(ms, ms)), bc2(R(-1.5)));   // -(1.5 - |u'|^2 / 2)
+  const Two<R> co = mul2(mc, nf), so = mul2(ms, nf);
+  R c0a, c0b, s0a, s0b, msa, msb, coa, cob, soa, sob;
+  un2(c, &c0a, &c0b); un2(s, &s0a, &s0b); un2(ms, &msa, &msb); un2(co, &coa, &cob); un2(so, &soa, &sob);
+  const bool oka = free_a && (f2a != R(0)) && (msa <= R(0));
+  const bool okb = free_b && (f2b != R(0)) && (msb <= R(0));
+  out[0] = oka ? coa : c0a; out[2] = oka ? soa : s0a;
+  out[1] = okb ? cob : c0b; out[3] = okb ? sob : s0b;
 }
 
 // Quench move (R8): the minimiser of the local energy, u = F/|F|.

@@ -4,7 +4,11 @@
 //
 // Layout.  Site (x, y) has colour (x + y) & 1 and lives in colour plane `col`
 // at row y, column j = x >> 1; a plane is L rows of Wp columns (Wp = ceil(L/2) rounded up to 16),
-// one vec (c, s) per site.  mask bit j of row y of plane col is 1 iff the site exists and is a
+// one spin (c, s) per site, stored PAIR-INTERLEAVED: the two sites of plane columns (2m, 2m + 1)
+// share one unit of four scalars (c_2m, c_2m+1, s_2m, s_2m+1), so that the tiled kernel reads a pair
+// with one 128-bit access whose register halves are already (site a, site b) lanes for the packed
+// f32x2 arithmetic.  With idx = row offset + j (always of j's parity), c sits at scalar
+// 2 idx - (j & 1) and s two scalars further (ld_spin / st_spin).  mask bit j of row y of plane col is 1 iff the site exists and is a
 // prediction site; Wm 32-bit words per row.
 #pragma once
 #include "mpr_device.cuh"
@@ -18,6 +22,20 @@ struct Geom {
 
 __device__ __forceinline__ bool mask_bit(const uint32_t* __restrict__ bits, const Geom& g, int col, int y, int j) {
   return (bits[(static_cast<size_t>(col) * g.L + y) * g.Wm + (j >> 5)] >> (j & 31)) & 1u;
+}
+
+// ---- pair-interleaved spin storage -----------------------------------------------------------
+template <typename V> __device__ __forceinline__ V ld_spin(const V* base, long long idx) {
+  using S = decltype(V::x);
+  const S* p = reinterpret_cast<const S*>(base) + (2 * idx - (idx & 1));
+  V v;
+  v.x = p[0]; v.y = p[2];
+  return v;
+}
+template <typename V> __device__ __forceinline__ void st_spin(V* base, long long idx, const V& v) {
+  using S = decltype(V::x);
+  S* p = reinterpret_cast<S*>(base) + (2 * idx - (idx & 1));
+  p[0] = v.x; p[2] = v.y;
 }
 
 // ---- block reduction helpers (deterministic order) -------------------------------------
@@ -172,7 +190,7 @@ __global__ void init_chain_kernel(const double* __restrict__ z, const uint8_t* _
     v.x = static_cast<decltype(v.x)>(cs);
     v.y = static_cast<decltype(v.y)>(sn);
   }
-  state[static_cast<size_t>(col) * g.plane + static_cast<size_t>(y) * g.Wp + j] = v;
+  st_spin(state, static_cast<long long>(col) * g.plane + static_cast<long long>(y) * g.Wp + j, v);
 }
 
 // Overwrite the free spins from angles (tests, checkpoint restore).
@@ -191,7 +209,7 @@ __global__ void set_state_kernel(const double* __restrict__ phi, Geom g, const u
   V v;
   v.x = static_cast<decltype(v.x)>(cs);
   v.y = static_cast<decltype(v.y)>(sn);
-  state[static_cast<size_t>(col) * g.plane + static_cast<size_t>(y) * g.Wp + j] = v;
+  st_spin(state, static_cast<long long>(col) * g.plane + static_cast<long long>(y) * g.Wp + j, v);
 }
 
 template <int MODE>
@@ -201,7 +219,7 @@ __global__ void get_state_kernel(const typename Traits<MODE>::vec* __restrict__ 
   const int x = blockIdx.x * blockDim.x + threadIdx.x;
   if (x >= g.L) return;
   const int col = (x + y) & 1, j = x >> 1;
-  const auto v = state[static_cast<size_t>(col) * g.plane + static_cast<size_t>(y) * g.Wp + j];
+  const auto v = ld_spin(state, static_cast<long long>(col) * g.plane + static_cast<long long>(y) * g.Wp + j);
   phi[static_cast<size_t>(y) * g.L + x] = 2.0 * atan2(static_cast<double>(v.y), static_cast<double>(v.x));
 }
 
@@ -224,13 +242,13 @@ plain_pass_kernel(typename Traits<MODE>::vec* __restrict__ state, const uint32_t
     const bool hl = x > 0, hr = x < g.L - 1, hu = y > 0, hd = y < g.L - 1;
     const int jl = j - 1 + par, jr = j + par;
     V zero; zero.x = 0; zero.y = 0;
-    const V l = hl ? oth[jl] : zero;
-    const V r = hr ? oth[jr] : zero;
-    const V u = hu ? oth[j - g.Wp] : zero;
-    const V d = hd ? oth[j + g.Wp] : zero;
+    const V l = hl ? ld_spin(oth, jl) : zero;
+    const V r = hr ? ld_spin(oth, jr) : zero;
+    const V u = hu ? ld_spin(oth, j - g.Wp) : zero;
+    const V d = hd ? ld_spin(oth, j + g.Wp) : zero;
     R A, B;
     local_field<R>(R(l.x), R(l.y), R(r.x), R(r.y), R(u.x), R(u.y), R(d.x), R(d.y), hl, hr, hu, hd, &A, &B);
-    const V me = own[j];
+    const V me = ld_spin(own, j);
     R c = R(me.x), s = R(me.y);
     if constexpr (KIND == KIND_MET) {
       // R9: the pair (2m, 2m + 1) of plane columns shares one Philox block in the float modes
@@ -238,16 +256,23 @@ plain_pass_kernel(typename Traits<MODE>::vec* __restrict__ state, const uint32_t
                                  static_cast<uint32_t>(2 * (j & ~1) + par);
       MetWords w0, w1;
       met_words_pair<MODE>(pair_site, sweep, k, &w0, &w1);
-      accepted = met_update<MODE>(&c, &s, A, B, (j & 1) ? w1 : w0, true, k);
+      const MetWords w = (j & 1) ? w1 : w0;
+      R o[4];
+      bool ok[2];
+      met_update2<MODE>(bc2(c), bc2(s), bc2(A), bc2(B), w, w, true, true, k, o, ok);   // the site in both lanes
+      c = o[0]; s = o[2];
+      accepted = ok[0];
     } else if constexpr (KIND == KIND_OR) {
-      or_update<MODE>(&c, &s, A, B, true);
+      R o[4];
+      or_update2<MODE>(bc2(c), bc2(s), bc2(A), bc2(B), true, true, o);
+      c = o[0]; s = o[2];
     } else {
       quench_update<MODE>(&c, &s, A, B);
     }
     V out;
     out.x = static_cast<decltype(out.x)>(c);
     out.y = static_cast<decltype(out.y)>(s);
-    own[j] = out;
+    st_spin(own, j, out);
   }
   if constexpr (KIND == KIND_MET) {
     const int n = __syncthreads_count(accepted);
@@ -275,13 +300,13 @@ plain_energy_kernel(const typename Traits<MODE>::vec* __restrict__ state, Geom g
       if (x >= g.L) continue;
       const bool hl = x > 0, hr = x < g.L - 1, hu = y > 0, hd = y < g.L - 1;
       V zero; zero.x = 0; zero.y = 0;
-      const V l = hl ? oth[j - 1 + par] : zero;
-      const V r = hr ? oth[j + par] : zero;
-      const V u = hu ? oth[j - g.Wp] : zero;
-      const V d = hd ? oth[j + g.Wp] : zero;
+      const V l = hl ? ld_spin(oth, j - 1 + par) : zero;
+      const V r = hr ? ld_spin(oth, j + par) : zero;
+      const V u = hu ? ld_spin(oth, j - g.Wp) : zero;
+      const V d = hd ? ld_spin(oth, j + g.Wp) : zero;
       R A, B;
       local_field<R>(R(l.x), R(l.y), R(r.x), R(r.y), R(u.x), R(u.y), R(d.x), R(d.y), hl, hr, hu, hd, &A, &B);
-      const V me = own[j];
+      const V me = ld_spin(own, j);
       sum += static_cast<double>(fma_(R(me.x), A, R(me.y) * B));
     }
   }
@@ -298,7 +323,7 @@ __global__ void plain_accumulate_kernel(const typename Traits<MODE>::vec* __rest
   const int j = blockIdx.x * blockDim.x + threadIdx.x;
   if (j >= g.Wp || !mask_bit(bits, g, col, y, j)) return;
   const size_t i = static_cast<size_t>(col) * g.plane + static_cast<size_t>(y) * g.Wp + j;
-  const auto v = state[i];
+  const auto v = ld_spin(state, static_cast<long long>(i));
   acc[i] += spin_angle<MODE>(R(v.x), R(v.y));
 }
 

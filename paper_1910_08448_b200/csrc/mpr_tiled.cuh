@@ -104,83 +104,97 @@ template <int MODE> constexpr size_t tile_smem_bytes() {
          + 64;                                                                      // mbarrier
 }
 
-// Two adjacent plane columns of one row: one 128-bit access in the float-storage modes, two in DP.
-template <typename V> struct alignas(2 * sizeof(V)) Pair { V a, b; };
+// Storage unit (mpr_plain.cuh): the two sites of plane columns (2m, 2m + 1) as (c_a, c_b, s_a, s_b):
+// one 128-bit access in the float-storage modes, two in DP; (ca, cb) and (sa, sb) land in
+// adjacent registers, i.e. they ARE the two-lane operands of the packed arithmetic.
+template <typename S> struct alignas(4 * sizeof(S)) Unit { S ca, cb, sa, sb; };
+constexpr int kRowScalars = 2 * kTileCols;
 
 template <int MODE> struct TileView {
-  using V = typename Traits<MODE>::vec;
+  using S = decltype(Traits<MODE>::vec::x);
   static constexpr int TH = TileCfg<MODE>::TH;
-  V* base;   // [2][TH][kTileCols]
-  __device__ __forceinline__ V* at(int pl, int r, int j) const { return base + (pl * TH + r) * kTileCols + j; }
-  __device__ __forceinline__ Pair<V> pair(int pl, int r, int j) const {
-    return *reinterpret_cast<const Pair<V>*>(at(pl, r, j));
-  }
+  S* base;   // [2][TH][kRowScalars]
+  // unit of columns (2 u, 2 u + 1) in row r of plane pl
+  __device__ __forceinline__ S* unit(int pl, int r, int u) const { return base + (pl * TH + r) * kRowScalars + 4 * u; }
 };
 
-// Local fields of the two sites (columns jj, jj + 1) of a pair in row r of colour `col`.
-// PAR = x-parity of the row for this colour: the left/right neighbours of column j are the
-// other plane's columns (j - 1 + PAR, j + PAR).  jx = clamped column of the one neighbour that
-// lies outside the aligned pair (jj - 1 for PAR = 0, jj + 2 for PAR = 1).  Sum order l, r, u, d.
+// Local fields of the two sites of a unit; `oth` points at the unit of the same row and columns in
+// the OTHER colour plane.  PAR = x-parity of the row for this colour: the left/right neighbours
+// of column j are the other plane's columns (j - 1 + PAR, j + PAR), so besides the unit itself
+// (mid) one more site is needed: column jj - 1 (PAR = 0; lane b of the previous unit) or jj + 2
+// (PAR = 1; lane a of the next unit).  At the rim of the staged region that address falls into
+// the adjacent row -- inside shared memory, and read only by sites that are stale anyway.
+// Sum order l, r, u, d, lanes = (site a, site b): one packed add per term in the float modes.
 template <int MODE, int PAR>
-__device__ __forceinline__ void pair_fields(const TileView<MODE>& t, int col, int r, int jj, int jx,
-                                            typename Traits<MODE>::real* Aa, typename Traits<MODE>::real* Ba,
-                                            typename Traits<MODE>::real* Ab, typename Traits<MODE>::real* Bb) {
+__device__ __forceinline__ void pair_fields(const decltype(Traits<MODE>::vec::x)* oth,
+                                            Two<typename Traits<MODE>::real>* A, Two<typename Traits<MODE>::real>* B) {
   using R = typename Traits<MODE>::real;
-  using V = typename Traits<MODE>::vec;
-  const Pair<V> mid = t.pair(1 - col, r, jj);
-  const Pair<V> up = t.pair(1 - col, r - 1, jj);
-  const Pair<V> dn = t.pair(1 - col, r + 1, jj);
-  const V ex = *t.at(1 - col, r, jx);
-  R aa, ba, ab, bb;
+  using S = decltype(Traits<MODE>::vec::x);
+  const Unit<S> mid = *reinterpret_cast<const Unit<S>*>(oth);
+  const Unit<S> up = *reinterpret_cast<const Unit<S>*>(oth - kRowScalars);
+  const Unit<S> dn = *reinterpret_cast<const Unit<S>*>(oth + kRowScalars);
+  const S exc = oth[PAR ? 4 : -3], exs = oth[PAR ? 6 : -1];
+  const Two<R> midc = mk2(R(mid.ca), R(mid.cb)), mids = mk2(R(mid.sa), R(mid.sb));
+  Two<R> a, b;
   if constexpr (PAR == 0) {         // a: l = ex, r = mid.a     b: l = mid.a, r = mid.b
-    aa = R(ex.x) + R(mid.a.x);    ba = R(ex.y) + R(mid.a.y);
-    ab = R(mid.a.x) + R(mid.b.x); bb = R(mid.a.y) + R(mid.b.y);
+    a = add2(mk2(R(exc), R(mid.ca)), midc);
+    b = add2(mk2(R(exs), R(mid.sa)), mids);
   } else {                          // a: l = mid.a, r = mid.b  b: l = mid.b, r = ex
-    aa = R(mid.a.x) + R(mid.b.x); ba = R(mid.a.y) + R(mid.b.y);
-    ab = R(mid.b.x) + R(ex.x);    bb = R(mid.b.y) + R(ex.y);
+    a = add2(midc, mk2(R(mid.cb), R(exc)));
+    b = add2(mids, mk2(R(mid.sb), R(exs)));
   }
-  aa = aa + R(up.a.x); ba = ba + R(up.a.y); ab = ab + R(up.b.x); bb = bb + R(up.b.y);
-  aa = aa + R(dn.a.x); ba = ba + R(dn.a.y); ab = ab + R(dn.b.x); bb = bb + R(dn.b.y);
-  *Aa = aa; *Ba = ba; *Ab = ab; *Bb = bb;
+  a = add2(a, mk2(R(up.ca), R(up.cb))); b = add2(b, mk2(R(up.sa), R(up.sb)));
+  a = add2(a, mk2(R(dn.ca), R(dn.cb))); b = add2(b, mk2(R(dn.sa), R(dn.sb)));
+  *A = a; *B = b;
 }
 
-// One colour pass (p-th pass of the launch, 1-based) over the rows of this warp.  Returns the
-// number of accepted Metropolis moves at sites this CTA owns (its interior).
-template <int MODE, int KIND, int PAR>
-__device__ __forceinline__ int pass_rows(const TileView<MODE>& t, int col, int p, int h, uint64_t mbits,
-                                         bool col_interior, uint32_t site_row0, uint32_t L, uint32_t sweep,
+// One colour pass (p-th pass of the launch, 1-based) over the rows of this warp.  COL, PAR and
+// KIND are compiled in: every shared-memory access is one pointer plus an immediate offset.
+// Returns the number of accepted Metropolis moves at sites this CTA owns (its interior).
+template <int MODE, int KIND, int PAR, int COL>
+__device__ __forceinline__ int pass_rows(const TileView<MODE>& t, int p, int h, uint32_t mcol, bool col_interior,
+                                         uint32_t site_row0, uint32_t L, uint32_t sweep,
                                          const ChainConst<typename Traits<MODE>::real>& kc) {
   using R = typename Traits<MODE>::real;
-  using V = typename Traits<MODE>::vec;
+  using S = decltype(Traits<MODE>::vec::x);
   constexpr int TH = TileCfg<MODE>::TH, NW = TileCfg<MODE>::NT / 32, RPW = TH / NW;
+  constexpr int kOther = (COL ? -1 : 1) * TH * kRowScalars;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  const int jj = 2 * lane;
-  const int jx = PAR ? (jj + 2 > kTileCols - 1 ? kTileCols - 1 : jj + 2) : (jj - 1 < 0 ? 0 : jj - 1);
+  // rows r = warp + NW i with p <= r < TH - p (the rest is the stale rim of the staged region)
+  const int i_lo = p > warp ? (p - warp + NW - 1) / NW : 0;
+  int i_hi = (TH - p - warp + NW - 1) / NW;
+  i_hi = i_hi > RPW ? RPW : i_hi;
+  // ... of which the CTA owns rows h <= r < TH - h
+  const int c_lo = h > warp ? (h - warp + NW - 1) / NW : 0;
+  const int c_hi = col_interior ? (TH - h - warp + NW - 1) / NW : 0;
+  S* own = t.unit(COL, warp + NW * i_lo, lane);
+  uint32_t m = mcol >> (2 * i_lo);
+  uint32_t site = site_row0 + static_cast<uint32_t>(warp + NW * i_lo) * L + static_cast<uint32_t>(PAR);
   int n_acc = 0;
 #pragma unroll 1
-  for (int i = 0; i < RPW; ++i) {
-    const int r = warp + NW * i;
-    if (r < p || r >= TH - p) continue;            // stale rim of the staged region (warp-uniform)
-    const uint32_t mm = static_cast<uint32_t>(mbits >> (4 * i + 2 * col));
-    const bool fa = mm & 1u, fb = mm & 2u;
-    R Aa, Ba, Ab, Bb;
-    pair_fields<MODE, PAR>(t, col, r, jj, jx, &Aa, &Ba, &Ab, &Bb);
-    const Pair<V> me = t.pair(col, r, jj);
-    R ca = R(me.a.x), sa = R(me.a.y), cb = R(me.b.x), sb = R(me.b.y);
+  for (int i = i_lo; i < i_hi; ++i) {
+    Two<R> A, B;
+    pair_fields<MODE, PAR>(own + kOther, &A, &B);
+    const Unit<S> me = *reinterpret_cast<const Unit<S>*>(own);
+    const Two<R> c = mk2(R(me.ca), R(me.cb)), s = mk2(R(me.sa), R(me.sb));
+    const bool fa = m & 1u, fb = m & 2u;
+    R o[4];
     if constexpr (KIND == KIND_MET) {
       MetWords w0, w1;
-      met_words_pair<MODE>(site_row0 + static_cast<uint32_t>(r) * L + static_cast<uint32_t>(PAR), sweep, kc, &w0, &w1);
-      const bool oka = met_update<MODE>(&ca, &sa, Aa, Ba, w0, fa, kc);
-      const bool okb = met_update<MODE>(&cb, &sb, Ab, Bb, w1, fb, kc);
-      if (col_interior && r >= h && r < TH - h) n_acc += static_cast<int>(oka) + static_cast<int>(okb);
+      met_words_pair<MODE>(site, sweep, kc, &w0, &w1);
+      bool ok[2];
+      met_update2<MODE>(c, s, A, B, w0, w1, fa, fb, kc, o, ok);
+      if (i >= c_lo && i < c_hi) n_acc += static_cast<int>(ok[0]) + static_cast<int>(ok[1]);
     } else {
-      or_update<MODE>(&ca, &sa, Aa, Ba, fa);
-      or_update<MODE>(&cb, &sb, Ab, Bb, fb);
+      or_update2<MODE>(c, s, A, B, fa, fb, o);
     }
-    Pair<V> out;
-    out.a.x = static_cast<decltype(out.a.x)>(ca); out.a.y = static_cast<decltype(out.a.y)>(sa);
-    out.b.x = static_cast<decltype(out.b.x)>(cb); out.b.y = static_cast<decltype(out.b.y)>(sb);
-    *reinterpret_cast<Pair<V>*>(t.at(col, r, jj)) = out;
+    Unit<S> out;
+    out.ca = static_cast<S>(o[0]); out.cb = static_cast<S>(o[1]);
+    out.sa = static_cast<S>(o[2]); out.sb = static_cast<S>(o[3]);
+    *reinterpret_cast<Unit<S>*>(own) = out;
+    own += NW * kRowScalars;
+    m >>= 2;
+    site += static_cast<uint32_t>(NW) * L;
   }
   return n_acc;
 }
@@ -194,9 +208,10 @@ tiled_sweep_kernel(const __grid_constant__ CUtensorMap tmap, typename Traits<MOD
   using R = typename Traits<MODE>::real;
   using V = typename Traits<MODE>::vec;
   constexpr int TH = TileCfg<MODE>::TH, NT = TileCfg<MODE>::NT, NW = NT / 32, RPW = TH / NW;
-  static_assert(TH % NW == 0 && NW % 2 == 0 && RPW * 4 <= 64, "row ownership / mask register layout");
+  static_assert(TH % NW == 0 && NW % 2 == 0 && RPW * 2 <= 32, "row ownership / mask register layout");
   extern __shared__ __align__(128) unsigned char smem_raw[];
-  TileView<MODE> t{reinterpret_cast<V*>(smem_raw)};
+  using S = decltype(V::x);
+  TileView<MODE> t{reinterpret_cast<S*>(smem_raw)};
   uint64_t* bar = reinterpret_cast<uint64_t*>(smem_raw + sizeof(V) * 2 * TH * kTileCols);
   __shared__ double red[32];
 
@@ -212,20 +227,22 @@ tiled_sweep_kernel(const __grid_constant__ CUtensorMap tmap, typename Traits<MOD
     mbar_expect_tx(bar, static_cast<uint32_t>(sizeof(V) * 2 * TH * kTileCols));
     tma_load_3d(t.base, &tmap, bar, 2 * j0, y0, 0);
   }
-  // mask bits of this thread's sites: bit 4 i + 2 col + {0, 1} = site (row warp + NW i, colour col,
-  // column jj + {0, 1}) is a prediction site.  (j0 + jj) is even, so both bits sit in one word.
-  uint64_t mbits = 0;
+  // mask bits of this thread's sites, one register per colour: bit 2 i + {0, 1} of mreg[col] = site
+  // (row warp + NW i, colour col, column jj + {0, 1}) is a prediction site.  (j0 + jj) is even, so
+  // both bits sit in one word of the bitmap.
+  uint32_t mreg[2] = {0u, 0u};
   {
     const int j = j0 + jj;
     const int wi = j >> 5, sh = j & 31;
+    if (wi >= 0 && wi < g.Wm) {
+      const uint32_t* b0 = bits + wi;
 #pragma unroll
-    for (int i = 0; i < RPW; ++i) {
-      const int y = y0 + warp + NW * i;
-      if (y >= 0 && y < g.L && wi >= 0 && wi < g.Wm) {
-#pragma unroll
-        for (int col = 0; col < 2; ++col) {
-          const uint32_t w = __ldg(bits + (static_cast<size_t>(col) * g.L + y) * g.Wm + wi);
-          mbits |= static_cast<uint64_t>((w >> sh) & 3u) << (4 * i + 2 * col);
+      for (int i = 0; i < RPW; ++i) {
+        const int y = y0 + warp + NW * i;
+        if (y >= 0 && y < g.L) {
+          const uint32_t* bp = b0 + static_cast<size_t>(y) * g.Wm;
+          mreg[0] |= ((__ldg(bp) >> sh) & 3u) << (2 * i);
+          mreg[1] |= ((__ldg(bp + static_cast<size_t>(g.L) * g.Wm) >> sh) & 3u) << (2 * i);
         }
       }
     }
@@ -238,20 +255,28 @@ tiled_sweep_kernel(const __grid_constant__ CUtensorMap tmap, typename Traits<MOD
   mbar_wait(bar, 0);
 
   int n_acc = 0;
+  const int par0 = (y0 + warp) & 1;               // x-parity of this warp's rows for colour 0 (NW is even)
+#pragma unroll 1
   for (int sw = 0; sw < nsweeps; ++sw) {
     const uint32_t sweep = first_sweep + static_cast<uint32_t>(sw);
-#pragma unroll 1
-    for (int pass = 0; pass < 4; ++pass) {
-      const int col = pass & 1;
-      const int p = 4 * sw + pass + 1;
-      const int par = (y0 + warp + col) & 1;       // same for all rows of this warp (NW even)
-      if (pass < 2) {
-        n_acc += par ? pass_rows<MODE, KIND_MET, 1>(t, col, p, h, mbits, col_interior, site_row0, Lu, sweep, kc)
-                     : pass_rows<MODE, KIND_MET, 0>(t, col, p, h, mbits, col_interior, site_row0, Lu, sweep, kc);
-      } else {
-        if (par) pass_rows<MODE, KIND_OR, 1>(t, col, p, h, mbits, col_interior, site_row0, Lu, sweep, kc);
-        else     pass_rows<MODE, KIND_OR, 0>(t, col, p, h, mbits, col_interior, site_row0, Lu, sweep, kc);
-      }
+    const int p = 4 * sw;
+    if (par0) {
+      n_acc += pass_rows<MODE, KIND_MET, 1, 0>(t, p + 1, h, mreg[0], col_interior, site_row0, Lu, sweep, kc);
+      __syncthreads();
+      n_acc += pass_rows<MODE, KIND_MET, 0, 1>(t, p + 2, h, mreg[1], col_interior, site_row0, Lu, sweep, kc);
+      __syncthreads();
+      pass_rows<MODE, KIND_OR, 1, 0>(t, p + 3, h, mreg[0], col_interior, site_row0, Lu, sweep, kc);
+      __syncthreads();
+      pass_rows<MODE, KIND_OR, 0, 1>(t, p + 4, h, mreg[1], col_interior, site_row0, Lu, sweep, kc);
+      __syncthreads();
+    } else {
+      n_acc += pass_rows<MODE, KIND_MET, 0, 0>(t, p + 1, h, mreg[0], col_interior, site_row0, Lu, sweep, kc);
+      __syncthreads();
+      n_acc += pass_rows<MODE, KIND_MET, 1, 1>(t, p + 2, h, mreg[1], col_interior, site_row0, Lu, sweep, kc);
+      __syncthreads();
+      pass_rows<MODE, KIND_OR, 0, 0>(t, p + 3, h, mreg[0], col_interior, site_row0, Lu, sweep, kc);
+      __syncthreads();
+      pass_rows<MODE, KIND_OR, 1, 1>(t, p + 4, h, mreg[1], col_interior, site_row0, Lu, sweep, kc);
       __syncthreads();
     }
   }
@@ -267,23 +292,24 @@ tiled_sweep_kernel(const __grid_constant__ CUtensorMap tmap, typename Traits<MOD
       if (r < h || r >= TH - h || y >= g.L) continue;
 #pragma unroll
       for (int pl = 0; pl < 2; ++pl) {
-        const Pair<V> me = t.pair(pl, r, jj);
-        const size_t gi = static_cast<size_t>(pl) * g.plane + static_cast<size_t>(y) * g.Wp + j;
-        *reinterpret_cast<Pair<V>*>(dst + gi) = me;
+        const Unit<S> me = *reinterpret_cast<const Unit<S>*>(t.unit(pl, r, lane));
+        const size_t gi = static_cast<size_t>(pl) * g.plane + static_cast<size_t>(y) * g.Wp + j;   // j is even
+        *reinterpret_cast<Unit<S>*>(reinterpret_cast<S*>(dst) + 2 * gi) = me;
         if constexpr (MEASURE) {
           if (pl == 1) {   // every bond has exactly one colour-1 end: H = -J sum over colour-1 sites of u.F
-            R Aa, Ba, Ab, Bb;
-            const int jl = jj - 1, jr = jj + 2;   // interior columns: both in the staged region
-            if ((y + 1) & 1) pair_fields<MODE, 1>(t, 1, r, jj, jr, &Aa, &Ba, &Ab, &Bb);
-            else             pair_fields<MODE, 0>(t, 1, r, jj, jl, &Aa, &Ba, &Ab, &Bb);
-            esum += static_cast<double>(fma_(R(me.a.x), Aa, R(me.a.y) * Ba));
-            esum += static_cast<double>(fma_(R(me.b.x), Ab, R(me.b.y) * Bb));
+            Two<R> A, B;
+            if ((y + 1) & 1) pair_fields<MODE, 1>(t.unit(0, r, lane), &A, &B);
+            else             pair_fields<MODE, 0>(t.unit(0, r, lane), &A, &B);
+            R Aa, Ab, Ba, Bb;
+            un2(A, &Aa, &Ab); un2(B, &Ba, &Bb);
+            esum += static_cast<double>(fma_(R(me.ca), Aa, R(me.sa) * Ba));
+            esum += static_cast<double>(fma_(R(me.cb), Ab, R(me.sb) * Bb));
           }
-          const uint32_t mm = static_cast<uint32_t>(mbits >> (4 * i + 2 * pl)) & 3u;
+          const uint32_t mm = (mreg[pl] >> (2 * i)) & 3u;
           if (mm) {
             double2 a2 = *reinterpret_cast<const double2*>(acc + gi);
-            if (mm & 1u) a2.x += spin_angle<MODE>(R(me.a.x), R(me.a.y));
-            if (mm & 2u) a2.y += spin_angle<MODE>(R(me.b.x), R(me.b.y));
+            if (mm & 1u) a2.x += spin_angle<MODE>(R(me.ca), R(me.sa));
+            if (mm & 2u) a2.y += spin_angle<MODE>(R(me.cb), R(me.sb));
             *reinterpret_cast<double2*>(acc + gi) = a2;
           }
         }
