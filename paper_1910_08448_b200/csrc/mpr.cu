@@ -136,6 +136,10 @@ ChainConst<R> chain_const(const mpr_ctx* c) {
   k.k0 = static_cast<uint32_t>(c->seed);
   k.k1 = static_cast<uint32_t>(c->seed >> 32);
   k.trial = c->trial;
+  for (int r = 0; r < 10; ++r) {
+    k.rk.a[r] = k.k0 + static_cast<uint32_t>(r) * 0x9E3779B9u;
+    k.rk.b[r] = k.k1 + static_cast<uint32_t>(r) * 0xBB67AE85u;
+  }
   return k;
 }
 

@@ -49,6 +49,26 @@ __device__ __forceinline__ uint4 philox4x32_10(uint32_t c0, uint32_t c1, uint32_
   return make_uint4(c0, c1, c2, c3);
 }
 
+// The same with the ten round keys (k0 + r W0, k1 + r W1) precomputed by the host and passed as
+// kernel parameters: each xor reads its key straight from the constant bank -- no key
+// registers, no key additions in the inner loop.
+struct PhiloxKeys { uint32_t a[10], b[10]; };
+__device__ __forceinline__ uint4 philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3,
+                                               const PhiloxKeys& rk) {
+  constexpr uint32_t M0 = 0xD2511F53u, M1 = 0xCD9E8D57u;
+#pragma unroll
+  for (int r = 0; r < 10; ++r) {
+    const uint64_t p0 = static_cast<uint64_t>(M0) * c0;
+    const uint64_t p1 = static_cast<uint64_t>(M1) * c2;
+    const uint32_t hi0 = static_cast<uint32_t>(p0 >> 32), lo0 = static_cast<uint32_t>(p0);
+    const uint32_t hi1 = static_cast<uint32_t>(p1 >> 32), lo1 = static_cast<uint32_t>(p1);
+    const uint32_t n0 = hi1 ^ c1 ^ rk.a[r];
+    const uint32_t n2 = hi0 ^ c3 ^ rk.b[r];
+    c0 = n0; c1 = lo1; c2 = n2; c3 = lo0;
+  }
+  return make_uint4(c0, c1, c2, c3);
+}
+
 // 53-bit uniform in [0,1): 27 high bits of a, 26 high bits of b (exact in double).
 __device__ __forceinline__ double u53(uint32_t a, uint32_t b) {
   const double hi = static_cast<double>(a >> 5);
@@ -111,6 +131,7 @@ template <typename R> struct ChainConst {
   R hscale;    // float modes: q Delta / 2 = hscale * float(int32 word) = (delta / 4) 2^-31 word
   R xscale;    // SP_INTRINSIC: -log2(e) / T, so that exp(-dE / T) 2^32 = ex2(dE * xscale + 32)
   uint32_t k0, k1, trial;
+  PhiloxKeys rk;   // round keys of (k0, k1)
 };
 
 // Local field from the four neighbours in the fixed order left, right, up, down; a missing
@@ -181,12 +202,12 @@ __device__ __forceinline__ void met_words_pair(uint32_t pair_site, uint32_t swee
                                                const ChainConst<typename Traits<MODE>::real>& k,
                                                MetWords* w0, MetWords* w1) {
   if constexpr (sizeof(typename Traits<MODE>::real) == 8) {
-    const uint4 r0 = philox4x32_10(pair_site, sweep, PASS_MET, k.trial, k.k0, k.k1);
-    const uint4 r1 = philox4x32_10(pair_site + 2u, sweep, PASS_MET, k.trial, k.k0, k.k1);
+    const uint4 r0 = philox4x32_10(pair_site, sweep, PASS_MET, k.trial, k.rk);
+    const uint4 r1 = philox4x32_10(pair_site + 2u, sweep, PASS_MET, k.trial, k.rk);
     *w0 = MetWords{r0.x, r0.y, r0.z, r0.w};
     *w1 = MetWords{r1.x, r1.y, r1.z, r1.w};
   } else {
-    const uint4 r = philox4x32_10(pair_site, sweep, PASS_MET, k.trial, k.k0, k.k1);
+    const uint4 r = philox4x32_10(pair_site, sweep, PASS_MET, k.trial, k.rk);
     *w0 = MetWords{r.x, 0u, r.z, 0u};
     *w1 = MetWords{r.y, 0u, r.w, 0u};
   }

@@ -100,8 +100,8 @@ __device__ __forceinline__ void tma_load_3d(void* dst, const CUtensorMap* map, u
 }
 
 template <int MODE> constexpr size_t tile_smem_bytes() {
-  return sizeof(typename Traits<MODE>::vec) * 2 * TileCfg<MODE>::TH * kTileCols   // spins
-         + 64;                                                                      // mbarrier
+  return sizeof(typename Traits<MODE>::vec) * (2 * TileCfg<MODE>::TH + 1) * kTileCols   // spins + one pad row
+         + 64;                                                                            // mbarrier
 }
 
 // Storage unit (mpr_plain.cuh): the two sites of plane columns (2m, 2m + 1) as (c_a, c_b, s_a, s_b):
@@ -118,25 +118,22 @@ template <int MODE> struct TileView {
   __device__ __forceinline__ S* unit(int pl, int r, int u) const { return base + (pl * TH + r) * kRowScalars + 4 * u; }
 };
 
-// Local fields of the two sites of a unit; `oth` points at the unit of the same row and columns in
-// the OTHER colour plane.  PAR = x-parity of the row for this colour: the left/right neighbours
-// of column j are the other plane's columns (j - 1 + PAR, j + PAR), so besides the unit itself
-// (mid) one more site is needed: column jj - 1 (PAR = 0; lane b of the previous unit) or jj + 2
-// (PAR = 1; lane a of the next unit).  At the rim of the staged region that address falls into
-// the adjacent row -- inside shared memory, and read only by sites that are stale anyway.
+// Local fields of the two sites of a unit of colour-plane row r from the other plane's units of
+// the same columns in rows r - 1 (up), r (mid), r + 1 (dn) and the one extra site `ex`.
+// par = x-parity of the row for this colour: the left/right neighbours of column j are the other
+// plane's columns (j - 1 + par, j + par), so besides mid one more site is needed: column jj - 1
+// (par = 0; lane b of the previous unit) or jj + 2 (par = 1; lane a of the next unit).
 // Sum order l, r, u, d, lanes = (site a, site b): one packed add per term in the float modes.
-template <int MODE, int PAR>
-__device__ __forceinline__ void pair_fields(const decltype(Traits<MODE>::vec::x)* oth,
-                                            Two<typename Traits<MODE>::real>* A, Two<typename Traits<MODE>::real>* B) {
+template <int MODE>
+__device__ __forceinline__ void combine_fields(int par, const Unit<decltype(Traits<MODE>::vec::x)>& up,
+                                               const Unit<decltype(Traits<MODE>::vec::x)>& mid,
+                                               const Unit<decltype(Traits<MODE>::vec::x)>& dn,
+                                               decltype(Traits<MODE>::vec::x) exc, decltype(Traits<MODE>::vec::x) exs,
+                                               Two<typename Traits<MODE>::real>* A, Two<typename Traits<MODE>::real>* B) {
   using R = typename Traits<MODE>::real;
-  using S = decltype(Traits<MODE>::vec::x);
-  const Unit<S> mid = *reinterpret_cast<const Unit<S>*>(oth);
-  const Unit<S> up = *reinterpret_cast<const Unit<S>*>(oth - kRowScalars);
-  const Unit<S> dn = *reinterpret_cast<const Unit<S>*>(oth + kRowScalars);
-  const S exc = oth[PAR ? 4 : -3], exs = oth[PAR ? 6 : -1];
   const Two<R> midc = mk2(R(mid.ca), R(mid.cb)), mids = mk2(R(mid.sa), R(mid.sb));
   Two<R> a, b;
-  if constexpr (PAR == 0) {         // a: l = ex, r = mid.a     b: l = mid.a, r = mid.b
+  if (par == 0) {                   // a: l = ex, r = mid.a     b: l = mid.a, r = mid.b
     a = add2(mk2(R(exc), R(mid.ca)), midc);
     b = add2(mk2(R(exs), R(mid.sa)), mids);
   } else {                          // a: l = mid.a, r = mid.b  b: l = mid.b, r = ex
@@ -148,53 +145,93 @@ __device__ __forceinline__ void pair_fields(const decltype(Traits<MODE>::vec::x)
   *A = a; *B = b;
 }
 
-// One colour pass (p-th pass of the launch, 1-based) over the rows of this warp.  COL, PAR and
-// KIND are compiled in: every shared-memory access is one pointer plus an immediate offset.
+// The same from shared memory (`oth` = the unit of the same row and columns in the other plane);
+// used by the energy sample, interior columns only.
+template <int MODE>
+__device__ __forceinline__ void pair_fields(int par, const decltype(Traits<MODE>::vec::x)* oth,
+                                            Two<typename Traits<MODE>::real>* A, Two<typename Traits<MODE>::real>* B) {
+  using S = decltype(Traits<MODE>::vec::x);
+  const Unit<S> mid = *reinterpret_cast<const Unit<S>*>(oth);
+  const Unit<S> up = *reinterpret_cast<const Unit<S>*>(oth - kRowScalars);
+  const Unit<S> dn = *reinterpret_cast<const Unit<S>*>(oth + kRowScalars);
+  combine_fields<MODE>(par, up, mid, dn, oth[par ? 4 : -3], oth[par ? 6 : -1], A, B);
+}
+
+// One row of a colour pass: the unit at `own` (row r, x-parity `par`) from the register window
+// (up, mid, dn) of the other plane.  The extra neighbour comes from the adjacent lane by warp
+// shuffle (wrong at lanes 0 / 31, for sites that are stale anyway).  Returns inc x accepted moves.
+template <int MODE, int KIND>
+__device__ __forceinline__ int row_step(int par, decltype(Traits<MODE>::vec::x)* own,
+                                        const Unit<decltype(Traits<MODE>::vec::x)>& up,
+                                        const Unit<decltype(Traits<MODE>::vec::x)>& mid,
+                                        const Unit<decltype(Traits<MODE>::vec::x)>& dn,
+                                        bool fa, bool fb, int inc, uint32_t pair_site, uint32_t sweep,
+                                        const ChainConst<typename Traits<MODE>::real>& kc) {
+  using R = typename Traits<MODE>::real;
+  using S = decltype(Traits<MODE>::vec::x);
+  const S exc = par ? __shfl_down_sync(0xffffffffu, mid.ca, 1) : __shfl_up_sync(0xffffffffu, mid.cb, 1);
+  const S exs = par ? __shfl_down_sync(0xffffffffu, mid.sa, 1) : __shfl_up_sync(0xffffffffu, mid.sb, 1);
+  Two<R> A, B;
+  combine_fields<MODE>(par, up, mid, dn, exc, exs, &A, &B);
+  const Unit<S> me = *reinterpret_cast<const Unit<S>*>(own);
+  const Two<R> c = mk2(R(me.ca), R(me.cb)), s = mk2(R(me.sa), R(me.sb));
+  R o[4];
+  int n = 0;
+  if constexpr (KIND == KIND_MET) {
+    MetWords w0, w1;
+    met_words_pair<MODE>(pair_site, sweep, kc, &w0, &w1);
+    bool ok[2];
+    met_update2<MODE>(c, s, A, B, w0, w1, fa, fb, kc, o, ok);
+    if (ok[0]) n += inc;
+    if (ok[1]) n += inc;
+  } else {
+    or_update2<MODE>(c, s, A, B, fa, fb, o);
+  }
+  Unit<S> out;
+  out.ca = static_cast<S>(o[0]); out.cb = static_cast<S>(o[1]);
+  out.sa = static_cast<S>(o[2]); out.sb = static_cast<S>(o[3]);
+  *reinterpret_cast<Unit<S>*>(own) = out;
+  return n;
+}
+
+// One colour pass over the RPW contiguous rows of this warp.  The other plane's rows slide through
+// a register window: each row is read from shared memory once per pass (RPW + 2 reads for RPW
+// rows instead of 3 RPW).  COL, KIND and the row parities are compile-time constants: the first
+// row of every warp has x-parity COL (y0 and RPW are even).  EVERY row is computed in every pass,
+// without a test: the rows and columns within p sites of the rim of the staged region are stale
+// after pass p whatever is done to them (they are recomputed by the neighbouring tile, never
+// stored and never counted), and leaving the tests out keeps the warp free of branches.
+// cnt = bit i set iff the CTA owns row i of this warp and this thread's columns.
 // Returns the number of accepted Metropolis moves at sites this CTA owns (its interior).
-template <int MODE, int KIND, int PAR, int COL>
-__device__ __forceinline__ int pass_rows(const TileView<MODE>& t, int p, int h, uint32_t mcol, bool col_interior,
+template <int MODE, int KIND, int COL>
+__device__ __forceinline__ int pass_rows(const TileView<MODE>& t, uint32_t mcol, uint32_t cnt,
                                          uint32_t site_row0, uint32_t L, uint32_t sweep,
                                          const ChainConst<typename Traits<MODE>::real>& kc) {
-  using R = typename Traits<MODE>::real;
   using S = decltype(Traits<MODE>::vec::x);
   constexpr int TH = TileCfg<MODE>::TH, NW = TileCfg<MODE>::NT / 32, RPW = TH / NW;
   constexpr int kOther = (COL ? -1 : 1) * TH * kRowScalars;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  // rows r = warp + NW i with p <= r < TH - p (the rest is the stale rim of the staged region)
-  const int i_lo = p > warp ? (p - warp + NW - 1) / NW : 0;
-  int i_hi = (TH - p - warp + NW - 1) / NW;
-  i_hi = i_hi > RPW ? RPW : i_hi;
-  // ... of which the CTA owns rows h <= r < TH - h
-  const int c_lo = h > warp ? (h - warp + NW - 1) / NW : 0;
-  const int c_hi = col_interior ? (TH - h - warp + NW - 1) / NW : 0;
-  S* own = t.unit(COL, warp + NW * i_lo, lane);
-  uint32_t m = mcol >> (2 * i_lo);
-  uint32_t site = site_row0 + static_cast<uint32_t>(warp + NW * i_lo) * L + static_cast<uint32_t>(PAR);
+  S* own = t.unit(COL, warp * RPW, lane);
+  // row -1 does not exist: warp 0 reads row 0 instead (used by row 0 only, which is always stale);
+  // row TH of plane 1 is the pad row behind the tile
+  Unit<S> up = *reinterpret_cast<const Unit<S>*>(own + kOther - (warp > 0 ? kRowScalars : 0));
+  Unit<S> mid = *reinterpret_cast<const Unit<S>*>(own + kOther);
+  const uint32_t site = site_row0 + static_cast<uint32_t>(warp * RPW) * L;
   int n_acc = 0;
-#pragma unroll 1
-  for (int i = i_lo; i < i_hi; ++i) {
-    Two<R> A, B;
-    pair_fields<MODE, PAR>(own + kOther, &A, &B);
-    const Unit<S> me = *reinterpret_cast<const Unit<S>*>(own);
-    const Two<R> c = mk2(R(me.ca), R(me.cb)), s = mk2(R(me.sa), R(me.sb));
-    const bool fa = m & 1u, fb = m & 2u;
-    R o[4];
-    if constexpr (KIND == KIND_MET) {
-      MetWords w0, w1;
-      met_words_pair<MODE>(site, sweep, kc, &w0, &w1);
-      bool ok[2];
-      met_update2<MODE>(c, s, A, B, w0, w1, fa, fb, kc, o, ok);
-      if (i >= c_lo && i < c_hi) n_acc += static_cast<int>(ok[0]) + static_cast<int>(ok[1]);
-    } else {
-      or_update2<MODE>(c, s, A, B, fa, fb, o);
-    }
-    Unit<S> out;
-    out.ca = static_cast<S>(o[0]); out.cb = static_cast<S>(o[1]);
-    out.sa = static_cast<S>(o[2]); out.sb = static_cast<S>(o[3]);
-    *reinterpret_cast<Unit<S>*>(own) = out;
-    own += NW * kRowScalars;
-    m >>= 2;
-    site += static_cast<uint32_t>(NW) * L;
+  // keeps the bit tests where they are used (hoisted out of the sweep loop they cost 24 registers)
+  asm volatile("" : "+r"(mcol), "+r"(cnt));
+  // float arithmetic: fully unrolled (the window rotation is register renaming); double arithmetic:
+  // two rows per iteration, which keeps the parities constant and the code within the registers
+  constexpr int kUnroll = sizeof(typename Traits<MODE>::real) == 8 ? 2 : RPW;
+#pragma unroll kUnroll
+  for (int i = 0; i < RPW; ++i) {
+    const int par = (COL + i) & 1;
+    const Unit<S> dn = *reinterpret_cast<const Unit<S>*>(own + kOther + (i + 1) * kRowScalars);
+    n_acc += row_step<MODE, KIND>(par, own + i * kRowScalars, up, mid, dn, (mcol >> (2 * i)) & 1u,
+                                  (mcol >> (2 * i + 1)) & 1u, (cnt >> i) & 1u,
+                                  site + static_cast<uint32_t>(i) * L + static_cast<uint32_t>(par), sweep, kc);
+    up = mid;
+    mid = dn;
   }
   return n_acc;
 }
@@ -208,11 +245,12 @@ tiled_sweep_kernel(const __grid_constant__ CUtensorMap tmap, typename Traits<MOD
   using R = typename Traits<MODE>::real;
   using V = typename Traits<MODE>::vec;
   constexpr int TH = TileCfg<MODE>::TH, NT = TileCfg<MODE>::NT, NW = NT / 32, RPW = TH / NW;
-  static_assert(TH % NW == 0 && NW % 2 == 0 && RPW * 2 <= 32, "row ownership / mask register layout");
+  static_assert(TH % NW == 0 && RPW % 2 == 0 && RPW * 2 <= 32, "row ownership / mask register layout");
+  static_assert(TH % 2 == 0, "y0 = ty (TH - 8 k) - 4 k must be even: the first row of a warp has x-parity = colour");
   extern __shared__ __align__(128) unsigned char smem_raw[];
   using S = decltype(V::x);
   TileView<MODE> t{reinterpret_cast<S*>(smem_raw)};
-  uint64_t* bar = reinterpret_cast<uint64_t*>(smem_raw + sizeof(V) * 2 * TH * kTileCols);
+  uint64_t* bar = reinterpret_cast<uint64_t*>(smem_raw + sizeof(V) * (2 * TH + 1) * kTileCols);
   __shared__ double red[32];
 
   const int h = 4 * nsweeps, hc = 2 * nsweeps;
@@ -228,7 +266,7 @@ tiled_sweep_kernel(const __grid_constant__ CUtensorMap tmap, typename Traits<MOD
     tma_load_3d(t.base, &tmap, bar, 2 * j0, y0, 0);
   }
   // mask bits of this thread's sites, one register per colour: bit 2 i + {0, 1} of mreg[col] = site
-  // (row warp + NW i, colour col, column jj + {0, 1}) is a prediction site.  (j0 + jj) is even, so
+  // (row warp RPW + i, colour col, column jj + {0, 1}) is a prediction site.  (j0 + jj) is even, so
   // both bits sit in one word of the bitmap.
   uint32_t mreg[2] = {0u, 0u};
   {
@@ -238,7 +276,7 @@ tiled_sweep_kernel(const __grid_constant__ CUtensorMap tmap, typename Traits<MOD
       const uint32_t* b0 = bits + wi;
 #pragma unroll
       for (int i = 0; i < RPW; ++i) {
-        const int y = y0 + warp + NW * i;
+        const int y = y0 + warp * RPW + i;
         if (y >= 0 && y < g.L) {
           const uint32_t* bp = b0 + static_cast<size_t>(y) * g.Wm;
           mreg[0] |= ((__ldg(bp) >> sh) & 3u) << (2 * i);
@@ -254,31 +292,27 @@ tiled_sweep_kernel(const __grid_constant__ CUtensorMap tmap, typename Traits<MOD
   __syncthreads();          // mbarrier initialised before anyone polls it
   mbar_wait(bar, 0);
 
+  // rows and columns this CTA owns (for the accepted-move count)
+  uint32_t cnt = 0;
+  if (col_interior) {
+#pragma unroll
+    for (int i = 0; i < RPW; ++i) {
+      const int r = warp * RPW + i;
+      if (r >= h && r < TH - h) cnt |= 1u << i;
+    }
+  }
   int n_acc = 0;
-  const int par0 = (y0 + warp) & 1;               // x-parity of this warp's rows for colour 0 (NW is even)
 #pragma unroll 1
   for (int sw = 0; sw < nsweeps; ++sw) {
     const uint32_t sweep = first_sweep + static_cast<uint32_t>(sw);
-    const int p = 4 * sw;
-    if (par0) {
-      n_acc += pass_rows<MODE, KIND_MET, 1, 0>(t, p + 1, h, mreg[0], col_interior, site_row0, Lu, sweep, kc);
-      __syncthreads();
-      n_acc += pass_rows<MODE, KIND_MET, 0, 1>(t, p + 2, h, mreg[1], col_interior, site_row0, Lu, sweep, kc);
-      __syncthreads();
-      pass_rows<MODE, KIND_OR, 1, 0>(t, p + 3, h, mreg[0], col_interior, site_row0, Lu, sweep, kc);
-      __syncthreads();
-      pass_rows<MODE, KIND_OR, 0, 1>(t, p + 4, h, mreg[1], col_interior, site_row0, Lu, sweep, kc);
-      __syncthreads();
-    } else {
-      n_acc += pass_rows<MODE, KIND_MET, 0, 0>(t, p + 1, h, mreg[0], col_interior, site_row0, Lu, sweep, kc);
-      __syncthreads();
-      n_acc += pass_rows<MODE, KIND_MET, 1, 1>(t, p + 2, h, mreg[1], col_interior, site_row0, Lu, sweep, kc);
-      __syncthreads();
-      pass_rows<MODE, KIND_OR, 0, 0>(t, p + 3, h, mreg[0], col_interior, site_row0, Lu, sweep, kc);
-      __syncthreads();
-      pass_rows<MODE, KIND_OR, 1, 1>(t, p + 4, h, mreg[1], col_interior, site_row0, Lu, sweep, kc);
-      __syncthreads();
-    }
+    n_acc += pass_rows<MODE, KIND_MET, 0>(t, mreg[0], cnt, site_row0, Lu, sweep, kc);
+    __syncthreads();
+    n_acc += pass_rows<MODE, KIND_MET, 1>(t, mreg[1], cnt, site_row0, Lu, sweep, kc);
+    __syncthreads();
+    pass_rows<MODE, KIND_OR, 0>(t, mreg[0], cnt, site_row0, Lu, sweep, kc);
+    __syncthreads();
+    pass_rows<MODE, KIND_OR, 1>(t, mreg[1], cnt, site_row0, Lu, sweep, kc);
+    __syncthreads();
   }
 
   // interior -> other state buffer (+ energy sample and accumulation of phi when measuring)
@@ -287,7 +321,7 @@ tiled_sweep_kernel(const __grid_constant__ CUtensorMap tmap, typename Traits<MOD
   if (col_interior && j < g.Wp) {
 #pragma unroll 1
     for (int i = 0; i < RPW; ++i) {
-      const int r = warp + NW * i;
+      const int r = warp * RPW + i;
       const int y = y0 + r;
       if (r < h || r >= TH - h || y >= g.L) continue;
 #pragma unroll
@@ -298,8 +332,7 @@ tiled_sweep_kernel(const __grid_constant__ CUtensorMap tmap, typename Traits<MOD
         if constexpr (MEASURE) {
           if (pl == 1) {   // every bond has exactly one colour-1 end: H = -J sum over colour-1 sites of u.F
             Two<R> A, B;
-            if ((y + 1) & 1) pair_fields<MODE, 1>(t.unit(0, r, lane), &A, &B);
-            else             pair_fields<MODE, 0>(t.unit(0, r, lane), &A, &B);
+            pair_fields<MODE>((y + 1) & 1, t.unit(0, r, lane), &A, &B);
             R Aa, Ab, Ba, Bb;
             un2(A, &Aa, &Ab); un2(B, &Ba, &Bb);
             esum += static_cast<double>(fma_(R(me.ca), Aa, R(me.sa) * Ba));
