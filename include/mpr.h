@@ -81,7 +81,11 @@ int mpr_workspace_bytes(int L, size_t* bytes);
  *   cuda_stream         a cudaStream_t (0 = default stream)
  * Does R1 (z_min, z_max over the measured sample, phi = 2pi (z - z_min)/(z_max - z_min)),
  * the sample energy of R6 (e_s over measured nearest-neighbour pairs), packs the mask into
- * per-colour bitmaps, selects MPR_DP, seed 0, and resets the chain (R8).
+ * per-colour bitmaps, selects MPR_DP, seed 0, and resets the chain (R8).  "Resets the chain"
+ * here and in the setters below means: the chain is marked for re-initialisation (uniform
+ * spins + quench passes, trial 0), which runs once, on the stream, when the chain is next
+ * used (run, sweep, pass, get/set_state, energy, counters) -- create + set_precision +
+ * set_seed costs one initialisation, not three.
  * Fails with INVALID_ARG, WORKSPACE, NO_MEASURED, DEGENERATE_RANGE, NONFINITE or CUDA;
  * *out is null on failure.                                                                 */
 int mpr_create(mpr_ctx** out, int L, const double* d_values, const uint8_t* d_mask,

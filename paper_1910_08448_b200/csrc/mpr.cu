@@ -42,13 +42,15 @@ Layout make_layout(int L) {
   lo.g.L = L;
   lo.g.Wp = static_cast<int>(align_up(static_cast<size_t>((L + 1) / 2), 16));
   lo.g.Wm = (lo.g.Wp + 31) / 32;
+  lo.g.Wb = lo.g.Wm + kBitPadLeft + kBitPadRight;
+  lo.g.Hb = L + kBitPadTop + kBitPadBot;
   lo.g.plane = static_cast<size_t>(L) * lo.g.Wp;
   size_t o = 0;
   const size_t state_bytes = 2 * lo.g.plane * sizeof(double2);
   lo.off_state[0] = o; o = align_up(o + state_bytes, 256);
   lo.off_state[1] = o; o = align_up(o + state_bytes, 256);
   lo.off_acc = o;      o = align_up(o + 2 * lo.g.plane * sizeof(double), 256);
-  lo.off_bits = o;     o = align_up(o + static_cast<size_t>(2) * L * lo.g.Wm * sizeof(uint32_t), 256);
+  lo.off_bits = o;     o = align_up(o + static_cast<size_t>(2) * lo.g.Hb * lo.g.Wb * sizeof(uint32_t), 256);
   lo.off_part = o;     o = align_up(o + kPartials * sizeof(double), 256);
   lo.off_series = o;   o = align_up(o + kSeriesCap * sizeof(double), 256);
   lo.off_slots = o;    o = align_up(o + kAcceptSlots * sizeof(unsigned long long), 256);
@@ -82,12 +84,15 @@ struct mpr_ctx {
   long long n_free = 0;
   uint64_t launches = 0;
   std::vector<double> series;
+  bool stale = true;     // the chain has to be (re)initialised before its next use (ensure_chain)
   std::string err;
   TiledPlan tiled;
 
   void* state(int b) const { return ws + lo.off_state[b]; }
   double* acc() const { return reinterpret_cast<double*>(ws + lo.off_acc); }
-  uint32_t* bits() const { return reinterpret_cast<uint32_t*>(ws + lo.off_bits); }
+  uint32_t* bits_base() const { return reinterpret_cast<uint32_t*>(ws + lo.off_bits); }
+  // word 0 of row 0 of colour 0 inside the padded bitmaps (mpr_plain.cuh)
+  uint32_t* bits() const { return bits_base() + static_cast<size_t>(kBitPadTop) * lo.g.Wb + kBitPadLeft; }
   double* part() const { return reinterpret_cast<double*>(ws + lo.off_part); }
   double* dseries() const { return reinterpret_cast<double*>(ws + lo.off_series); }
   unsigned long long* slots() const { return reinterpret_cast<unsigned long long*>(ws + lo.off_slots); }
@@ -313,6 +318,7 @@ int do_tiled(mpr_ctx* c, int k, bool measure, double* d_e) {
 // R8: uniform initial spins, then n_quench x (quench colour 0, quench colour 1); everything
 // that belongs to the chain is cleared.
 int reset_chain(mpr_ctx* c, uint32_t trial) {
+  c->stale = false;
   c->trial = trial;
   c->sweep = 0;
   c->attempted = 0;
@@ -330,11 +336,24 @@ int reset_chain(mpr_ctx* c, uint32_t trial) {
   return MPR_OK;
 }
 
+// Setters only mark the chain stale; the reset (init + quench passes, R8) runs once, when the
+// chain is next used -- mpr_create followed by mpr_set_precision pays for one reset, not two.
+void mark_stale(mpr_ctx* c) {
+  c->stale = true;
+  c->trial = 0;
+  c->sweep = 0;
+  c->attempted = 0;
+  c->n_acc = 0;
+  c->series.clear();
+}
+int ensure_chain(mpr_ctx* c) { return c->stale ? reset_chain(c, 0) : MPR_OK; }
+
 // n hybrid sweeps (R4); with `measure`, each is followed by the energy sample into
 // dseries[first_slot + i] and the accumulation of phi.
 int hybrid_sweeps(mpr_ctx* c, int n, bool measure, int first_slot) {
   if (n <= 0) return MPR_OK;
   if (!(c->T > 0.0)) return fail(c, MPR_ERR_NOT_READY, "temperature not set");
+  TRY(ensure_chain(c));
   if (c->path == MPR_PATH_PLAIN) {
     for (int i = 0; i < n; ++i) {
       const uint64_t sw = c->sweep + 1;
@@ -408,11 +427,11 @@ int setup(mpr_ctx* c) {
   pair_final_kernel<<<1, 32, 0, c->stream>>>(c->part(), nblk, c->scal());
   LAUNCH_OK(c);
   // mask bitmaps and the number of prediction sites
-  const size_t nwords = static_cast<size_t>(2) * g.L * g.Wm;
+  const size_t nwords = static_cast<size_t>(2) * g.Hb * g.Wb;
   const int mblk = static_cast<int>((nwords + 255) / 256);
   if (mblk > kPartials) return fail(c, MPR_ERR_INVALID_ARG, "grid too large");
   double* cnt_part = c->part() + 2 * nblk;
-  pack_mask_kernel<<<mblk, 256, 0, c->stream>>>(c->d_mask, g, c->bits(), cnt_part);
+  pack_mask_kernel<<<mblk, 256, 0, c->stream>>>(c->d_mask, g, c->bits_base(), cnt_part);
   LAUNCH_OK(c);
   final_sum_kernel<<<1, 1024, 0, c->stream>>>(cnt_part, mblk, 1.0, c->scal() + 2);
   LAUNCH_OK(c);
@@ -475,7 +494,7 @@ int mpr_create(mpr_ctx** out, int L, const double* d_values, const uint8_t* d_ma
     const int ts = tiled_plan_init(&c->tiled, c->lo.g);
     if (ts != 0) st = fail(c, MPR_ERR_CUDA, std::string("tiled plan: ") + tiled_error(ts));
   }
-  if (st == MPR_OK) st = reset_chain(c, 0);
+  if (st == MPR_OK) mark_stale(c);
   if (st != MPR_OK) { delete c; return st; }
   *out = c;
   return MPR_OK;
@@ -486,12 +505,14 @@ void mpr_destroy(mpr_ctx* ctx) { delete ctx; }
 int mpr_set_precision(mpr_ctx* c, mpr_precision mode) {
   if (!c || mode < MPR_DP || mode > MPR_SP_INTRINSIC) return fail(c, MPR_ERR_INVALID_ARG, "bad mode");
   c->mode = mode;
-  return reset_chain(c, 0);
+  mark_stale(c);
+  return MPR_OK;
 }
 int mpr_set_seed(mpr_ctx* c, uint64_t seed) {
   if (!c) return MPR_ERR_INVALID_ARG;
   c->seed = seed;
-  return reset_chain(c, 0);
+  mark_stale(c);
+  return MPR_OK;
 }
 int mpr_set_temperature(mpr_ctx* c, double T) {
   if (!c || !(T > 0.0) || !std::isfinite(T)) return fail(c, MPR_ERR_INVALID_ARG, "T must be finite and > 0");
@@ -501,7 +522,8 @@ int mpr_set_temperature(mpr_ctx* c, double T) {
 int mpr_set_quench(mpr_ctx* c, int n) {
   if (!c || n < 0) return fail(c, MPR_ERR_INVALID_ARG, "n_quench < 0");
   c->n_quench = n;
-  return reset_chain(c, 0);
+  mark_stale(c);
+  return MPR_OK;
 }
 int mpr_set_path(mpr_ctx* c, mpr_path path) {
   if (!c || (path != MPR_PATH_TILED && path != MPR_PATH_PLAIN)) return fail(c, MPR_ERR_INVALID_ARG, "bad path");
@@ -581,12 +603,14 @@ int mpr_sweep(mpr_ctx* c, int n) {
 int mpr_pass(mpr_ctx* c, int kind, int colour, uint64_t sweep) {
   if (!c || kind < 0 || kind > 2) return fail(c, MPR_ERR_INVALID_ARG, "bad pass kind");
   if (kind == KIND_MET && !(c->T > 0.0)) return fail(c, MPR_ERR_NOT_READY, "temperature not set");
+  TRY(ensure_chain(c));
   return do_pass(c, kind, colour & 1, sweep);
 }
 
 int mpr_run(mpr_ctx* c, int n_eq, int n_meas, double* d_pred, double* e_mean, double* e_stderr) {
   if (!c || n_eq < 0 || n_meas < 0 || n_meas > kSeriesCap) return fail(c, MPR_ERR_INVALID_ARG, "bad sweep counts");
   if (!(c->T > 0.0)) return fail(c, MPR_ERR_NOT_READY, "temperature not set");
+  TRY(ensure_chain(c));
   TRY(hybrid_sweeps(c, n_eq, false, 0));
   TRY(hybrid_sweeps(c, n_meas, true, 0));
   if (d_pred) {
@@ -603,6 +627,7 @@ int mpr_run(mpr_ctx* c, int n_eq, int n_meas, double* d_pred, double* e_mean, do
 
 int mpr_get_state(mpr_ctx* c, double* d_phi) {
   if (!c || !d_phi) return fail(c, MPR_ERR_INVALID_ARG, "null pointer");
+  TRY(ensure_chain(c));
   switch (c->mode) {
     case MPR_DP: return get_state<MODE_DP>(c, d_phi);
     case MPR_SP: return get_state<MODE_SP>(c, d_phi);
@@ -612,6 +637,7 @@ int mpr_get_state(mpr_ctx* c, double* d_phi) {
 }
 int mpr_set_state(mpr_ctx* c, const double* d_phi) {
   if (!c || !d_phi) return fail(c, MPR_ERR_INVALID_ARG, "null pointer");
+  TRY(ensure_chain(c));
   switch (c->mode) {
     case MPR_DP: return set_state<MODE_DP>(c, d_phi);
     case MPR_SP: return set_state<MODE_SP>(c, d_phi);
@@ -622,6 +648,7 @@ int mpr_set_state(mpr_ctx* c, const double* d_phi) {
 
 int mpr_energy(mpr_ctx* c, double* H, double* e) {
   if (!c) return MPR_ERR_INVALID_ARG;
+  TRY(ensure_chain(c));
   TRY(do_energy(c, c->scal() + 8, false));
   double h = 0.0;
   CUDA_OK(c, cudaMemcpyAsync(&h, c->scal() + 8, sizeof(double), cudaMemcpyDeviceToHost, c->stream));
@@ -642,6 +669,7 @@ int mpr_sample_energy(mpr_ctx* c, double* e_sample, int64_t* n_pairs) {
 
 int mpr_get_counters(mpr_ctx* c, uint64_t* accepted, uint64_t* attempted, uint64_t* sweeps) {
   if (!c) return MPR_ERR_INVALID_ARG;
+  TRY(ensure_chain(c));
   unsigned long long h[kAcceptSlots];
   CUDA_OK(c, cudaMemcpyAsync(h, c->slots(), sizeof(h), cudaMemcpyDeviceToHost, c->stream));
   CUDA_OK(c, cudaStreamSynchronize(c->stream));

@@ -192,7 +192,7 @@ template <typename R> __device__ __forceinline__ Two<R> bc2(R k) { return mk2(k,
 
 // Random words of the Metropolis move at a site (R9).  Double-arithmetic modes (DP, SP): one
 // Philox block per site, counter word 0 = the site's row-major index; all four words are used
-// (two 53-bit uniforms), exactly as in the oracle.  Float-arithmetic modes: one block per PAIR of
+// (two 53-bit uniforms): the R9 reading in full.  Float-arithmetic modes: one block per PAIR of
 // sites of the same colour and row whose plane columns are (2m, 2m + 1); counter word 0 = the index
 // of the first site of the pair (pair_site); that site takes words (0, 2), the other one (1, 3).
 struct MetWords { uint32_t p, q, a, b; };   // proposal (p [, q]) and acceptance (a [, b]) words

@@ -17,11 +17,22 @@ namespace mpr {
 
 struct Geom {
   int L, Wp, Wm;
+  int Wb, Hb;            // padded bitmap: words per row, rows per colour
   size_t plane;          // elements per colour plane = L * Wp
 };
 
+// The mask bitmaps are padded with zero words (kBitPadTop rows above, kBitPadBot below, kBitPadLeft
+// words to the left, kBitPadRight to the right of every row), so that the tiled kernel can read
+// the words of a whole staged region -- halo and out-of-grid part included -- without a bounds
+// test.  `bits` always points at word 0 of row 0 of colour 0 INSIDE the padded array.
+constexpr int kBitPadTop = 16, kBitPadBot = 96, kBitPadLeft = 1, kBitPadRight = 3;
+
+__device__ __forceinline__ const uint32_t* mask_word(const uint32_t* __restrict__ bits, const Geom& g, int col, int y,
+                                                     int wi) {
+  return bits + (static_cast<long long>(col) * g.Hb + y) * g.Wb + wi;
+}
 __device__ __forceinline__ bool mask_bit(const uint32_t* __restrict__ bits, const Geom& g, int col, int y, int j) {
-  return (bits[(static_cast<size_t>(col) * g.L + y) * g.Wm + (j >> 5)] >> (j & 31)) & 1u;
+  return (*mask_word(bits, g, col, y, j >> 5) >> (j & 31)) & 1u;
 }
 
 // ---- pair-interleaved spin storage -----------------------------------------------------------
@@ -139,24 +150,27 @@ __global__ void pair_final_kernel(const double* __restrict__ part, int nblocks, 
   out[0] = s; out[1] = c;
 }
 
-// Mask bitmaps: one thread per 32-bit word; per-block partial = number of set bits.
-__global__ void pack_mask_kernel(const uint8_t* __restrict__ mask, Geom g, uint32_t* __restrict__ bits,
+// Mask bitmaps: one thread per 32-bit word of the PADDED arrays (`base` = their first word);
+// per-block partial = number of set bits.
+__global__ void pack_mask_kernel(const uint8_t* __restrict__ mask, Geom g, uint32_t* __restrict__ base,
                                  double* __restrict__ part) {
   __shared__ double sh[32];
-  const size_t nwords = static_cast<size_t>(2) * g.L * g.Wm;
+  const size_t nwords = static_cast<size_t>(2) * g.Hb * g.Wb;
   const size_t w = blockIdx.x * static_cast<size_t>(blockDim.x) + threadIdx.x;
   double cnt = 0.0;
   if (w < nwords) {
-    const int wi = static_cast<int>(w % g.Wm);
-    const size_t row = w / g.Wm;
-    const int y = static_cast<int>(row % g.L), col = static_cast<int>(row / g.L);
-    const int par = x_parity(y, col);
+    const int wi = static_cast<int>(w % g.Wb) - kBitPadLeft;
+    const size_t row = w / g.Wb;
+    const int y = static_cast<int>(row % g.Hb) - kBitPadTop, col = static_cast<int>(row / g.Hb);
     uint32_t word = 0;
-    for (int b = 0; b < 32; ++b) {
-      const int x = 2 * (32 * wi + b) + par;
-      if (x < g.L && mask[static_cast<size_t>(y) * g.L + x]) word |= (1u << b);
+    if (y >= 0 && y < g.L && wi >= 0 && wi < g.Wm) {
+      const int par = x_parity(y, col);
+      for (int b = 0; b < 32; ++b) {
+        const int x = 2 * (32 * wi + b) + par;
+        if (x < g.L && mask[static_cast<size_t>(y) * g.L + x]) word |= (1u << b);
+      }
     }
-    bits[w] = word;
+    base[w] = word;
     cnt = static_cast<double>(__popc(word));
   }
   const double s = block_sum(cnt, sh);

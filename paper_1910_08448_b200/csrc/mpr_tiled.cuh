@@ -270,19 +270,16 @@ tiled_sweep_kernel(const __grid_constant__ CUtensorMap tmap, typename Traits<MOD
   // both bits sit in one word of the bitmap.
   uint32_t mreg[2] = {0u, 0u};
   {
+    // the bitmaps are padded with zero words: no bounds test (mpr_plain.cuh)
     const int j = j0 + jj;
-    const int wi = j >> 5, sh = j & 31;
-    if (wi >= 0 && wi < g.Wm) {
-      const uint32_t* b0 = bits + wi;
+    const int sh = j & 31;
+    const uint32_t* bp = mask_word(bits, g, 0, y0 + warp * RPW, j >> 5);
+    const size_t colour = static_cast<size_t>(g.Hb) * g.Wb;
 #pragma unroll
-      for (int i = 0; i < RPW; ++i) {
-        const int y = y0 + warp * RPW + i;
-        if (y >= 0 && y < g.L) {
-          const uint32_t* bp = b0 + static_cast<size_t>(y) * g.Wm;
-          mreg[0] |= ((__ldg(bp) >> sh) & 3u) << (2 * i);
-          mreg[1] |= ((__ldg(bp + static_cast<size_t>(g.L) * g.Wm) >> sh) & 3u) << (2 * i);
-        }
-      }
+    for (int i = 0; i < RPW; ++i) {
+      mreg[0] |= ((__ldg(bp) >> sh) & 3u) << (2 * i);
+      mreg[1] |= ((__ldg(bp + colour) >> sh) & 3u) << (2 * i);
+      bp += g.Wb;
     }
   }
   const bool col_interior = jj >= hc && jj < kTileCols - hc;
@@ -315,35 +312,47 @@ tiled_sweep_kernel(const __grid_constant__ CUtensorMap tmap, typename Traits<MOD
     __syncthreads();
   }
 
-  // interior -> other state buffer (+ energy sample and accumulation of phi when measuring)
+  // interior -> other state buffer (+ energy sample and accumulation of phi when measuring).
+  // cnt already says which rows of this warp and whether this thread's columns are owned; what
+  // is left is the edge of the grid (rows >= L, plane columns >= Wp).  Unrolled: one pointer each
+  // for shared and global memory plus immediate / strided offsets.
   double esum = 0.0;
-  const int j = j0 + jj;
-  if (col_interior && j < g.Wp) {
-#pragma unroll 1
+  {
+    const int j = j0 + jj;                                        // even
+    const int row0 = y0 + warp * RPW;
+    const int nrows = g.L - row0;                                 // rows i < nrows lie in the grid
+    const uint32_t own_rows = j < g.Wp ? cnt : 0u;
+    const long long g0 = static_cast<long long>(row0) * g.Wp + j; // never dereferenced for rows outside
+    S* gp = reinterpret_cast<S*>(dst) + 2 * g0;
+    const S* sp = t.unit(0, warp * RPW, lane);
+    const size_t grow = 2 * static_cast<size_t>(g.Wp), gplane = 2 * g.plane;
+    constexpr int kEpiUnroll = MEASURE ? 1 : RPW;   // the measuring variant carries two atan2 per unit: keep it rolled
+#pragma unroll kEpiUnroll
     for (int i = 0; i < RPW; ++i) {
-      const int r = warp * RPW + i;
-      const int y = y0 + r;
-      if (r < h || r >= TH - h || y >= g.L) continue;
-#pragma unroll
-      for (int pl = 0; pl < 2; ++pl) {
-        const Unit<S> me = *reinterpret_cast<const Unit<S>*>(t.unit(pl, r, lane));
-        const size_t gi = static_cast<size_t>(pl) * g.plane + static_cast<size_t>(y) * g.Wp + j;   // j is even
-        *reinterpret_cast<Unit<S>*>(reinterpret_cast<S*>(dst) + 2 * gi) = me;
+      if (((own_rows >> i) & 1u) && i < nrows) {
+        const Unit<S> u0 = *reinterpret_cast<const Unit<S>*>(sp + i * kRowScalars);
+        const Unit<S> u1 = *reinterpret_cast<const Unit<S>*>(sp + (TH + i) * kRowScalars);
+        *reinterpret_cast<Unit<S>*>(gp + i * grow) = u0;
+        *reinterpret_cast<Unit<S>*>(gp + i * grow + gplane) = u1;
         if constexpr (MEASURE) {
-          if (pl == 1) {   // every bond has exactly one colour-1 end: H = -J sum over colour-1 sites of u.F
-            Two<R> A, B;
-            pair_fields<MODE>((y + 1) & 1, t.unit(0, r, lane), &A, &B);
-            R Aa, Ab, Ba, Bb;
-            un2(A, &Aa, &Ab); un2(B, &Ba, &Bb);
-            esum += static_cast<double>(fma_(R(me.ca), Aa, R(me.sa) * Ba));
-            esum += static_cast<double>(fma_(R(me.cb), Ab, R(me.sb) * Bb));
-          }
-          const uint32_t mm = (mreg[pl] >> (2 * i)) & 3u;
-          if (mm) {
-            double2 a2 = *reinterpret_cast<const double2*>(acc + gi);
-            if (mm & 1u) a2.x += spin_angle<MODE>(R(me.ca), R(me.sa));
-            if (mm & 2u) a2.y += spin_angle<MODE>(R(me.cb), R(me.sb));
-            *reinterpret_cast<double2*>(acc + gi) = a2;
+          // every bond has exactly one colour-1 end: H = -J sum over colour-1 sites of u.F
+          Two<R> A, B;
+          pair_fields<MODE>((row0 + i + 1) & 1, sp + i * kRowScalars, &A, &B);
+          R Aa, Ab, Ba, Bb;
+          un2(A, &Aa, &Ab); un2(B, &Ba, &Bb);
+          esum += static_cast<double>(fma_(R(u1.ca), Aa, R(u1.sa) * Ba));
+          esum += static_cast<double>(fma_(R(u1.cb), Ab, R(u1.sb) * Bb));
+#pragma unroll
+          for (int pl = 0; pl < 2; ++pl) {
+            const Unit<S>& me = pl ? u1 : u0;
+            const uint32_t mm = (mreg[pl] >> (2 * i)) & 3u;
+            if (mm) {
+              double* ap = acc + (g0 + static_cast<long long>(i) * g.Wp + static_cast<long long>(pl) * g.plane);
+              double2 a2 = *reinterpret_cast<const double2*>(ap);
+              if (mm & 1u) a2.x += spin_angle<MODE>(R(me.ca), R(me.sa));
+              if (mm & 2u) a2.y += spin_angle<MODE>(R(me.cb), R(me.sb));
+              *reinterpret_cast<double2*>(ap) = a2;
+            }
           }
         }
       }
