@@ -250,7 +250,7 @@ template <int MODE> int set_state(mpr_ctx* c, const double* d_phi) {
 
 // k hybrid sweeps of the tiled path (k <= fused depth), with the energy sample and the
 // accumulation of phi after the last one when `measure`; d_e receives e_n.
-template <int MODE> int tiled_sweeps(mpr_ctx* c, int k, bool measure, double* d_e) {
+template <int MODE> int tiled_sweeps(mpr_ctx* c, int k, int measure, double* d_e) {
   using R = typename Traits<MODE>::real;
   const Geom& g = c->lo.g;
   int ntiles = 0;
@@ -260,7 +260,7 @@ template <int MODE> int tiled_sweeps(mpr_ctx* c, int k, bool measure, double* d_
   if (st != 0) return fail(c, MPR_ERR_CUDA, std::string("tiled launch: ") + tiled_error(st));
   c->launches += 1;
   c->cur = 1 - c->cur;
-  if (measure) {
+  if (measure == 1 || measure == 2) {
     const double nb = 2.0 * g.L * (g.L - 1.0);
     final_sum_kernel<<<1, 1024, 0, c->stream>>>(c->part(), ntiles, -kJ * 2.0 / nb, d_e);
     LAUNCH_OK(c);
@@ -306,7 +306,7 @@ int do_accumulate(mpr_ctx* c) {
     default: return plain_accumulate<MODE_SP_INTRINSIC>(c);
   }
 }
-int do_tiled(mpr_ctx* c, int k, bool measure, double* d_e) {
+int do_tiled(mpr_ctx* c, int k, int measure, double* d_e) {
   switch (c->mode) {
     case MPR_DP: return tiled_sweeps<MODE_DP>(c, k, measure, d_e);
     case MPR_SP: return tiled_sweeps<MODE_SP>(c, k, measure, d_e);
@@ -325,7 +325,17 @@ int reset_chain(mpr_ctx* c, uint32_t trial) {
   c->n_acc = 0;
   c->series.clear();
   TRY(do_init(c));
-  for (int k = 0; k < c->n_quench; ++k) {
+  // quench double passes (colour 0, colour 1): the tiled kernel runs them 2 k at a time (k <= 2,
+  // halo 4 k), an odd remainder goes through the plain kernels -- same moves, same order
+  int left = c->n_quench;
+  if (c->path == MPR_PATH_TILED) {
+    while (left >= 2) {
+      const int k = left / 2 < 2 ? left / 2 : 2;
+      TRY(do_tiled(c, k, kTiledQuench, nullptr));
+      left -= 2 * k;
+    }
+  }
+  for (; left > 0; --left) {
     TRY(do_pass(c, KIND_QUENCH, 0, 0));
     TRY(do_pass(c, KIND_QUENCH, 1, 0));
   }
@@ -348,9 +358,10 @@ void mark_stale(mpr_ctx* c) {
 }
 int ensure_chain(mpr_ctx* c) { return c->stale ? reset_chain(c, 0) : MPR_OK; }
 
+// measure: 0 = sweeps only, 1 = + energy sample per sweep, 2 = + accumulation of phi.
 // n hybrid sweeps (R4); with `measure`, each is followed by the energy sample into
 // dseries[first_slot + i] and the accumulation of phi.
-int hybrid_sweeps(mpr_ctx* c, int n, bool measure, int first_slot) {
+int hybrid_sweeps(mpr_ctx* c, int n, int measure, int first_slot) {
   if (n <= 0) return MPR_OK;
   if (!(c->T > 0.0)) return fail(c, MPR_ERR_NOT_READY, "temperature not set");
   TRY(ensure_chain(c));
@@ -365,8 +376,10 @@ int hybrid_sweeps(mpr_ctx* c, int n, bool measure, int first_slot) {
       c->attempted += static_cast<uint64_t>(c->n_free);
       if (measure) {
         TRY(do_energy(c, c->dseries() + first_slot + i, true));
-        TRY(do_accumulate(c));
-        c->n_acc += 1;
+        if (measure == 2) {
+          TRY(do_accumulate(c));
+          c->n_acc += 1;
+        }
       }
     }
     return MPR_OK;
@@ -378,7 +391,7 @@ int hybrid_sweeps(mpr_ctx* c, int n, bool measure, int first_slot) {
     TRY(do_tiled(c, k, measure, measure ? c->dseries() + first_slot + done : nullptr));
     c->sweep += static_cast<uint64_t>(k);
     c->attempted += static_cast<uint64_t>(k) * static_cast<uint64_t>(c->n_free);
-    if (measure) c->n_acc += 1;
+    if (measure == 2) c->n_acc += 1;
     done += k;
   }
   return MPR_OK;
@@ -397,8 +410,8 @@ int trial_energy(mpr_ctx* c, int* est_trials, double T, double* e, double* se) {
   *est_trials += 1;
   c->T = T;
   TRY(reset_chain(c, static_cast<uint32_t>(*est_trials)));
-  TRY(hybrid_sweeps(c, kTrialEq, false, 0));
-  TRY(hybrid_sweeps(c, kTrialMeas, true, 0));
+  TRY(hybrid_sweeps(c, kTrialEq, 0, 0));
+  TRY(hybrid_sweeps(c, kTrialMeas, 1, 0));   // energy only: a trial's phi average is never used
   TRY(fetch_series(c, kTrialMeas));
   mean_stderr(c->series, e, se);
   return MPR_OK;
@@ -597,7 +610,7 @@ int mpr_estimate_temperature(mpr_ctx* c, double* T_hat, double* e_sample, int* n
 
 int mpr_sweep(mpr_ctx* c, int n) {
   if (!c || n < 0) return fail(c, MPR_ERR_INVALID_ARG, "n < 0");
-  return hybrid_sweeps(c, n, false, 0);
+  return hybrid_sweeps(c, n, 0, 0);
 }
 
 int mpr_pass(mpr_ctx* c, int kind, int colour, uint64_t sweep) {
@@ -611,8 +624,8 @@ int mpr_run(mpr_ctx* c, int n_eq, int n_meas, double* d_pred, double* e_mean, do
   if (!c || n_eq < 0 || n_meas < 0 || n_meas > kSeriesCap) return fail(c, MPR_ERR_INVALID_ARG, "bad sweep counts");
   if (!(c->T > 0.0)) return fail(c, MPR_ERR_NOT_READY, "temperature not set");
   TRY(ensure_chain(c));
-  TRY(hybrid_sweeps(c, n_eq, false, 0));
-  TRY(hybrid_sweeps(c, n_meas, true, 0));
+  TRY(hybrid_sweeps(c, n_eq, 0, 0));
+  TRY(hybrid_sweeps(c, n_meas, 2, 0));
   if (d_pred) {
     const Geom& g = c->lo.g;
     dim3 block(128), grid((g.L + 127) / 128, g.L);

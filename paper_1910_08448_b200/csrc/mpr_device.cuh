@@ -314,6 +314,23 @@ __device__ __forceinline__ void quench_update(typename Traits<MODE>::real* c, ty
   *c = A * inv; *s = B * inv;
 }
 
+// Quench move of two sites at once (same per-lane operations as quench_update).
+template <int MODE>
+__device__ __forceinline__ void quench_update2(Two<typename Traits<MODE>::real> c, Two<typename Traits<MODE>::real> s,
+                                               Two<typename Traits<MODE>::real> A, Two<typename Traits<MODE>::real> B,
+                                               bool free_a, bool free_b,
+                                               typename Traits<MODE>::real out[4] /* ca, cb, sa, sb */) {
+  using R = typename Traits<MODE>::real;
+  R f2a, f2b, c0a, c0b, s0a, s0b, coa, cob, soa, sob;
+  un2(fma2(A, A, mul2(B, B)), &f2a, &f2b);
+  const Two<R> inv = mk2(Fn<MODE>::rsqrt_(f2a), Fn<MODE>::rsqrt_(f2b));
+  un2(mul2(A, inv), &coa, &cob); un2(mul2(B, inv), &soa, &sob);
+  un2(c, &c0a, &c0b); un2(s, &s0a, &s0b);
+  const bool oka = free_a && (f2a != R(0)), okb = free_b && (f2b != R(0));
+  out[0] = oka ? coa : c0a; out[2] = oka ? soa : s0a;
+  out[1] = okb ? cob : c0b; out[3] = okb ? sob : s0b;
+}
+
 // phi = 2 atan2(s, c) in [0, 2pi] (s >= 0).
 template <int MODE>
 __device__ __forceinline__ double spin_angle(typename Traits<MODE>::real c, typename Traits<MODE>::real s) {

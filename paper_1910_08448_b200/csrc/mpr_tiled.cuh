@@ -184,8 +184,10 @@ __device__ __forceinline__ int row_step(int par, decltype(Traits<MODE>::vec::x)*
     met_update2<MODE>(c, s, A, B, w0, w1, fa, fb, kc, o, ok);
     if (ok[0]) n += inc;
     if (ok[1]) n += inc;
-  } else {
+  } else if constexpr (KIND == KIND_OR) {
     or_update2<MODE>(c, s, A, B, fa, fb, o);
+  } else {
+    quench_update2<MODE>(c, s, A, B, fa, fb, o);
   }
   Unit<S> out;
   out.ca = static_cast<S>(o[0]); out.cb = static_cast<S>(o[1]);
@@ -236,7 +238,10 @@ __device__ __forceinline__ int pass_rows(const TileView<MODE>& t, uint32_t mcol,
   return n_acc;
 }
 
-template <int MODE, bool MEASURE>
+// MEASURE: 0 = sweeps only; 1 = + energy sample (temperature trials, R6); 2 = + accumulation of phi (R15);
+// 3 (kTiledQuench) = no sweeps but 2 nsweeps quench double passes (R8), same halo bookkeeping
+constexpr int kTiledQuench = 3;
+template <int MODE, int MEASURE>
 __global__ void __launch_bounds__(TileCfg<MODE>::NT, 2)
 tiled_sweep_kernel(const __grid_constant__ CUtensorMap tmap, typename Traits<MODE>::vec* __restrict__ dst,
                    const uint32_t* __restrict__ bits, double* __restrict__ acc, double* __restrict__ part,
@@ -302,6 +307,16 @@ tiled_sweep_kernel(const __grid_constant__ CUtensorMap tmap, typename Traits<MOD
 #pragma unroll 1
   for (int sw = 0; sw < nsweeps; ++sw) {
     const uint32_t sweep = first_sweep + static_cast<uint32_t>(sw);
+    if constexpr (MEASURE == kTiledQuench) {
+#pragma unroll 1
+      for (int d = 0; d < 2; ++d) {
+        pass_rows<MODE, KIND_QUENCH, 0>(t, mreg[0], cnt, site_row0, Lu, sweep, kc);
+        __syncthreads();
+        pass_rows<MODE, KIND_QUENCH, 1>(t, mreg[1], cnt, site_row0, Lu, sweep, kc);
+        __syncthreads();
+      }
+      continue;
+    }
     n_acc += pass_rows<MODE, KIND_MET, 0>(t, mreg[0], cnt, site_row0, Lu, sweep, kc);
     __syncthreads();
     n_acc += pass_rows<MODE, KIND_MET, 1>(t, mreg[1], cnt, site_row0, Lu, sweep, kc);
@@ -326,7 +341,7 @@ tiled_sweep_kernel(const __grid_constant__ CUtensorMap tmap, typename Traits<MOD
     S* gp = reinterpret_cast<S*>(dst) + 2 * g0;
     const S* sp = t.unit(0, warp * RPW, lane);
     const size_t grow = 2 * static_cast<size_t>(g.Wp), gplane = 2 * g.plane;
-    constexpr int kEpiUnroll = MEASURE ? 1 : RPW;   // the measuring variant carries two atan2 per unit: keep it rolled
+    constexpr int kEpiUnroll = MEASURE == 2 ? 1 : RPW;   // the measuring variant carries two atan2 per unit: keep it rolled
 #pragma unroll kEpiUnroll
     for (int i = 0; i < RPW; ++i) {
       if (((own_rows >> i) & 1u) && i < nrows) {
@@ -334,7 +349,7 @@ tiled_sweep_kernel(const __grid_constant__ CUtensorMap tmap, typename Traits<MOD
         const Unit<S> u1 = *reinterpret_cast<const Unit<S>*>(sp + (TH + i) * kRowScalars);
         *reinterpret_cast<Unit<S>*>(gp + i * grow) = u0;
         *reinterpret_cast<Unit<S>*>(gp + i * grow + gplane) = u1;
-        if constexpr (MEASURE) {
+        if constexpr (MEASURE == 1 || MEASURE == 2) {
           // every bond has exactly one colour-1 end: H = -J sum over colour-1 sites of u.F
           Two<R> A, B;
           pair_fields<MODE>((row0 + i + 1) & 1, sp + i * kRowScalars, &A, &B);
@@ -342,6 +357,8 @@ tiled_sweep_kernel(const __grid_constant__ CUtensorMap tmap, typename Traits<MOD
           un2(A, &Aa, &Ab); un2(B, &Ba, &Bb);
           esum += static_cast<double>(fma_(R(u1.ca), Aa, R(u1.sa) * Ba));
           esum += static_cast<double>(fma_(R(u1.cb), Ab, R(u1.sb) * Bb));
+        }
+        if constexpr (MEASURE == 2) {
 #pragma unroll
           for (int pl = 0; pl < 2; ++pl) {
             const Unit<S>& me = pl ? u1 : u0;
@@ -358,7 +375,7 @@ tiled_sweep_kernel(const __grid_constant__ CUtensorMap tmap, typename Traits<MOD
       }
     }
   }
-  if constexpr (MEASURE) {
+  if constexpr (MEASURE == 1 || MEASURE == 2) {
     const double e = block_sum(esum, red);
     if (threadIdx.x == 0) part[blockIdx.x] = e;
   }
@@ -384,7 +401,7 @@ int tiled_encode(TiledPlan& plan, const Geom& g, void* src, CUtensorMap* map) {
 template <int MODE>
 int tiled_launch(TiledPlan& plan, const Geom& g, void* src, void* dst, const uint32_t* bits, double* acc, double* part,
                  unsigned long long* slots, ChainConst<typename Traits<MODE>::real> kc, uint32_t first_sweep, int k,
-                 bool measure, cudaStream_t stream, int* ntiles_out) {
+                 int measure, cudaStream_t stream, int* ntiles_out) {
   using V = typename Traits<MODE>::vec;
   constexpr int TH = TileCfg<MODE>::TH, NT = TileCfg<MODE>::NT;
   if (!plan.encode) return TILED_NO_DRIVER;
@@ -393,9 +410,13 @@ int tiled_launch(TiledPlan& plan, const Geom& g, void* src, void* dst, const uin
   if (es != TILED_OK) return es;
   constexpr size_t smem = tile_smem_bytes<MODE>();
   if (!plan.attr_set[MODE]) {
-    if (cudaFuncSetAttribute(tiled_sweep_kernel<MODE, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+    if (cudaFuncSetAttribute(tiled_sweep_kernel<MODE, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                              static_cast<int>(smem)) != cudaSuccess ||
-        cudaFuncSetAttribute(tiled_sweep_kernel<MODE, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+        cudaFuncSetAttribute(tiled_sweep_kernel<MODE, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                             static_cast<int>(smem)) != cudaSuccess ||
+        cudaFuncSetAttribute(tiled_sweep_kernel<MODE, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                             static_cast<int>(smem)) != cudaSuccess ||
+        cudaFuncSetAttribute(tiled_sweep_kernel<MODE, kTiledQuench>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                              static_cast<int>(smem)) != cudaSuccess)
       return TILED_ATTR;
     plan.attr_set[MODE] = true;
@@ -404,11 +425,17 @@ int tiled_launch(TiledPlan& plan, const Geom& g, void* src, void* dst, const uin
   const int tiles_x = (g.Wp + IC - 1) / IC, tiles_y = (g.L + IR - 1) / IR;
   const long long ntiles = static_cast<long long>(tiles_x) * tiles_y;
   if (ntiles > (1 << 18)) return TILED_TOO_MANY;
-  if (measure)
-    tiled_sweep_kernel<MODE, true><<<static_cast<unsigned>(ntiles), NT, smem, stream>>>(
+  if (measure == kTiledQuench)
+    tiled_sweep_kernel<MODE, kTiledQuench><<<static_cast<unsigned>(ntiles), NT, smem, stream>>>(
+        map, static_cast<V*>(dst), bits, acc, part, slots, g, kc, first_sweep, k, tiles_x);
+  else if (measure == 2)
+    tiled_sweep_kernel<MODE, 2><<<static_cast<unsigned>(ntiles), NT, smem, stream>>>(
+        map, static_cast<V*>(dst), bits, acc, part, slots, g, kc, first_sweep, k, tiles_x);
+  else if (measure == 1)
+    tiled_sweep_kernel<MODE, 1><<<static_cast<unsigned>(ntiles), NT, smem, stream>>>(
         map, static_cast<V*>(dst), bits, acc, part, slots, g, kc, first_sweep, k, tiles_x);
   else
-    tiled_sweep_kernel<MODE, false><<<static_cast<unsigned>(ntiles), NT, smem, stream>>>(
+    tiled_sweep_kernel<MODE, 0><<<static_cast<unsigned>(ntiles), NT, smem, stream>>>(
         map, static_cast<V*>(dst), bits, acc, part, slots, g, kc, first_sweep, k, tiles_x);
   if (cudaGetLastError() != cudaSuccess) return TILED_LAUNCH;
   *ntiles_out = static_cast<int>(ntiles);
