@@ -33,7 +33,7 @@ template <int MODE> struct TileCfg;
 template <> struct TileCfg<MODE_DP>           { static constexpr int TH = 48, NT = 256; };
 template <> struct TileCfg<MODE_SP>           { static constexpr int TH = 96, NT = 256; };
 template <> struct TileCfg<MODE_SP_PRECISE>   { static constexpr int TH = 96, NT = 512; };
-template <> struct TileCfg<MODE_SP_INTRINSIC> { static constexpr int TH = 96, NT = 512; };
+template <> struct TileCfg<MODE_SP_INTRINSIC> { static constexpr int TH = 96, NT = 384; };
 
 inline int tiled_max_fused() { return 4; }
 
