@@ -279,3 +279,64 @@ def test_sp_modes_statistics_config2_shape(mpr, oracle_mod, inputs):
         rmse = float(np.mean([r for _, r in maes]))
         assert abs(mae / mae_o - 1.0) <= 0.01, (mode, mae, mae_o)
         assert abs(rmse / rmse_o - 1.0) <= 0.01, (mode, rmse, rmse_o)
+
+
+# --------------------------------------------------------------------------- large grids
+def test_dp_large_ragged_grid_matches_oracle(mpr, oracle_mod, inputs):
+    """L = 4100 (69 x 103 DP tiles, ragged tail in both directions, plane padding columns): every
+    site after the tiled quench passes and 2 hybrid sweeps, and the accepted-move count."""
+    L = 4100
+    values, mask, _ = make(inputs, L, 64.0, 21, 0.9)
+    g = mpr.Mpr(values, mask, seed=1234)
+    o = oracle_mod.Oracle(values=values, mask=mask, seed=1234, threads=oracle_mod.threads_available())
+    g.set_quench(2)
+    o.set_quench(2)
+    g.set_temperature(0.004)
+    o.set_temperature(0.004)
+    g.sweep(2)
+    o.hybrid_sweeps(2)
+    sg, so = g.get_state().cpu().numpy(), o.get_state()
+    assert phi_diff(sg, so) <= PHI_TOL
+    assert g.counters() == o.counters()
+    assert abs(g.energy()[1] - o.energy()[1]) <= 1e-10
+
+
+def test_bench_configuration_full_size_properties(mpr, inputs):
+    """BASELINE.json configs[4] (L = 16384, 90 % masked) in the launch configuration bench.py times
+    (SP_INTRINSIC, tiled, one hybrid sweep per launch).  The oracle cannot finish this size in
+    seconds, so the full grid is checked through what holds at any size: the tiled kernel equals the
+    plain per-pass kernels bit for bit (spins, accepted moves), measured spins never move, every
+    angle stays in [0, 2 pi], the fused energy sample equals the plain energy kernel's, and the
+    prediction leaves measured sites bit-exact."""
+    import torch
+    c, values, mask, truth = inputs.make_config(5)
+    d_values = torch.from_numpy(values).cuda()
+    d_mask = torch.from_numpy(mask).cuda()
+    out = {}
+    for path in ("TILED", "PLAIN"):
+        g = mpr.Mpr(d_values, d_mask, mode="SP_INTRINSIC", seed=c.mpr_seed)
+        g.set_path(path)
+        g.set_quench(2)
+        g.set_temperature(1.1e-3)
+        s0 = g.get_state()
+        g.sweep(3)
+        s1 = g.get_state()
+        cnt = g.counters()
+        pred, e, se = g.run(0, 2)
+        out[path] = (s1, cnt, g.series(), pred)
+        if path == "TILED":
+            m0 = d_mask == 0
+            assert torch.equal(s0[m0], s1[m0])                       # measured spins never move
+            assert float(s1.min()) >= 0.0 and float(s1.max()) <= TWO_PI + 1e-15
+            assert torch.equal(pred[m0], d_values[m0])               # measured values come back bit-exact
+            free = pred[~m0]
+            assert bool(torch.isfinite(free).all())
+            zmin, zmax = g.info()["z_min"], g.info()["z_max"]
+            assert float(free.min()) >= zmin - 1e-9 and float(free.max()) <= zmax + 1e-9   # R1 confines predictions
+            assert cnt[1] == 3 * int(mask.sum()) and cnt[0] > 0
+        g.close()
+        del g
+    assert torch.equal(out["TILED"][0], out["PLAIN"][0])
+    assert out["TILED"][1] == out["PLAIN"][1]
+    np.testing.assert_allclose(out["TILED"][2], out["PLAIN"][2], rtol=0, atol=1e-12)
+    assert torch.equal(out["TILED"][3], out["PLAIN"][3])
