@@ -34,6 +34,10 @@ METRIC = "mpr_site_updates_per_s"
 UNIT = "site-updates/s"
 CPU_CROP = 2048          # cpu_baseline / reference arm: top-left CPU_CROP^2 window of the workload
 CPU_EQ, CPU_MEAS = 10, 1
+ALG_WARP_INST_PER_32_UNITS = 125.0   # Metropolis 91 + over-relaxation 34 per unit and sweep
+# dram__bytes_read.sum + dram__bytes_write.sum of one launch of the dominant kernel at L = 16384, from the
+# committed `ncu --set full` capture (profiles/r01g_ncu_full_tiled_v4.md); None for configurations not captured.
+NCU_TRAFFIC_BYTES = {("SP_INTRINSIC", 1): None}
 
 
 def parse():
@@ -250,10 +254,19 @@ def run_ours(args, rank, world, local_rank):
     alg_bytes = stored * 2 * w + 2 * stored / 8.0          # read + write of every stored spin, mask bits
     peak, peak_src = peaks()
     achieved = alg_bytes / (kern_ms * 1e-3) / 1e9
+    # second ceiling: warp-instruction issue.  Algorithmic count = 125 warp instructions per
+    # 32 units (unit = 2 sites of one colour and row) per hybrid sweep; peak = 148 SMs x 4 schedulers x 1 / clk.
+    alg_inst = (stored / 2.0) / 32.0 * ALG_WARP_INST_PER_32_UNITS * args.fused
+    sm_hz = (clk.get("sm_max_mhz") or 1965.0) * 1e6
+    issue_peak = 148 * 4 * sm_hz
+    alu = {"bound": "alu", "achieved": alg_inst / (kern_ms * 1e-3), "peak": issue_peak, "unit": "warp-inst/s",
+           "frac": alg_inst / (kern_ms * 1e-3) / issue_peak, "algorithmic_warp_inst_per_launch": alg_inst}
     roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                "traffic": None, "kernel": "tiled_sweep_kernel<%s,false>" % mode, "kernel_ms": kern_ms,
+                "traffic": NCU_TRAFFIC_BYTES.get((mode, args.fused)) if L == 16384 else None, "kernel": "tiled_sweep_kernel<%s,0>" % mode,
+                "kernel_ms": kern_ms,
                 "algorithmic_bytes_per_launch": alg_bytes, "sweeps_per_launch": args.fused, "peak_source": peak_src,
-                "kernel_site_updates_per_s": 2.0 * state["n_free"] * args.fused / (kern_ms * 1e-3)}
+                "kernel_site_updates_per_s": 2.0 * state["n_free"] * args.fused / (kern_ms * 1e-3),
+                "second_ceiling": alu}
 
     # ---- per-mode sweep rates (BASELINE.json: "per precision mode") ----------------------------
     modes = {}
