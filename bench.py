@@ -159,7 +159,7 @@ def run_ours(args, rank, world, local_rank):
     import torch
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device: there is no CPU fallback")
-    from paper_1910_08448_b200 import inputs, mpr
+    from paper_1910_08448_b200 import inputs, mpr, sharding
     import torch.distributed as dist
     dev = torch.device("cuda", local_rank)
     torch.cuda.set_device(dev)
@@ -172,13 +172,14 @@ def run_ours(args, rank, world, local_rank):
     mode = args.mode
     # every rank its own problem of the same recipe (weak scaling; rank 0 = BASELINE.json's seed)
     t_gen = time.perf_counter()
-    values, mask, truth = inputs.make_problem(c.L, c.xi, c.field_seed + 1000 * rank, c.f, c.lognormal)
+    rp = sharding.rank_problem(c.field_seed, c.mpr_seed, rank, world)
+    values, mask, truth = inputs.make_problem(c.L, c.xi, rp.field_seed, c.f, c.lognormal)
     t_gen = time.perf_counter() - t_gen
     L, N = c.L, c.L * c.L
     d_values = torch.from_numpy(values).to(dev)
     d_mask = torch.from_numpy(mask).to(dev)
     d_truth = torch.from_numpy(truth).to(dev)
-    seed = c.mpr_seed + rank
+    seed = rp.mpr_seed
 
     state = {"launches": 0, "sweeps": 0, "n_free": int(mask.sum()), "T": None, "trials": None, "pred": None,
              "e": None, "se": None}
@@ -218,14 +219,9 @@ def run_ours(args, rank, world, local_rank):
     barrier()
     ms = ev0.elapsed_time(ev1)
     clk = clocks.stop()
-    tt = torch.tensor([ms], dtype=torch.float64, device=dev)
-    units = torch.tensor([2.0 * state["n_free"] * state["sweeps"], float(state["launches"])], dtype=torch.float64,
-                         device=dev)
-    if world > 1:
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-        dist.all_reduce(units, op=dist.ReduceOp.SUM)
-    ms_max = float(tt.item())
-    value = float(units[0].item()) / (ms_max * 1e-3)
+    ms_max, units_total, launches_total = sharding.aggregate(
+        ms, 2.0 * state["n_free"] * state["sweeps"], state["launches"], world, device=dev)
+    value = sharding.throughput(units_total, ms_max)
 
     # prediction error of the last step (metric of PAPER.md Eq. 4; post-processing, not the path)
     m1 = d_mask.bool()
@@ -316,16 +312,12 @@ def run_ours(args, rank, world, local_rank):
             e2e_step()
         b.record()
         barrier()
-        te = torch.tensor([a.elapsed_time(b)], dtype=torch.float64, device=dev)
-        if world > 1:
-            dist.all_reduce(te, op=dist.ReduceOp.MAX)
         # same problem, seed and mode => same number of T trials as the device-resident steps
         sweeps_e2e = state["sweeps"]
-        ue = torch.tensor([2.0 * state["n_free"] * sweeps_e2e], dtype=torch.float64, device=dev)
-        if world > 1:
-            dist.all_reduce(ue, op=dist.ReduceOp.SUM)
-        e2e = {"value": float(ue.item()) / (float(te.item()) * 1e-3), "unit": UNIT, "h2d_bytes_per_step": 9 * N,
-               "d2h_bytes_per_step": 8 * N, "ms_per_step": float(te.item()) / args.steps}
+        te_max, ue_total, _ = sharding.aggregate(a.elapsed_time(b), 2.0 * state["n_free"] * sweeps_e2e, 0, world,
+                                                 device=dev)
+        e2e = {"value": sharding.throughput(ue_total, te_max), "unit": UNIT, "h2d_bytes_per_step": 9 * N,
+               "d2h_bytes_per_step": 8 * N, "ms_per_step": te_max / args.steps}
         del ws
 
     cpu = None
@@ -348,7 +340,7 @@ def run_ours(args, rank, world, local_rank):
                        "n_meas": n_meas, "T_trials": state["trials"], "sweeps_per_step": state["sweeps"] // args.steps,
                        "fused_sweeps": args.fused, "parallelism": "replicas x%d" % world,
                        "l2": "state (%.1f GiB) larger than L2; no flush" % (stored * w / 2 ** 30)},
-            "clocks": clk, "e2e": e2e, "gpu_launches": int(units[1].item()), "roofline": roofline,
+            "clocks": clk, "e2e": e2e, "gpu_launches": launches_total, "roofline": roofline,
             "cpu_baseline": cpu, "modes": modes, "T_hat": T_hat, "e_sample": state.get("e_sample"),
             "e_mean": state["e"], "e_stderr": state["se"], "mae": mae, "rmse": rmse,
             "mae_of_sample_mean_predictor": base_mae, "input_generation_s": t_gen,
