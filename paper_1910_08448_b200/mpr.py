@@ -134,6 +134,9 @@ class Mpr:
         self._stream = stream
         sptr = stream.cuda_stream if stream is not None else torch.cuda.current_stream(dev).cuda_stream
         self.h = C.c_void_p()
+        # bound here so that close() works from __del__ at interpreter shutdown, when module
+        # globals (lib, C) may already be cleared
+        self._destroy, self._null = lib().mpr_destroy, C.c_void_p
         with torch.cuda.device(dev):
             st = lib().mpr_create(C.byref(self.h), self.L, self.values.data_ptr(), self.mask.data_ptr(),
                                   self._ws_ptr, self.ws.numel() - off, sptr)
@@ -146,9 +149,10 @@ class Mpr:
             self.set_seed(seed)
 
     def close(self):
-        if getattr(self, "h", None) and self.h.value:
-            lib().mpr_destroy(self.h)
-            self.h = C.c_void_p()
+        h = getattr(self, "h", None)
+        if h is not None and h.value and getattr(self, "_destroy", None) is not None:
+            self._destroy(h)
+            self.h = self._null()
 
     __del__ = close
 
