@@ -285,7 +285,10 @@ def run_ours(args, rank, world, local_rank):
             b.record()
             torch.cuda.synchronize(dev)
             modes[md] = {"ms_per_sweep": t, "site_updates_per_s": 2.0 * state["n_free"] / (t * 1e-3),
-                         "ms_per_measurement_sweep": a.elapsed_time(b) / 5, "e": e_m}
+                         "ms_per_measurement_sweep": a.elapsed_time(b) / 5,
+                         # mean of 5 samples taken 3 + n_sw sweeps after the chain reset: NOT an equilibrium
+                         # value and not comparable between modes (n_sw differs); a plausibility figure only
+                         "e_unequilibrated_after_%d_sweeps" % (3 + n_sw): e_m}
             gm.close()
 
     # ---- end to end through the C ABI with HOST buffers (mpr_predict_host) ---------------------

@@ -147,6 +147,40 @@ __device__ __forceinline__ void local_field(R lc, R ls, R rc, R rs, R uc, R us, 
   *A = a; *B = b;
 }
 
+// ---- per-site energy term of S5 (R3, R13): sum over the existing neighbours j of cos[q(phi - phi_j)] ----
+// Double arithmetic (DP, SP): u . F with F = sum_j u_j, as Eq. 2 reads in the unit-vector form.
+// Float arithmetic (SP_PRECISE, SP_INTRINSIC): the same quantity per bond as 1 - |u - u_j|^2 / 2.
+// u . u_j = |u||u_j| cos(theta) carries the norm error of the stored float vectors and the
+// rounding of a value near 1 (measured on the B200: a constant +2.1e-8 .. +2.6e-8 in e at L = 16384,
+// T = 1.1e-3, i.e. ~3 standard errors of e there), whereas |u - u_j|^2 = (|u|^2 + |u_j|^2)/2 x
+// 2 (1 - cos(theta)) up to second order: the same errors now multiply the small thermal part only.
+// A missing neighbour (open boundary, R2) and an out-of-grid padding site are the zero vector in
+// both kernels; a real spin is never (0, 0).  Neighbour order l, r, u, d; the bond terms are float
+// (the mode's arithmetic), the count is exact and the combination is done in double (R13).
+template <typename R>
+__device__ __forceinline__ double site_energy_term(R c, R s, R lc, R ls, R rc, R rs, R uc, R us, R dc, R ds) {
+  if constexpr (sizeof(R) == 8) {
+    const R A = ((lc + rc) + uc) + dc, B = ((ls + rs) + us) + ds;
+    return static_cast<double>(fma_(c, A, s * B));
+  } else {
+    const R z = R(0);
+    const bool me = (c != z) || (s != z);
+    const bool hl = (lc != z) || (ls != z), hr = (rc != z) || (rs != z);
+    const bool hu = (uc != z) || (us != z), hd = (dc != z) || (ds != z);
+    R ec, es;
+    ec = c - lc; es = s - ls; const R tl = fma_(ec, ec, es * es);
+    ec = c - rc; es = s - rs; const R tr = fma_(ec, ec, es * es);
+    ec = c - uc; es = s - us; const R tu = fma_(ec, ec, es * es);
+    ec = c - dc; es = s - ds; const R td = fma_(ec, ec, es * es);
+    R t = hl ? tl : z;
+    t = t + (hr ? tr : z);
+    t = t + (hu ? tu : z);
+    t = t + (hd ? td : z);
+    const int n = static_cast<int>(hl) + static_cast<int>(hr) + static_cast<int>(hu) + static_cast<int>(hd);
+    return me ? static_cast<double>(n) - 0.5 * static_cast<double>(t) : 0.0;
+  }
+}
+
 // ---- two-lane arithmetic -----------------------------------------------------------------
 // Every move is written once, for TWO sites at a time (lanes a, b).  In the float modes the two
 // lanes are the halves of one 64-bit register and every add / mul / fma is ONE packed sm_100

@@ -296,7 +296,9 @@ plain_pass_kernel(typename Traits<MODE>::vec* __restrict__ state, const uint32_t
 }
 
 // ---- energy (R3): every bond has exactly one colour-1 end, so H = -J sum over colour-1
-// sites of u_s . F_s.  Terms in the mode's arithmetic, sums in double (R13).
+// sites of site_energy_term (mpr_device.cuh): u_s . F_s in the double-arithmetic modes, the
+// per-bond form n - sum_j |u_s - u_j|^2 / 2 in the float-arithmetic modes.  Terms in the mode's
+// arithmetic, sums in double (R13).  Missing neighbours are passed as the zero vector.
 template <int MODE>
 __global__ void __launch_bounds__(256)
 plain_energy_kernel(const typename Traits<MODE>::vec* __restrict__ state, Geom g, double* __restrict__ part) {
@@ -318,10 +320,8 @@ plain_energy_kernel(const typename Traits<MODE>::vec* __restrict__ state, Geom g
       const V r = hr ? ld_spin(oth, j + par) : zero;
       const V u = hu ? ld_spin(oth, j - g.Wp) : zero;
       const V d = hd ? ld_spin(oth, j + g.Wp) : zero;
-      R A, B;
-      local_field<R>(R(l.x), R(l.y), R(r.x), R(r.y), R(u.x), R(u.y), R(d.x), R(d.y), hl, hr, hu, hd, &A, &B);
       const V me = ld_spin(own, j);
-      sum += static_cast<double>(fma_(R(me.x), A, R(me.y) * B));
+      sum += site_energy_term<R>(R(me.x), R(me.y), R(l.x), R(l.y), R(r.x), R(r.y), R(u.x), R(u.y), R(d.x), R(d.y));
     }
   }
   const double s = block_sum(sum, sh);

@@ -145,18 +145,6 @@ __device__ __forceinline__ void combine_fields(int par, const Unit<decltype(Trai
   *A = a; *B = b;
 }
 
-// The same from shared memory (`oth` = the unit of the same row and columns in the other plane);
-// used by the energy sample, interior columns only.
-template <int MODE>
-__device__ __forceinline__ void pair_fields(int par, const decltype(Traits<MODE>::vec::x)* oth,
-                                            Two<typename Traits<MODE>::real>* A, Two<typename Traits<MODE>::real>* B) {
-  using S = decltype(Traits<MODE>::vec::x);
-  const Unit<S> mid = *reinterpret_cast<const Unit<S>*>(oth);
-  const Unit<S> up = *reinterpret_cast<const Unit<S>*>(oth - kRowScalars);
-  const Unit<S> dn = *reinterpret_cast<const Unit<S>*>(oth + kRowScalars);
-  combine_fields<MODE>(par, up, mid, dn, oth[par ? 4 : -3], oth[par ? 6 : -1], A, B);
-}
-
 // One row of a colour pass: the unit at `own` (row r, x-parity `par`) from the register window
 // (up, mid, dn) of the other plane.  The extra neighbour comes from the adjacent lane by warp
 // shuffle (wrong at lanes 0 / 31, for sites that are stale anyway).  Returns inc x accepted moves.
@@ -350,13 +338,23 @@ tiled_sweep_kernel(const __grid_constant__ CUtensorMap tmap, typename Traits<MOD
         *reinterpret_cast<Unit<S>*>(gp + i * grow) = u0;
         *reinterpret_cast<Unit<S>*>(gp + i * grow + gplane) = u1;
         if constexpr (MEASURE == 1 || MEASURE == 2) {
-          // every bond has exactly one colour-1 end: H = -J sum over colour-1 sites of u.F
-          Two<R> A, B;
-          pair_fields<MODE>((row0 + i + 1) & 1, sp + i * kRowScalars, &A, &B);
-          R Aa, Ab, Ba, Bb;
-          un2(A, &Aa, &Ab); un2(B, &Ba, &Bb);
-          esum += static_cast<double>(fma_(R(u1.ca), Aa, R(u1.sa) * Ba));
-          esum += static_cast<double>(fma_(R(u1.cb), Ab, R(u1.sb) * Bb));
+          // every bond has exactly one colour-1 end: H = -J sum over colour-1 sites of their
+          // site_energy_term (mpr_device.cuh; the same function as plain_energy_kernel).  The
+          // neighbours are the other plane's units of rows r - 1, r, r + 1 and one extra site:
+          // x-parity par = 0: site a has (l, r) = (ex, mid.a), site b (mid.a, mid.b);
+          // par = 1: site a (mid.a, mid.b), site b (mid.b, ex)  -- as in combine_fields
+          const S* oth = sp + i * kRowScalars;
+          const int par = (row0 + i + 1) & 1;
+          const Unit<S> mid = *reinterpret_cast<const Unit<S>*>(oth);
+          const Unit<S> up = *reinterpret_cast<const Unit<S>*>(oth - kRowScalars);
+          const Unit<S> dn = *reinterpret_cast<const Unit<S>*>(oth + kRowScalars);
+          const R exc = R(oth[par ? 4 : -3]), exs = R(oth[par ? 6 : -1]);
+          const R alc = par ? R(mid.ca) : exc, als = par ? R(mid.sa) : exs;
+          const R arc = par ? R(mid.cb) : R(mid.ca), ars = par ? R(mid.sb) : R(mid.sa);
+          const R blc = par ? R(mid.cb) : R(mid.ca), bls = par ? R(mid.sb) : R(mid.sa);
+          const R brc = par ? exc : R(mid.cb), brs = par ? exs : R(mid.sb);
+          esum += site_energy_term<R>(R(u1.ca), R(u1.sa), alc, als, arc, ars, R(up.ca), R(up.sa), R(dn.ca), R(dn.sa));
+          esum += site_energy_term<R>(R(u1.cb), R(u1.sb), blc, bls, brc, brs, R(up.cb), R(up.sb), R(dn.cb), R(dn.sb));
         }
         if constexpr (MEASURE == 2) {
 #pragma unroll

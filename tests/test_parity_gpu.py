@@ -281,6 +281,54 @@ def test_sp_modes_statistics_config2_shape(mpr, oracle_mod, inputs):
         assert abs(rmse / rmse_o - 1.0) <= 0.01, (mode, rmse, rmse_o)
 
 
+@pytest.mark.parametrize("lognormal,f,T", [(False, 0.9, 1.1e-3), (True, 0.33, 1.5e-3)])
+def test_float_modes_at_low_temperature(mpr, inputs, lognormal, f, T):
+    """The low-T stress point (T_hat ~ 1e-3 at configs 3 and 5; lognormal = spins crowded
+    near phi = 0).  Two separate statements about the float modes, on chain snapshots whose energy is
+    evaluated twice -- by the mode's own S5 arithmetic and by a DP context loaded with the same phi:
+
+    (a) evaluation: the mode's own e of a state equals the DP evaluation of that state to 5e-10.  With
+        u.F in float arithmetic this was a constant +1e-8 .. +2.6e-8, ~3 standard errors of e at
+        L = 16384 (u_s.u_t is sensitive to the norm error of the stored float vectors and to the
+        rounding of a value near 1; which of the two dominated was not separated); the per-bond form
+        1 - |u_s - u_t|^2 / 2 (site_energy_term), sensitive to neither, brings it to ~1e-11.
+    (b) chain: the DP-evaluated mean e of each mode's chain is within 3 standard errors of the DP
+        chain's (north_star's statistical gate).  The reference is the GPU DP chain, which the tests
+        above show to be decision-identical to the oracle; seeds are fixed, so the outcome is
+        reproducible rather than a draw."""
+    L, n_eq, n_snap, gap, seeds = 2048, 400, 12, 25, (11, 22, 33)
+    values, mask, _ = make(inputs, L, 64.0, 4, f, lognormal)
+    import torch
+    dv, dm = torch.from_numpy(values).cuda(), torch.from_numpy(mask).cuda()
+    ev = mpr.Mpr(dv, dm, mode="DP", seed=1)
+    ev.set_temperature(T)
+    stats = {}
+    for mode in ("DP", "SP", "SP_PRECISE", "SP_INTRINSIC"):
+        per_seed, worst_eval = [], 0.0
+        for seed in seeds:
+            g = mpr.Mpr(dv, dm, mode=mode, seed=seed)
+            g.set_temperature(T)
+            g.sweep(n_eq)
+            dp = []
+            for _ in range(n_snap):
+                g.sweep(gap)
+                own = g.energy()[1]
+                ev.set_state(g.get_state())
+                e_dp = ev.energy()[1]
+                worst_eval = max(worst_eval, abs(own - e_dp))
+                dp.append(e_dp)
+            per_seed.append(float(np.mean(dp)))
+            g.close()
+        stats[mode] = (float(np.mean(per_seed)), float(np.std(per_seed, ddof=1) / math.sqrt(len(seeds))), worst_eval)
+    ev.close()
+    e_ref, se_ref, _ = stats["DP"]
+    assert -2.0 < e_ref < -1.99                                   # a low-temperature state, not a frozen one
+    for mode in ("SP", "SP_PRECISE", "SP_INTRINSIC"):
+        e_m, se_m, worst_eval = stats[mode]
+        assert worst_eval <= 5e-10, (mode, worst_eval)                                   # (a)
+        assert abs(e_m - e_ref) <= 3.0 * math.hypot(se_m, se_ref), (mode, e_m, e_ref, se_m, se_ref)   # (b)
+
+
 # --------------------------------------------------------------------------- large grids
 def test_dp_large_ragged_grid_matches_oracle(mpr, oracle_mod, inputs):
     """L = 4100 (69 x 103 DP tiles, ragged tail in both directions, plane padding columns): every
