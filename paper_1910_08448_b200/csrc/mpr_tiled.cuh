@@ -30,10 +30,16 @@ namespace mpr {
 constexpr int kTileCols = 64;   // plane columns staged per tile (incl. halo)
 
 template <int MODE> struct TileCfg;
-template <> struct TileCfg<MODE_DP>           { static constexpr int TH = 48, NT = 256; };
-template <> struct TileCfg<MODE_SP>           { static constexpr int TH = 96, NT = 256; };
-template <> struct TileCfg<MODE_SP_PRECISE>   { static constexpr int TH = 96, NT = 512; };
-template <> struct TileCfg<MODE_SP_INTRINSIC> { static constexpr int TH = 96, NT = 384; };
+// PAIR_SYNC: synchronise two colour passes by pairwise named barriers between neighbouring warps
+// (neighbour_sync) instead of __syncthreads.  Chosen per mode from an A/B run on one B200 at a
+// constant 1965 MHz (L = 16384, ms per hybrid sweep, __syncthreads -> pairwise, two runs each):
+// DP 4.279 -> 4.221, SP 3.555 -> 3.531, SP_PRECISE 1.616 -> 1.570, but SP_INTRINSIC 1.229 -> 1.247
+// (at its 80-register cap the barrier ids spill, and its barrier waits were already covered by the
+// second resident CTA), so that mode keeps __syncthreads.
+template <> struct TileCfg<MODE_DP>           { static constexpr int TH = 48, NT = 256; static constexpr bool PAIR_SYNC = true; };
+template <> struct TileCfg<MODE_SP>           { static constexpr int TH = 96, NT = 256; static constexpr bool PAIR_SYNC = true; };
+template <> struct TileCfg<MODE_SP_PRECISE>   { static constexpr int TH = 96, NT = 512; static constexpr bool PAIR_SYNC = true; };
+template <> struct TileCfg<MODE_SP_INTRINSIC> { static constexpr int TH = 96, NT = 384; static constexpr bool PAIR_SYNC = false; };
 
 inline int tiled_max_fused() { return 4; }
 
@@ -184,6 +190,30 @@ __device__ __forceinline__ int row_step(int par, decltype(Traits<MODE>::vec::x)*
   return n;
 }
 
+// Synchronisation between two colour passes.  In a pass warp w writes its own RPW rows of one plane
+// and reads rows w RPW - 1 .. (w + 1) RPW of the other: the only warps it exchanges data with are
+// w - 1 and w + 1, so it need not wait for the whole CTA.  Two rounds of PAIRWISE named barriers
+// (bar.sync id, 64): round A pairs (0,1), (2,3), ..., round B pairs (1,2), (3,4), ...  The pairs of a
+// round are disjoint, so every round resolves in parallel (no ripple from warp 0 upwards), and a
+// warp that has passed both rounds knows that both neighbours have finished the pass -- their
+// writes are visible to it (RAW) and their reads of its rows are done (WAR for the next pass).
+// Warps may drift apart by one pass per warp of distance, which also spreads the Philox /
+// arithmetic / MUFU phases of the resident warps over time.  Ids 1 .. NW - 1; id 0 stays
+// __syncthreads.  NW is even and <= 16.
+template <int NW>
+__device__ __forceinline__ void neighbour_sync(int warp) {
+  static_assert(NW % 2 == 0 && NW >= 2 && NW <= 16, "pair barriers use ids 1 .. NW - 1 of the 16 hardware barriers");
+  asm volatile("bar.sync %0, 64;" ::"r"(1 + (warp >> 1)) : "memory");                       // A: (w, w ^ 1)
+  if (warp > 0 && warp < NW - 1)                                                             // B: odd w with w + 1
+    asm volatile("bar.sync %0, 64;" ::"r"(NW / 2 + ((warp + 1) >> 1)) : "memory");
+}
+
+template <int MODE>
+__device__ __forceinline__ void pass_sync(int warp) {
+  if constexpr (TileCfg<MODE>::PAIR_SYNC) neighbour_sync<TileCfg<MODE>::NT / 32>(warp);
+  else __syncthreads();
+}
+
 // One colour pass over the RPW contiguous rows of this warp.  The other plane's rows slide through
 // a register window: each row is read from shared memory once per pass (RPW + 2 reads for RPW
 // rows instead of 3 RPW).  COL, KIND and the row parities are compile-time constants: the first
@@ -299,20 +329,20 @@ tiled_sweep_kernel(const __grid_constant__ CUtensorMap tmap, typename Traits<MOD
 #pragma unroll 1
       for (int d = 0; d < 2; ++d) {
         pass_rows<MODE, KIND_QUENCH, 0>(t, mreg[0], cnt, site_row0, Lu, sweep, kc);
-        __syncthreads();
+        pass_sync<MODE>(warp);
         pass_rows<MODE, KIND_QUENCH, 1>(t, mreg[1], cnt, site_row0, Lu, sweep, kc);
-        __syncthreads();
+        pass_sync<MODE>(warp);
       }
       continue;
     }
     n_acc += pass_rows<MODE, KIND_MET, 0>(t, mreg[0], cnt, site_row0, Lu, sweep, kc);
-    __syncthreads();
+    pass_sync<MODE>(warp);
     n_acc += pass_rows<MODE, KIND_MET, 1>(t, mreg[1], cnt, site_row0, Lu, sweep, kc);
-    __syncthreads();
+    pass_sync<MODE>(warp);
     pass_rows<MODE, KIND_OR, 0>(t, mreg[0], cnt, site_row0, Lu, sweep, kc);
-    __syncthreads();
+    pass_sync<MODE>(warp);
     pass_rows<MODE, KIND_OR, 1>(t, mreg[1], cnt, site_row0, Lu, sweep, kc);
-    __syncthreads();
+    pass_sync<MODE>(warp);
   }
 
   // interior -> other state buffer (+ energy sample and accumulation of phi when measuring).

@@ -253,6 +253,39 @@ def test_paths_and_fused_depths_are_bit_identical(mpr, inputs, mode):
     np.testing.assert_allclose(out[0][1], out[1][1], rtol=0, atol=1e-13)
 
 
+@pytest.mark.parametrize("mode", ["DP", "SP", "SP_PRECISE", "SP_INTRINSIC"])
+def test_pass_synchronisation_stress(mpr, inputs, mode):
+    """DP, SP and SP_PRECISE separate the colour passes of a tile by pairwise named barriers between
+    neighbouring warps instead of a CTA-wide barrier (mpr_tiled.cuh, neighbour_sync).  A missing or
+    misplaced synchronisation shows up as a spin that differs from the one-launch-per-pass PLAIN
+    path, most likely where the warps of a CTA can drift furthest apart: the deepest fusion (k = 4,
+    16 passes per launch) on a grid of many tiles, repeated.  compute-sanitizer's racecheck is not
+    available on the GPU pool, so this bitwise comparison is the check that stands in for it; it
+    is evidence, not a proof of race freedom."""
+    import torch
+    L = 2048
+    values, mask, _ = make(inputs, L, 48.0, 9, 0.9)
+    dv, dm = torch.from_numpy(values).cuda(), torch.from_numpy(mask).cuda()
+    out = {}
+    for path, k in (("PLAIN", 1), ("TILED", 4), ("TILED", 1)):
+        g = mpr.Mpr(dv, dm, mode=mode, seed=4242)
+        g.set_path(path)
+        g.set_fused_sweeps(k)
+        g.set_temperature(0.02)
+        states = []
+        for _ in range(3):                    # 3 x 8 sweeps: six launches of 16 passes at k = 4
+            g.sweep(8)
+            states.append(g.get_state())
+        out[(path, k)] = (states, g.counters())
+        g.close()
+    ref_states, ref_cnt = out[("PLAIN", 1)]
+    for key in (("TILED", 4), ("TILED", 1)):
+        states, cnt = out[key]
+        assert cnt == ref_cnt, (mode, key, cnt, ref_cnt)
+        for i, (a, b) in enumerate(zip(states, ref_states)):
+            assert torch.equal(a, b), (mode, key, i, int((a != b).sum()))
+
+
 # --------------------------------------------------------------------------- SP modes: statistics
 def test_sp_modes_statistics_config2_shape(mpr, oracle_mod, inputs):
     """e within 3 standard errors of the DP value; MAE / RMSE within 1 % of the DP oracle's."""
