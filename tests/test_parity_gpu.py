@@ -382,20 +382,27 @@ def test_dp_large_ragged_grid_matches_oracle(mpr, oracle_mod, inputs):
     assert abs(g.energy()[1] - o.energy()[1]) <= 1e-10
 
 
-def test_bench_configuration_full_size_properties(mpr, inputs):
-    """BASELINE.json configs[4] (L = 16384, 90 % masked) in the launch configuration bench.py times
-    (SP_INTRINSIC, tiled, one hybrid sweep per launch).  The oracle cannot finish this size in
+@pytest.fixture(scope="module")
+def config5(inputs):
+    """BASELINE.json configs[4] on the device, generated once for all full-size cases (15 s, 2 GiB)."""
+    import torch
+    c, values, mask, truth = inputs.make_config(5)
+    return c, torch.from_numpy(values).cuda(), torch.from_numpy(mask).cuda(), int(mask.sum())
+
+
+@pytest.mark.parametrize("mode", ["SP_INTRINSIC", "SP_PRECISE", "SP", "DP"])
+def test_bench_configuration_full_size_properties(mpr, config5, mode):
+    """BASELINE.json configs[4] (L = 16384, 90 % masked) in the launch configurations bench.py times
+    (every precision mode, tiled, one hybrid sweep per launch).  The oracle cannot finish this size in
     seconds, so the full grid is checked through what holds at any size: the tiled kernel equals the
     plain per-pass kernels bit for bit (spins, accepted moves), measured spins never move, every
     angle stays in [0, 2 pi], the fused energy sample equals the plain energy kernel's, and the
     prediction leaves measured sites bit-exact."""
     import torch
-    c, values, mask, truth = inputs.make_config(5)
-    d_values = torch.from_numpy(values).cuda()
-    d_mask = torch.from_numpy(mask).cuda()
+    c, d_values, d_mask, n_free = config5
     out = {}
     for path in ("TILED", "PLAIN"):
-        g = mpr.Mpr(d_values, d_mask, mode="SP_INTRINSIC", seed=c.mpr_seed)
+        g = mpr.Mpr(d_values, d_mask, mode=mode, seed=c.mpr_seed)
         g.set_path(path)
         g.set_quench(2)
         g.set_temperature(1.1e-3)
@@ -414,7 +421,7 @@ def test_bench_configuration_full_size_properties(mpr, inputs):
             assert bool(torch.isfinite(free).all())
             zmin, zmax = g.info()["z_min"], g.info()["z_max"]
             assert float(free.min()) >= zmin - 1e-9 and float(free.max()) <= zmax + 1e-9   # R1 confines predictions
-            assert cnt[1] == 3 * int(mask.sum()) and cnt[0] > 0
+            assert cnt[1] == 3 * n_free and cnt[0] > 0
         g.close()
         del g
     assert torch.equal(out["TILED"][0], out["PLAIN"][0])
