@@ -82,11 +82,64 @@ __device__ __forceinline__ double u53(uint32_t a, uint32_t b) {
 __device__ __forceinline__ float sym_word(uint32_t a) { return static_cast<float>(static_cast<int32_t>(a)); }
 __device__ __forceinline__ float pos_word(uint32_t a) { return static_cast<float>(a); }
 
+// ---- double-precision sin/cos/exp on the ranges the Metropolis move needs ---------------------
+// The library sincos(double) / exp(double) are written for any argument: Cody-Waite reduction,
+// quadrant logic, a Payne-Hanek slow path behind a branch, and coefficients that the compiler
+// rebuilds from immediates at every use (ncu, DP sweep kernel: UMOV 13.7 % of all executed
+// instructions, BRA/BSSY/BSYNC 4.3 % of the instructions and 13 % of the stall samples, real
+// DFMA/DMUL/DADD only 32 %).  The move calls them on fixed, small ranges:
+//   sincos(q Delta / 2):  |q Delta / 2| = |Delta| / 4 <= delta / 4 <= pi / 4   (R7: delta <= pi, q = 1/2)
+//   exp(-dE / T) is compared with u2 in [0, 1): only arguments <= 0 decide anything.
+// So both are branch-free Taylor polynomials whose coefficients +-1/n! (exact quotients of integers
+// below 2^53, correctly rounded by the host compiler) sit in constant memory and enter each DFMA
+// as a constant-bank operand.  Truncation errors are below half an ulp: sin stops at x^17
+// (next term (pi/4)^19 / 19! = 8e-20), cos at x^16 ((pi/4)^18 / 18! = 2e-18), exp at r^13 with
+// |r| <= ln 2 / 2 (r^14 / 14! = 4e-18).
+__constant__ double kSinC[8] = {-1.0 / 6.0, 1.0 / 120.0, -1.0 / 5040.0, 1.0 / 362880.0, -1.0 / 39916800.0,
+                                1.0 / 6227020800.0, -1.0 / 1307674368000.0, 1.0 / 355687428096000.0};
+__constant__ double kCosC[8] = {-1.0 / 2.0, 1.0 / 24.0, -1.0 / 720.0, 1.0 / 40320.0, -1.0 / 3628800.0,
+                                1.0 / 479001600.0, -1.0 / 87178291200.0, 1.0 / 20922789888000.0};
+__constant__ double kExpC[12] = {1.0 / 2.0, 1.0 / 6.0, 1.0 / 24.0, 1.0 / 120.0, 1.0 / 720.0, 1.0 / 5040.0,
+                                 1.0 / 40320.0, 1.0 / 362880.0, 1.0 / 3628800.0, 1.0 / 39916800.0,
+                                 1.0 / 479001600.0, 1.0 / 6227020800.0};
+
+// sin and cos of x, |x| <= pi/4 (no range reduction: the caller guarantees the range)
+__device__ __forceinline__ void sincos_quarter(double x, double* s, double* c) {
+  const double z = x * x;
+  double ps = kSinC[7], pc = kCosC[7];
+#pragma unroll
+  for (int i = 6; i >= 0; --i) { ps = fma(ps, z, kSinC[i]); pc = fma(pc, z, kCosC[i]); }
+  *s = fma(x * z, ps, x);        // x + x^3 (S1 + S2 z + ...)
+  *c = fma(z, pc, 1.0);          // 1 + z (C1 + C2 z + ...)
+}
+
+// exp(min(y, 0)): for y >= 0 the result is exactly 1, which exceeds every u2 in [0, 1) -- the same
+// decision as "accept if dE <= 0".  y = k ln 2 + r, |r| <= ln 2 / 2; 2^k is applied as two exact
+// power-of-two factors 2^(k >> 1) 2^(k - (k >> 1)), both normal for k >= -1075, so that results in
+// the subnormal range are rounded once, by the last multiplication.  Below -745.2 the result is 0.
+__device__ __forceinline__ double exp_nonpos(double y) {
+  y = fmin(y, 0.0);
+  const double yc = fmax(y, -745.2);
+  const double t = fma(yc, 1.4426950408889634, 6755399441055744.0);   // rint(y log2 e) in the low word
+  const int k = __double2loint(t);
+  const double kd = t - 6755399441055744.0;
+  double r = fma(kd, -0.6931471805599453, yc);                        // ln 2, high part
+  r = fma(kd, -2.3190468138462996e-17, r);                            // ln 2, low part
+  double p = kExpC[11];
+#pragma unroll
+  for (int i = 10; i >= 0; --i) p = fma(p, r, kExpC[i]);
+  p = fma(r * r, p, r) + 1.0;                                         // 1 + r + r^2 (1/2 + r/6 + ...)
+  const int k1 = k >> 1, k2 = k - k1;
+  p = p * __hiloint2double((k1 + 1023) << 20, 0);
+  p = p * __hiloint2double((k2 + 1023) << 20, 0);
+  return y < -745.2 ? 0.0 : p;
+}
+
 // ---- function-precision policies (X_F) -----------------------------------
 template <int MODE> struct Fn;
 template <> struct Fn<MODE_DP> {
-  static __device__ __forceinline__ void sincos_(double x, double* s, double* c) { sincos(x, s, c); }
-  static __device__ __forceinline__ double exp_(double x) { return exp(x); }
+  static __device__ __forceinline__ void sincos_(double x, double* s, double* c) { sincos_quarter(x, s, c); }
+  static __device__ __forceinline__ double exp_(double x) { return exp_nonpos(x); }
   static __device__ __forceinline__ double div_(double a, double b) { return a / b; }
   static __device__ __forceinline__ double rsqrt_(double x) { return 1.0 / sqrt(x); }
   static __device__ __forceinline__ double atan2_(double y, double x) { return atan2(y, x); }
