@@ -33,7 +33,7 @@ if ROOT not in sys.path:
 METRIC = "mpr_site_updates_per_s"
 UNIT = "site-updates/s"
 CPU_CROP = 4096          # cpu_baseline / reference arm: top-left CPU_CROP^2 window of the workload
-CPU_EQ, CPU_MEAS = 60, 2  # ~1.9e9 site-updates: 10-20 s on 16 host threads
+CPU_EQ, CPU_MEAS = 110, 4  # ~3.4e9 site-updates: ~15 s on the 16 host threads of the B200 box (measured 2.3e8 /s)
 ALG_WARP_INST_PER_32_UNITS = 125.0   # Metropolis 91 + over-relaxation 34 per unit and sweep
 # dram__bytes_read.sum + dram__bytes_write.sum of one launch of the dominant kernel at L = 16384, from the
 # committed `ncu --set full` capture (profiles/r01g_ncu_full_tiled_v4.md); None for configurations not captured.
