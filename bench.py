@@ -284,7 +284,10 @@ def run_ours(args, rank, world, local_rank):
             _, e_m, se_m = gm.run(0, 5, want_pred=False)
             b.record()
             torch.cuda.synchronize(dev)
+            # same definitions as `roofline` above: every stored spin read and written once + the mask bits
+            md_bytes = stored * 2 * (16 if md == "DP" else 8) + 2 * stored / 8.0
             modes[md] = {"ms_per_sweep": t, "site_updates_per_s": 2.0 * state["n_free"] / (t * 1e-3),
+                         "hbm_roofline_frac": md_bytes / (t * 1e-3) / 1e9 / peak,
                          "ms_per_measurement_sweep": a.elapsed_time(b) / 5,
                          # mean of 5 samples taken 3 + n_sw sweeps after the chain reset: NOT an equilibrium
                          # value and not comparable between modes (n_sw differs); a plausibility figure only
