@@ -18,7 +18,8 @@ def mpr_mod():
 
 
 def declared_symbols():
-    text = open(os.path.join(ROOT, "include", "mpr.h")).read()
+    with open(os.path.join(ROOT, "include", "mpr.h")) as fh:
+        text = fh.read()
     text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
     return sorted(set(re.findall(r"\b(mpr_[a-z_0-9]+)\s*\(", text)))
 
@@ -69,6 +70,7 @@ def test_product_does_not_import_oracle():
     for dirpath, _, files in os.walk(pkg):
         for f in files:
             if f.endswith((".py", ".cu", ".cuh", ".h")):
-                text = open(os.path.join(dirpath, f)).read()
+                with open(os.path.join(dirpath, f)) as fh:
+                    text = fh.read()
                 for needle in ("import oracle", "from oracle", "mpr_oracle", "oracle/", "oracle."):
                     assert needle not in text, (f, needle)
