@@ -182,7 +182,7 @@ def run_ours(args, rank, world, local_rank):
     seed = rp.mpr_seed
 
     state = {"launches": 0, "sweeps": 0, "n_free": int(mask.sum()), "T": None, "trials": None, "pred": None,
-             "e": None, "se": None}
+             "e": None, "se": None, "eq_ms": 0.0, "eq_launches": 0}
 
     def step():
         g = mpr.Mpr(d_values, d_mask, mode=mode, seed=seed, device=dev)
@@ -193,6 +193,11 @@ def run_ours(args, rank, world, local_rank):
         else:
             T, es, nt = g.estimate_temperature()
         pred, e, se = g.run(n_eq, n_meas)
+        # the equilibration phase of run() = back-to-back launches of the dominant kernel alone, timed by
+        # CUDA events on the library's stream INSIDE this step (mpr_get_run_timing)
+        eq_ms, eq_l, _ = g.run_timing()
+        state["eq_ms"] += eq_ms
+        state["eq_launches"] += eq_l
         state["launches"] += g.launches()
         sw = nt * 250 + n_eq + n_meas
         state["sweeps"] += sw
@@ -209,6 +214,8 @@ def run_ours(args, rank, world, local_rank):
         step()
     state["launches"] = 0
     state["sweeps"] = 0
+    state["eq_ms"] = 0.0
+    state["eq_launches"] = 0
     barrier()
     clocks = ClockSampler(local_rank)
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
@@ -242,8 +249,12 @@ def run_ours(args, rank, world, local_rank):
     g.sweep(n_l * args.fused)
     k1.record()
     torch.cuda.synchronize(dev)
-    kern_ms = k0.elapsed_time(k1) / n_l
+    kern_ms_burst = k0.elapsed_time(k1) / n_l      # the kernel timed alone, 50 launches after the steps
     g.close()
+    # roofline uses the average launch duration INSIDE the timed steps (sustained clocks); the burst leg
+    # is reported beside it and stands in only when the steps had no equilibration sweeps
+    in_step = state["eq_launches"] > 0
+    kern_ms = state["eq_ms"] / state["eq_launches"] if in_step else kern_ms_burst
     w = 16 if mode == "DP" else 8
     Wp = (((L + 1) // 2 + 15) // 16) * 16
     stored = 2 * L * Wp
@@ -260,6 +271,9 @@ def run_ours(args, rank, world, local_rank):
     roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                 "traffic": NCU_TRAFFIC_BYTES.get((mode, args.fused)) if L == 16384 else None, "kernel": "tiled_sweep_kernel<%s,0>" % mode,
                 "kernel_ms": kern_ms,
+                "kernel_ms_source": ("CUDA events around the %d equilibration launches inside the timed steps "
+                                     "(mpr_get_run_timing)" % state["eq_launches"]) if in_step else "burst leg",
+                "kernel_ms_burst": kern_ms_burst, "frac_burst": alg_bytes / (kern_ms_burst * 1e-3) / 1e9 / peak,
                 "algorithmic_bytes_per_launch": alg_bytes, "sweeps_per_launch": args.fused, "peak_source": peak_src,
                 "kernel_site_updates_per_s": 2.0 * state["n_free"] * args.fused / (kern_ms * 1e-3),
                 "second_ceiling": alu}

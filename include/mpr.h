@@ -140,6 +140,15 @@ int mpr_energy(mpr_ctx* ctx, double* H, double* e);
 int mpr_sample_energy(mpr_ctx* ctx, double* e_sample, int64_t* n_pairs);
 /* Accepted / attempted Metropolis moves and hybrid sweeps since the last chain reset.      */
 int mpr_get_counters(mpr_ctx* ctx, uint64_t* accepted, uint64_t* attempted, uint64_t* sweeps);
+/* Device time of the EQUILIBRATION phase of the last mpr_run: the n_eq hybrid sweeps that carry no
+ * measurement, i.e. back-to-back launches of the sweep kernel alone (on the tiled path with fused
+ * depth k: ceil(n_eq / k) launches of tiled_sweep_kernel<mode, 0>), timed by two CUDA events on the
+ * ctx stream; the chain reset before them and the measurement sweeps after them are outside.  This
+ * is what bench.py divides to get the dominant kernel's average launch duration INSIDE the timed
+ * step.  HOST outs, each may be NULL.  eq_ms = 0 and eq_launches = 0 when n_eq
+ * was 0.  MPR_ERR_NOT_READY before the first mpr_run.  The two events are the only CUDA objects the
+ * library creates; mpr_destroy releases them.                                               */
+int mpr_get_run_timing(mpr_ctx* ctx, double* eq_ms, int64_t* eq_launches, int64_t* eq_sweeps);
 /* e_n of the last mpr_run, copied to HOST out[0..cap); returns their number (>= 0).        */
 int64_t mpr_get_energy_series(mpr_ctx* ctx, double* out, int64_t cap);
 /* z_min, z_max of the measured sample and the number of prediction sites.  HOST outs.      */

@@ -77,6 +77,11 @@ struct mpr_ctx {
   uint64_t attempted = 0;
   long long n_acc = 0;
   int cur = 0;                 // which state buffer holds the chain
+  // timing of the equilibration phase of the last mpr_run (mpr_get_run_timing): two events on the
+  // ctx stream, created on first use, destroyed with the ctx
+  cudaEvent_t ev_eq[2] = {nullptr, nullptr};
+  double last_eq_ms = -1.0;
+  long long last_eq_launches = 0, last_eq_sweeps = 0;
   double T = -1.0;
   double zmin = 0.0, zmax = 0.0;
   double e_sample = 0.0;
@@ -513,7 +518,12 @@ int mpr_create(mpr_ctx** out, int L, const double* d_values, const uint8_t* d_ma
   return MPR_OK;
 }
 
-void mpr_destroy(mpr_ctx* ctx) { delete ctx; }
+void mpr_destroy(mpr_ctx* ctx) {
+  if (!ctx) return;
+  for (cudaEvent_t e : ctx->ev_eq)
+    if (e) cudaEventDestroy(e);
+  delete ctx;
+}
 
 int mpr_set_precision(mpr_ctx* c, mpr_precision mode) {
   if (!c || mode < MPR_DP || mode > MPR_SP_INTRINSIC) return fail(c, MPR_ERR_INVALID_ARG, "bad mode");
@@ -624,7 +634,13 @@ int mpr_run(mpr_ctx* c, int n_eq, int n_meas, double* d_pred, double* e_mean, do
   if (!c || n_eq < 0 || n_meas < 0 || n_meas > kSeriesCap) return fail(c, MPR_ERR_INVALID_ARG, "bad sweep counts");
   if (!(c->T > 0.0)) return fail(c, MPR_ERR_NOT_READY, "temperature not set");
   TRY(ensure_chain(c));
+  for (cudaEvent_t& e : c->ev_eq)
+    if (!e) CUDA_OK(c, cudaEventCreate(&e));
+  const uint64_t launches0 = c->launches;
+  CUDA_OK(c, cudaEventRecord(c->ev_eq[0], c->stream));      // after the chain reset, if one was due
   TRY(hybrid_sweeps(c, n_eq, 0, 0));
+  CUDA_OK(c, cudaEventRecord(c->ev_eq[1], c->stream));
+  const long long eq_launches = static_cast<long long>(c->launches - launches0);
   TRY(hybrid_sweeps(c, n_meas, 2, 0));
   if (d_pred) {
     const Geom& g = c->lo.g;
@@ -635,6 +651,21 @@ int mpr_run(mpr_ctx* c, int n_eq, int n_meas, double* d_pred, double* e_mean, do
   }
   TRY(fetch_series(c, n_meas));
   mean_stderr(c->series, e_mean, e_stderr);
+  CUDA_OK(c, cudaEventSynchronize(c->ev_eq[1]));
+  float ms = 0.0f;
+  CUDA_OK(c, cudaEventElapsedTime(&ms, c->ev_eq[0], c->ev_eq[1]));
+  c->last_eq_ms = n_eq > 0 ? static_cast<double>(ms) : 0.0;   // two adjacent events are a few us apart, not 0
+  c->last_eq_launches = eq_launches;
+  c->last_eq_sweeps = n_eq;
+  return MPR_OK;
+}
+
+int mpr_get_run_timing(mpr_ctx* c, double* eq_ms, int64_t* eq_launches, int64_t* eq_sweeps) {
+  if (!c) return MPR_ERR_INVALID_ARG;
+  if (c->last_eq_ms < 0.0) return fail(c, MPR_ERR_NOT_READY, "no mpr_run yet");
+  if (eq_ms) *eq_ms = c->last_eq_ms;
+  if (eq_launches) *eq_launches = c->last_eq_launches;
+  if (eq_sweeps) *eq_sweeps = c->last_eq_sweeps;
   return MPR_OK;
 }
 

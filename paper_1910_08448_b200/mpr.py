@@ -27,7 +27,8 @@ SYMBOLS = [
     "mpr_workspace_bytes", "mpr_create", "mpr_destroy", "mpr_set_precision", "mpr_set_seed",
     "mpr_set_temperature", "mpr_set_quench", "mpr_set_path", "mpr_set_fused_sweeps", "mpr_reset_chain",
     "mpr_estimate_temperature", "mpr_run", "mpr_sweep", "mpr_pass", "mpr_get_state", "mpr_set_state",
-    "mpr_energy", "mpr_sample_energy", "mpr_get_counters", "mpr_get_energy_series", "mpr_get_info",
+    "mpr_energy", "mpr_sample_energy", "mpr_get_counters", "mpr_get_run_timing", "mpr_get_energy_series",
+    "mpr_get_info",
     "mpr_get_launch_stats", "mpr_workspace_bytes_host", "mpr_predict_host", "mpr_debug_philox",
     "mpr_last_error", "mpr_status_string",
 ]
@@ -79,6 +80,7 @@ def lib():
         "mpr_energy": (C.c_int, [vp, dp, dp]),
         "mpr_sample_energy": (C.c_int, [vp, dp, i64p]),
         "mpr_get_counters": (C.c_int, [vp, u64p, u64p, u64p]),
+        "mpr_get_run_timing": (C.c_int, [vp, dp, i64p, i64p]),
         "mpr_get_energy_series": (i64, [vp, dp, i64]),
         "mpr_get_info": (C.c_int, [vp, dp, dp, i64p, dp]),
         "mpr_get_launch_stats": (C.c_int, [vp, u64p]),
@@ -244,6 +246,12 @@ class Mpr:
         a, b, n, T = C.c_double(), C.c_double(), C.c_int64(), C.c_double()
         self._call(lib().mpr_get_info, C.byref(a), C.byref(b), C.byref(n), C.byref(T))
         return {"z_min": a.value, "z_max": b.value, "n_free": n.value, "T": T.value}
+
+    def run_timing(self):
+        """(device ms, launches, sweeps) of the equilibration phase of the last run() -- mpr_get_run_timing."""
+        ms, nl, ns = C.c_double(), C.c_int64(), C.c_int64()
+        self._call(lib().mpr_get_run_timing, C.byref(ms), C.byref(nl), C.byref(ns))
+        return ms.value, nl.value, ns.value
 
     def launches(self):
         n = C.c_uint64()

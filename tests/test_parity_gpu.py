@@ -222,6 +222,30 @@ def test_no_root_is_reported(mpr):
     assert ei.value.code == mpr.ERR_NO_ROOT
 
 
+def test_run_timing_reports_the_equilibration_launches(mpr, inputs):
+    """mpr_get_run_timing: device time, launches and sweeps of the equilibration phase of the last run
+    (what bench.py divides to get the dominant kernel's average duration inside the timed step)."""
+    values, mask, _ = make(inputs, 300, 12.0, 4, 0.66)
+    g = mpr.Mpr(values, mask, mode="SP_INTRINSIC", seed=5)
+    g.set_temperature(0.05)
+    with pytest.raises(mpr.MprError) as ei:
+        g.run_timing()
+    assert ei.value.code == mpr.ERR_NOT_READY
+    g.run(20, 3)
+    ms, launches, sweeps = g.run_timing()
+    assert (launches, sweeps) == (20, 20) and 0.0 < ms < 1000.0       # tiled, one sweep per launch
+    g.set_fused_sweeps(4)
+    g.run(18, 2)
+    ms4, launches4, sweeps4 = g.run_timing()
+    assert (launches4, sweeps4) == (5, 18) and ms4 > 0.0                # 4 + 4 + 4 + 4 + 2
+    g.run(0, 2)
+    assert g.run_timing() == (0.0, 0, 0)
+    g.set_path("PLAIN")
+    g.run(3, 1)
+    assert g.run_timing()[1:] == (12, 3)                                # one launch per colour pass
+    g.close()
+
+
 # --------------------------------------------------------------------------- determinism contract
 @pytest.mark.parametrize("mode", ["DP", "SP", "SP_PRECISE", "SP_INTRINSIC"])
 def test_paths_and_fused_depths_are_bit_identical(mpr, inputs, mode):
