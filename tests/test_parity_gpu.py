@@ -386,6 +386,74 @@ def test_float_modes_at_low_temperature(mpr, inputs, lognormal, f, T):
         assert abs(e_m - e_ref) <= 3.0 * math.hypot(se_m, se_ref), (mode, e_m, e_ref, se_m, se_ref)   # (b)
 
 
+# --------------------------------------------------------------------------- BASELINE configs at their actual sizes
+def _float_mode_gates(mpr, inputs, dv, dm, truth, mask, modes, seed, T, n_eq, n_meas, e_o, se_o, mae_o, rmse_o):
+    """north_star's statistical gates for the float modes against the DP oracle run (e_o, se_o, mae_o, rmse_o)."""
+    for mode in modes:
+        g = mpr.Mpr(dv, dm, mode=mode, seed=seed)
+        g.set_temperature(T)
+        pred, e, se = g.run(n_eq, n_meas)
+        mae, rmse = inputs.prediction_errors(pred.cpu().numpy(), truth, mask)
+        g.close()
+        assert abs(e - e_o) <= 3.0 * math.hypot(se, se_o), (mode, e, e_o, se, se_o)
+        assert abs(mae / mae_o - 1.0) <= 0.01, (mode, mae, mae_o)
+        assert abs(rmse / rmse_o - 1.0) <= 0.01, (mode, rmse, rmse_o)
+
+
+def test_config2_actual_size(mpr, oracle_mod, inputs):
+    """BASELINE.json configs[1] as stated: L = 512, 66 % masked, temperature inferred by energy matching,
+    1000 + 100 sweeps, DP versus SP storage.  DP: the whole procedure (T-matching trials, run) equals the
+    oracle's -- same T_hat, same accepted-move count, same prediction; SP: the statistical gates."""
+    import torch
+    c, values, mask, truth = inputs.make_config(2)
+    dv, dm = torch.from_numpy(values).cuda(), torch.from_numpy(mask).cuda()
+    o = oracle_mod.Oracle(values=values, mask=mask, seed=c.mpr_seed, threads=oracle_mod.threads_available())
+    g = mpr.Mpr(dv, dm, seed=c.mpr_seed)
+    T_o, es_o, n_o = o.estimate_temperature()
+    T_g, es_g, n_g = g.estimate_temperature()
+    assert n_g == n_o and abs(es_g - es_o) <= 1e-12 and abs(T_g - T_o) <= 1e-9 * T_o
+    pred_o, e_o, se_o = o.run(c.n_eq, c.n_meas)
+    pred_g, e_g, se_g = g.run(c.n_eq, c.n_meas)
+    pred_g = pred_g.cpu().numpy()
+    m1 = mask == 1
+    zmin, zmax = o.zrange()
+    assert g.counters() == o.counters()                               # every accept/reject decision of 1100 sweeps
+    assert np.array_equal(pred_g[~m1], values[~m1])
+    assert np.max(np.abs(pred_g[m1] - pred_o[m1])) <= 1e-8 * (zmax - zmin)
+    assert abs(e_g - e_o) <= 1e-11
+    g.close()
+    mae_o, rmse_o = inputs.prediction_errors(pred_o, truth, mask)
+    assert mae_o < 0.5 * float(np.mean(np.abs(truth[m1] - values[~m1].mean())))     # it predicts (sanity, not parity)
+    _float_mode_gates(mpr, inputs, dv, dm, truth, mask, ("SP",), c.mpr_seed, T_o, c.n_eq, c.n_meas, e_o, se_o,
+                      mae_o, rmse_o)
+
+
+def test_config3_actual_size(mpr, oracle_mod, inputs):
+    """BASELINE.json configs[2] as stated: L = 2048 lognormal field (spins crowded near phi = 0, T_hat ~ 1e-3: the
+    float-precision stress case), 33 % masked, 1000 + 100 sweeps, all four modes at the oracle's T_hat.
+    DP equals the oracle over the whole run; SP, SP_PRECISE and SP_INTRINSIC meet the statistical gates."""
+    import torch
+    c, values, mask, truth = inputs.make_config(3)
+    dv, dm = torch.from_numpy(values).cuda(), torch.from_numpy(mask).cuda()
+    o = oracle_mod.Oracle(values=values, mask=mask, seed=c.mpr_seed, threads=oracle_mod.threads_available())
+    T_o, _, _ = o.estimate_temperature()
+    assert 1e-4 < T_o < 1e-2
+    pred_o, e_o, se_o = o.run(c.n_eq, c.n_meas)
+    g = mpr.Mpr(dv, dm, seed=c.mpr_seed)
+    g.set_temperature(T_o)
+    pred_g, e_g, se_g = g.run(c.n_eq, c.n_meas)
+    pred_g = pred_g.cpu().numpy()
+    m1 = mask == 1
+    zmin, zmax = o.zrange()
+    assert g.counters() == o.counters()
+    assert np.max(np.abs(pred_g[m1] - pred_o[m1])) <= 1e-8 * (zmax - zmin)
+    assert abs(e_g - e_o) <= 1e-11
+    g.close()
+    mae_o, rmse_o = inputs.prediction_errors(pred_o, truth, mask)
+    _float_mode_gates(mpr, inputs, dv, dm, truth, mask, ("SP", "SP_PRECISE", "SP_INTRINSIC"), c.mpr_seed, T_o,
+                      c.n_eq, c.n_meas, e_o, se_o, mae_o, rmse_o)
+
+
 # --------------------------------------------------------------------------- large grids
 def test_dp_large_ragged_grid_matches_oracle(mpr, oracle_mod, inputs):
     """L = 4100 (69 x 103 DP tiles, ragged tail in both directions, plane padding columns): every
