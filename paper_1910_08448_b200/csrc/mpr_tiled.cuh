@@ -36,10 +36,14 @@ template <int MODE> struct TileCfg;
 // DP 4.279 -> 4.221, SP 3.555 -> 3.531, SP_PRECISE 1.616 -> 1.570, but SP_INTRINSIC 1.229 -> 1.247
 // (at its 80-register cap the barrier ids spill, and its barrier waits were already covered by the
 // second resident CTA), so that mode keeps __syncthreads.
-template <> struct TileCfg<MODE_DP>           { static constexpr int TH = 48, NT = 256; static constexpr bool PAIR_SYNC = true; };
-template <> struct TileCfg<MODE_SP>           { static constexpr int TH = 96, NT = 256; static constexpr bool PAIR_SYNC = true; };
-template <> struct TileCfg<MODE_SP_PRECISE>   { static constexpr int TH = 96, NT = 512; static constexpr bool PAIR_SYNC = true; };
-template <> struct TileCfg<MODE_SP_INTRINSIC> { static constexpr int TH = 96, NT = 384; static constexpr bool PAIR_SYNC = false; };
+// UNROLL: rows of a warp per iteration of the pass loop (0 = all RPW rows).  Even, so the row
+// parities stay compile-time.  Double arithmetic: 2 keeps the code within the registers.  Float
+// arithmetic, A/B at 1965 MHz, ms per sweep, full unroll -> 4: SP_INTRINSIC 1.2266 -> 1.2199 (and half
+// the code), SP_PRECISE 1.570 -> 1.630, so only SP_INTRINSIC takes 4.
+template <> struct TileCfg<MODE_DP>           { static constexpr int TH = 48, NT = 256, UNROLL = 2; static constexpr bool PAIR_SYNC = true; };
+template <> struct TileCfg<MODE_SP>           { static constexpr int TH = 96, NT = 256, UNROLL = 2; static constexpr bool PAIR_SYNC = true; };
+template <> struct TileCfg<MODE_SP_PRECISE>   { static constexpr int TH = 96, NT = 512, UNROLL = 0; static constexpr bool PAIR_SYNC = true; };
+template <> struct TileCfg<MODE_SP_INTRINSIC> { static constexpr int TH = 96, NT = 384, UNROLL = 4; static constexpr bool PAIR_SYNC = false; };
 
 inline int tiled_max_fused() { return 4; }
 
@@ -240,9 +244,9 @@ __device__ __forceinline__ int pass_rows(const TileView<MODE>& t, uint32_t mcol,
   int n_acc = 0;
   // keeps the bit tests where they are used (hoisted out of the sweep loop they cost 24 registers)
   asm volatile("" : "+r"(mcol), "+r"(cnt));
-  // float arithmetic: fully unrolled (the window rotation is register renaming); double arithmetic:
-  // two rows per iteration, which keeps the parities constant and the code within the registers
-  constexpr int kUnroll = sizeof(typename Traits<MODE>::real) == 8 ? 2 : RPW;
+  // unrolled bodies rotate the window by register renaming; the depth is per mode (TileCfg::UNROLL)
+  constexpr int kUnroll = TileCfg<MODE>::UNROLL == 0 ? RPW : TileCfg<MODE>::UNROLL;
+  static_assert(kUnroll % 2 == 0 && RPW % kUnroll == 0, "row parities must be compile-time constants");
 #pragma unroll kUnroll
   for (int i = 0; i < RPW; ++i) {
     const int par = (COL + i) & 1;
