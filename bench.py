@@ -56,6 +56,8 @@ def parse():
     ap.add_argument("--skip-cpu-baseline", action="store_true")
     ap.add_argument("--skip-modes", action="store_true")
     ap.add_argument("--skip-e2e", action="store_true")
+    ap.add_argument("--microbench", action="store_true",
+                    help="build and run tests/helpers/pipe_microbench.cu (pipe throughputs, L2 / HBM copy) and exit")
     return ap.parse_args()
 
 
@@ -369,8 +371,22 @@ def run_ours(args, rank, world, local_rank):
         dist.destroy_process_group()
 
 
+def run_microbench():
+    """Measured per-SM pipe throughputs and copy bandwidths (JSON lines on stdout): the denominators of the
+    "alu" ceilings, taken on the box the bench runs on."""
+    src = os.path.join(ROOT, "tests", "helpers", "pipe_microbench.cu")
+    with tempfile.TemporaryDirectory() as td:
+        exe = os.path.join(td, "pipe_microbench")
+        subprocess.run([os.environ.get("NVCC", "nvcc"), "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-o", exe, src],
+                       check=True)
+        subprocess.run([exe], check=True)
+
+
 def main():
     args = parse()
+    if args.microbench:
+        run_microbench()
+        return
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))

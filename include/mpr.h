@@ -25,7 +25,7 @@
  *   - Errors: every call returns 0 (MPR_OK) or a negative mpr_status.  Nothing is thrown,
  *     printed or aborted.  mpr_last_error() gives a text for the last failure of a context.
  *   - Ordering: all device work is enqueued on the context's stream.  Calls that return
- *     host scalars (create, estimate_temperature, run, get_counters, get_energy_series,
+ *     host scalars (create, set_workspace, estimate_temperature, run, get_counters, get_energy_series,
  *     get_launch_stats) synchronise that stream before returning; the others are asynchronous.
  *   - Determinism: for fixed (inputs, seed, mode, T) the spin state after any number of
  *     sweeps is bit-identical for every kernel path, tile size and fused depth.
@@ -87,10 +87,24 @@ int mpr_workspace_bytes(int L, size_t* bytes);
  * used (run, sweep, pass, get/set_state, energy, counters) -- create + set_precision +
  * set_seed costs one initialisation, not three.
  * Fails with INVALID_ARG, WORKSPACE, NO_MEASURED, DEGENERATE_RANGE, NONFINITE or CUDA;
- * *out is null on failure.                                                                 */
+ * *out is null on failure.
+ * Two-step form (the problem statement first, resources afterwards): pass d_workspace = NULL and
+ * workspace_bytes = 0; the context is then created without touching the device and every compute
+ * call returns MPR_ERR_WORKSPACE until mpr_set_workspace has attached one.                  */
 int mpr_create(mpr_ctx** out, int L, const double* d_values, const uint8_t* d_mask,
                void* d_workspace, size_t workspace_bytes, void* cuda_stream);
 void mpr_destroy(mpr_ctx* ctx); /* frees the host struct only */
+
+/* Attaches (or replaces) the caller-owned device workspace: >= mpr_workspace_bytes(L) bytes, 256-byte
+ * aligned, borrowed for the life of the context.  Runs the set-up described under mpr_create on the
+ * context's stream (R1 range and map, sample energy of R6, mask bitmaps) and marks the chain for
+ * re-initialisation; mode, seed, temperature and the other settings are kept.  Synchronises the
+ * stream.  Fails with WORKSPACE, NO_MEASURED, DEGENERATE_RANGE, NONFINITE or CUDA; on failure the
+ * context has no workspace.                                                                 */
+int mpr_set_workspace(mpr_ctx* ctx, void* d_workspace, size_t workspace_bytes);
+/* The cudaStream_t all later device work of the context is enqueued on (0 = default stream).  Work
+ * already enqueued on the previous stream is waited for first, so the chain continues unchanged. */
+int mpr_set_stream(mpr_ctx* ctx, void* cuda_stream);
 
 /* Re-encodes the spins for `mode` and resets the chain (trial 0).                          */
 int mpr_set_precision(mpr_ctx* ctx, mpr_precision mode);
@@ -130,9 +144,11 @@ int mpr_sweep(mpr_ctx* ctx, int n);
  * stream of sweep number `sweep`), 1 = over-relaxation, 2 = quench.                        */
 int mpr_pass(mpr_ctx* ctx, int kind, int colour, uint64_t sweep);
 
-/* Spins as angles, d_phi f64[L*L] row-major (parity tests, checkpoint).                    */
+/* Spins as angles, d_phi f64[L*L] row-major (parity tests).  State only: the sweep counter, the move
+ * counters and the prediction accumulator are not part of it.                              */
 int mpr_get_state(mpr_ctx* ctx, double* d_phi);
-/* Overwrites the spins at the prediction sites from d_phi (measured sites keep R1's map). */
+/* Overwrites the spins at the prediction sites from d_phi (measured sites keep R1's map); angles
+ * outside [0, 2pi] are clamped to the nearer end.  Counters and accumulator are left alone.  */
 int mpr_set_state(mpr_ctx* ctx, const double* d_phi);
 /* Energy of the current state: H (Eq. 2) and e = 2H/N_b.  HOST outs.                       */
 int mpr_energy(mpr_ctx* ctx, double* H, double* e);
@@ -166,6 +182,22 @@ int mpr_predict_host(int L, const double* h_values, const uint8_t* h_mask, mpr_p
                      uint64_t seed, double T, int n_eq, int n_meas, void* d_workspace,
                      size_t workspace_bytes, void* cuda_stream, double* h_pred, double* e_mean,
                      double* e_stderr, double* T_used, uint64_t* launches);
+
+/* HOST-only hooks into the library's host-side numerics, so that they can be pinned against
+ * hand-worked numbers without a GPU (tests/test_host_logic.py); no device work, no context.
+ *   mpr_debug_series_stats       mean and binned standard error (R16) of h_series[0..n), exactly
+ *                                the routine mpr_run and the temperature trials use.
+ *   mpr_debug_match_temperature  the root search of R6 (steps 1-5 in DESIGN.md) as
+ *                                mpr_estimate_temperature runs it, with the trial chains replaced by
+ *                                the caller's function: trial(T, trial_index (1, 2, ...), &e, &se, user)
+ *                                returns 0 and the mean energy / standard error "measured" at T.
+ *                                Returns MPR_OK and T_hat, or MPR_ERR_NO_ROOT; *n_trials = trials made.
+ *   mpr_debug_proposal_width     the Metropolis proposal half-width delta(T) of R7 the kernels are given. */
+double mpr_debug_proposal_width(double T);
+typedef int (*mpr_trial_fn)(double T, int trial_index, double* e, double* se, void* user);
+int mpr_debug_series_stats(const double* h_series, int64_t n, double* mean, double* se);
+int mpr_debug_match_temperature(double e_sample, mpr_trial_fn trial, void* user, double* T_hat,
+                                int* n_trials);
 
 /* The Philox4x32-10 block function and the uniform the kernels use, evaluated on the DEVICE
  * for n counters (tests pin the in-kernel generator against the CUDA toolkit's own).

@@ -134,7 +134,9 @@ double proposal_width(double T) {
 // O2 / R8 first half: free spins i.i.d. uniform on [0, 2pi) from Philox (pass = INIT).
 void init_random(Oracle& o, uint32_t trial) {
   const uint32_t key[2] = {static_cast<uint32_t>(o.seed), static_cast<uint32_t>(o.seed >> 32)};
-  for (size_t s = 0; s < o.N(); ++s) {
+  const long long n = static_cast<long long>(o.N());
+#pragma omp parallel for schedule(static) num_threads(o.threads)
+  for (long long s = 0; s < n; ++s) {
     if (!o.mask[s]) continue;
     const uint32_t ctr[4] = {static_cast<uint32_t>(s), 0u, PASS_INIT, trial};
     uint32_t r[4];
@@ -348,32 +350,30 @@ void trial_energy(Oracle& o, double T, double* e, double* se) {
 
 // R6: conditional energy matching.  Find T with e_cond(T) = e_s by bracketing on
 // [1e-4, 1] (expanded by decades within [1e-6, 1e2]) and Illinois regula falsi.
-int estimate_temperature(Oracle& o, double* T_hat, double* e_sample) {
-  double es = 0.0;
-  long long nsp = 0;
-  const int st = sample_energy(o, &es, &nsp);
-  if (st != OK) return st;
-  if (e_sample) *e_sample = es;
-  o.est_trials = 0;
+// `trial(T, &e, &se)` runs one temperature trial; the search itself never looks at the chain,
+// so a test can hand it a synthetic e(T) (orc_debug_match_temperature) and follow the
+// iterates by hand.
+template <typename Trial>
+int match_temperature(double es, Trial&& trial, double* T_hat) {
   double T_lo = 1e-4, T_hi = 1.0, g_lo, g_hi, e, se;
   bool have_hi = false;
-  trial_energy(o, T_lo, &e, &se);
+  trial(T_lo, &e, &se);
   g_lo = e - es;
   while (g_lo > 0.0) {
     if (T_lo <= 1.5e-6) return ERR_NO_ROOT;
     T_hi = T_lo; g_hi = g_lo; have_hi = true;
     T_lo /= 10.0;
-    trial_energy(o, T_lo, &e, &se);
+    trial(T_lo, &e, &se);
     g_lo = e - es;
   }
   if (!have_hi) {
-    trial_energy(o, T_hi, &e, &se);
+    trial(T_hi, &e, &se);
     g_hi = e - es;
     while (g_hi < 0.0) {
       if (T_hi >= 0.99e2) return ERR_NO_ROOT;
       T_lo = T_hi; g_lo = g_hi;
       T_hi *= 10.0;
-      trial_energy(o, T_hi, &e, &se);
+      trial(T_hi, &e, &se);
       g_hi = e - es;
     }
   }
@@ -382,7 +382,7 @@ int estimate_temperature(Oracle& o, double* T_hat, double* e_sample) {
   for (int it = 0; it < kMaxIllinois; ++it) {
     T_new = T_hi - g_hi * (T_hi - T_lo) / (g_hi - g_lo);
     if (!(T_new > T_lo && T_new < T_hi)) T_new = 0.5 * (T_lo + T_hi);
-    trial_energy(o, T_new, &e, &se);
+    trial(T_new, &e, &se);
     const double g = e - es;
     if (std::fabs(g) <= 2.0 * se) break;
     if (g < 0.0) {
@@ -397,9 +397,23 @@ int estimate_temperature(Oracle& o, double* T_hat, double* e_sample) {
     if (it > 0 && std::fabs(T_new - T_prev) / T_new < 0.01) break;
     T_prev = T_new;
   }
-  o.T = T_new;
-  reset_chain(o, 0);
   if (T_hat) *T_hat = T_new;
+  return OK;
+}
+
+int estimate_temperature(Oracle& o, double* T_hat, double* e_sample) {
+  double es = 0.0;
+  long long nsp = 0;
+  const int st = sample_energy(o, &es, &nsp);
+  if (st != OK) return st;
+  if (e_sample) *e_sample = es;
+  o.est_trials = 0;
+  double T_found = 0.0;
+  const int sr = match_temperature(es, [&](double T, double* e, double* se) { trial_energy(o, T, e, se); }, &T_found);
+  if (sr != OK) return sr;
+  o.T = T_found;
+  reset_chain(o, 0);
+  if (T_hat) *T_hat = T_found;
   return OK;
 }
 
@@ -419,7 +433,17 @@ void orc_mean_stderr(const double* v, long n, double* mean, double* se) {
 
 // O0 (R1): phi = 2pi (z - zmin)/(zmax - zmin), min/max over the measured sample.
 // mask[s] = 1 -> prediction site (value never read).  Returns a handle or null + status.
+static void* create_impl(int L, const double* values, const uint8_t* mask, int* status, bool reset);
 void* orc_create(int L, const double* values, const uint8_t* mask, int* status) {
+  return create_impl(L, values, mask, status, true);
+}
+// Same map, but the chain is NOT initialised: the caller sets threads / seed / quench count first and
+// then calls orc_configure, so that a large grid pays for one R8 initialisation (on all threads)
+// instead of three single-threaded ones.
+void* orc_create_deferred(int L, const double* values, const uint8_t* mask, int* status) {
+  return create_impl(L, values, mask, status, false);
+}
+static void* create_impl(int L, const double* values, const uint8_t* mask, int* status, bool reset) {
   auto fail = [&](int code) -> void* { if (status) *status = code; return nullptr; };
   if (L < 2 || !values || !mask) return fail(ERR_INVALID_ARG);
   Oracle* o = new Oracle;
@@ -443,7 +467,7 @@ void* orc_create(int L, const double* values, const uint8_t* mask, int* status) 
   o->zmin = zmin; o->zmax = zmax;
   for (size_t s = 0; s < N; ++s)
     if (!mask[s]) o->phi[s] = kTwoPi * ((values[s] - zmin) / (zmax - zmin));
-  reset_chain(*o, 0);
+  if (reset) reset_chain(*o, 0);
   if (status) *status = OK;
   return o;
 }
@@ -479,6 +503,14 @@ int orc_set_quench(void* h, int n) {
   if (n < 0) return ERR_INVALID_ARG;
   Oracle& o = *static_cast<Oracle*>(h);
   o.n_quench = n;
+  reset_chain(o, 0);
+  return OK;
+}
+int orc_configure(void* h, uint64_t seed, int n_quench) {
+  if (n_quench < 0) return ERR_INVALID_ARG;
+  Oracle& o = *static_cast<Oracle*>(h);
+  o.seed = seed;
+  o.n_quench = n_quench;
   reset_chain(o, 0);
   return OK;
 }
@@ -602,6 +634,15 @@ int orc_estimate_temperature(void* h, double* T_hat, double* e_sample, int* n_tr
   Oracle& o = *static_cast<Oracle*>(h);
   const int st = estimate_temperature(o, T_hat, e_sample);
   if (n_trials) *n_trials = o.est_trials;
+  return st;
+}
+
+// Pins: the R6 search on a caller-supplied e(T) (no chain involved).  trial(T, index, &e, &se, user).
+int orc_debug_match_temperature(double e_sample, int (*trial)(double, int, double*, double*, void*), void* user,
+                                double* T_hat, int* n_trials) {
+  int n = 0;
+  const int st = match_temperature(e_sample, [&](double T, double* e, double* se) { trial(T, ++n, e, se, user); }, T_hat);
+  if (n_trials) *n_trials = n;
   return st;
 }
 

@@ -30,6 +30,8 @@ def build(force: bool = False) -> str:
     return _LIB
 
 
+TRIAL_FN = C.CFUNCTYPE(C.c_int, C.c_double, C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_double), C.c_void_p)
+
 _lib = None
 
 
@@ -46,6 +48,8 @@ def lib():
             "orc_proposal_width": (C.c_double, [C.c_double]),
             "orc_mean_stderr": (None, [dp, C.c_long, dp, dp]),
             "orc_create": (vp, [C.c_int, dp, u8p, C.POINTER(C.c_int)]),
+            "orc_create_deferred": (vp, [C.c_int, dp, u8p, C.POINTER(C.c_int)]),
+            "orc_configure": (C.c_int, [vp, C.c_uint64, C.c_int]),
             "orc_create_from_phi": (vp, [C.c_int, dp, u8p]),
             "orc_destroy": (None, [vp]),
             "orc_set_seed": (C.c_int, [vp, C.c_uint64]),
@@ -72,6 +76,7 @@ def lib():
             "orc_get_series": (C.c_long, [vp, dp, C.c_long]),
             "orc_estimate_temperature": (C.c_int, [vp, dp, dp, C.POINTER(C.c_int)]),
             "orc_trial_energy": (C.c_int, [vp, C.c_double, C.c_int, dp, dp]),
+            "orc_debug_match_temperature": (C.c_int, [C.c_double, TRIAL_FN, vp, dp, C.POINTER(C.c_int)]),
         }
         for name, (res, args) in sig.items():
             fn = getattr(L, name)
@@ -116,7 +121,9 @@ def mean_stderr(v):
 class Oracle:
     """One MPR problem held by the CPU oracle.  `mask` = 1 marks a prediction site."""
 
-    def __init__(self, values=None, mask=None, phi=None, seed=None, threads=1):
+    def __init__(self, values=None, mask=None, phi=None, seed=None, threads=1, n_quench=None):
+        """n_quench given: large-grid form -- the chain is initialised once, on `threads` threads, with
+        (seed, n_quench) (orc_create_deferred + orc_configure) instead of once per setter."""
         L_ = lib()
         mask = np.ascontiguousarray(mask, dtype=np.uint8)
         self.L = int(mask.shape[0])
@@ -130,9 +137,14 @@ class Oracle:
         else:
             values = np.ascontiguousarray(values, dtype=np.float64)
             st = C.c_int()
-            self.h = L_.orc_create(self.L, _dp(values), mask.ctypes.data_as(C.POINTER(C.c_uint8)), C.byref(st))
+            create = L_.orc_create if n_quench is None else L_.orc_create_deferred
+            self.h = create(self.L, _dp(values), mask.ctypes.data_as(C.POINTER(C.c_uint8)), C.byref(st))
             if not self.h:
                 raise OracleError(st.value)
+            if n_quench is not None:
+                self.set_threads(threads)
+                self._chk(L_.orc_configure(self.h, int(seed or 0), int(n_quench)))
+                return
         if threads != 1:
             self.set_threads(threads)
         if seed is not None:
@@ -244,6 +256,20 @@ class Oracle:
         e, se = C.c_double(), C.c_double()
         self._chk(lib().orc_trial_energy(self.h, float(T), int(trial_index), C.byref(e), C.byref(se)))
         return e.value, se.value
+
+
+def match_temperature(e_sample, energy_of_T):
+    """The oracle's R6 search on a Python function T -> (e, se).  Returns (status, T_hat, [T asked])."""
+    asked = []
+
+    def cb(T, idx, e, se, _user):
+        asked.append(T)
+        e[0], se[0] = energy_of_T(T)
+        return 0
+
+    T, n = C.c_double(), C.c_int()
+    st = lib().orc_debug_match_temperature(float(e_sample), TRIAL_FN(cb), None, C.byref(T), C.byref(n))
+    return st, T.value, asked
 
 
 def threads_available():

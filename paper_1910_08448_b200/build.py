@@ -12,7 +12,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 LIB = os.path.join(_HERE, "libmpr.so")
 SOURCES = ["mpr.cu"]
-HEADERS = ["mpr_device.cuh", "mpr_plain.cuh", "mpr_tiled.cuh", os.path.join("..", "..", "include", "mpr.h")]
+HEADERS = ["mpr_device.cuh", "mpr_host_math.hpp", "mpr_plain.cuh", "mpr_tiled.cuh", os.path.join("..", "..", "include", "mpr.h")]
 
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",

@@ -15,6 +15,7 @@
 #include <cuda_runtime.h>
 
 #include "mpr_device.cuh"
+#include "mpr_host_math.hpp"
 #include "mpr_plain.cuh"
 #include "mpr_tiled.cuh"
 
@@ -28,7 +29,7 @@ constexpr int kMaxL = 32768;
 constexpr int kPartials = 1 << 18;       // doubles
 constexpr int kSeriesCap = 1 << 16;      // energy samples per mpr_run
 constexpr int kAcceptSlots = 1024;
-constexpr int kTrialEq = 200, kTrialMeas = 50, kMaxIllinois = 20;   // R6
+constexpr int kTrialEq = 200, kTrialMeas = 50;   // R6: sweeps of one temperature trial
 
 size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
@@ -153,32 +154,11 @@ ChainConst<R> chain_const(const mpr_ctx* c) {
   return k;
 }
 
-// Mean and binned standard error (R16): 10 equal bins if n >= 20, else bins of one sample;
-// unbiased variance of the bin means over the number of bins.
+// Mean and binned standard error of a series (R16): mpr_host_math.hpp.
 void mean_stderr(const std::vector<double>& v, double* mean, double* se) {
-  const size_t n = v.size();
-  double m = 0.0;
-  for (double x : v) m += x;
-  m = n ? m / static_cast<double>(n) : std::numeric_limits<double>::quiet_NaN();
-  double s = 0.0;
-  if (n >= 2) {
-    const size_t nb = n >= 20 ? 10 : n;
-    const size_t len = n / nb;
-    std::vector<double> bm(nb, 0.0);
-    double bmean = 0.0;
-    for (size_t b = 0; b < nb; ++b) {
-      for (size_t k = 0; k < len; ++k) bm[b] += v[b * len + k];
-      bm[b] /= static_cast<double>(len);
-      bmean += bm[b];
-    }
-    bmean /= static_cast<double>(nb);
-    double var = 0.0;
-    for (size_t b = 0; b < nb; ++b) var += (bm[b] - bmean) * (bm[b] - bmean);
-    var /= static_cast<double>(nb - 1);
-    s = std::sqrt(var / static_cast<double>(nb));
-  }
-  if (mean) *mean = m;
-  if (se) *se = s;
+  const mpr_host::SeriesStats st = mpr_host::series_stats(v.data(), v.size());
+  if (mean) *mean = st.mean;
+  if (se) *se = st.stderr_;
 }
 
 // ---- mode dispatch ---------------------------------------------------------------------------
@@ -261,7 +241,7 @@ template <int MODE> int tiled_sweeps(mpr_ctx* c, int k, int measure, double* d_e
   int ntiles = 0;
   const int st = tiled_launch<MODE>(c->tiled, g, c->state(c->cur), c->state(1 - c->cur), c->bits(), c->acc(),
                                     c->part(), c->slots(), chain_const<R>(c), static_cast<uint32_t>(c->sweep + 1), k,
-                                    measure, c->stream, &ntiles);
+                                    measure, c->stream, &ntiles, kPartials);
   if (st != 0) return fail(c, MPR_ERR_CUDA, std::string("tiled launch: ") + tiled_error(st));
   c->launches += 1;
   c->cur = 1 - c->cur;
@@ -323,6 +303,7 @@ int do_tiled(mpr_ctx* c, int k, int measure, double* d_e) {
 // R8: uniform initial spins, then n_quench x (quench colour 0, quench colour 1); everything
 // that belongs to the chain is cleared.
 int reset_chain(mpr_ctx* c, uint32_t trial) {
+  if (!c->ws) return fail(c, MPR_ERR_WORKSPACE, "no workspace attached (mpr_set_workspace)");
   c->stale = false;
   c->trial = trial;
   c->sweep = 0;
@@ -361,7 +342,10 @@ void mark_stale(mpr_ctx* c) {
   c->n_acc = 0;
   c->series.clear();
 }
-int ensure_chain(mpr_ctx* c) { return c->stale ? reset_chain(c, 0) : MPR_OK; }
+int ensure_chain(mpr_ctx* c) {
+  if (!c->ws) return fail(c, MPR_ERR_WORKSPACE, "no workspace attached (mpr_set_workspace)");
+  return c->stale ? reset_chain(c, 0) : MPR_OK;
+}
 
 // measure: 0 = sweeps only, 1 = + energy sample per sweep, 2 = + accumulation of phi.
 // n hybrid sweeps (R4); with `measure`, each is followed by the energy sample into
@@ -496,7 +480,8 @@ int mpr_create(mpr_ctx** out, int L, const double* d_values, const uint8_t* d_ma
   *out = nullptr;
   if (L < 2 || L > kMaxL || !d_values || !d_mask) return MPR_ERR_INVALID_ARG;
   const Layout lo = make_layout(L);
-  if (!d_workspace || (reinterpret_cast<uintptr_t>(d_workspace) & 255u) || workspace_bytes < lo.total)
+  const bool with_ws = d_workspace || workspace_bytes;
+  if (with_ws && (!d_workspace || (reinterpret_cast<uintptr_t>(d_workspace) & 255u) || workspace_bytes < lo.total))
     return MPR_ERR_WORKSPACE;
   int ndev = 0;
   if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) return MPR_ERR_CUDA;
@@ -505,16 +490,39 @@ int mpr_create(mpr_ctx** out, int L, const double* d_values, const uint8_t* d_ma
   c->lo = lo;
   c->d_values = d_values;
   c->d_mask = d_mask;
-  c->ws = static_cast<char*>(d_workspace);
   c->stream = static_cast<cudaStream_t>(cuda_stream);
+  // SURVEY 8(b) form: create(L, values, mask) first, mpr_set_workspace / mpr_set_stream afterwards
+  if (with_ws) {
+    const int st = mpr_set_workspace(c, d_workspace, workspace_bytes);
+    if (st != MPR_OK) { delete c; return st; }
+  }
+  *out = c;
+  return MPR_OK;
+}
+
+int mpr_set_workspace(mpr_ctx* c, void* d_workspace, size_t workspace_bytes) {
+  if (!c) return MPR_ERR_INVALID_ARG;
+  if (!d_workspace || (reinterpret_cast<uintptr_t>(d_workspace) & 255u) || workspace_bytes < c->lo.total)
+    return fail(c, MPR_ERR_WORKSPACE, "workspace null, misaligned or too small");
+  if (c->ws) CUDA_OK(c, cudaStreamSynchronize(c->stream));   // nothing of ours still runs on the old one
+  c->ws = static_cast<char*>(d_workspace);
   int st = setup(c);
   if (st == MPR_OK) {
     const int ts = tiled_plan_init(&c->tiled, c->lo.g);
     if (ts != 0) st = fail(c, MPR_ERR_CUDA, std::string("tiled plan: ") + tiled_error(ts));
   }
-  if (st == MPR_OK) mark_stale(c);
-  if (st != MPR_OK) { delete c; return st; }
-  *out = c;
+  if (st != MPR_OK) { c->ws = nullptr; return st; }
+  mark_stale(c);
+  return MPR_OK;
+}
+
+int mpr_set_stream(mpr_ctx* c, void* cuda_stream) {
+  if (!c) return MPR_ERR_INVALID_ARG;
+  cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
+  if (s == c->stream) return MPR_OK;
+  // work already enqueued on the old stream must be finished before the new one touches the state
+  if (c->ws) CUDA_OK(c, cudaStreamSynchronize(c->stream));
+  c->stream = s;
   return MPR_OK;
 }
 
@@ -565,57 +573,34 @@ int mpr_reset_chain(mpr_ctx* c, uint32_t trial) {
 
 int mpr_estimate_temperature(mpr_ctx* c, double* T_hat, double* e_sample, int* n_trials) {
   if (!c) return MPR_ERR_INVALID_ARG;
+  if (!c->ws) return fail(c, MPR_ERR_WORKSPACE, "no workspace attached (mpr_set_workspace)");
   if (c->n_pairs == 0) return fail(c, MPR_ERR_NO_MEASURED, "no measured nearest-neighbour pair");
-  const double es = c->e_sample;
-  if (e_sample) *e_sample = es;
-  int trials = 0;
-  double T_lo = 1e-4, T_hi = 1.0, g_lo = 0.0, g_hi = 0.0, e = 0.0, se = 0.0;
-  bool have_hi = false;
-  auto done = [&](int st) { if (n_trials) *n_trials = trials; return st; };
-  TRY(trial_energy(c, &trials, T_lo, &e, &se));
-  g_lo = e - es;
-  while (g_lo > 0.0) {
-    if (T_lo <= 1.5e-6) return done(fail(c, MPR_ERR_NO_ROOT, "e_sample below e(T) for every T >= 1e-6"));
-    T_hi = T_lo; g_hi = g_lo; have_hi = true;
-    T_lo /= 10.0;
-    TRY(trial_energy(c, &trials, T_lo, &e, &se));
-    g_lo = e - es;
+  if (e_sample) *e_sample = c->e_sample;
+  // R6 steps 1-5: the search itself is mpr_host::TemperatureMatcher; this loop only runs the trial
+  // chains it asks for (trial i = fresh chain with i in Philox counter word 3, 200 + 50 sweeps).
+  const double T_before = c->T;
+  mpr_host::TemperatureMatcher search;
+  int trials = 0, st = MPR_OK;
+  while (st == MPR_OK && search.want_trial()) {
+    double e = 0.0, se = 0.0;
+    st = trial_energy(c, &trials, search.T(), &e, &se);
+    if (st == MPR_OK) search.report(e - c->e_sample, se);
   }
-  if (!have_hi) {
-    TRY(trial_energy(c, &trials, T_hi, &e, &se));
-    g_hi = e - es;
-    while (g_hi < 0.0) {
-      if (T_hi >= 0.99e2) return done(fail(c, MPR_ERR_NO_ROOT, "e_sample above e(T) for every T <= 1e2"));
-      T_lo = T_hi; g_lo = g_hi;
-      T_hi *= 10.0;
-      TRY(trial_energy(c, &trials, T_hi, &e, &se));
-      g_hi = e - es;
-    }
+  if (n_trials) *n_trials = trials;
+  if (st == MPR_OK && search.outcome() != mpr_host::TemperatureMatcher::FOUND)
+    st = fail(c, MPR_ERR_NO_ROOT, search.outcome() == mpr_host::TemperatureMatcher::NO_ROOT_BELOW
+                                      ? "e_sample below e(T) for every T >= 1e-6"
+                                      : "e_sample above e(T) for every T <= 1e2");
+  if (st != MPR_OK) {
+    // a failed estimate leaves no trial temperature behind: T as before the call, chain to be rebuilt
+    c->T = T_before;
+    mark_stale(c);
+    return st;
   }
-  double T_new = T_hi, T_prev = T_hi;
-  int last_side = 0;
-  for (int it = 0; it < kMaxIllinois; ++it) {
-    T_new = T_hi - g_hi * (T_hi - T_lo) / (g_hi - g_lo);
-    if (!(T_new > T_lo && T_new < T_hi)) T_new = 0.5 * (T_lo + T_hi);
-    TRY(trial_energy(c, &trials, T_new, &e, &se));
-    const double g = e - es;
-    if (std::fabs(g) <= 2.0 * se) break;
-    if (g < 0.0) {
-      T_lo = T_new; g_lo = g;
-      if (last_side == -1) g_hi *= 0.5;
-      last_side = -1;
-    } else {
-      T_hi = T_new; g_hi = g;
-      if (last_side == +1) g_lo *= 0.5;
-      last_side = +1;
-    }
-    if (it > 0 && std::fabs(T_new - T_prev) / T_new < 0.01) break;
-    T_prev = T_new;
-  }
-  c->T = T_new;
+  c->T = search.result();
   TRY(reset_chain(c, 0));
-  if (T_hat) *T_hat = T_new;
-  return done(MPR_OK);
+  if (T_hat) *T_hat = c->T;
+  return MPR_OK;
 }
 
 int mpr_sweep(mpr_ctx* c, int n) {
@@ -705,6 +690,7 @@ int mpr_energy(mpr_ctx* c, double* H, double* e) {
 
 int mpr_sample_energy(mpr_ctx* c, double* e_sample, int64_t* n_pairs) {
   if (!c) return MPR_ERR_INVALID_ARG;
+  if (!c->ws) return fail(c, MPR_ERR_WORKSPACE, "no workspace attached (mpr_set_workspace)");
   if (n_pairs) *n_pairs = c->n_pairs;
   if (c->n_pairs == 0) return fail(c, MPR_ERR_NO_MEASURED, "no measured nearest-neighbour pair");
   if (e_sample) *e_sample = c->e_sample;
@@ -734,6 +720,7 @@ int64_t mpr_get_energy_series(mpr_ctx* c, double* out, int64_t cap) {
 
 int mpr_get_info(mpr_ctx* c, double* z_min, double* z_max, int64_t* n_free, double* T) {
   if (!c) return MPR_ERR_INVALID_ARG;
+  if (!c->ws) return fail(c, MPR_ERR_WORKSPACE, "no workspace attached (mpr_set_workspace)");
   if (z_min) *z_min = c->zmin;
   if (z_max) *z_max = c->zmax;
   if (n_free) *n_free = c->n_free;
@@ -776,7 +763,8 @@ int mpr_predict_host(int L, const double* h_values, const uint8_t* h_mask, mpr_p
   mpr_ctx* c = nullptr;
   int st = mpr_create(&c, L, d_values, d_mask, d_workspace, core, cuda_stream);
   if (st != MPR_OK) return st;
-  c->mode = mode;
+  st = mpr_set_precision(c, mode);
+  if (st != MPR_OK) { mpr_destroy(c); return st; }
   c->seed = seed;
   if (T > 0.0) {
     c->T = T;
@@ -794,6 +782,30 @@ int mpr_predict_host(int L, const double* h_values, const uint8_t* h_mask, mpr_p
   if (launches) *launches = c->launches;
   mpr_destroy(c);
   return st;
+}
+
+double mpr_debug_proposal_width(double T) { return proposal_width(T); }
+
+int mpr_debug_series_stats(const double* h_series, int64_t n, double* mean, double* se) {
+  if (n < 0 || (n > 0 && !h_series)) return MPR_ERR_INVALID_ARG;
+  const mpr_host::SeriesStats st = mpr_host::series_stats(h_series, static_cast<size_t>(n));
+  if (mean) *mean = st.mean;
+  if (se) *se = st.stderr_;
+  return MPR_OK;
+}
+
+int mpr_debug_match_temperature(double e_sample, mpr_trial_fn trial, void* user, double* T_hat, int* n_trials) {
+  if (!trial) return MPR_ERR_INVALID_ARG;
+  mpr_host::TemperatureMatcher search;
+  while (search.want_trial()) {
+    double e = 0.0, se = 0.0;
+    if (trial(search.T(), search.trials() + 1, &e, &se, user) != 0) return MPR_ERR_INVALID_ARG;
+    search.report(e - e_sample, se);
+  }
+  if (n_trials) *n_trials = search.trials();
+  if (search.outcome() != mpr_host::TemperatureMatcher::FOUND) return MPR_ERR_NO_ROOT;
+  if (T_hat) *T_hat = search.result();
+  return MPR_OK;
 }
 
 int mpr_debug_philox(const uint32_t* d_ctr, const uint32_t key[2], uint32_t* d_out, int64_t n, void* cuda_stream) {

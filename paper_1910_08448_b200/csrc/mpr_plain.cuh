@@ -218,8 +218,11 @@ __global__ void set_state_kernel(const double* __restrict__ phi, Geom g, const u
   if (!mask_bit(bits, g, col, y, j)) return;
   const int x = 2 * j + x_parity(y, col);
   double sn, cs;
-  sincos(0.5 * phi[static_cast<size_t>(y) * g.L + x], &sn, &cs);
-  if (sn < 0.0) sn = 0.0;
+  // angles outside [0, 2pi] are clamped to the nearer end: the stored vector is always a
+  // unit vector on the upper half circle
+  const double p = fmin(fmax(phi[static_cast<size_t>(y) * g.L + x], 0.0), 6.283185307179586476925286766559);
+  sincos(0.5 * p, &sn, &cs);
+  if (sn < 0.0) { sn = 0.0; cs = cs < 0.0 ? -1.0 : 1.0; }
   V v;
   v.x = static_cast<decltype(v.x)>(cs);
   v.y = static_cast<decltype(v.y)>(sn);

@@ -250,7 +250,12 @@ __device__ __forceinline__ int pass_rows(const TileView<MODE>& t, uint32_t mcol,
 #pragma unroll kUnroll
   for (int i = 0; i < RPW; ++i) {
     const int par = (COL + i) & 1;
-    const Unit<S> dn = *reinterpret_cast<const Unit<S>*>(own + kOther + (i + 1) * kRowScalars);
+    // the last row of the last warp has no row below it inside the tile: in a colour-1 pass the address
+    // one row further is row 0 of plane 1, which warp 0 is writing -- read the row itself instead (the
+    // value only feeds row TH - 1, which is stale from the first pass on); in a colour-0 pass it is the
+    // zero-filled pad row behind plane 1
+    const int dn_row = (COL == 1 && i == RPW - 1 && warp == NW - 1) ? i : i + 1;
+    const Unit<S> dn = *reinterpret_cast<const Unit<S>*>(own + kOther + dn_row * kRowScalars);
     n_acc += row_step<MODE, KIND>(par, own + i * kRowScalars, up, mid, dn, (mcol >> (2 * i)) & 1u,
                                   (mcol >> (2 * i + 1)) & 1u, (cnt >> i) & 1u,
                                   site + static_cast<uint32_t>(i) * L + static_cast<uint32_t>(par), sweep, kc);
@@ -292,6 +297,8 @@ tiled_sweep_kernel(const __grid_constant__ CUtensorMap tmap, typename Traits<MOD
     mbar_expect_tx(bar, static_cast<uint32_t>(sizeof(V) * 2 * TH * kTileCols));
     tma_load_3d(t.base, &tmap, bar, 2 * j0, y0, 0);
   }
+  // pad row behind plane 1 (read as "row TH" by the last warp in colour-0 passes): the zero vector
+  if (threadIdx.x < kRowScalars) t.base[2 * TH * kRowScalars + threadIdx.x] = S(0);
   // mask bits of this thread's sites, one register per colour: bit 2 i + {0, 1} of mreg[col] = site
   // (row warp RPW + i, colour col, column jj + {0, 1}) is a prediction site.  (j0 + jj) is even, so
   // both bits sit in one word of the bitmap.
@@ -433,7 +440,7 @@ int tiled_encode(TiledPlan& plan, const Geom& g, void* src, CUtensorMap* map) {
 template <int MODE>
 int tiled_launch(TiledPlan& plan, const Geom& g, void* src, void* dst, const uint32_t* bits, double* acc, double* part,
                  unsigned long long* slots, ChainConst<typename Traits<MODE>::real> kc, uint32_t first_sweep, int k,
-                 int measure, cudaStream_t stream, int* ntiles_out) {
+                 int measure, cudaStream_t stream, int* ntiles_out, long long max_partials) {
   using V = typename Traits<MODE>::vec;
   constexpr int TH = TileCfg<MODE>::TH, NT = TileCfg<MODE>::NT;
   if (!plan.encode) return TILED_NO_DRIVER;
@@ -456,7 +463,9 @@ int tiled_launch(TiledPlan& plan, const Geom& g, void* src, void* dst, const uin
   const int IC = kTileCols - 4 * k, IR = TH - 8 * k;
   const int tiles_x = (g.Wp + IC - 1) / IC, tiles_y = (g.L + IR - 1) / IR;
   const long long ntiles = static_cast<long long>(tiles_x) * tiles_y;
-  if (ntiles > (1 << 18)) return TILED_TOO_MANY;
+  // only the measuring launches write one partial per tile (they always run at k = 1)
+  if ((measure == 1 || measure == 2) && ntiles > max_partials) return TILED_TOO_MANY;
+  if (ntiles > 0x7fffffffLL) return TILED_TOO_MANY;
   if (measure == kTiledQuench)
     tiled_sweep_kernel<MODE, kTiledQuench><<<static_cast<unsigned>(ntiles), NT, smem, stream>>>(
         map, static_cast<V*>(dst), bits, acc, part, slots, g, kc, first_sweep, k, tiles_x);

@@ -24,7 +24,8 @@ PASS_KINDS = {"MET": 0, "OR": 1, "QUENCH": 2}
 
 # every symbol include/mpr.h declares
 SYMBOLS = [
-    "mpr_workspace_bytes", "mpr_create", "mpr_destroy", "mpr_set_precision", "mpr_set_seed",
+    "mpr_workspace_bytes", "mpr_create", "mpr_destroy", "mpr_set_workspace", "mpr_set_stream",
+    "mpr_debug_series_stats", "mpr_debug_match_temperature", "mpr_debug_proposal_width", "mpr_set_precision", "mpr_set_seed",
     "mpr_set_temperature", "mpr_set_quench", "mpr_set_path", "mpr_set_fused_sweeps", "mpr_reset_chain",
     "mpr_estimate_temperature", "mpr_run", "mpr_sweep", "mpr_pass", "mpr_get_state", "mpr_set_state",
     "mpr_energy", "mpr_sample_energy", "mpr_get_counters", "mpr_get_run_timing", "mpr_get_energy_series",
@@ -32,6 +33,9 @@ SYMBOLS = [
     "mpr_get_launch_stats", "mpr_workspace_bytes_host", "mpr_predict_host", "mpr_debug_philox",
     "mpr_last_error", "mpr_status_string",
 ]
+
+# int trial(double T, int trial_index, double* e, double* se, void* user) -- mpr_debug_match_temperature
+TRIAL_FN = C.CFUNCTYPE(C.c_int, C.c_double, C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_double), C.c_void_p)
 
 _lib = None
 
@@ -64,6 +68,11 @@ def lib():
         "mpr_workspace_bytes": (C.c_int, [C.c_int, C.POINTER(C.c_size_t)]),
         "mpr_create": (C.c_int, [C.POINTER(vp), C.c_int, vp, vp, vp, C.c_size_t, vp]),
         "mpr_destroy": (None, [vp]),
+        "mpr_set_workspace": (C.c_int, [vp, vp, C.c_size_t]),
+        "mpr_set_stream": (C.c_int, [vp, vp]),
+        "mpr_debug_proposal_width": (C.c_double, [C.c_double]),
+        "mpr_debug_series_stats": (C.c_int, [dp, i64, dp, dp]),
+        "mpr_debug_match_temperature": (C.c_int, [C.c_double, TRIAL_FN, vp, dp, C.POINTER(C.c_int)]),
         "mpr_set_precision": (C.c_int, [vp, C.c_int]),
         "mpr_set_seed": (C.c_int, [vp, C.c_uint64]),
         "mpr_set_temperature": (C.c_int, [vp, C.c_double]),
@@ -167,6 +176,16 @@ class Mpr:
             self._chk(fn(self.h, *args))
 
     # -- setters -------------------------------------------------------------------------
+    def set_workspace(self, ws):
+        """Attach another caller-owned workspace tensor (uint8, CUDA)."""
+        off = (-ws.data_ptr()) % 256
+        self._call(lib().mpr_set_workspace, ws.data_ptr() + off, ws.numel() - off)
+        self.ws = ws
+
+    def set_stream(self, stream):
+        self._call(lib().mpr_set_stream, stream.cuda_stream if stream is not None else None)
+        self._stream = stream
+
     def set_precision(self, mode):
         self._call(lib().mpr_set_precision, MODES[mode] if isinstance(mode, str) else int(mode))
 
@@ -282,6 +301,40 @@ def predict_host(values, mask, mode="DP", seed=0, T=-1.0, n_eq=100, n_meas=100, 
     if st != MPR_OK:
         raise MprError(st)
     return pred_out, m.value, s.value, Tu.value, nl.value
+
+
+def debug_proposal_width(T):
+    return lib().mpr_debug_proposal_width(float(T))
+
+
+def debug_series_stats(series):
+    """(mean, binned standard error) of a host series by the library's own routine (R16).  No GPU needed."""
+    v = np.ascontiguousarray(series, dtype=np.float64)
+    m, s = C.c_double(), C.c_double()
+    st = lib().mpr_debug_series_stats(v.ctypes.data_as(C.POINTER(C.c_double)), len(v), C.byref(m), C.byref(s))
+    if st != MPR_OK:
+        raise MprError(st)
+    return m.value, s.value
+
+
+def debug_match_temperature(e_sample, energy_of_T):
+    """The library's R6 root search driven by a Python function T -> (e, se).  No GPU needed.
+    Returns (T_hat, [trial temperatures in order])."""
+    asked = []
+
+    def cb(T, idx, e, se, _user):
+        asked.append(T)
+        e[0], se[0] = energy_of_T(T)
+        return 0
+
+    T, n = C.c_double(), C.c_int()
+    st = lib().mpr_debug_match_temperature(float(e_sample), TRIAL_FN(cb), None, C.byref(T), C.byref(n))
+    if st != MPR_OK:
+        err = MprError(st)
+        err.asked = asked
+        raise err
+    assert n.value == len(asked)
+    return T.value, asked
 
 
 def debug_philox(ctr, key, device="cuda:0"):

@@ -49,7 +49,8 @@ def test_create_rejects_bad_arguments_without_gpu(mpr_mod):
     lib = mpr_mod.lib()
     h = C.c_void_p()
     assert lib.mpr_create(C.byref(h), 1, None, None, None, 0, None) == mpr_mod.ERR_INVALID_ARG
-    assert lib.mpr_create(C.byref(h), 8, 256, 256, None, 0, None) == mpr_mod.ERR_WORKSPACE
+    assert lib.mpr_create(C.byref(h), 8, 256, 256, None, 1 << 30, None) == mpr_mod.ERR_WORKSPACE
+    assert lib.mpr_create(C.byref(h), 8, 256, 256, 256, 1024, None) == mpr_mod.ERR_WORKSPACE     # too small
     assert lib.mpr_create(C.byref(h), 8, 256, 256, 257, 1 << 30, None) == mpr_mod.ERR_WORKSPACE
     assert not h.value
 
