@@ -63,12 +63,24 @@ typedef enum {
  * Energy sums are accumulated in double in every mode (R13).                              */
 typedef enum { MPR_DP = 0, MPR_SP = 1, MPR_SP_PRECISE = 2, MPR_SP_INTRINSIC = 3 } mpr_precision;
 
-/* Kernel paths.  Both give bit-identical spin states (determinism contract).
+/* Kernel paths.  All give bit-identical spin states (determinism contract).
+ *   MPR_PATH_STRIP   (default) one launch per k <= 2 hybrid sweeps: every warp streams a column strip of
+ *                    the grid through a private shared-memory ring fed by TMA and runs the colour
+ *                    passes as a software pipeline down the rows (no barriers, no redundant rows).
  *   MPR_PATH_TILED   one launch per hybrid sweep group: TMA stages a tile + halo of both colour
  *                    planes in shared memory, all 4*k colour passes of k sweeps run there.
  *   MPR_PATH_PLAIN   one launch per colour pass on the global colour planes (reference path
- *                    for the self-consistency tests; also used for the R8 quench passes).  */
-typedef enum { MPR_PATH_TILED = 0, MPR_PATH_PLAIN = 1 } mpr_path;
+ *                    for the self-consistency tests; also used for odd R8 quench passes).  */
+typedef enum { MPR_PATH_TILED = 0, MPR_PATH_PLAIN = 1, MPR_PATH_STRIP = 2 } mpr_path;
+
+/* Order of the colour passes inside one hybrid sweep ("hybrid algorithm" -- the paper
+ * leaves the order to its ref. [5]; both orders leave the conditional Boltzmann density invariant):
+ *   MPR_SCHEDULE_R4          (default, R4)  Metropolis colour 0, colour 1, over-relaxation colour 0, 1
+ *   MPR_SCHEDULE_SITE_FUSED  (R4b)  per colour, every site gets its Metropolis move and at once its
+ *                            over-relaxation move (both read only the other colour): colour 0, colour 1.
+ * Same random numbers per (site, sweep); a different, equally valid Markov chain.  Runs on the STRIP
+ * and PLAIN paths.                                                                          */
+typedef enum { MPR_SCHEDULE_R4 = 0, MPR_SCHEDULE_SITE_FUSED = 1 } mpr_schedule;
 
 /* Bytes of workspace mpr_create needs for an L x L grid (any mode).  HOST out pointer.     */
 int mpr_workspace_bytes(int L, size_t* bytes);
@@ -114,10 +126,12 @@ int mpr_set_seed(mpr_ctx* ctx, uint64_t seed);
 int mpr_set_temperature(mpr_ctx* ctx, double T);
 /* Number of quench double-passes of the R8 initialisation (default 32).  Resets the chain. */
 int mpr_set_quench(mpr_ctx* ctx, int n);
-/* Kernel path (default MPR_PATH_TILED) and temporal-blocking depth k >= 1 (hybrid sweeps
- * fused per launch of the tiled kernel, default 1).  Results do not depend on either.      */
+/* Kernel path (default MPR_PATH_STRIP) and temporal-blocking depth 1 <= k <= 4 (hybrid sweeps
+ * fused per launch, default 1; the STRIP path uses min(k, 2)).  Results do not depend on either. */
 int mpr_set_path(mpr_ctx* ctx, mpr_path path);
 int mpr_set_fused_sweeps(mpr_ctx* ctx, int k);
+/* Pass order of a hybrid sweep (see mpr_schedule).  Does not touch the chain.               */
+int mpr_set_schedule(mpr_ctx* ctx, mpr_schedule schedule);
 /* R8: free spins i.i.d. uniform from Philox (pass INIT, `trial` in counter word 3), then the
  * quench passes; sweep counter, move counters and the prediction accumulator are cleared.  */
 int mpr_reset_chain(mpr_ctx* ctx, uint32_t trial);
@@ -141,7 +155,8 @@ int mpr_run(mpr_ctx* ctx, int n_eq, int n_meas, double* d_pred, double* e_mean, 
 /* n hybrid sweeps without measurement (asynchronous).                                      */
 int mpr_sweep(mpr_ctx* ctx, int n);
 /* Single colour passes on the plain path, for tests: kind 0 = Metropolis (uses the Philox
- * stream of sweep number `sweep`), 1 = over-relaxation, 2 = quench.                        */
+ * stream of sweep number `sweep`), 1 = over-relaxation, 2 = quench, 3 = Metropolis followed at
+ * once by over-relaxation at every site of the colour (the pass of the site-fused schedule). */
 int mpr_pass(mpr_ctx* ctx, int kind, int colour, uint64_t sweep);
 
 /* Spins as angles, d_phi f64[L*L] row-major (parity tests).  State only: the sweep counter, the move

@@ -18,6 +18,7 @@
 #include "mpr_host_math.hpp"
 #include "mpr_plain.cuh"
 #include "mpr_tiled.cuh"
+#include "mpr_strip.cuh"
 
 using namespace mpr;
 
@@ -69,7 +70,8 @@ struct mpr_ctx {
   char* ws = nullptr;
   cudaStream_t stream = nullptr;
   int mode = MPR_DP;
-  int path = MPR_PATH_TILED;
+  int path = MPR_PATH_STRIP;
+  int schedule = MPR_SCHEDULE_R4;
   int fused = 1;
   int n_quench = 32;
   uint64_t seed = 0;
@@ -93,6 +95,7 @@ struct mpr_ctx {
   bool stale = true;     // the chain has to be (re)initialised before its next use (ensure_chain)
   std::string err;
   TiledPlan tiled;
+  StripPlan strip;
 
   void* state(int b) const { return ws + lo.off_state[b]; }
   double* acc() const { return reinterpret_cast<double*>(ws + lo.off_acc); }
@@ -172,6 +175,8 @@ template <int MODE> int plain_pass(mpr_ctx* c, int kind, int col, uint64_t sweep
   const uint32_t sw = static_cast<uint32_t>(sweep);
   if (kind == KIND_MET)
     plain_pass_kernel<MODE, KIND_MET><<<grid, block, 0, c->stream>>>(st, c->bits(), g, col, sw, k, c->slots());
+  else if (kind == KIND_MO)
+    plain_pass_kernel<MODE, KIND_MO><<<grid, block, 0, c->stream>>>(st, c->bits(), g, col, sw, k, c->slots());
   else if (kind == KIND_OR)
     plain_pass_kernel<MODE, KIND_OR><<<grid, block, 0, c->stream>>>(st, c->bits(), g, col, sw, k, c->slots());
   else
@@ -253,6 +258,28 @@ template <int MODE> int tiled_sweeps(mpr_ctx* c, int k, int measure, double* d_e
   return MPR_OK;
 }
 
+// One launch of the STRIP path: k sweeps of the current schedule (prog = PROG_R4 / PROG_FUSED) or two quench double
+// passes (PROG_QUENCH, k = 2); `measure` as in tiled_sweeps.
+template <int MODE> int strip_sweeps(mpr_ctx* c, int prog, int k, int measure, double* d_e) {
+  using R = typename Traits<MODE>::real;
+  const Geom& g = c->lo.g;
+  const ChainConst<R> kc = chain_const<R>(c);
+  int nblocks = 0;
+  StripArgs a{&c->strip, &c->tiled, g, c->cur, c->state(c->cur), c->state(1 - c->cur), c->bits(), c->acc(), c->part(),
+              c->slots(), &kc, static_cast<uint32_t>(c->sweep + 1), prog, k, measure, c->stream, &nblocks, kPartials};
+  const int st = MODE == MODE_DP ? strip_launch_mode0(a) : MODE == MODE_SP ? strip_launch_mode1(a)
+                 : MODE == MODE_SP_PRECISE ? strip_launch_mode2(a) : strip_launch_mode3(a);
+  if (st != 0) return fail(c, MPR_ERR_CUDA, std::string("strip launch: ") + tiled_error(st));
+  c->launches += 1;
+  c->cur = 1 - c->cur;
+  if (measure == 1 || measure == 2) {
+    const double nb = 2.0 * g.L * (g.L - 1.0);
+    final_sum_kernel<<<1, 1024, 0, c->stream>>>(c->part(), nblocks, -kJ * 2.0 / nb, d_e);
+    LAUNCH_OK(c);
+  }
+  return MPR_OK;
+}
+
 #define DISPATCH(c, call)                                                     \
   ((c)->mode == MPR_DP           ? call<MODE_DP>                              \
    : (c)->mode == MPR_SP         ? call<MODE_SP>                              \
@@ -300,6 +327,15 @@ int do_tiled(mpr_ctx* c, int k, int measure, double* d_e) {
   }
 }
 
+int do_strip(mpr_ctx* c, int prog, int k, int measure, double* d_e) {
+  switch (c->mode) {
+    case MPR_DP: return strip_sweeps<MODE_DP>(c, prog, k, measure, d_e);
+    case MPR_SP: return strip_sweeps<MODE_SP>(c, prog, k, measure, d_e);
+    case MPR_SP_PRECISE: return strip_sweeps<MODE_SP_PRECISE>(c, prog, k, measure, d_e);
+    default: return strip_sweeps<MODE_SP_INTRINSIC>(c, prog, k, measure, d_e);
+  }
+}
+
 // R8: uniform initial spins, then n_quench x (quench colour 0, quench colour 1); everything
 // that belongs to the chain is cleared.
 int reset_chain(mpr_ctx* c, uint32_t trial) {
@@ -320,6 +356,8 @@ int reset_chain(mpr_ctx* c, uint32_t trial) {
       TRY(do_tiled(c, k, kTiledQuench, nullptr));
       left -= 2 * k;
     }
+  } else if (c->path == MPR_PATH_STRIP) {
+    for (; left >= 2; left -= 2) TRY(do_strip(c, PROG_QUENCH, 2, 0, nullptr));     // two double passes per launch
   }
   for (; left > 0; --left) {
     TRY(do_pass(c, KIND_QUENCH, 0, 0));
@@ -357,10 +395,15 @@ int hybrid_sweeps(mpr_ctx* c, int n, int measure, int first_slot) {
   if (c->path == MPR_PATH_PLAIN) {
     for (int i = 0; i < n; ++i) {
       const uint64_t sw = c->sweep + 1;
-      TRY(do_pass(c, KIND_MET, 0, sw));
-      TRY(do_pass(c, KIND_MET, 1, sw));
-      TRY(do_pass(c, KIND_OR, 0, sw));
-      TRY(do_pass(c, KIND_OR, 1, sw));
+      if (c->schedule == MPR_SCHEDULE_SITE_FUSED) {      // R4b
+        TRY(do_pass(c, KIND_MO, 0, sw));
+        TRY(do_pass(c, KIND_MO, 1, sw));
+      } else {                                            // R4
+        TRY(do_pass(c, KIND_MET, 0, sw));
+        TRY(do_pass(c, KIND_MET, 1, sw));
+        TRY(do_pass(c, KIND_OR, 0, sw));
+        TRY(do_pass(c, KIND_OR, 1, sw));
+      }
       c->sweep = sw;
       c->attempted += static_cast<uint64_t>(c->n_free);
       if (measure) {
@@ -373,11 +416,19 @@ int hybrid_sweeps(mpr_ctx* c, int n, int measure, int first_slot) {
     }
     return MPR_OK;
   }
+  if (c->path == MPR_PATH_TILED && c->schedule != MPR_SCHEDULE_R4)
+    return fail(c, MPR_ERR_INVALID_ARG, "the site-fused schedule runs on the STRIP and PLAIN paths");
   int done = 0;
   while (done < n) {
     // measurement needs the state after every sweep: one sweep per launch there
-    const int k = measure ? 1 : (n - done < c->fused ? n - done : c->fused);
-    TRY(do_tiled(c, k, measure, measure ? c->dseries() + first_slot + done : nullptr));
+    int k = measure ? 1 : (n - done < c->fused ? n - done : c->fused);
+    double* d_e = measure ? c->dseries() + first_slot + done : nullptr;
+    if (c->path == MPR_PATH_STRIP) {
+      if (k > 2) k = 2;                                   // the strip pipeline carries at most two sweeps
+      TRY(do_strip(c, c->schedule == MPR_SCHEDULE_SITE_FUSED ? PROG_FUSED : PROG_R4, k, measure, d_e));
+    } else {
+      TRY(do_tiled(c, k, measure, d_e));
+    }
     c->sweep += static_cast<uint64_t>(k);
     c->attempted += static_cast<uint64_t>(k) * static_cast<uint64_t>(c->n_free);
     if (measure == 2) c->n_acc += 1;
@@ -557,8 +608,15 @@ int mpr_set_quench(mpr_ctx* c, int n) {
   return MPR_OK;
 }
 int mpr_set_path(mpr_ctx* c, mpr_path path) {
-  if (!c || (path != MPR_PATH_TILED && path != MPR_PATH_PLAIN)) return fail(c, MPR_ERR_INVALID_ARG, "bad path");
+  if (!c || (path != MPR_PATH_TILED && path != MPR_PATH_PLAIN && path != MPR_PATH_STRIP))
+    return fail(c, MPR_ERR_INVALID_ARG, "bad path");
   c->path = path;
+  return MPR_OK;
+}
+int mpr_set_schedule(mpr_ctx* c, mpr_schedule schedule) {
+  if (!c || (schedule != MPR_SCHEDULE_R4 && schedule != MPR_SCHEDULE_SITE_FUSED))
+    return fail(c, MPR_ERR_INVALID_ARG, "bad schedule");
+  c->schedule = schedule;     // the chain continues: both orders are valid Markov kernels for the same density
   return MPR_OK;
 }
 int mpr_set_fused_sweeps(mpr_ctx* c, int k) {
@@ -609,8 +667,8 @@ int mpr_sweep(mpr_ctx* c, int n) {
 }
 
 int mpr_pass(mpr_ctx* c, int kind, int colour, uint64_t sweep) {
-  if (!c || kind < 0 || kind > 2) return fail(c, MPR_ERR_INVALID_ARG, "bad pass kind");
-  if (kind == KIND_MET && !(c->T > 0.0)) return fail(c, MPR_ERR_NOT_READY, "temperature not set");
+  if (!c || kind < 0 || kind > 3) return fail(c, MPR_ERR_INVALID_ARG, "bad pass kind");
+  if ((kind == KIND_MET || kind == KIND_MO) && !(c->T > 0.0)) return fail(c, MPR_ERR_NOT_READY, "temperature not set");
   TRY(ensure_chain(c));
   return do_pass(c, kind, colour & 1, sweep);
 }

@@ -22,7 +22,7 @@ namespace mpr {
 
 enum { MODE_DP = 0, MODE_SP = 1, MODE_SP_PRECISE = 2, MODE_SP_INTRINSIC = 3 };
 enum { PASS_INIT = 0, PASS_MET = 1 };  // Philox counter word 2 (R9)
-enum { KIND_MET = 0, KIND_OR = 1, KIND_QUENCH = 2 };
+enum { KIND_MET = 0, KIND_OR = 1, KIND_QUENCH = 2, KIND_MO = 3 };   // MO: Metropolis then over-relaxation in one visit (R4b)
 
 template <int MODE> struct Traits;
 template <> struct Traits<MODE_DP>           { using real = double; using vec = double2; };
@@ -95,11 +95,11 @@ __device__ __forceinline__ float pos_word(uint32_t a) { return static_cast<float
 // as a constant-bank operand.  Truncation errors are below half an ulp: sin stops at x^17
 // (next term (pi/4)^19 / 19! = 8e-20), cos at x^16 ((pi/4)^18 / 18! = 2e-18), exp at r^13 with
 // |r| <= ln 2 / 2 (r^14 / 14! = 4e-18).
-__constant__ double kSinC[8] = {-1.0 / 6.0, 1.0 / 120.0, -1.0 / 5040.0, 1.0 / 362880.0, -1.0 / 39916800.0,
+static __constant__ double kSinC[8] = {-1.0 / 6.0, 1.0 / 120.0, -1.0 / 5040.0, 1.0 / 362880.0, -1.0 / 39916800.0,
                                 1.0 / 6227020800.0, -1.0 / 1307674368000.0, 1.0 / 355687428096000.0};
-__constant__ double kCosC[8] = {-1.0 / 2.0, 1.0 / 24.0, -1.0 / 720.0, 1.0 / 40320.0, -1.0 / 3628800.0,
+static __constant__ double kCosC[8] = {-1.0 / 2.0, 1.0 / 24.0, -1.0 / 720.0, 1.0 / 40320.0, -1.0 / 3628800.0,
                                 1.0 / 479001600.0, -1.0 / 87178291200.0, 1.0 / 20922789888000.0};
-__constant__ double kExpC[12] = {1.0 / 2.0, 1.0 / 6.0, 1.0 / 24.0, 1.0 / 120.0, 1.0 / 720.0, 1.0 / 5040.0,
+static __constant__ double kExpC[12] = {1.0 / 2.0, 1.0 / 6.0, 1.0 / 24.0, 1.0 / 120.0, 1.0 / 720.0, 1.0 / 5040.0,
                                  1.0 / 40320.0, 1.0 / 362880.0, 1.0 / 3628800.0, 1.0 / 39916800.0,
                                  1.0 / 479001600.0, 1.0 / 6227020800.0};
 

@@ -70,7 +70,7 @@ __device__ __forceinline__ double block_sum(double v, double* sh /* >= 32 */) {
 }
 
 // out[0] = scale * sum(partials[0..n)), fixed order; one block.
-__global__ void final_sum_kernel(const double* __restrict__ partials, int n, double scale, double* out) {
+static __global__ void final_sum_kernel(const double* __restrict__ partials, int n, double scale, double* out) {
   __shared__ double sh[32];
   double v = 0.0;
   for (int i = threadIdx.x; i < n; i += blockDim.x) v += partials[i];
@@ -80,7 +80,7 @@ __global__ void final_sum_kernel(const double* __restrict__ partials, int n, dou
 
 // ---- set-up ---------------------------------------------------------------------------------
 // Per-block partials of the measured sample: [0] min, [1] max, [2] count, [3] non-finite count.
-__global__ void sample_range_kernel(const double* __restrict__ z, const uint8_t* __restrict__ mask, size_t N,
+static __global__ void sample_range_kernel(const double* __restrict__ z, const uint8_t* __restrict__ mask, size_t N,
                                     double* __restrict__ part /* 4 per block */) {
   double mn = INFINITY, mx = -INFINITY, cnt = 0.0, bad = 0.0;
   for (size_t i = blockIdx.x * static_cast<size_t>(blockDim.x) + threadIdx.x; i < N;
@@ -110,7 +110,7 @@ __global__ void sample_range_kernel(const double* __restrict__ z, const uint8_t*
     p[0] = mn; p[1] = mx; p[2] = cnt; p[3] = bad;
   }
 }
-__global__ void sample_range_final_kernel(const double* __restrict__ part, int nblocks, double* out /* 4 */) {
+static __global__ void sample_range_final_kernel(const double* __restrict__ part, int nblocks, double* out /* 4 */) {
   if (threadIdx.x != 0 || blockIdx.x != 0) return;
   double mn = INFINITY, mx = -INFINITY, cnt = 0.0, bad = 0.0;
   for (int b = 0; b < nblocks; ++b) {
@@ -126,7 +126,7 @@ __device__ __forceinline__ double map_to_phi(double z, double zmin, double zmax)
 
 // R6 first half: e_s = -2J mean over measured nearest-neighbour pairs of cos[q(phi_s - phi_t)].
 // Per-block partials: [0] sum of cos, [1] pair count.
-__global__ void sample_energy_kernel(const double* __restrict__ z, const uint8_t* __restrict__ mask, int L,
+static __global__ void sample_energy_kernel(const double* __restrict__ z, const uint8_t* __restrict__ mask, int L,
                                      double zmin, double zmax, double* __restrict__ part /* 2 per block */) {
   __shared__ double sh[32];
   double sum = 0.0, cnt = 0.0;
@@ -143,7 +143,7 @@ __global__ void sample_energy_kernel(const double* __restrict__ z, const uint8_t
   const double c = block_sum(cnt, sh);
   if (threadIdx.x == 0) { part[2 * blockIdx.x] = s; part[2 * blockIdx.x + 1] = c; }
 }
-__global__ void pair_final_kernel(const double* __restrict__ part, int nblocks, double* out /* 2 */) {
+static __global__ void pair_final_kernel(const double* __restrict__ part, int nblocks, double* out /* 2 */) {
   if (threadIdx.x != 0 || blockIdx.x != 0) return;
   double s = 0.0, c = 0.0;
   for (int b = 0; b < nblocks; ++b) { s += part[2 * b]; c += part[2 * b + 1]; }
@@ -152,7 +152,7 @@ __global__ void pair_final_kernel(const double* __restrict__ part, int nblocks, 
 
 // Mask bitmaps: one thread per 32-bit word of the PADDED arrays (`base` = their first word);
 // per-block partial = number of set bits.
-__global__ void pack_mask_kernel(const uint8_t* __restrict__ mask, Geom g, uint32_t* __restrict__ base,
+static __global__ void pack_mask_kernel(const uint8_t* __restrict__ mask, Geom g, uint32_t* __restrict__ base,
                                  double* __restrict__ part) {
   __shared__ double sh[32];
   const size_t nwords = static_cast<size_t>(2) * g.Hb * g.Wb;
@@ -267,7 +267,7 @@ plain_pass_kernel(typename Traits<MODE>::vec* __restrict__ state, const uint32_t
     local_field<R>(R(l.x), R(l.y), R(r.x), R(r.y), R(u.x), R(u.y), R(d.x), R(d.y), hl, hr, hu, hd, &A, &B);
     const V me = ld_spin(own, j);
     R c = R(me.x), s = R(me.y);
-    if constexpr (KIND == KIND_MET) {
+    if constexpr (KIND == KIND_MET || KIND == KIND_MO) {
       // R9: the pair (2m, 2m + 1) of plane columns shares one Philox block in the float modes
       const uint32_t pair_site = static_cast<uint32_t>(y) * static_cast<uint32_t>(g.L) +
                                  static_cast<uint32_t>(2 * (j & ~1) + par);
@@ -279,6 +279,11 @@ plain_pass_kernel(typename Traits<MODE>::vec* __restrict__ state, const uint32_t
       met_update2<MODE>(bc2(c), bc2(s), bc2(A), bc2(B), w, w, true, true, k, o, ok);   // the site in both lanes
       c = o[0]; s = o[2];
       accepted = ok[0];
+      if constexpr (KIND == KIND_MO) {     // site-fused schedule (R4b): the over-relaxation move follows at once
+        R o2[4];
+        or_update2<MODE>(bc2(c), bc2(s), bc2(A), bc2(B), true, true, o2);
+        c = o2[0]; s = o2[2];
+      }
     } else if constexpr (KIND == KIND_OR) {
       R o[4];
       or_update2<MODE>(bc2(c), bc2(s), bc2(A), bc2(B), true, true, o);
@@ -291,7 +296,7 @@ plain_pass_kernel(typename Traits<MODE>::vec* __restrict__ state, const uint32_t
     out.y = static_cast<decltype(out.y)>(s);
     st_spin(own, j, out);
   }
-  if constexpr (KIND == KIND_MET) {
+  if constexpr (KIND == KIND_MET || KIND == KIND_MO) {
     const int n = __syncthreads_count(accepted);
     if (threadIdx.x == 0 && n)
       atomicAdd(accept_slots + ((blockIdx.y * gridDim.x + blockIdx.x) & 1023u), static_cast<unsigned long long>(n));
@@ -344,14 +349,14 @@ __global__ void plain_accumulate_kernel(const typename Traits<MODE>::vec* __rest
   acc[i] += spin_angle<MODE>(R(v.x), R(v.y));
 }
 
-__global__ void clear_acc_kernel(double* __restrict__ acc, size_t n) {
+static __global__ void clear_acc_kernel(double* __restrict__ acc, size_t n) {
   for (size_t i = blockIdx.x * static_cast<size_t>(blockDim.x) + threadIdx.x; i < n;
        i += static_cast<size_t>(gridDim.x) * blockDim.x)
     acc[i] = 0.0;
 }
 
 // pred = zmin + (zmax - zmin) * acc / (2pi n_acc) at prediction sites, the input value elsewhere.
-__global__ void predict_kernel(const double* __restrict__ z, const uint8_t* __restrict__ mask, Geom g,
+static __global__ void predict_kernel(const double* __restrict__ z, const uint8_t* __restrict__ mask, Geom g,
                                const double* __restrict__ acc, double zmin, double zmax, long long n_acc,
                                double* __restrict__ pred) {
   const int y = blockIdx.y;
@@ -366,7 +371,7 @@ __global__ void predict_kernel(const double* __restrict__ z, const uint8_t* __re
   pred[s] = zmin + (zmax - zmin) * frac;
 }
 
-__global__ void philox_debug_kernel(const uint32_t* __restrict__ ctr, uint32_t k0, uint32_t k1,
+static __global__ void philox_debug_kernel(const uint32_t* __restrict__ ctr, uint32_t k0, uint32_t k1,
                                     uint32_t* __restrict__ out, long long n) {
   const long long i = blockIdx.x * static_cast<long long>(blockDim.x) + threadIdx.x;
   if (i >= n) return;

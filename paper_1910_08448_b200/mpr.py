@@ -19,14 +19,15 @@ ERR_INVALID_ARG, ERR_NO_MEASURED, ERR_DEGENERATE_RANGE, ERR_NONFINITE = -1, -2, 
 ERR_WORKSPACE, ERR_NOT_READY, ERR_NO_ROOT, ERR_CUDA = -5, -6, -7, -8
 
 MODES = {"DP": 0, "SP": 1, "SP_PRECISE": 2, "SP_INTRINSIC": 3}
-PATHS = {"TILED": 0, "PLAIN": 1}
-PASS_KINDS = {"MET": 0, "OR": 1, "QUENCH": 2}
+PATHS = {"TILED": 0, "PLAIN": 1, "STRIP": 2}
+SCHEDULES = {"R4": 0, "SITE_FUSED": 1}
+PASS_KINDS = {"MET": 0, "OR": 1, "QUENCH": 2, "MO": 3}
 
 # every symbol include/mpr.h declares
 SYMBOLS = [
     "mpr_workspace_bytes", "mpr_create", "mpr_destroy", "mpr_set_workspace", "mpr_set_stream",
     "mpr_debug_series_stats", "mpr_debug_match_temperature", "mpr_debug_proposal_width", "mpr_set_precision", "mpr_set_seed",
-    "mpr_set_temperature", "mpr_set_quench", "mpr_set_path", "mpr_set_fused_sweeps", "mpr_reset_chain",
+    "mpr_set_temperature", "mpr_set_quench", "mpr_set_path", "mpr_set_fused_sweeps", "mpr_set_schedule", "mpr_reset_chain",
     "mpr_estimate_temperature", "mpr_run", "mpr_sweep", "mpr_pass", "mpr_get_state", "mpr_set_state",
     "mpr_energy", "mpr_sample_energy", "mpr_get_counters", "mpr_get_run_timing", "mpr_get_energy_series",
     "mpr_get_info",
@@ -79,6 +80,7 @@ def lib():
         "mpr_set_quench": (C.c_int, [vp, C.c_int]),
         "mpr_set_path": (C.c_int, [vp, C.c_int]),
         "mpr_set_fused_sweeps": (C.c_int, [vp, C.c_int]),
+        "mpr_set_schedule": (C.c_int, [vp, C.c_int]),
         "mpr_reset_chain": (C.c_int, [vp, C.c_uint32]),
         "mpr_estimate_temperature": (C.c_int, [vp, dp, dp, C.POINTER(C.c_int)]),
         "mpr_run": (C.c_int, [vp, C.c_int, C.c_int, vp, dp, dp]),
@@ -200,6 +202,9 @@ class Mpr:
 
     def set_path(self, path):
         self._call(lib().mpr_set_path, PATHS[path] if isinstance(path, str) else int(path))
+
+    def set_schedule(self, schedule):
+        self._call(lib().mpr_set_schedule, SCHEDULES[schedule] if isinstance(schedule, str) else int(schedule))
 
     def set_fused_sweeps(self, k):
         self._call(lib().mpr_set_fused_sweeps, int(k))

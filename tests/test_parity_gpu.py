@@ -97,7 +97,7 @@ def test_error_paths(mpr, inputs):
 
 
 # --------------------------------------------------------------------------- DP parity, pass by pass
-@pytest.mark.parametrize("path", ["PLAIN", "TILED"])
+@pytest.mark.parametrize("path", ["PLAIN", "TILED", "STRIP"])
 @pytest.mark.parametrize("L,xi,f,T", [(64, 8.0, 0.33, 0.07), (97, 8.0, 0.9, 0.02), (250, 16.0, 0.66, 0.3)])
 def test_dp_ten_sweeps_match_oracle(mpr, oracle_mod, inputs, L, xi, f, T, path):
     values, mask, _ = make(inputs, L, xi, 3, f)
@@ -154,7 +154,7 @@ def test_tiny_grids(mpr, oracle_mod, L):
     mask[-1, -1] = 0
     g = mpr.Mpr(z, mask, seed=3)
     o = oracle_mod.Oracle(values=z, mask=mask, seed=3)
-    for path in ("PLAIN", "TILED"):
+    for path in ("PLAIN", "TILED", "STRIP"):
         g.set_path(path)
         g.set_seed(3)
         o.set_seed(3)
@@ -231,6 +231,7 @@ def test_run_timing_reports_the_equilibration_launches(mpr, inputs):
     with pytest.raises(mpr.MprError) as ei:
         g.run_timing()
     assert ei.value.code == mpr.ERR_NOT_READY
+    g.set_path("TILED")
     g.run(20, 3)
     ms, launches, sweeps = g.run_timing()
     assert (launches, sweeps) == (20, 20) and 0.0 < ms < 1000.0       # tiled, one sweep per launch
@@ -243,6 +244,9 @@ def test_run_timing_reports_the_equilibration_launches(mpr, inputs):
     g.set_path("PLAIN")
     g.run(3, 1)
     assert g.run_timing()[1:] == (12, 3)                                # one launch per colour pass
+    g.set_path("STRIP")
+    g.run(9, 1)
+    assert g.run_timing()[1:] == (5, 9)                                 # 2 + 2 + 2 + 2 + 1 at depth min(4, 2)
     g.close()
 
 
@@ -254,7 +258,7 @@ def test_paths_and_fused_depths_are_bit_identical(mpr, inputs, mode):
     g = mpr.Mpr(values, mask, mode=mode, seed=77)
     g.set_temperature(0.05)
     ref = None
-    for path, k in [("PLAIN", 1), ("TILED", 1), ("TILED", 2), ("TILED", 3), ("TILED", 4)]:
+    for path, k in [("PLAIN", 1), ("TILED", 1), ("TILED", 2), ("TILED", 3), ("TILED", 4), ("STRIP", 1), ("STRIP", 2)]:
         g.set_path(path)
         g.set_fused_sweeps(k)
         g.reset_chain(0)
@@ -268,13 +272,30 @@ def test_paths_and_fused_depths_are_bit_identical(mpr, inputs, mode):
             assert cnt == ref[1], (path, k)
     # measurement launches: energies and accumulators agree between the paths
     out = []
-    for path in ("PLAIN", "TILED"):
+    for path in ("PLAIN", "TILED", "STRIP"):
         g.set_path(path)
         g.reset_chain(0)
         pred, e, se = g.run(5, 7)
         out.append((pred.cpu().numpy(), g.series()))
-    assert np.array_equal(out[0][0], out[1][0])
-    np.testing.assert_allclose(out[0][1], out[1][1], rtol=0, atol=1e-13)
+    for other in out[1:]:
+        assert np.array_equal(out[0][0], other[0])
+        np.testing.assert_allclose(out[0][1], other[1], rtol=0, atol=1e-13)
+    # the site-fused schedule (R4b): STRIP at both depths equals the plain per-pass kernels
+    g.set_schedule("SITE_FUSED")
+    ref = None
+    for path, k in [("PLAIN", 1), ("STRIP", 1), ("STRIP", 2)]:
+        g.set_path(path)
+        g.set_fused_sweeps(k)
+        g.reset_chain(0)
+        g.sweep(7)
+        pred, e, se = g.run(2, 3)
+        cur = (g.get_state().cpu().numpy(), g.counters(), pred.cpu().numpy(), g.series())
+        if ref is None:
+            ref = cur
+        else:
+            assert np.array_equal(cur[0], ref[0]) and cur[1] == ref[1], (path, k)
+            assert np.array_equal(cur[2], ref[2]), (path, k)
+            np.testing.assert_allclose(cur[3], ref[3], rtol=0, atol=1e-13)
 
 
 @pytest.mark.parametrize("mode", ["DP", "SP", "SP_PRECISE", "SP_INTRINSIC"])
@@ -291,7 +312,7 @@ def test_pass_synchronisation_stress(mpr, inputs, mode):
     values, mask, _ = make(inputs, L, 48.0, 9, 0.9)
     dv, dm = torch.from_numpy(values).cuda(), torch.from_numpy(mask).cuda()
     out = {}
-    for path, k in (("PLAIN", 1), ("TILED", 4), ("TILED", 1)):
+    for path, k in (("PLAIN", 1), ("TILED", 4), ("TILED", 1), ("STRIP", 2), ("STRIP", 1)):
         g = mpr.Mpr(dv, dm, mode=mode, seed=4242)
         g.set_path(path)
         g.set_fused_sweeps(k)
@@ -303,7 +324,7 @@ def test_pass_synchronisation_stress(mpr, inputs, mode):
         out[(path, k)] = (states, g.counters())
         g.close()
     ref_states, ref_cnt = out[("PLAIN", 1)]
-    for key in (("TILED", 4), ("TILED", 1)):
+    for key in (("TILED", 4), ("TILED", 1), ("STRIP", 2), ("STRIP", 1)):
         states, cnt = out[key]
         assert cnt == ref_cnt, (mode, key, cnt, ref_cnt)
         for i, (a, b) in enumerate(zip(states, ref_states)):
@@ -534,7 +555,7 @@ def test_bench_configuration_full_size_properties(mpr, config5, mode):
     import torch
     c, d_values, d_mask, n_free = config5
     out = {}
-    for path in ("TILED", "PLAIN"):
+    for path in ("TILED", "PLAIN", "STRIP"):
         g = mpr.Mpr(d_values, d_mask, mode=mode, seed=c.mpr_seed)
         g.set_path(path)
         g.set_quench(2)
@@ -545,7 +566,7 @@ def test_bench_configuration_full_size_properties(mpr, config5, mode):
         cnt = g.counters()
         pred, e, se = g.run(0, 2)
         out[path] = (s1, cnt, g.series(), pred)
-        if path == "TILED":
+        if path == "STRIP":                                           # bench.py's path
             m0 = d_mask == 0
             assert torch.equal(s0[m0], s1[m0])                       # measured spins never move
             assert float(s1.min()) >= 0.0 and float(s1.max()) <= TWO_PI + 1e-15
@@ -557,7 +578,8 @@ def test_bench_configuration_full_size_properties(mpr, config5, mode):
             assert cnt[1] == 3 * n_free and cnt[0] > 0
         g.close()
         del g
-    assert torch.equal(out["TILED"][0], out["PLAIN"][0])
-    assert out["TILED"][1] == out["PLAIN"][1]
-    np.testing.assert_allclose(out["TILED"][2], out["PLAIN"][2], rtol=0, atol=1e-12)
-    assert torch.equal(out["TILED"][3], out["PLAIN"][3])
+    for path in ("TILED", "STRIP"):
+        assert torch.equal(out[path][0], out["PLAIN"][0]), path
+        assert out[path][1] == out["PLAIN"][1], path
+        np.testing.assert_allclose(out[path][2], out["PLAIN"][2], rtol=0, atol=1e-12)
+        assert torch.equal(out[path][3], out["PLAIN"][3]), path
