@@ -25,6 +25,7 @@
 // shuffle has no partner) and the rows above the first loaded one do not exist; none of them is
 // ever stored to global memory or counted.
 #pragma once
+#include <type_traits>
 #include <cuda.h>
 #include "mpr_device.cuh"
 #include "mpr_plain.cuh"
@@ -63,9 +64,12 @@ template <int MODE, int NS> struct StripCfg {
   static constexpr int NW = kFit < 12 ? kFit : 12;
 };
 
+// Work distribution.  The rows of all strips are laid end to end (strip s occupies [s Lp, (s + 1) Lp), Lp = L rounded
+// up to a multiple of 4) and cut into equal quotas of `quota` rows (a multiple of 4): warp w of the launch takes
+// [w quota, (w + 1) quota).  A quota that crosses the end of a strip is worked off as two segments.  Warp w is warp
+// slot w / gridDim.x of CTA w % gridDim.x, so that a launch with fewer warps than slots still uses every SM.
 struct StripGeom {
-  int n_strips, n_seg, seg_rows;   // items = n_strips * n_seg, item -> (strip = item % n_strips, seg = item / n_strips)
-  int n_items;
+  int n_strips, Lp, quota, n_warps;
 };
 
 template <int MODE, int NS> constexpr size_t strip_smem_bytes() {
@@ -88,209 +92,239 @@ strip_kernel(const __grid_constant__ CUtensorMap tmap, typename Traits<MODE>::ve
   using P = StripProg<PROG, K>;
   constexpr int NS = P::NS, NW = StripCfg<MODE, NS>::NW, RB = kStripRB, LAG = kStripLag;
   constexpr int NSLOT = strip_slots(NS), HL = strip_halo_lanes(NS), IC = strip_interior_cols(NS);
+  constexpr int LEAD = strip_lead_rows(NS);
   constexpr int CHUNK = 2 * RB * kRowScalars;          // scalars per chunk: [plane][row][128]
   constexpr int PLANE = RB * kRowScalars;
+  constexpr uint32_t kChunkBytes = CHUNK * sizeof(S);
   static_assert(MEASURE == 0 || K == 1, "measuring launches carry one sweep");
   static_assert(LAG * (NS - 1) * 2 + 4 <= 32, "mask queue: 2 bits per row in a 32-bit register");
 
   extern __shared__ __align__(128) unsigned char smem_raw[];
   __shared__ double red[32];
-  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int lane = threadIdx.x & 31;
+  // the shuffle tells the compiler that the warp index is warp-uniform: everything derived from it (quota, strip,
+  // row range, loop bounds) then lives in uniform registers and the loops are known not to diverge
+  const int warp = __shfl_sync(0xffffffffu, static_cast<int>(threadIdx.x >> 5), 0);
   S* const ring = reinterpret_cast<S*>(smem_raw) + static_cast<size_t>(warp) * NSLOT * CHUNK;
   uint64_t* const bars = reinterpret_cast<uint64_t*>(smem_raw + static_cast<size_t>(NW) * NSLOT * CHUNK * sizeof(S)) + warp * NSLOT;
 
-  const int item = blockIdx.x * NW + warp;
   int n_acc = 0;
   double esum = 0.0;
-  if (item < sg.n_items) {
-    const int strip = item % sg.n_strips, seg = item / sg.n_strips;
-    const int j0 = strip * IC - 2 * HL;                       // plane column of lane 0 (even)
-    const int yb = seg * sg.seg_rows;
-    const int ye = min(g.L, yb + sg.seg_rows);
-    const int t0 = yb - strip_lead_rows(NS);                  // first loaded row (multiple of 4 below yb, even)
-    const int n_steps = ye - t0 + LAG * (NS - 1);             // the last stage finishes row ye - 1 in the last step
-    const int n_iter = (n_steps + RB - 1) / RB;
-    const int j = j0 + 2 * lane;
-    const bool lane_ok = lane >= HL && lane < 32 - HL && j < g.Wp;
-
+  const int wg = warp * static_cast<int>(gridDim.x) + static_cast<int>(blockIdx.x);
+  if (wg < sg.n_warps) {
     if (lane == 0) {
 #pragma unroll
       for (int k = 0; k < NSLOT; ++k) mbar_init(bars + k, 1);
     }
     __syncwarp();
-    constexpr uint32_t kChunkBytes = CHUNK * sizeof(S);
-    if (lane == 0) {                                          // chunk 0 -> slot 0
-      mbar_expect_tx(bars, kChunkBytes);
-      tma_load_3d(ring, &tmap, bars, 2 * j0, t0, 0);
-    }
-    // cb[k] = scalar offset (inside this warp's ring) of the chunk  i + 2 - NSLOT + k,  i.e. cb[NSLOT-1] holds
-    // chunk i + 1 (in flight), cb[NSLOT-2] chunk i, cb[0] the oldest live one.  Chunk c lives in slot c % NSLOT.
-    int cb[NSLOT];
-#pragma unroll
-    for (int k = 0; k < NSLOT; ++k) cb[k] = ((k + 2) % NSLOT) * CHUNK;    // iteration 0: chunk k + 2 - NSLOT
-    int slot_next = 1 % NSLOT;                                // slot of chunk i + 1
     uint32_t phase_bits = 0;                                  // bit s = parity the next wait on slot s expects
-
-    // mask bits: queue per colour, 2 bits per row, row t at bits 0..1, row t - d at bits 2d..2d+1
-    uint32_t mq[2] = {0u, 0u};
-    const int sh = j & 31;
-    const uint32_t* bp = mask_word(bits, g, 0, t0, j >> 5);
-    const size_t colour_words = static_cast<size_t>(g.Hb) * g.Wb;
-    uint32_t nxt0 = (__ldg(bp) >> sh) & 3u, nxt1 = (__ldg(bp + colour_words) >> sh) & 3u;    // row t0
-
+    const long long total = static_cast<long long>(sg.n_strips) * sg.Lp;
+    long long q0 = static_cast<long long>(wg) * sg.quota;
+    const long long q1 = min(total, q0 + sg.quota);
     const uint32_t Lu = static_cast<uint32_t>(g.L);
-    uint32_t site_t = static_cast<uint32_t>(t0) * Lu + static_cast<uint32_t>(2 * j);         // Philox word 0 of row t, no parity
-    // global pointers of this lane's unit in row t of plane 0 (dst / accumulator); never dereferenced outside the grid
-    const long long g_t0 = static_cast<long long>(t0) * g.Wp + j;
-    S* gp = reinterpret_cast<S*>(dst) + 2 * g_t0;
-    double* ap = acc + g_t0;
     const long long grow = 2 * static_cast<long long>(g.Wp), gplane = 2 * static_cast<long long>(g.plane);
-
-    mbar_wait(bars, 0);
-    phase_bits ^= 1u;
+    const size_t colour_words = static_cast<size_t>(g.Hb) * g.Wb;
 
 #pragma unroll 1
-    for (int i = 0; i < n_iter; ++i) {
-      // prefetch chunk i + 1 into the slot whose old chunk (i + 1 - NSLOT) nobody reads any more
+    while (q0 < q1) {
+      // ---- one segment: rows [yb, ye) of one strip
+      const int strip = static_cast<int>(q0 / sg.Lp);
+      const int yb = static_cast<int>(q0 - static_cast<long long>(strip) * sg.Lp);     // multiple of 4
+      const int ye_pad = static_cast<int>(min(static_cast<long long>(sg.Lp), yb + (q1 - q0)));
+      q0 += ye_pad - yb;
+      const int ye = min(g.L, ye_pad);
+      if (yb >= ye) continue;
+      const int j0 = strip * IC - 2 * HL;                     // plane column of lane 0 (even)
+      const int t0 = yb - LEAD;                               // first loaded row (a multiple of 4, so even)
+      const int n_steps = ye - t0 + LAG * (NS - 1);           // the last stage finishes row ye - 1 in the last step
+      const int n_iter = (n_steps + RB - 1) / RB;
+      // iterations in which every stage works on an owned, loaded row in all four steps: no predicates needed
+      const int i_lo = (LEAD + LAG * (NS - 1) + RB - 1) / RB;
+      const int i_hi = (ye - t0) / RB;                        // RB i + RB - 1 < ye - t0
+      const int j = j0 + 2 * lane;
+      const bool lane_ok = lane >= HL && lane < 32 - HL && j < g.Wp;
+      int seg_acc = 0;
+
       __syncwarp();
-      if (lane == 0) {
+      if (lane == 0) {                                        // chunk 0 -> slot 0
         fence_proxy_async_smem();
-        mbar_expect_tx(bars + slot_next, kChunkBytes);
-        tma_load_3d(ring + cb[NSLOT - 1], &tmap, bars + slot_next, 2 * j0, t0 + RB * (i + 1), 0);
+        mbar_expect_tx(bars, kChunkBytes);
+        tma_load_3d(ring, &tmap, bars, 2 * j0, t0, 0);
       }
+      // cb[k] = scalar offset (inside this warp's ring) of the chunk  i + 2 - NSLOT + k,  i.e. cb[NSLOT-1] holds
+      // chunk i + 1 (in flight), cb[NSLOT-2] chunk i, cb[0] the oldest live one.  Chunk c lives in slot c % NSLOT.
+      int cb[NSLOT];
 #pragma unroll
-      for (int u = 0; u < RB; ++u) {
-        if (u == RB - 1) {                                    // row 4 i + 4 (first of chunk i + 1) is read from here on
-          mbar_wait(bars + slot_next, (phase_bits >> slot_next) & 1u);
-          phase_bits ^= 1u << slot_next;
-        }
-        const int n = RB * i + u;                             // step number; row t = t0 + n
-        const int t = t0 + n;
-        // ---- mask bits of row t enter the queues; those of row t + 1 are fetched for the next step
-        mq[0] = (mq[0] << 2) | nxt0;
-        mq[1] = (mq[1] << 2) | nxt1;
-        bp += g.Wb;
-        nxt0 = (__ldg(bp) >> sh) & 3u;
-        nxt1 = (__ldg(bp + colour_words) >> sh) & 3u;
+      for (int k = 0; k < NSLOT; ++k) cb[k] = ((k + 2) % NSLOT) * CHUNK;    // iteration 0: chunk k + 2 - NSLOT
+      int slot_next = 1 % NSLOT;                              // slot of chunk i + 1
 
-        // ---- gather: own unit and local fields of every stage (all reads before any write of this step)
-        Two<R> A[NS], B[NS], c[NS], s[NS];
-        S* own[NS];
-        Unit<S> nb_l[1], nb_m[1], nb_u[1], nb_d[1];           // float-mode energy: the last stage's neighbours
-        S exc_last = S(0), exs_last = S(0);
+      // mask bits: one queue per colour, 2 bits per row, row t at bits 0..1, row t - d at bits 2d..2d+1.  The words
+      // are fetched TWO steps ahead (raw, shifted only when they enter the queue) so that their L2 latency is hidden.
+      uint32_t mq[2] = {0u, 0u};
+      const int sh = j & 31;
+      const uint32_t* bp = mask_word(bits, g, 0, t0, j >> 5);
+      uint32_t rawA0 = __ldg(bp), rawA1 = __ldg(bp + colour_words);                       // row t
+      uint32_t rawB0 = __ldg(bp + g.Wb), rawB1 = __ldg(bp + g.Wb + colour_words);         // row t + 1
+      bp += 2 * g.Wb;
+
+      uint32_t site_t = static_cast<uint32_t>(t0) * Lu + static_cast<uint32_t>(2 * j);   // Philox word 0 of row t, no parity
+      // global pointers of this lane's unit in row t of plane 0 (dst / accumulator); never dereferenced outside the grid
+      const long long g_t0 = static_cast<long long>(t0) * g.Wp + j;
+      S* gp = reinterpret_cast<S*>(dst) + 2 * g_t0;
+      double* ap = acc + g_t0;
+
+      mbar_wait(bars, phase_bits & 1u);
+      phase_bits ^= 1u;
+
+      // ---- one iteration = RB steps = the rows of one chunk entering the pipeline
+      auto iteration = [&](int i, auto edge_tag) {
+        constexpr bool EDGE = decltype(edge_tag)::value;
+        // prefetch chunk i + 1 into the slot whose old chunk (i + 1 - NSLOT) nobody reads any more
+        __syncwarp();
+        if (lane == 0) {
+          fence_proxy_async_smem();
+          mbar_expect_tx(bars + slot_next, kChunkBytes);
+          tma_load_3d(ring + cb[NSLOT - 1], &tmap, bars + slot_next, 2 * j0, t0 + RB * (i + 1), 0);
+        }
 #pragma unroll
-        for (int p = 0; p < NS; ++p) {
-          const int col = p & 1, par = (u + col) & 1;         // t0 and LAG are even: x-parity of row t - 2p is (u + col) & 1
-          const int rel = u - LAG * p;                        // row relative to 4 i
-          auto at = [&](int plane, int r) -> S* {
-            const int q = (r >= 0) ? r / RB : -((-r + RB - 1) / RB);      // floor(r / RB)
-            return ring + cb[NSLOT - 2 + q] + plane * PLANE + (r - q * RB) * kRowScalars + 4 * lane;
-          };
-          own[p] = at(col, rel);
-          const Unit<S> up = *reinterpret_cast<const Unit<S>*>(at(1 - col, rel - 1));
-          const Unit<S> mid = *reinterpret_cast<const Unit<S>*>(at(1 - col, rel));
-          const Unit<S> dn = *reinterpret_cast<const Unit<S>*>(at(1 - col, rel + 1));
-          const Unit<S> me = *reinterpret_cast<const Unit<S>*>(own[p]);
-          const S exc = par ? __shfl_down_sync(0xffffffffu, mid.ca, 1) : __shfl_up_sync(0xffffffffu, mid.cb, 1);
-          const S exs = par ? __shfl_down_sync(0xffffffffu, mid.sa, 1) : __shfl_up_sync(0xffffffffu, mid.sb, 1);
-          combine_fields<MODE>(par, up, mid, dn, exc, exs, &A[p], &B[p]);
-          c[p] = mk2(R(me.ca), R(me.cb));
-          s[p] = mk2(R(me.sa), R(me.sb));
-          if (MEASURE != 0 && sizeof(R) == 4 && p == NS - 1) {
-            nb_u[0] = up; nb_m[0] = mid; nb_d[0] = dn; exc_last = exc; exs_last = exs;
+        for (int u = 0; u < RB; ++u) {
+          if (u == RB - 1) {                                  // row 4 i + 4 (first of chunk i + 1) is read from here on
+            mbar_wait(bars + slot_next, (phase_bits >> slot_next) & 1u);
+            phase_bits ^= 1u << slot_next;
           }
-        }
-        (void)nb_l;
+          const int n = RB * i + u;                           // step number; row t = t0 + n
+          const int t = t0 + n;
+          // ---- mask bits of row t enter the queues; those of row t + 2 are requested
+          mq[0] = (mq[0] << 2) | ((rawA0 >> sh) & 3u);
+          mq[1] = (mq[1] << 2) | ((rawA1 >> sh) & 3u);
+          rawA0 = rawB0; rawA1 = rawB1;
+          rawB0 = __ldg(bp); rawB1 = __ldg(bp + colour_words);
+          bp += g.Wb;
 
-        // ---- compute
-        R o[NS][4];
+          // ---- gather: own unit and local fields of every stage (all reads before any write of this step)
+          Two<R> A[NS], B[NS], c[NS], s[NS];
+          S* own[NS];
+          Unit<S> nb_m, nb_u, nb_d;                           // float-mode energy: the last stage's neighbours
+          S exc_last = S(0), exs_last = S(0);
 #pragma unroll
-        for (int p = 0; p < NS; ++p) {
-          const int col = p & 1, par = (u + col) & 1;
-          const uint32_t mbits = mq[col] >> (2 * LAG * p);
-          const bool fa = mbits & 1u, fb = mbits & 2u;
-          const int row = t - LAG * p;
-          const bool counted = lane_ok && row >= yb && row < ye;
-          constexpr int dummy = 0; (void)dummy;
-          const int kind = P::kind(p);
-          if (kind == KIND_MET || kind == KIND_MO) {
-            const uint32_t pair_site = site_t - static_cast<uint32_t>(LAG * p) * Lu + static_cast<uint32_t>(par);
-            MetWords w0, w1;
-            met_words_pair<MODE>(pair_site, first_sweep + static_cast<uint32_t>(P::sweep_off(p)), kc, &w0, &w1);
-            bool ok[2];
-            met_update2<MODE>(c[p], s[p], A[p], B[p], w0, w1, fa, fb, kc, o[p], ok);
-            if (counted) n_acc += static_cast<int>(ok[0]) + static_cast<int>(ok[1]);
-            if (kind == KIND_MO) {
-              R o2[4];
-              or_update2<MODE>(mk2(o[p][0], o[p][1]), mk2(o[p][2], o[p][3]), A[p], B[p], fa, fb, o2);
-              o[p][0] = o2[0]; o[p][1] = o2[1]; o[p][2] = o2[2]; o[p][3] = o2[3];
-            }
-          } else if (kind == KIND_OR) {
-            or_update2<MODE>(c[p], s[p], A[p], B[p], fa, fb, o[p]);
-          } else {
-            quench_update2<MODE>(c[p], s[p], A[p], B[p], fa, fb, o[p]);
-          }
-        }
-
-        // ---- scatter: ring (stages whose row is loaded), global memory (final stage of each colour, owned rows)
-#pragma unroll
-        for (int p = 0; p < NS; ++p) {
-          const int col = p & 1;
-          const int row = t - LAG * p;
-          Unit<S> out;
-          out.ca = static_cast<S>(o[p][0]); out.cb = static_cast<S>(o[p][1]);
-          out.sa = static_cast<S>(o[p][2]); out.sb = static_cast<S>(o[p][3]);
-          if (n >= LAG * p) *reinterpret_cast<Unit<S>*>(own[p]) = out;       // rows above t0 do not exist
-          if (p >= NS - 2) {                                                   // last stage of this colour
-            const bool owned = lane_ok && row >= yb && row < ye;
-            if (owned) {
-              *reinterpret_cast<Unit<S>*>(gp - (LAG * p) * grow + col * gplane) = out;
-              if (MEASURE == 2) {
-                const uint32_t mm = (mq[col] >> (2 * LAG * p)) & 3u;
-                if (mm) {
-                  double* a = ap - static_cast<long long>(LAG * p) * g.Wp + static_cast<long long>(col) * static_cast<long long>(g.plane);
-                  double2 a2 = *reinterpret_cast<const double2*>(a);
-                  if (mm & 1u) a2.x += spin_angle<MODE>(o[p][0], o[p][2]);
-                  if (mm & 2u) a2.y += spin_angle<MODE>(o[p][1], o[p][3]);
-                  *reinterpret_cast<double2*>(a) = a2;
-                }
-              }
-              if (MEASURE != 0 && p == NS - 1) {
-                // every bond has exactly one colour-1 end: H = -J sum over colour-1 sites of site_energy_term
-                // with the final spins; the neighbours (colour 0) were final when this stage gathered them
-                if constexpr (sizeof(R) == 8) {
-                  R Aa, Ab, Ba, Bb;
-                  un2(A[p], &Aa, &Ab); un2(B[p], &Ba, &Bb);
-                  esum += static_cast<double>(fma_(o[p][0], Aa, o[p][2] * Ba));
-                  esum += static_cast<double>(fma_(o[p][1], Ab, o[p][3] * Bb));
-                } else {
-                  const int par = (u + col) & 1;
-                  const Unit<S>& mid = nb_m[0];
-                  const R alc = par ? R(mid.ca) : R(exc_last), als = par ? R(mid.sa) : R(exs_last);
-                  const R arc = par ? R(mid.cb) : R(mid.ca), ars = par ? R(mid.sb) : R(mid.sa);
-                  const R blc = par ? R(mid.cb) : R(mid.ca), bls = par ? R(mid.sb) : R(mid.sa);
-                  const R brc = par ? R(exc_last) : R(mid.cb), brs = par ? R(exs_last) : R(mid.sb);
-                  esum += site_energy_term<R>(o[p][0], o[p][2], alc, als, arc, ars, R(nb_u[0].ca), R(nb_u[0].sa),
-                                              R(nb_d[0].ca), R(nb_d[0].sa));
-                  esum += site_energy_term<R>(o[p][1], o[p][3], blc, bls, brc, brs, R(nb_u[0].cb), R(nb_u[0].sb),
-                                              R(nb_d[0].cb), R(nb_d[0].sb));
-                }
-              }
+          for (int p = 0; p < NS; ++p) {
+            const int col = p & 1, par = (u + col) & 1;       // t0 and LAG are even: x-parity of row t - 2p is (u + col) & 1
+            const int rel = u - LAG * p;                      // row relative to 4 i
+            auto at = [&](int plane, int r) -> S* {
+              const int q = (r >= 0) ? r / RB : -((-r + RB - 1) / RB);      // floor(r / RB)
+              return ring + cb[NSLOT - 2 + q] + plane * PLANE + (r - q * RB) * kRowScalars + 4 * lane;
+            };
+            own[p] = at(col, rel);
+            const Unit<S> up = *reinterpret_cast<const Unit<S>*>(at(1 - col, rel - 1));
+            const Unit<S> mid = *reinterpret_cast<const Unit<S>*>(at(1 - col, rel));
+            const Unit<S> dn = *reinterpret_cast<const Unit<S>*>(at(1 - col, rel + 1));
+            const Unit<S> me = *reinterpret_cast<const Unit<S>*>(own[p]);
+            const S exc = par ? __shfl_down_sync(0xffffffffu, mid.ca, 1) : __shfl_up_sync(0xffffffffu, mid.cb, 1);
+            const S exs = par ? __shfl_down_sync(0xffffffffu, mid.sa, 1) : __shfl_up_sync(0xffffffffu, mid.sb, 1);
+            combine_fields<MODE>(par, up, mid, dn, exc, exs, &A[p], &B[p]);
+            c[p] = mk2(R(me.ca), R(me.cb));
+            s[p] = mk2(R(me.sa), R(me.sb));
+            if (MEASURE != 0 && sizeof(R) == 4 && p == NS - 1) {
+              nb_u = up; nb_m = mid; nb_d = dn; exc_last = exc; exs_last = exs;
             }
           }
-        }
-        site_t += Lu;
-        gp += grow;
-        ap += g.Wp;
-      }
-      // rotate: the oldest chunk's slot receives chunk i + 2 in the next iteration
-      const int freed = cb[0];
+
+          // ---- compute
+          R o[NS][4];
 #pragma unroll
-      for (int k = 0; k + 1 < NSLOT; ++k) cb[k] = cb[k + 1];
-      cb[NSLOT - 1] = freed;
-      slot_next = slot_next + 1 == NSLOT ? 0 : slot_next + 1;
+          for (int p = 0; p < NS; ++p) {
+            const int col = p & 1, par = (u + col) & 1;
+            const bool fa = (mq[col] & (1u << (2 * LAG * p))) != 0u, fb = (mq[col] & (2u << (2 * LAG * p))) != 0u;
+            const int kind = P::kind(p);
+            if (kind == KIND_MET || kind == KIND_MO) {
+              const uint32_t pair_site = site_t - static_cast<uint32_t>(LAG * p) * Lu + static_cast<uint32_t>(par);
+              MetWords w0, w1;
+              met_words_pair<MODE>(pair_site, first_sweep + static_cast<uint32_t>(P::sweep_off(p)), kc, &w0, &w1);
+              bool ok[2];
+              met_update2<MODE>(c[p], s[p], A[p], B[p], w0, w1, fa, fb, kc, o[p], ok);
+              // accepted moves are counted per lane; the lanes that do not own their columns are dropped at the end
+              const int row = t - LAG * p;
+              if (!EDGE || (row >= yb && row < ye)) seg_acc += static_cast<int>(ok[0]) + static_cast<int>(ok[1]);
+              if (kind == KIND_MO) {
+                R o2[4];
+                or_update2<MODE>(mk2(o[p][0], o[p][1]), mk2(o[p][2], o[p][3]), A[p], B[p], fa, fb, o2);
+                o[p][0] = o2[0]; o[p][1] = o2[1]; o[p][2] = o2[2]; o[p][3] = o2[3];
+              }
+            } else if (kind == KIND_OR) {
+              or_update2<MODE>(c[p], s[p], A[p], B[p], fa, fb, o[p]);
+            } else {
+              quench_update2<MODE>(c[p], s[p], A[p], B[p], fa, fb, o[p]);
+            }
+          }
+
+          // ---- scatter: ring (stages whose row is loaded), global memory (final stage of each colour, owned rows)
+#pragma unroll
+          for (int p = 0; p < NS; ++p) {
+            const int col = p & 1;
+            const int row = t - LAG * p;
+            Unit<S> out;
+            out.ca = static_cast<S>(o[p][0]); out.cb = static_cast<S>(o[p][1]);
+            out.sa = static_cast<S>(o[p][2]); out.sb = static_cast<S>(o[p][3]);
+            if (!EDGE || n >= LAG * p) *reinterpret_cast<Unit<S>*>(own[p]) = out;       // rows above t0 do not exist
+            if (p >= NS - 2) {                                                            // last stage of this colour
+              const bool owned = lane_ok && (!EDGE || (row >= yb && row < ye));
+              if (owned) {
+                *reinterpret_cast<Unit<S>*>(gp - (LAG * p) * grow + col * gplane) = out;
+                if (MEASURE == 2) {
+                  const uint32_t mm = (mq[col] >> (2 * LAG * p)) & 3u;
+                  if (mm) {
+                    double* a = ap - static_cast<long long>(LAG * p) * g.Wp + static_cast<long long>(col) * static_cast<long long>(g.plane);
+                    double2 a2 = *reinterpret_cast<const double2*>(a);
+                    if (mm & 1u) a2.x += spin_angle<MODE>(o[p][0], o[p][2]);
+                    if (mm & 2u) a2.y += spin_angle<MODE>(o[p][1], o[p][3]);
+                    *reinterpret_cast<double2*>(a) = a2;
+                  }
+                }
+                if (MEASURE != 0 && p == NS - 1) {
+                  // every bond has exactly one colour-1 end: H = -J sum over colour-1 sites of site_energy_term
+                  // with the final spins; the neighbours (colour 0) were final when this stage gathered them
+                  if constexpr (sizeof(R) == 8) {
+                    R Aa, Ab, Ba, Bb;
+                    un2(A[p], &Aa, &Ab); un2(B[p], &Ba, &Bb);
+                    esum += static_cast<double>(fma_(o[p][0], Aa, o[p][2] * Ba));
+                    esum += static_cast<double>(fma_(o[p][1], Ab, o[p][3] * Bb));
+                  } else {
+                    const int par = (u + col) & 1;
+                    const R alc = par ? R(nb_m.ca) : R(exc_last), als = par ? R(nb_m.sa) : R(exs_last);
+                    const R arc = par ? R(nb_m.cb) : R(nb_m.ca), ars = par ? R(nb_m.sb) : R(nb_m.sa);
+                    const R blc = par ? R(nb_m.cb) : R(nb_m.ca), bls = par ? R(nb_m.sb) : R(nb_m.sa);
+                    const R brc = par ? R(exc_last) : R(nb_m.cb), brs = par ? R(exs_last) : R(nb_m.sb);
+                    esum += site_energy_term<R>(o[p][0], o[p][2], alc, als, arc, ars, R(nb_u.ca), R(nb_u.sa),
+                                                R(nb_d.ca), R(nb_d.sa));
+                    esum += site_energy_term<R>(o[p][1], o[p][3], blc, bls, brc, brs, R(nb_u.cb), R(nb_u.sb),
+                                                R(nb_d.cb), R(nb_d.sb));
+                  }
+                }
+              }
+            }
+          }
+          site_t += Lu;
+          gp += grow;
+          ap += g.Wp;
+        }
+        // rotate: the oldest chunk's slot receives chunk i + 2 in the next iteration
+        const int freed = cb[0];
+#pragma unroll
+        for (int k = 0; k + 1 < NSLOT; ++k) cb[k] = cb[k + 1];
+        cb[NSLOT - 1] = freed;
+        slot_next = slot_next + 1 == NSLOT ? 0 : slot_next + 1;
+      };
+
+      int i = 0;
+#pragma unroll 1
+      for (; i < n_iter && i < i_lo; ++i) iteration(i, std::true_type{});
+#pragma unroll 1
+      for (; i < n_iter && i < i_hi; ++i) iteration(i, std::false_type{});
+#pragma unroll 1
+      for (; i < n_iter; ++i) iteration(i, std::true_type{});
+      // every chunk issued was awaited inside its iteration: nothing is in flight here
+      if (lane_ok) n_acc += seg_acc;
     }
-    // every chunk issued was awaited inside its iteration: nothing is in flight here
   }
   if constexpr (MEASURE != 0) {
     const double e = block_sum(esum, red);
@@ -326,31 +360,22 @@ int strip_encode(TiledPlan& tp, const Geom& g, void* src, CUtensorMap* map) {
   return r == CUDA_SUCCESS ? TILED_OK : TILED_ENCODE;
 }
 
-// Segments per strip: as many as fill the resident warps (sm_count * NW), but no shorter than the point where the
-// warm-up / drain rows (2 NS + 6 per segment) would cost more than the idle warps they save.
-inline StripGeom strip_geometry(const Geom& g, int ns, int nw, int sm_count) {
+// Quota of rows per warp: all warp slots of the device (sm_count x NW) when that leaves at least 8 rows each,
+// fewer warps otherwise (a warp pays LEAD + 2 (NS - 1) + 3 warm-up / drain steps per segment whatever its quota).
+inline StripGeom strip_geometry(const Geom& g, int ns, int nw, int sm_count, int* nblocks) {
   StripGeom sg;
   const int ic = strip_interior_cols(ns);
   sg.n_strips = (g.Wp + ic - 1) / ic;
-  const int slots = sm_count * nw;
-  const int overhead = strip_lead_rows(ns) + kStripLag * (ns - 1) + 3;      // steps a segment runs beyond its own rows
-  int best_seg = 1;
-  double best_cost = 1e300;
-  const int max_seg = (g.L + 7) / 8;
-  for (int nseg = 1; nseg <= max_seg && static_cast<long long>(nseg) * sg.n_strips <= 4LL * slots; ++nseg) {
-    const int rows = ((g.L + nseg - 1) / nseg + 3) / 4 * 4;
-    const long long items = static_cast<long long>(sg.n_strips) * ((g.L + rows - 1) / rows);
-    const long long waves = (items + slots - 1) / slots;
-    // a wave with few warps per SM runs each warp faster, but not proportionally: model the per-step time as
-    // 1 + 0.35 (w - 1) for w resident warps per SM (measured shape: issue-bound beyond ~4 warps per scheduler)
-    const double per_sm = static_cast<double>(items) / waves / sm_count;
-    const double w = per_sm < 1.0 ? 1.0 : per_sm;
-    const double cost = static_cast<double>(waves) * (rows + overhead) * (1.0 + 0.35 * (w - 1.0));
-    if (cost < best_cost) { best_cost = cost; best_seg = nseg; }
-  }
-  sg.seg_rows = ((g.L + best_seg - 1) / best_seg + 3) / 4 * 4;
-  sg.n_seg = (g.L + sg.seg_rows - 1) / sg.seg_rows;
-  sg.n_items = sg.n_strips * sg.n_seg;
+  sg.Lp = (g.L + 3) / 4 * 4;
+  const long long total = static_cast<long long>(sg.n_strips) * sg.Lp;
+  const long long slots = static_cast<long long>(sm_count) * nw;
+  long long warps = total / 8 < slots ? total / 8 : slots;
+  if (warps < 1) warps = 1;
+  long long quota = (total + warps - 1) / warps;
+  quota = (quota + 3) / 4 * 4;
+  sg.quota = static_cast<int>(quota);
+  sg.n_warps = static_cast<int>((total + quota - 1) / quota);
+  *nblocks = sg.n_warps < sm_count ? sg.n_warps : sm_count;
   return sg;
 }
 
@@ -368,8 +393,8 @@ int strip_launch_one(StripPlan& plan, const CUtensorMap& map, const Geom& g, voi
       return TILED_ATTR;
     attr_done = true;
   }
-  const StripGeom sg = strip_geometry(g, NS, NW, plan.sm_count);
-  const int nblocks = (sg.n_items + NW - 1) / NW;
+  int nblocks = 0;
+  const StripGeom sg = strip_geometry(g, NS, NW, plan.sm_count, &nblocks);
   if (MEASURE != 0 && nblocks > max_partials) return TILED_TOO_MANY;
   strip_kernel<MODE, PROG, K, MEASURE><<<nblocks, NW * 32, smem, stream>>>(map, static_cast<V*>(dst), bits, acc, part, slots,
                                                                             g, kc, first_sweep, sg);
