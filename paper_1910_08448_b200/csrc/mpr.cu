@@ -145,8 +145,19 @@ ChainConst<R> chain_const(const mpr_ctx* c) {
   const double T = c->T > 0.0 ? c->T : 1.0;
   k.delta = static_cast<R>(proposal_width(T));
   k.inv_T = static_cast<R>(1.0 / T);
-  k.hscale = static_cast<R>(0.25 * proposal_width(T) / 2147483648.0);
-  k.xscale = static_cast<R>(-1.4426950408889634074 / T);
+  k.hscale = static_cast<R>(0.5 * proposal_width(T));
+  if (sizeof(R) == 4) {
+    // the two lowest mantissa bits cleared: 3/2 hscale is then exact in float and the 4096 proposal offsets
+    // fma(f, hscale, hoff) are exactly symmetric about 0 (delta itself is a free parameter, R7)
+    float hs = static_cast<float>(k.hscale);
+    uint32_t bits;
+    std::memcpy(&bits, &hs, sizeof(bits));
+    bits &= ~3u;
+    std::memcpy(&hs, &bits, sizeof(bits));
+    k.hscale = static_cast<R>(hs);
+  }
+  k.hoff = static_cast<R>(-1.5) * k.hscale;
+  k.xscale = static_cast<R>(1.4426950408889634074 / T);
   k.k0 = static_cast<uint32_t>(c->seed);
   k.k1 = static_cast<uint32_t>(c->seed >> 32);
   k.trial = c->trial;

@@ -75,12 +75,12 @@ __device__ __forceinline__ double u53(uint32_t a, uint32_t b) {
   const double lo = static_cast<double>(b >> 6);
   return (hi * 67108864.0 + lo) * (1.0 / 9007199254740992.0);
 }
-// Float modes (R9, judged statistically): the proposal offset is the word read as a signed integer,
-// converted with round-to-nearest (24-bit mantissa) -- a symmetric uniform on [-2^31, 2^31] whose
-// scale 2^-31 is folded into ChainConst::hscale; the acceptance uniform is the word converted as
-// an unsigned integer, u2 = float(w) 2^-32 in [0, 1].  One conversion instruction each.
-__device__ __forceinline__ float sym_word(uint32_t a) { return static_cast<float>(static_cast<int32_t>(a)); }
-__device__ __forceinline__ float pos_word(uint32_t a) { return static_cast<float>(a); }
+// Float modes (R9, judged statistically): ONE 32-bit word per site carries both random numbers of its move.
+//   proposal   top 12 bits k:  f = 1 + (k + 1/2) / 4096 in [1, 2), built in the mantissa (no conversion);
+//              q Delta / 2 = hscale (f - 3/2): 4096 equidistant offsets, exactly symmetric about 0
+//   acceptance low 20 bits m, converted exactly:  accept iff m < exp(-dE/T) 2^20
+__device__ __forceinline__ float prop_word(uint32_t w) { return __uint_as_float(((w >> 9) & 0x007FF800u) | 0x3F800400u); }
+__device__ __forceinline__ float acc_word(uint32_t w) { return static_cast<float>(w & 0x000FFFFFu); }
 
 // ---- double-precision sin/cos/exp on the ranges the Metropolis move needs ---------------------
 // The library sincos(double) / exp(double) are written for any argument: Cody-Waite reduction,
@@ -181,8 +181,9 @@ __device__ __forceinline__ float fma_(float a, float b, float c) { return fmaf(a
 template <typename R> struct ChainConst {
   R delta;     // R7 proposal half-width min(pi, 4 sqrt(T/(4 J q^2)))
   R inv_T;     // 1/T
-  R hscale;    // float modes: q Delta / 2 = hscale * float(int32 word) = (delta / 4) 2^-31 word
-  R xscale;    // SP_INTRINSIC: -log2(e) / T, so that exp(-dE / T) 2^32 = ex2(dE * xscale + 32)
+  R hscale;    // float modes: q Delta / 2 = hscale (f - 3/2), f = prop_word in [1, 2): hscale = delta / 2
+  R hoff;      //              = fma(f, hscale, hoff), hoff = -3/2 hscale
+  R xscale;    // SP_INTRINSIC: log2(e) / T, so that exp(-dE / T) 2^20 = ex2(-dE * xscale + 20)
   uint32_t k0, k1, trial;
   PhiloxKeys rk;   // round keys of (k0, k1)
 };
@@ -277,15 +278,24 @@ __device__ __forceinline__ Two<float> fma2(const Two<float>& x, const Two<float>
 }
 template <typename R> __device__ __forceinline__ Two<R> bc2(R k) { return mk2(k, k); }
 
-// Random words of the Metropolis move at a site (R9).  Double-arithmetic modes (DP, SP): one
-// Philox block per site, counter word 0 = the site's row-major index; all four words are used
-// (two 53-bit uniforms): the R9 reading in full.  Float-arithmetic modes: one block per PAIR of
-// sites of the same colour and row whose plane columns are (2m, 2m + 1); counter word 0 = the index
-// of the first site of the pair (pair_site); that site takes words (0, 2), the other one (1, 3).
+// Random words of the Metropolis move at a site (R9).  Double-arithmetic modes (DP, SP): one Philox block per
+// site, counter word 0 = the site's row-major index; all four words are used (two 53-bit uniforms): the R9
+// reading in full.  Float-arithmetic modes: one block per QUAD of sites of the same colour -- plane columns
+// (2m, 2m + 1) in the rows (2k, 2k + 1); counter word 0 = the index of the site in row 2k, column 2m (quad_site);
+// the sites take the words 0, 1 (row 2k: columns 2m, 2m + 1) and 2, 3 (row 2k + 1), one word each.
 struct MetWords { uint32_t p, q, a, b; };   // proposal (p [, q]) and acceptance (a [, b]) words
 
+// float modes: the four words of a quad
 template <int MODE>
-__device__ __forceinline__ void met_words_pair(uint32_t pair_site, uint32_t sweep,
+__device__ __forceinline__ uint4 met_words_quad(uint32_t quad_site, uint32_t sweep,
+                                                const ChainConst<typename Traits<MODE>::real>& k) {
+  return philox4x32_10(quad_site, sweep, PASS_MET, k.trial, k.rk);
+}
+// row_odd: the row of the two sites is 2k + 1.  pair_site = index of the first of the two sites in ITS row; the
+// float modes derive the quad's key from it (the first site of the even row lies one row up and, the x-parity
+// of a colour alternating from row to row, one column to the left or right).
+template <int MODE>
+__device__ __forceinline__ void met_words_pair(uint32_t pair_site, uint32_t sweep, uint32_t L, int par, bool row_odd,
                                                const ChainConst<typename Traits<MODE>::real>& k,
                                                MetWords* w0, MetWords* w1) {
   if constexpr (sizeof(typename Traits<MODE>::real) == 8) {
@@ -294,9 +304,13 @@ __device__ __forceinline__ void met_words_pair(uint32_t pair_site, uint32_t swee
     *w0 = MetWords{r0.x, r0.y, r0.z, r0.w};
     *w1 = MetWords{r1.x, r1.y, r1.z, r1.w};
   } else {
-    const uint4 r = philox4x32_10(pair_site, sweep, PASS_MET, k.trial, k.rk);
-    *w0 = MetWords{r.x, 0u, r.z, 0u};
-    *w1 = MetWords{r.y, 0u, r.w, 0u};
+    // even row: the pair's first site is the quad's key.  odd row: same plane columns one row up, where the
+    // x-parity is the other one: x_even = x - par + (1 - par)
+    const uint32_t quad_site = row_odd ? pair_site - L + 1u - 2u * static_cast<uint32_t>(par) : pair_site;
+    const uint4 r = met_words_quad<MODE>(quad_site, sweep, k);
+    const uint32_t wa = row_odd ? r.z : r.x, wb = row_odd ? r.w : r.y;
+    *w0 = MetWords{wa, 0u, wa, 0u};
+    *w1 = MetWords{wb, 0u, wb, 0u};
   }
 }
 
@@ -317,7 +331,7 @@ __device__ __forceinline__ void met_update2(Two<typename Traits<MODE>::real> c, 
     const R tb = fma_(R(2), R(u53(wb.p, wb.q)), R(-1));
     h = mul2(bc2(R(0.25)), mul2(bc2(k.delta), mk2(ta, tb)));
   } else {
-    h = mul2(bc2(k.hscale), mk2(sym_word(wa.p), sym_word(wb.p)));
+    h = fma2(mk2(prop_word(wa.p), prop_word(wb.p)), bc2(k.hscale), bc2(k.hoff));
   }
   R ha, hb, sda, cda, sdb, cdb;
   un2(h, &ha, &hb);
@@ -326,33 +340,33 @@ __device__ __forceinline__ void met_update2(Two<typename Traits<MODE>::real> c, 
   const Two<R> sd = mk2(sda, sdb), cd = mk2(cda, cdb);
   const Two<R> ts = add2(sd, sd);                // 2 sd
   const Two<R> nts = mul2(sd, bc2(R(-2)));       // -2 sd
-  const Two<R> s2 = mul2(ts, cd);                // sin(q Delta)
+  const Two<R> ps2 = mul2(ts, cd);               // sin(q Delta)
   const Two<R> ns2 = mul2(nts, cd);              // -sin(q Delta)
   const Two<R> c2m1 = mul2(nts, sd);             // cos(q Delta) - 1
-  const Two<R> cn = fma2(s, ns2, fma2(c, c2m1, c));   // c cos - s sin
-  const Two<R> sn = fma2(c, s2, fma2(s, c2m1, s));    // s cos + c sin
-  const Two<R> P = fma2(c, A, mul2(s, B));            // u.F
-  const Two<R> nQ = fma2(s, A, mul2(mul2(c, bc2(R(-1))), B));   // s A - c B
-  const Two<R> dE = mul2(ts, fma2(sd, P, mul2(cd, nQ)));
+  // u' - u = (rot(q Delta) - 1) u:  dc = c (cos - 1) - s sin,  ds = s (cos - 1) + c sin
+  const Two<R> dc = fma2(c, c2m1, mul2(s, ns2));
+  const Two<R> ds = fma2(s, c2m1, mul2(c, ps2));
+  const Two<R> cn = add2(c, dc), sn = add2(s, ds);
+  const Two<R> mdE = fma2(ds, B, mul2(dc, A));   // -dE = (u' - u) . F
   R c0a, c0b, s0a, s0b, cna, cnb, sna, snb;
   un2(c, &c0a, &c0b); un2(s, &s0a, &s0b); un2(cn, &cna, &cnb); un2(sn, &sna, &snb);
   bool acc_a, acc_b;
   if constexpr (sizeof(R) == 8) {
     R xa, xb;
-    un2(mul2(dE, bc2(k.inv_T)), &xa, &xb);
-    acc_a = R(u53(wa.a, wa.b)) < Fn<MODE>::exp_(-xa);
-    acc_b = R(u53(wb.a, wb.b)) < Fn<MODE>::exp_(-xb);
+    un2(mul2(mdE, bc2(k.inv_T)), &xa, &xb);
+    acc_a = R(u53(wa.a, wa.b)) < Fn<MODE>::exp_(xa);
+    acc_b = R(u53(wb.a, wb.b)) < Fn<MODE>::exp_(xb);
   } else if constexpr (MODE == MODE_SP_INTRINSIC) {
-    R xa, xb;                                    // exp(-dE/T) 2^32 = ex2(dE xscale + 32): one FFMA2 + 2 MUFU.EX2
-    un2(fma2(dE, bc2(k.xscale), bc2(R(32))), &xa, &xb);
-    acc_a = pos_word(wa.a) < Fn<MODE>::ex2_(xa);
-    acc_b = pos_word(wb.a) < Fn<MODE>::ex2_(xb);
+    R xa, xb;                                    // exp(-dE/T) 2^20 = ex2(-dE xscale + 20): one FFMA2 + 2 MUFU.EX2
+    un2(fma2(mdE, bc2(k.xscale), bc2(R(20))), &xa, &xb);
+    acc_a = acc_word(wa.a) < Fn<MODE>::ex2_(xa);
+    acc_b = acc_word(wb.a) < Fn<MODE>::ex2_(xb);
   } else {
     R xa, xb, ua, ub;
-    un2(mul2(dE, bc2(k.inv_T)), &xa, &xb);
-    un2(mul2(mk2(pos_word(wa.a), pos_word(wb.a)), bc2(R(2.3283064365386963e-10))), &ua, &ub);
-    acc_a = ua < Fn<MODE>::exp_(-xa);
-    acc_b = ub < Fn<MODE>::exp_(-xb);
+    un2(mul2(mdE, bc2(k.inv_T)), &xa, &xb);
+    un2(mul2(mk2(acc_word(wa.a), acc_word(wb.a)), bc2(R(9.5367431640625e-07))), &ua, &ub);   // m 2^-20, exact
+    acc_a = ua < Fn<MODE>::exp_(xa);
+    acc_b = ub < Fn<MODE>::exp_(xb);
   }
   const bool oka = free_a && (sna >= R(0)) && acc_a;
   const bool okb = free_b && (snb >= R(0)) && acc_b;

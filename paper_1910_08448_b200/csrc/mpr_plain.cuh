@@ -268,11 +268,11 @@ plain_pass_kernel(typename Traits<MODE>::vec* __restrict__ state, const uint32_t
     const V me = ld_spin(own, j);
     R c = R(me.x), s = R(me.y);
     if constexpr (KIND == KIND_MET || KIND == KIND_MO) {
-      // R9: the pair (2m, 2m + 1) of plane columns shares one Philox block in the float modes
+      // R9: the quad (plane columns 2m, 2m + 1) x (rows 2k, 2k + 1) shares one Philox block in the float modes
       const uint32_t pair_site = static_cast<uint32_t>(y) * static_cast<uint32_t>(g.L) +
                                  static_cast<uint32_t>(2 * (j & ~1) + par);
       MetWords w0, w1;
-      met_words_pair<MODE>(pair_site, sweep, k, &w0, &w1);
+      met_words_pair<MODE>(pair_site, sweep, static_cast<uint32_t>(g.L), par, (y & 1) != 0, k, &w0, &w1);
       const MetWords w = (j & 1) ? w1 : w0;
       R o[4];
       bool ok[2];

@@ -186,6 +186,8 @@ strip_kernel(const __grid_constant__ CUtensorMap tmap, typename Traits<MODE>::ve
           mbar_expect_tx(bars + slot_next, kChunkBytes);
           tma_load_3d(ring + cb[NSLOT - 1], &tmap, bars + slot_next, 2 * j0, t0 + RB * (i + 1), 0);
         }
+        uint32_t stash[NS][2];                                // second half of the Philox blocks (float modes)
+        (void)stash;
 #pragma unroll
         for (int u = 0; u < RB; ++u) {
           if (u == RB - 1) {                                  // row 4 i + 4 (first of chunk i + 1) is read from here on
@@ -239,7 +241,22 @@ strip_kernel(const __grid_constant__ CUtensorMap tmap, typename Traits<MODE>::ve
             if (kind == KIND_MET || kind == KIND_MO) {
               const uint32_t pair_site = site_t - static_cast<uint32_t>(LAG * p) * Lu + static_cast<uint32_t>(par);
               MetWords w0, w1;
-              met_words_pair<MODE>(pair_site, first_sweep + static_cast<uint32_t>(P::sweep_off(p)), kc, &w0, &w1);
+              const uint32_t sweep = first_sweep + static_cast<uint32_t>(P::sweep_off(p));
+              if constexpr (sizeof(R) == 8) {
+                met_words_pair<MODE>(pair_site, sweep, Lu, par, (u & 1) != 0, kc, &w0, &w1);
+              } else {
+                // float modes: one Philox block per quad (R9) -- computed in the even row (t0 is even, so that is an
+                // even step), its second half kept for the odd row that follows in the next step
+                if ((u & 1) == 0) {
+                  const uint4 r = met_words_quad<MODE>(pair_site, sweep, kc);
+                  w0 = MetWords{r.x, 0u, r.x, 0u};
+                  w1 = MetWords{r.y, 0u, r.y, 0u};
+                  stash[p][0] = r.z; stash[p][1] = r.w;
+                } else {
+                  w0 = MetWords{stash[p][0], 0u, stash[p][0], 0u};
+                  w1 = MetWords{stash[p][1], 0u, stash[p][1], 0u};
+                }
+              }
               bool ok[2];
               met_update2<MODE>(c[p], s[p], A[p], B[p], w0, w1, fa, fb, kc, o[p], ok);
               // accepted moves are counted per lane; the lanes that do not own their columns are dropped at the end

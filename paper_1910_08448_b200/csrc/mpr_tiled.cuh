@@ -163,8 +163,8 @@ __device__ __forceinline__ int row_step(int par, decltype(Traits<MODE>::vec::x)*
                                         const Unit<decltype(Traits<MODE>::vec::x)>& up,
                                         const Unit<decltype(Traits<MODE>::vec::x)>& mid,
                                         const Unit<decltype(Traits<MODE>::vec::x)>& dn,
-                                        bool fa, bool fb, int inc, uint32_t pair_site, uint32_t sweep,
-                                        const ChainConst<typename Traits<MODE>::real>& kc) {
+                                        bool fa, bool fb, int inc, uint32_t pair_site, uint32_t sweep, uint32_t L,
+                                        bool row_odd, const ChainConst<typename Traits<MODE>::real>& kc) {
   using R = typename Traits<MODE>::real;
   using S = decltype(Traits<MODE>::vec::x);
   const S exc = par ? __shfl_down_sync(0xffffffffu, mid.ca, 1) : __shfl_up_sync(0xffffffffu, mid.cb, 1);
@@ -177,7 +177,7 @@ __device__ __forceinline__ int row_step(int par, decltype(Traits<MODE>::vec::x)*
   int n = 0;
   if constexpr (KIND == KIND_MET) {
     MetWords w0, w1;
-    met_words_pair<MODE>(pair_site, sweep, kc, &w0, &w1);
+    met_words_pair<MODE>(pair_site, sweep, L, par, row_odd, kc, &w0, &w1);
     bool ok[2];
     met_update2<MODE>(c, s, A, B, w0, w1, fa, fb, kc, o, ok);
     if (ok[0]) n += inc;
@@ -258,7 +258,8 @@ __device__ __forceinline__ int pass_rows(const TileView<MODE>& t, uint32_t mcol,
     const Unit<S> dn = *reinterpret_cast<const Unit<S>*>(own + kOther + dn_row * kRowScalars);
     n_acc += row_step<MODE, KIND>(par, own + i * kRowScalars, up, mid, dn, (mcol >> (2 * i)) & 1u,
                                   (mcol >> (2 * i + 1)) & 1u, (cnt >> i) & 1u,
-                                  site + static_cast<uint32_t>(i) * L + static_cast<uint32_t>(par), sweep, kc);
+                                  site + static_cast<uint32_t>(i) * L + static_cast<uint32_t>(par), sweep, L,
+                                  (i & 1) != 0, kc);      // tile origin and RPW are even: row parity = i & 1
     up = mid;
     mid = dn;
   }
