@@ -36,7 +36,7 @@ size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
 struct Layout {
   Geom g;
-  size_t off_state[2], off_acc, off_bits, off_part, off_series, off_slots, off_scal, total;
+  size_t off_state[2], off_acc, off_bits, off_smask[2], off_part, off_series, off_slots, off_scal, total;
 };
 
 Layout make_layout(int L) {
@@ -53,6 +53,10 @@ Layout make_layout(int L) {
   lo.off_state[1] = o; o = align_up(o + state_bytes, 256);
   lo.off_acc = o;      o = align_up(o + 2 * lo.g.plane * sizeof(double), 256);
   lo.off_bits = o;     o = align_up(o + static_cast<size_t>(2) * lo.g.Hb * lo.g.Wb * sizeof(uint32_t), 256);
+  for (int hl = 1; hl <= 2; ++hl) {
+    lo.off_smask[hl - 1] = o;
+    o = align_up(o + strip_mask_words(lo.g, hl) * sizeof(uint32_t), 256);
+  }
   lo.off_part = o;     o = align_up(o + kPartials * sizeof(double), 256);
   lo.off_series = o;   o = align_up(o + kSeriesCap * sizeof(double), 256);
   lo.off_slots = o;    o = align_up(o + kAcceptSlots * sizeof(unsigned long long), 256);
@@ -102,6 +106,7 @@ struct mpr_ctx {
   uint32_t* bits_base() const { return reinterpret_cast<uint32_t*>(ws + lo.off_bits); }
   // word 0 of row 0 of colour 0 inside the padded bitmaps (mpr_plain.cuh)
   uint32_t* bits() const { return bits_base() + static_cast<size_t>(kBitPadTop) * lo.g.Wb + kBitPadLeft; }
+  uint32_t* smask(int hl) const { return reinterpret_cast<uint32_t*>(ws + lo.off_smask[hl - 1]); }
   double* part() const { return reinterpret_cast<double*>(ws + lo.off_part); }
   double* dseries() const { return reinterpret_cast<double*>(ws + lo.off_series); }
   unsigned long long* slots() const { return reinterpret_cast<unsigned long long*>(ws + lo.off_slots); }
@@ -276,7 +281,7 @@ template <int MODE> int strip_sweeps(mpr_ctx* c, int prog, int k, int measure, d
   const Geom& g = c->lo.g;
   const ChainConst<R> kc = chain_const<R>(c);
   int nblocks = 0;
-  StripArgs a{&c->strip, &c->tiled, g, c->cur, c->state(c->cur), c->state(1 - c->cur), c->bits(), c->acc(), c->part(),
+  StripArgs a{&c->strip, &c->tiled, g, c->cur, c->state(c->cur), c->state(1 - c->cur), {c->smask(1), c->smask(2)}, c->acc(), c->part(),
               c->slots(), &kc, static_cast<uint32_t>(c->sweep + 1), prog, k, measure, c->stream, &nblocks, kPartials};
   const int st = MODE == MODE_DP ? strip_launch_mode0(a) : MODE == MODE_SP ? strip_launch_mode1(a)
                  : MODE == MODE_SP_PRECISE ? strip_launch_mode2(a) : strip_launch_mode3(a);
@@ -499,6 +504,11 @@ int setup(mpr_ctx* c) {
   LAUNCH_OK(c);
   final_sum_kernel<<<1, 1024, 0, c->stream>>>(cnt_part, mblk, 1.0, c->scal() + 2);
   LAUNCH_OK(c);
+  // the same bits in strip order, for the STRIP path (mpr_strip.cuh)
+  for (int hl = 1; hl <= 2; ++hl) {
+    CUDA_OK(c, strip_mask_build(c->d_mask, g, hl, c->smask(hl), c->stream));
+    c->launches += 1;
+  }
   double h2[3];
   CUDA_OK(c, cudaMemcpyAsync(h2, c->scal(), sizeof(h2), cudaMemcpyDeviceToHost, c->stream));
   CUDA_OK(c, cudaStreamSynchronize(c->stream));

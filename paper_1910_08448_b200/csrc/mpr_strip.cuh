@@ -70,20 +70,35 @@ template <int MODE, int NS> struct StripCfg {
 // slot w / gridDim.x of CTA w % gridDim.x, so that a launch with fewer warps than slots still uses every SM.
 struct StripGeom {
   int n_strips, Lp, quota, n_warps;
+  int n_mchunks;      // chunks per strip in the strip-ordered mask (strip_mask_chunks)
 };
+
+// Strip-ordered mask: for every strip and every chunk of 4 rows one 128-byte block, one 32-bit word per lane:
+// bit 4 r + 2 c + k = site (row 4 chunk + r, colour c, plane column j0 + 2 lane + k) exists and is a prediction site.
+// It travels into shared memory with the spins of the chunk (one 1-D bulk copy on the same mbarrier), so a lane gets
+// the mask bits of 4 rows x 2 colours with one LDS and tests them with immediate bit masks.  Chunk index 0 is the
+// chunk of rows -kStripMaskLead .. -kStripMaskLead + 3; rows outside the grid have no bits set.
+constexpr int kStripMaskLead = 8;      // rows (two chunks) above the grid
+constexpr int kStripMaskTail = 32;     // rows below it
+__host__ __device__ constexpr int strip_mask_chunks(int L) { return ((L + 3) / 4 * 4 + kStripMaskLead + kStripMaskTail) / kStripRB; }
 
 template <int MODE, int NS> constexpr size_t strip_smem_bytes() {
   using S = decltype(Traits<MODE>::vec::x);
-  return static_cast<size_t>(StripCfg<MODE, NS>::NW) * strip_slots(NS) * (2 * kStripRB * kRowScalars * sizeof(S) + sizeof(uint64_t)) + 128;
+  return static_cast<size_t>(StripCfg<MODE, NS>::NW) * strip_slots(NS) * (2 * kStripRB * kRowScalars * sizeof(S) + 128 + sizeof(uint64_t)) + 128;
 }
 
 __device__ __forceinline__ void fence_proxy_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+// 1-D bulk copy global -> shared, completion counted on an mbarrier (SASS UBLKCP)
+__device__ __forceinline__ void bulk_load_1d(void* dst, const void* src, uint32_t bytes, uint64_t* bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+               ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+}
 
 // MEASURE: 0 = none; 1 = + energy sample after the last stage; 2 = + accumulation of phi (R15)
 template <int MODE, int PROG, int K, int MEASURE>
 __global__ void __launch_bounds__(StripCfg<MODE, StripProg<PROG, K>::NS>::NW * 32, 1)
 strip_kernel(const __grid_constant__ CUtensorMap tmap, typename Traits<MODE>::vec* __restrict__ dst,
-             const uint32_t* __restrict__ bits, double* __restrict__ acc, double* __restrict__ part,
+             const uint32_t* __restrict__ smask, double* __restrict__ acc, double* __restrict__ part,
              unsigned long long* __restrict__ accept_slots, Geom g, ChainConst<typename Traits<MODE>::real> kc,
              uint32_t first_sweep, StripGeom sg) {
   using R = typename Traits<MODE>::real;
@@ -95,9 +110,10 @@ strip_kernel(const __grid_constant__ CUtensorMap tmap, typename Traits<MODE>::ve
   constexpr int LEAD = strip_lead_rows(NS);
   constexpr int CHUNK = 2 * RB * kRowScalars;          // scalars per chunk: [plane][row][128]
   constexpr int PLANE = RB * kRowScalars;
-  constexpr uint32_t kChunkBytes = CHUNK * sizeof(S);
+  constexpr uint32_t kSpinBytes = CHUNK * sizeof(S), kMaskBytes = 128, kChunkBytes = kSpinBytes + kMaskBytes;
+  constexpr int NQ = (LAG * (NS - 1) + RB - 1) / RB + 1;     // mask words a lane holds: chunks i, i - 1, ..., i - NQ + 1
   static_assert(MEASURE == 0 || K == 1, "measuring launches carry one sweep");
-  static_assert(LAG * (NS - 1) * 2 + 4 <= 32, "mask queue: 2 bits per row in a 32-bit register");
+  static_assert(LEAD <= kStripMaskLead, "the strip-ordered mask starts kStripMaskLead rows above the grid");
 
   extern __shared__ __align__(128) unsigned char smem_raw[];
   __shared__ double red[32];
@@ -106,7 +122,9 @@ strip_kernel(const __grid_constant__ CUtensorMap tmap, typename Traits<MODE>::ve
   // row range, loop bounds) then lives in uniform registers and the loops are known not to diverge
   const int warp = __shfl_sync(0xffffffffu, static_cast<int>(threadIdx.x >> 5), 0);
   S* const ring = reinterpret_cast<S*>(smem_raw) + static_cast<size_t>(warp) * NSLOT * CHUNK;
-  uint64_t* const bars = reinterpret_cast<uint64_t*>(smem_raw + static_cast<size_t>(NW) * NSLOT * CHUNK * sizeof(S)) + warp * NSLOT;
+  unsigned char* const after_rings = smem_raw + static_cast<size_t>(NW) * NSLOT * CHUNK * sizeof(S);
+  uint32_t* const mring = reinterpret_cast<uint32_t*>(after_rings) + warp * NSLOT * 32;          // 128 B of mask per slot
+  uint64_t* const bars = reinterpret_cast<uint64_t*>(after_rings + static_cast<size_t>(NW) * NSLOT * kMaskBytes) + warp * NSLOT;
 
   int n_acc = 0;
   double esum = 0.0;
@@ -123,7 +141,6 @@ strip_kernel(const __grid_constant__ CUtensorMap tmap, typename Traits<MODE>::ve
     const long long q1 = min(total, q0 + sg.quota);
     const uint32_t Lu = static_cast<uint32_t>(g.L);
     const long long grow = 2 * static_cast<long long>(g.Wp), gplane = 2 * static_cast<long long>(g.plane);
-    const size_t colour_words = static_cast<size_t>(g.Hb) * g.Wb;
 
 #pragma unroll 1
     while (q0 < q1) {
@@ -146,10 +163,13 @@ strip_kernel(const __grid_constant__ CUtensorMap tmap, typename Traits<MODE>::ve
       int seg_acc = 0;
 
       __syncwarp();
+      // this strip's mask blocks; block of the chunk whose first row is t0 + 4 c: index (t0 + lead) / 4 + c
+      const uint32_t* const mblk = smask + (static_cast<size_t>(strip) * sg.n_mchunks + (t0 + kStripMaskLead) / RB) * 32;
       if (lane == 0) {                                        // chunk 0 -> slot 0
         fence_proxy_async_smem();
         mbar_expect_tx(bars, kChunkBytes);
         tma_load_3d(ring, &tmap, bars, 2 * j0, t0, 0);
+        bulk_load_1d(mring, mblk, kMaskBytes, bars);
       }
       // cb[k] = scalar offset (inside this warp's ring) of the chunk  i + 2 - NSLOT + k,  i.e. cb[NSLOT-1] holds
       // chunk i + 1 (in flight), cb[NSLOT-2] chunk i, cb[0] the oldest live one.  Chunk c lives in slot c % NSLOT.
@@ -158,14 +178,10 @@ strip_kernel(const __grid_constant__ CUtensorMap tmap, typename Traits<MODE>::ve
       for (int k = 0; k < NSLOT; ++k) cb[k] = ((k + 2) % NSLOT) * CHUNK;    // iteration 0: chunk k + 2 - NSLOT
       int slot_next = 1 % NSLOT;                              // slot of chunk i + 1
 
-      // mask bits: one queue per colour, 2 bits per row, row t at bits 0..1, row t - d at bits 2d..2d+1.  The words
-      // are fetched TWO steps ahead (raw, shifted only when they enter the queue) so that their L2 latency is hidden.
-      uint32_t mq[2] = {0u, 0u};
-      const int sh = j & 31;
-      const uint32_t* bp = mask_word(bits, g, 0, t0, j >> 5);
-      uint32_t rawA0 = __ldg(bp), rawA1 = __ldg(bp + colour_words);                       // row t
-      uint32_t rawB0 = __ldg(bp + g.Wb), rawB1 = __ldg(bp + g.Wb + colour_words);         // row t + 1
-      bp += 2 * g.Wb;
+      // mask words of the chunks i, i - 1, ... (cw[0] = chunk i); chunks above t0 were never loaded: no bits
+      uint32_t cw[NQ];
+#pragma unroll
+      for (int k = 0; k < NQ; ++k) cw[k] = 0u;
 
       uint32_t site_t = static_cast<uint32_t>(t0) * Lu + static_cast<uint32_t>(2 * j);   // Philox word 0 of row t, no parity
       // global pointers of this lane's unit in row t of plane 0 (dst / accumulator); never dereferenced outside the grid
@@ -185,7 +201,12 @@ strip_kernel(const __grid_constant__ CUtensorMap tmap, typename Traits<MODE>::ve
           fence_proxy_async_smem();
           mbar_expect_tx(bars + slot_next, kChunkBytes);
           tma_load_3d(ring + cb[NSLOT - 1], &tmap, bars + slot_next, 2 * j0, t0 + RB * (i + 1), 0);
+          bulk_load_1d(mring + slot_next * 32, mblk + static_cast<size_t>(i + 1) * 32, kMaskBytes, bars + slot_next);
         }
+        // the mask word of chunk i (its slot is the one before slot_next; the chunk was awaited in iteration i - 1)
+#pragma unroll
+        for (int k = NQ - 1; k > 0; --k) cw[k] = cw[k - 1];
+        cw[0] = mring[(slot_next == 0 ? NSLOT - 1 : slot_next - 1) * 32 + lane];
         uint32_t stash[NS][2];                                // second half of the Philox blocks (float modes)
         (void)stash;
 #pragma unroll
@@ -196,13 +217,6 @@ strip_kernel(const __grid_constant__ CUtensorMap tmap, typename Traits<MODE>::ve
           }
           const int n = RB * i + u;                           // step number; row t = t0 + n
           const int t = t0 + n;
-          // ---- mask bits of row t enter the queues; those of row t + 2 are requested
-          mq[0] = (mq[0] << 2) | ((rawA0 >> sh) & 3u);
-          mq[1] = (mq[1] << 2) | ((rawA1 >> sh) & 3u);
-          rawA0 = rawB0; rawA1 = rawB1;
-          rawB0 = __ldg(bp); rawB1 = __ldg(bp + colour_words);
-          bp += g.Wb;
-
           // ---- gather: own unit and local fields of every stage (all reads before any write of this step)
           Two<R> A[NS], B[NS], c[NS], s[NS];
           S* own[NS];
@@ -236,7 +250,11 @@ strip_kernel(const __grid_constant__ CUtensorMap tmap, typename Traits<MODE>::ve
 #pragma unroll
           for (int p = 0; p < NS; ++p) {
             const int col = p & 1, par = (u + col) & 1;
-            const bool fa = (mq[col] & (1u << (2 * LAG * p))) != 0u, fb = (mq[col] & (2u << (2 * LAG * p))) != 0u;
+            // mask bits of row 4 i + u - 2 p: chunk i + mq (mq <= 0), row mr of it
+            const int rel = u - LAG * p;
+            const int mqk = (rel >= 0) ? 0 : (-rel + RB - 1) / RB;          // chunks back
+            const int mr = rel + mqk * RB;
+            const bool fa = (cw[mqk] & (1u << (4 * mr + 2 * col))) != 0u, fb = (cw[mqk] & (2u << (4 * mr + 2 * col))) != 0u;
             const int kind = P::kind(p);
             if (kind == KIND_MET || kind == KIND_MO) {
               const uint32_t pair_site = site_t - static_cast<uint32_t>(LAG * p) * Lu + static_cast<uint32_t>(par);
@@ -288,7 +306,9 @@ strip_kernel(const __grid_constant__ CUtensorMap tmap, typename Traits<MODE>::ve
               if (owned) {
                 *reinterpret_cast<Unit<S>*>(gp - (LAG * p) * grow + col * gplane) = out;
                 if (MEASURE == 2) {
-                  const uint32_t mm = (mq[col] >> (2 * LAG * p)) & 3u;
+                  const int rel = u - LAG * p;
+                  const int mqk = (rel >= 0) ? 0 : (-rel + RB - 1) / RB;
+                  const uint32_t mm = (cw[mqk] >> (4 * (rel + mqk * RB) + 2 * col)) & 3u;
                   if (mm) {
                     double* a = ap - static_cast<long long>(LAG * p) * g.Wp + static_cast<long long>(col) * static_cast<long long>(g.plane);
                     double2 a2 = *reinterpret_cast<const double2*>(a);
@@ -354,6 +374,40 @@ strip_kernel(const __grid_constant__ CUtensorMap tmap, typename Traits<MODE>::ve
   }
 }
 
+// Strip-ordered mask for strips with `hl` halo lanes per side (see strip_mask_chunks): one thread per word.
+static __global__ void pack_strip_mask_kernel(const uint8_t* __restrict__ mask, Geom g, int hl, int n_strips, int n_mchunks,
+                                              uint32_t* __restrict__ out) {
+  const long long w = blockIdx.x * static_cast<long long>(blockDim.x) + threadIdx.x;
+  const long long nwords = static_cast<long long>(n_strips) * n_mchunks * 32;
+  if (w >= nwords) return;
+  const int lane = static_cast<int>(w & 31);
+  const int chunk = static_cast<int>((w >> 5) % n_mchunks), strip = static_cast<int>((w >> 5) / n_mchunks);
+  const int ic = kTileCols - 4 * hl;
+  const int j = strip * ic - 2 * hl + 2 * lane;
+  uint32_t word = 0;
+  for (int r = 0; r < kStripRB; ++r) {
+    const int y = chunk * kStripRB - kStripMaskLead + r;
+    if (y < 0 || y >= g.L) continue;
+    for (int c = 0; c < 2; ++c)
+      for (int k = 0; k < 2; ++k) {
+        const int jj = j + k;
+        const int x = 2 * jj + x_parity(y, c);
+        if (jj >= 0 && x < g.L && mask[static_cast<size_t>(y) * g.L + x]) word |= 1u << (4 * r + 2 * c + k);
+      }
+  }
+  out[w] = word;
+}
+inline int strip_mask_strips(const Geom& g, int hl) { const int ic = kTileCols - 4 * hl; return (g.Wp + ic - 1) / ic; }
+inline size_t strip_mask_words(const Geom& g, int hl) {
+  return static_cast<size_t>(strip_mask_strips(g, hl)) * strip_mask_chunks(g.L) * 32;
+}
+inline cudaError_t strip_mask_build(const uint8_t* d_mask, const Geom& g, int hl, uint32_t* out, cudaStream_t stream) {
+  const size_t n = strip_mask_words(g, hl);
+  pack_strip_mask_kernel<<<static_cast<unsigned>((n + 255) / 256), 256, 0, stream>>>(d_mask, g, hl, strip_mask_strips(g, hl),
+                                                                                     strip_mask_chunks(g.L), out);
+  return cudaGetLastError();
+}
+
 // ---- host side -------------------------------------------------------------------------------
 struct StripPlan {
   int sm_count = 0;
@@ -392,12 +446,13 @@ inline StripGeom strip_geometry(const Geom& g, int ns, int nw, int sm_count, int
   quota = (quota + 3) / 4 * 4;
   sg.quota = static_cast<int>(quota);
   sg.n_warps = static_cast<int>((total + quota - 1) / quota);
+  sg.n_mchunks = strip_mask_chunks(g.L);
   *nblocks = sg.n_warps < sm_count ? sg.n_warps : sm_count;
   return sg;
 }
 
 template <int MODE, int PROG, int K, int MEASURE>
-int strip_launch_one(StripPlan& plan, const CUtensorMap& map, const Geom& g, void* dst, const uint32_t* bits, double* acc,
+int strip_launch_one(StripPlan& plan, const CUtensorMap& map, const Geom& g, void* dst, const uint32_t* const smask[2], double* acc,
                      double* part, unsigned long long* slots, const ChainConst<typename Traits<MODE>::real>& kc,
                      uint32_t first_sweep, cudaStream_t stream, int* nblocks_out, long long max_partials) {
   using V = typename Traits<MODE>::vec;
@@ -413,7 +468,7 @@ int strip_launch_one(StripPlan& plan, const CUtensorMap& map, const Geom& g, voi
   int nblocks = 0;
   const StripGeom sg = strip_geometry(g, NS, NW, plan.sm_count, &nblocks);
   if (MEASURE != 0 && nblocks > max_partials) return TILED_TOO_MANY;
-  strip_kernel<MODE, PROG, K, MEASURE><<<nblocks, NW * 32, smem, stream>>>(map, static_cast<V*>(dst), bits, acc, part, slots,
+  strip_kernel<MODE, PROG, K, MEASURE><<<nblocks, NW * 32, smem, stream>>>(map, static_cast<V*>(dst), smask[strip_halo_lanes(NS) - 1], acc, part, slots,
                                                                             g, kc, first_sweep, sg);
   if (cudaGetLastError() != cudaSuccess) return TILED_LAUNCH;
   *nblocks_out = nblocks;
@@ -423,7 +478,7 @@ int strip_launch_one(StripPlan& plan, const CUtensorMap& map, const Geom& g, voi
 // prog / k / measure -> instantiation.  Supported: R4 k = 1 (measure 0, 1, 2), R4 k = 2; FUSED k = 1 (measure 0, 1, 2),
 // FUSED k = 2; QUENCH k = 2 (two double passes).  Returns TILED_LAUNCH for anything else.
 template <int MODE>
-int strip_launch(StripPlan& plan, TiledPlan& tp, const Geom& g, int src_index, void* src, void* dst, const uint32_t* bits,
+int strip_launch(StripPlan& plan, TiledPlan& tp, const Geom& g, int src_index, void* src, void* dst, const uint32_t* const smask[2],
                  double* acc, double* part, unsigned long long* slots, const ChainConst<typename Traits<MODE>::real>& kc,
                  uint32_t first_sweep, int prog, int k, int measure, cudaStream_t stream, int* nblocks_out,
                  long long max_partials) {
@@ -443,7 +498,7 @@ int strip_launch(StripPlan& plan, TiledPlan& tp, const Geom& g, int src_index, v
   const CUtensorMap& map = plan.map[src_index][w];
 #define MPR_STRIP_CASE(PROG_, K_, M_)                                                                              \
   if (prog == PROG_ && k == K_ && measure == M_)                                                                   \
-    return strip_launch_one<MODE, PROG_, K_, M_>(plan, map, g, dst, bits, acc, part, slots, kc, first_sweep, stream, \
+    return strip_launch_one<MODE, PROG_, K_, M_>(plan, map, g, dst, smask, acc, part, slots, kc, first_sweep, stream, \
                                                  nblocks_out, max_partials);
   MPR_STRIP_CASE(PROG_R4, 1, 0)
   MPR_STRIP_CASE(PROG_R4, 1, 1)
@@ -467,7 +522,7 @@ struct StripArgs {
   int src_index;
   void* src;
   void* dst;
-  const uint32_t* bits;
+  const uint32_t* smask[2];   // strip-ordered masks for 1 and 2 halo lanes per side (NS <= 4, NS = 8)
   double* acc;
   double* part;
   unsigned long long* slots;

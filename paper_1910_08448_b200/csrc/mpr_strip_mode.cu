@@ -13,7 +13,7 @@ namespace mpr {
 int MPR_CAT(strip_launch_mode, MPR_STRIP_MODE)(const StripArgs& a) {
   constexpr int MODE = MPR_STRIP_MODE;
   using R = typename Traits<MODE>::real;
-  return strip_launch<MODE>(*a.plan, *a.tp, a.g, a.src_index, a.src, a.dst, a.bits, a.acc, a.part, a.slots,
+  return strip_launch<MODE>(*a.plan, *a.tp, a.g, a.src_index, a.src, a.dst, a.smask, a.acc, a.part, a.slots,
                             *static_cast<const ChainConst<R>*>(a.kc), a.first_sweep, a.prog, a.k, a.measure, a.stream,
                             a.nblocks_out, a.max_partials);
 }
