@@ -398,8 +398,11 @@ __device__ __forceinline__ void or_update2(Two<typename Traits<MODE>::real> c, T
   const Two<R> co = mul2(mc, nf), so = mul2(ms, nf);
   R c0a, c0b, s0a, s0b, msa, msb, coa, cob, soa, sob;
   un2(c, &c0a, &c0b); un2(s, &s0a, &s0b); un2(ms, &msa, &msb); un2(co, &coa, &cob); un2(so, &soa, &sob);
-  const bool oka = free_a && (f2a != R(0)) && (msa <= R(0));
-  const bool okb = free_b && (f2b != R(0)) && (msb <= R(0));
+  // F = 0 (no field: nothing to reflect about) needs no test of its own: t = -2 P / 0 is inf or NaN, t F - u is NaN
+  // (inf x 0), and NaN <= 0 is false -- the spin stays.  (void)f2a keeps the name for readers of the formula above.
+  (void)f2a; (void)f2b;
+  const bool oka = free_a && (msa <= R(0));
+  const bool okb = free_b && (msb <= R(0));
   out[0] = oka ? coa : c0a; out[2] = oka ? soa : s0a;
   out[1] = okb ? cob : c0b; out[3] = okb ? sob : s0b;
 }

@@ -56,12 +56,17 @@ __host__ __device__ constexpr int strip_interior_cols(int ns) { return kTileCols
 __host__ __device__ constexpr int strip_slots(int ns) { return (2 * ns + 1 + kStripRB - 1) / kStripRB + 1; }
 __host__ __device__ constexpr int strip_lead_rows(int ns) { return (ns + kStripRB - 1) / kStripRB * kStripRB; }   // rows loaded above a segment
 
-// warps per CTA (one CTA per SM): as many as their rings fit into 216 KiB of shared memory, at most 12
-// (the ring of a warp is 16 KiB with float storage and NS = 4, 32 KiB in DP)
+// warps per CTA (one CTA per SM): as many as their rings fit into 216 KiB of shared memory, at most 12 -- 168
+// registers per thread, which the four interleaved update chains of a 4-stage program need -- or 16 for the
+// 2-stage programs, whose two chains fit the 128 registers that leaves (measured at L = 16384, SP_INTRINSIC,
+// site-fused schedule, one sweep per launch: 12 warps 1.07 ms, 16 warps 0.78 ms per sweep; a 4-stage program
+// squeezed into 128 registers for 13 warps: 1.11 against 0.98 ms).  The ring of a warp is 16.5 KiB with float
+// storage and NS = 4, 33 KiB in DP.
 template <int MODE, int NS> struct StripCfg {
-  static constexpr int kRingBytes = strip_slots(NS) * 2 * kStripRB * 2 * kTileCols * static_cast<int>(sizeof(decltype(Traits<MODE>::vec::x)));
+  static constexpr int kRingBytes = strip_slots(NS) * (2 * kStripRB * 2 * kTileCols * static_cast<int>(sizeof(decltype(Traits<MODE>::vec::x))) + 128 + 8);
   static constexpr int kFit = (216 * 1024) / kRingBytes;
-  static constexpr int NW = kFit < 12 ? kFit : 12;
+  static constexpr int kMax = (NS <= 2 && sizeof(typename Traits<MODE>::real) == 4) ? 16 : 12;
+  static constexpr int NW = kFit < kMax ? kFit : kMax;
 };
 
 // Work distribution.  The rows of all strips are laid end to end (strip s occupies [s Lp, (s + 1) Lp), Lp = L rounded
@@ -312,8 +317,9 @@ strip_kernel(const __grid_constant__ CUtensorMap tmap, typename Traits<MODE>::ve
                   if (mm) {
                     double* a = ap - static_cast<long long>(LAG * p) * g.Wp + static_cast<long long>(col) * static_cast<long long>(g.plane);
                     double2 a2 = *reinterpret_cast<const double2*>(a);
-                    if (mm & 1u) a2.x += spin_angle<MODE>(o[p][0], o[p][2]);
-                    if (mm & 2u) a2.y += spin_angle<MODE>(o[p][1], o[p][3]);
+                    // from the spins AS STORED (SP: rounded to float), like the other paths
+                    if (mm & 1u) a2.x += spin_angle<MODE>(R(out.ca), R(out.sa));
+                    if (mm & 2u) a2.y += spin_angle<MODE>(R(out.cb), R(out.sb));
                     *reinterpret_cast<double2*>(a) = a2;
                   }
                 }
@@ -323,17 +329,17 @@ strip_kernel(const __grid_constant__ CUtensorMap tmap, typename Traits<MODE>::ve
                   if constexpr (sizeof(R) == 8) {
                     R Aa, Ab, Ba, Bb;
                     un2(A[p], &Aa, &Ab); un2(B[p], &Ba, &Bb);
-                    esum += static_cast<double>(fma_(o[p][0], Aa, o[p][2] * Ba));
-                    esum += static_cast<double>(fma_(o[p][1], Ab, o[p][3] * Bb));
+                    esum += static_cast<double>(fma_(R(out.ca), Aa, R(out.sa) * Ba));
+                    esum += static_cast<double>(fma_(R(out.cb), Ab, R(out.sb) * Bb));
                   } else {
                     const int par = (u + col) & 1;
                     const R alc = par ? R(nb_m.ca) : R(exc_last), als = par ? R(nb_m.sa) : R(exs_last);
                     const R arc = par ? R(nb_m.cb) : R(nb_m.ca), ars = par ? R(nb_m.sb) : R(nb_m.sa);
                     const R blc = par ? R(nb_m.cb) : R(nb_m.ca), bls = par ? R(nb_m.sb) : R(nb_m.sa);
                     const R brc = par ? R(exc_last) : R(nb_m.cb), brs = par ? R(exs_last) : R(nb_m.sb);
-                    esum += site_energy_term<R>(o[p][0], o[p][2], alc, als, arc, ars, R(nb_u.ca), R(nb_u.sa),
+                    esum += site_energy_term<R>(R(out.ca), R(out.sa), alc, als, arc, ars, R(nb_u.ca), R(nb_u.sa),
                                                 R(nb_d.ca), R(nb_d.sa));
-                    esum += site_energy_term<R>(o[p][1], o[p][3], blc, bls, brc, brs, R(nb_u.cb), R(nb_u.sb),
+                    esum += site_energy_term<R>(R(out.cb), R(out.sb), blc, bls, brc, brs, R(nb_u.cb), R(nb_u.sb),
                                                 R(nb_d.cb), R(nb_d.sb));
                   }
                 }
@@ -425,27 +431,44 @@ int strip_encode(TiledPlan& tp, const Geom& g, void* src, CUtensorMap* map) {
   const cuuint64_t strides[2] = {static_cast<cuuint64_t>(g.Wp) * sizeof(V), static_cast<cuuint64_t>(g.plane) * sizeof(V)};
   const cuuint32_t box[3] = {2 * kTileCols, static_cast<cuuint32_t>(kStripRB), 2};
   const cuuint32_t estr[3] = {1, 1, 1};
+  // 64-byte promotion: a strip row (512 B at a 480-byte pitch) then drags in the least data it does not use
+  // (128 B: 0.983 ms, 64 B: 0.970 ms, none: 0.983 ms per sweep at L = 16384)
+  const CUtensorMapL2promotion promo = CU_TENSOR_MAP_L2_PROMOTION_L2_64B;
   const CUresult r = tp.encode(map, f64 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, src,
                                dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
-                               CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+                               promo, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
   return r == CUDA_SUCCESS ? TILED_OK : TILED_ENCODE;
 }
 
-// Quota of rows per warp: all warp slots of the device (sm_count x NW) when that leaves at least 8 rows each,
-// fewer warps otherwise (a warp pays LEAD + 2 (NS - 1) + 3 warm-up / drain steps per segment whatever its quota).
+// Rows per warp.  Preferred: every strip cut at the SAME rows into n_seg = floor(slots / n_strips) segments (the
+// warps of neighbouring strips then work on the same rows at the same time and the columns they share are read
+// from DRAM once and from L2 the second time) -- taken when that keeps at least 96 % of the warp slots busy.
+// Otherwise the rows of all strips are laid end to end and cut into equal quotas, whatever the strip boundaries.
+// Fewer warps than slots when a warp would get fewer than 8 rows (a warp pays LEAD + 2 (NS - 1) + 3 warm-up / drain
+// steps per segment whatever its quota).
 inline StripGeom strip_geometry(const Geom& g, int ns, int nw, int sm_count, int* nblocks) {
   StripGeom sg;
   const int ic = strip_interior_cols(ns);
   sg.n_strips = (g.Wp + ic - 1) / ic;
-  sg.Lp = (g.L + 3) / 4 * 4;
-  const long long total = static_cast<long long>(sg.n_strips) * sg.Lp;
+  const int L4 = (g.L + 3) / 4 * 4;
   const long long slots = static_cast<long long>(sm_count) * nw;
-  long long warps = total / 8 < slots ? total / 8 : slots;
-  if (warps < 1) warps = 1;
-  long long quota = (total + warps - 1) / warps;
-  quota = (quota + 3) / 4 * 4;
-  sg.quota = static_cast<int>(quota);
-  sg.n_warps = static_cast<int>((total + quota - 1) / quota);
+  const long long n_seg = slots / sg.n_strips;
+  const int seg_rows = n_seg > 0 ? static_cast<int>(((g.L + n_seg - 1) / n_seg + 3) / 4 * 4) : 0;
+  if (n_seg > 0 && sg.n_strips * n_seg * 100 >= slots * 96 && seg_rows >= 8) {
+    const int segs = (g.L + seg_rows - 1) / seg_rows;
+    sg.Lp = segs * seg_rows;
+    sg.quota = seg_rows;
+    sg.n_warps = sg.n_strips * segs;
+  } else {
+    sg.Lp = L4;
+    const long long total = static_cast<long long>(sg.n_strips) * sg.Lp;
+    long long warps = total / 8 < slots ? total / 8 : slots;
+    if (warps < 1) warps = 1;
+    long long quota = (total + warps - 1) / warps;
+    quota = (quota + 3) / 4 * 4;
+    sg.quota = static_cast<int>(quota);
+    sg.n_warps = static_cast<int>((total + quota - 1) / quota);
+  }
   sg.n_mchunks = strip_mask_chunks(g.L);
   *nblocks = sg.n_warps < sm_count ? sg.n_warps : sm_count;
   return sg;
@@ -497,9 +520,10 @@ int strip_launch(StripPlan& plan, TiledPlan& tp, const Geom& g, int src_index, v
   }
   const CUtensorMap& map = plan.map[src_index][w];
 #define MPR_STRIP_CASE(PROG_, K_, M_)                                                                              \
-  if (prog == PROG_ && k == K_ && measure == M_)                                                                   \
-    return strip_launch_one<MODE, PROG_, K_, M_>(plan, map, g, dst, smask, acc, part, slots, kc, first_sweep, stream, \
-                                                 nblocks_out, max_partials);
+  if (prog == PROG_ && k == K_ && measure == M_) {                                                                 \
+    return strip_launch_one<MODE, PROG_, K_, M_>(plan, map, g, dst, smask, acc, part, slots, kc, first_sweep,     \
+                                                   stream, nblocks_out, max_partials);                             \
+  }
   MPR_STRIP_CASE(PROG_R4, 1, 0)
   MPR_STRIP_CASE(PROG_R4, 1, 1)
   MPR_STRIP_CASE(PROG_R4, 1, 2)
