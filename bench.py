@@ -32,12 +32,26 @@ if ROOT not in sys.path:
 
 METRIC = "mpr_site_updates_per_s"
 UNIT = "site-updates/s"
-CPU_CROP = 4096          # cpu_baseline / reference arm: top-left CPU_CROP^2 window of the workload
-CPU_EQ, CPU_MEAS = 110, 4  # ~3.4e9 site-updates: ~15 s on the 16 host threads of the B200 box (measured 2.3e8 /s)
-ALG_WARP_INST_PER_32_UNITS = 125.0   # Metropolis 91 + over-relaxation 34 per unit and sweep
-# dram__bytes_read.sum + dram__bytes_write.sum of one launch of the dominant kernel at L = 16384, from the
-# committed `ncu --set full` capture (profiles/r01g_ncu_full_tiled_v4.md); None for configurations not captured.
-NCU_TRAFFIC_BYTES = {("SP_INTRINSIC", 1): 2.182e9 + 2.099e9}
+# ---- CPU legs (the oracle as it stands).  One temperature per config for BOTH cpu legs (cpu_baseline and --impl
+# reference), close to the T_hat the GPU path infers, so that the two report the same quantity.
+CPU_T = {1: 0.07, 2: 0.03, 3: 1.5e-3, 4: 1.5e-3, 5: 1.1e-3}
+CPU_FULL_WARM, CPU_FULL_SWEEPS = 2, 3          # all host threads, the FULL grid: 2 warm-up + 3 timed hybrid sweeps
+CPU_ONE_CROP, CPU_ONE_SWEEPS = 2048, 3         # one thread: top-left 2048^2 window, 1 warm-up + 3 timed sweeps
+
+# ---- ceilings of the dominant kernel.  Algorithmic work of ONE unit (the two sites of one colour in
+# one row that a lane owns) in ONE hybrid sweep = one Metropolis + one over-relaxation move per site, in this ISA's
+# instructions, priced on the pipe that carries most of them, the FMA-heavy pipe (IMAD, IMAD.WIDE, packed f32x2):
+#   Metropolis  Philox4x32-10 block shared by 4 sites (R9): 10 IMAD.WIDE per unit; local field 6 FADD2;
+#               proposal 1 FFMA2; rotation / energy 13 packed (ts, nts, ps2, ns2, c2m1, 2 x (FMUL2 + FFMA2) for
+#               (dc, ds), cn, sn, FMUL2 + FFMA2 for -dE); acceptance 1 FFMA2                    = 10 W + 21 P
+#   over-relax. local field 6 FADD2; reflection 13 packed                                       = 19 P
+# measured cost per warp instruction and scheduler (tests/helpers/pipe_microbench.cu, profiles/r02_microbench.md):
+#   IMAD.WIDE.U32 4.27 cycles (inside a Philox block), FADD2 / FMUL2 2.03, FFMA2 2.34 -> packed average 2.1
+ALG_FMA_CYCLES_PER_UNIT_SWEEP = 10 * 4.27 + (21 + 19) * 2.1       # = 126.7 scheduler cycles
+SMS, SCHEDULERS = 148, 4
+# dram__bytes_read.sum + dram__bytes_write.sum of one launch at L = 16384 from the committed `ncu --set full` captures
+# (profiles/); None for configurations not captured.
+NCU_TRAFFIC_BYTES = {("SP_INTRINSIC", "R4", 1): 2.957e9 + 2.117e9}
 
 
 def parse():
@@ -50,7 +64,10 @@ def parse():
     ap.add_argument("--mode", default="SP_INTRINSIC")
     ap.add_argument("--n-eq", type=int, default=None)
     ap.add_argument("--n-meas", type=int, default=None)
-    ap.add_argument("--fused", type=int, default=1)
+    ap.add_argument("--fused", type=int, default=1, help="hybrid sweeps per launch (STRIP: 1 or 2)")
+    ap.add_argument("--path", default="AUTO", choices=["AUTO", "STRIP", "TILED", "PLAIN"])
+    ap.add_argument("--schedule", default="R4", choices=["R4", "SITE_FUSED"],
+                    help="pass order of a hybrid sweep (DESIGN.md R4 / R4b); the headline is R4")
     ap.add_argument("--temperature", type=float, default=None,
                     help="profiling only: fix T and skip the temperature estimate (not the benchmark step)")
     ap.add_argument("--skip-cpu-baseline", action="store_true")
@@ -117,35 +134,63 @@ class ClockSampler:
         return out
 
 
-def cpu_sample(values, mask, T, seed):
-    """The oracle, as it stands, on the top-left CPU_CROP^2 window: run(CPU_EQ, CPU_MEAS), all host threads."""
+def cpu_legs(values, mask, T, seed, full_sweeps=CPU_FULL_SWEEPS):
+    """The oracle, as it stands, on the host cores: (a) all threads on the FULL grid, CPU_FULL_WARM warm-up +
+    `full_sweeps` timed hybrid sweeps after an R8 start with 2 quench double passes; (b) one thread on the top-left
+    CPU_ONE_CROP^2 window.  Returns (all-thread dict, one-thread dict)."""
     from oracle import mpr_oracle
-    n = min(CPU_CROP, values.shape[0])
-    v = np.ascontiguousarray(values[:n, :n])
-    m = np.ascontiguousarray(mask[:n, :n])
+    L = values.shape[0]
     cores = mpr_oracle.threads_available()
-    o = mpr_oracle.Oracle(values=v, mask=m, seed=seed, threads=cores)
+    t0 = time.perf_counter()
+    o = mpr_oracle.Oracle(values=values, mask=mask, seed=seed, threads=cores, n_quench=2)
     o.set_temperature(T)
-    return o, int(m.sum()), cores, n
+    t_init = time.perf_counter() - t0
+    o.hybrid_sweeps(CPU_FULL_WARM)
+    t0 = time.perf_counter()
+    o.hybrid_sweeps(full_sweeps)
+    dt = time.perf_counter() - t0
+    n_free = int(mask.sum())
+    full = {"value": 2.0 * n_free * full_sweeps / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
+            "sample": "full %dx%d grid, %d warm-up + %d timed hybrid sweeps, T=%g, %.1f s (+ %.1f s set-up)" %
+                      (L, L, CPU_FULL_WARM, full_sweeps, T, dt, t_init)}
+    del o
+    n = min(CPU_ONE_CROP, L)
+    v1, m1 = np.ascontiguousarray(values[:n, :n]), np.ascontiguousarray(mask[:n, :n])
+    o1 = mpr_oracle.Oracle(values=v1, mask=m1, seed=seed, threads=1, n_quench=2)
+    o1.set_temperature(T)
+    o1.hybrid_sweeps(1)
+    t0 = time.perf_counter()
+    o1.hybrid_sweeps(CPU_ONE_SWEEPS)
+    dt1 = time.perf_counter() - t0
+    one = {"value": 2.0 * int(m1.sum()) * CPU_ONE_SWEEPS / dt1, "unit": UNIT, "cores": 1, "kind": "oracle",
+           "sample": "top-left %dx%d window, 1 warm-up + %d timed hybrid sweeps, T=%g, %.1f s" %
+                     (n, n, CPU_ONE_SWEEPS, T, dt1)}
+    return full, one
 
 
 def run_reference(args, rank, world):
-    """--impl reference: the CPU oracle on the box's host cores, bounded sample per step."""
+    """--impl reference: the CPU oracle on the box's host cores; a step = CPU_FULL_SWEEPS hybrid sweeps of the
+    full grid of the config (the same bounded sample cpu_baseline times)."""
     if rank != 0:
         return
+    from oracle import mpr_oracle
     from paper_1910_08448_b200 import inputs
     c = inputs.CONFIGS[args.config]
     values, mask, _ = inputs.make_problem(c.L, c.xi, c.field_seed, c.f, c.lognormal)
-    o, n_free, cores, n = cpu_sample(values, mask, 0.05, c.mpr_seed)
-    upd = 2.0 * n_free * (CPU_EQ + CPU_MEAS)
+    T = CPU_T[args.config]
+    cores = mpr_oracle.threads_available()
+    o = mpr_oracle.Oracle(values=values, mask=mask, seed=c.mpr_seed, threads=cores, n_quench=2)
+    o.set_temperature(T)
+    n_free = int(mask.sum())
     for _ in range(args.warmup):
-        o.run(CPU_EQ, CPU_MEAS)
+        o.hybrid_sweeps(1)
     t0 = time.perf_counter()
     for _ in range(args.steps):
-        o.run(CPU_EQ, CPU_MEAS)
+        o.hybrid_sweeps(CPU_FULL_SWEEPS)
     dt = time.perf_counter() - t0
-    val = upd * args.steps / dt
-    sample = "top-left %dx%d window of the L=%d workload, run(%d,%d) per step, T=0.05" % (n, n, c.L, CPU_EQ, CPU_MEAS)
+    val = 2.0 * n_free * CPU_FULL_SWEEPS * args.steps / dt
+    sample = "full %dx%d grid, %d hybrid sweeps per step (%d warm-up sweeps), T=%g" % (c.L, c.L, CPU_FULL_SWEEPS,
+                                                                                    args.warmup, T)
     print(json.dumps({
         "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True, "scaling": "weak",
@@ -188,6 +233,8 @@ def run_ours(args, rank, world, local_rank):
 
     def step():
         g = mpr.Mpr(d_values, d_mask, mode=mode, seed=seed, device=dev)
+        g.set_path(args.path)
+        g.set_schedule(args.schedule)
         g.set_fused_sweeps(args.fused)
         if args.temperature is not None:
             g.set_temperature(args.temperature)
@@ -239,76 +286,113 @@ def run_ours(args, rank, world, local_rank):
     base_mae = float((d_truth[m1] - d_values[~m1].mean()).abs().mean().item())
     T_hat = state["T"]
 
-    # ---- roofline of the dominant kernel: tiled_sweep_kernel<mode, false>, timed live ----------
-    g = mpr.Mpr(d_values, d_mask, mode=mode, seed=seed, device=dev)
-    g.set_fused_sweeps(args.fused)
-    g.set_temperature(T_hat)
-    g.sweep(8 * args.fused)
-    n_l = 50
-    torch.cuda.synchronize(dev)
-    k0, k1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    k0.record()
-    g.sweep(n_l * args.fused)
-    k1.record()
-    torch.cuda.synchronize(dev)
-    kern_ms_burst = k0.elapsed_time(k1) / n_l      # the kernel timed alone, 50 launches after the steps
-    g.close()
-    # roofline uses the average launch duration INSIDE the timed steps (sustained clocks); the burst leg
-    # is reported beside it and stands in only when the steps had no equilibration sweeps
+    # ---- ceilings of the dominant kernel (the sweep launch without measurement), timed live ------------------
+    def time_sweeps(md, path, schedule, k, n_launch, warm=6):
+        gk = mpr.Mpr(d_values, d_mask, mode=md, seed=seed, device=dev)
+        gk.set_path(path)
+        gk.set_schedule(schedule)
+        gk.set_fused_sweeps(k)
+        gk.set_temperature(T_hat)
+        gk.sweep(warm * k)
+        torch.cuda.synchronize(dev)
+        k0, k1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        k0.record()
+        gk.sweep(n_launch * k)
+        k1.record()
+        torch.cuda.synchronize(dev)
+        ms_launch = k0.elapsed_time(k1) / n_launch
+        k0.record()
+        gk.run(0, 5, want_pred=False)
+        k1.record()
+        torch.cuda.synchronize(dev)
+        gk.close()
+        return ms_launch, k0.elapsed_time(k1) / 5
+
+    # what MPR_PATH_AUTO resolves to (csrc/mpr.cu, eff_path)
+    def auto_path(md, schedule):
+        return "STRIP" if schedule == "SITE_FUSED" or (md == "SP_INTRINSIC" and L >= 4096) else "TILED"
+    path_used = auto_path(mode, args.schedule) if args.path == "AUTO" else args.path
+    k_eff = min(args.fused, 2) if path_used == "STRIP" else args.fused
+    kern_ms_burst, _ = time_sweeps(mode, args.path, args.schedule, args.fused, 50)   # the kernel timed alone, after the steps
+    # the in-step figure (sustained clocks) is the one the ceilings use; the burst leg stands in only when the steps had
+    # no equilibration sweeps
     in_step = state["eq_launches"] > 0
     kern_ms = state["eq_ms"] / state["eq_launches"] if in_step else kern_ms_burst
-    w = 16 if mode == "DP" else 8
-    Wp = (((L + 1) // 2 + 15) // 16) * 16
-    stored = 2 * L * Wp
-    alg_bytes = stored * 2 * w + 2 * stored / 8.0          # read + write of every stored spin, mask bits
     peak, peak_src = peaks()
-    achieved = alg_bytes / (kern_ms * 1e-3) / 1e9
-    # second ceiling: warp-instruction issue.  Algorithmic count = 125 warp instructions per
-    # 32 units (unit = 2 sites of one colour and row) per hybrid sweep; peak = 148 SMs x 4 schedulers x 1 / clk.
-    alg_inst = (stored / 2.0) / 32.0 * ALG_WARP_INST_PER_32_UNITS * args.fused
-    sm_hz = (clk.get("sm_max_mhz") or 1965.0) * 1e6
-    issue_peak = 148 * 4 * sm_hz
-    alu = {"bound": "alu", "achieved": alg_inst / (kern_ms * 1e-3), "peak": issue_peak, "unit": "warp-inst/s",
-           "frac": alg_inst / (kern_ms * 1e-3) / issue_peak, "algorithmic_warp_inst_per_launch": alg_inst}
-    roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                "traffic": NCU_TRAFFIC_BYTES.get((mode, args.fused)) if L == 16384 else None, "kernel": "tiled_sweep_kernel<%s,0>" % mode,
-                "kernel_ms": kern_ms,
-                "kernel_ms_source": ("CUDA events around the %d equilibration launches inside the timed steps "
-                                     "(mpr_get_run_timing)" % state["eq_launches"]) if in_step else "burst leg",
-                "kernel_ms_burst": kern_ms_burst, "frac_burst": alg_bytes / (kern_ms_burst * 1e-3) / 1e9 / peak,
-                "algorithmic_bytes_per_launch": alg_bytes, "sweeps_per_launch": args.fused, "peak_source": peak_src,
-                "kernel_site_updates_per_s": 2.0 * state["n_free"] * args.fused / (kern_ms * 1e-3),
-                "second_ceiling": alu}
+    sm_mhz = clk.get("sm_mhz") or 1965.0
 
-    # ---- per-mode sweep rates (BASELINE.json: "per precision mode") ----------------------------
+    def ceilings(md, ms_launch, k, sm_mhz_used):
+        """Ceilings of one sweep launch of k hybrid sweeps.  Bytes per SURVEY.md 8(d): every spin read once and written
+        once per LAUNCH at the paper's storage width w (4 B in the float-storage modes: one 32-bit angle; 8 B in DP),
+        plus the mask bits; `state_bytes` is what this library's layout moves (a unit vector per spin: 2 w)."""
+        w = 8 if md == "DP" else 4
+        alg_bytes = 2.0 * N * w + N / 8.0
+        state_bytes = 2.0 * N * 2 * w + N / 8.0
+        units = N / 2.0                                             # one unit = 2 sites of one colour and row
+        fma_cycles = units / 32.0 * k * ALG_FMA_CYCLES_PER_UNIT_SWEEP   # scheduler cycles on the FMA-heavy pipe
+        fma_peak = SMS * SCHEDULERS * sm_mhz_used * 1e6             # scheduler cycles per second at the sampled clock
+        t = ms_launch * 1e-3
+        out = {
+            "hbm_algorithmic": {"bytes_per_launch": alg_bytes, "achieved_gb_s": alg_bytes / t / 1e9,
+                                "frac": alg_bytes / t / 1e9 / peak, "lower_bound_ms": alg_bytes / (peak * 1e9) * 1e3},
+            "hbm_state_layout": {"bytes_per_launch": state_bytes, "achieved_gb_s": state_bytes / t / 1e9,
+                                 "frac": state_bytes / t / 1e9 / peak, "lower_bound_ms": state_bytes / (peak * 1e9) * 1e3},
+        }
+        if md in ("SP_INTRINSIC", "SP_PRECISE"):
+            out["fma_pipe"] = {"cycles_per_launch": fma_cycles, "achieved_cycles_per_s": fma_cycles / t,
+                               "peak_cycles_per_s": fma_peak, "frac": fma_cycles / t / fma_peak,
+                               "lower_bound_ms": fma_cycles / fma_peak * 1e3, "sm_mhz": sm_mhz_used,
+                               "cycles_per_unit_sweep": ALG_FMA_CYCLES_PER_UNIT_SWEEP}
+        return out
+
+    ceil = ceilings(mode, kern_ms, k_eff, sm_mhz)
+    # the binding ceiling = the one with the largest lower-bound time among those computed from ALGORITHMIC work
+    binding = "alu" if "fma_pipe" in ceil and ceil["fma_pipe"]["lower_bound_ms"] > ceil["hbm_algorithmic"]["lower_bound_ms"] \
+        else "hbm"
+    if binding == "alu":
+        fp = ceil["fma_pipe"]
+        roofline = {"bound": "alu", "achieved": fp["achieved_cycles_per_s"], "peak": fp["peak_cycles_per_s"],
+                    "unit": "FMA-pipe scheduler cycles/s", "frac": fp["frac"],
+                    "peak_source": "148 SMs x 4 schedulers x SM clock sampled during the timed steps (%.0f MHz); "
+                                   "instruction costs measured by tests/helpers/pipe_microbench.cu "
+                                   "(profiles/r02_microbench.md)" % sm_mhz,
+                    "binding_evidence": "ncu sm__pipe_fmaheavy_cycles_active is the busiest pipe (profiles/r02*_ncu_full*.md)"}
+    else:
+        ha = ceil["hbm_algorithmic"]
+        roofline = {"bound": "hbm", "achieved": ha["achieved_gb_s"], "peak": peak, "unit": "GB/s", "frac": ha["frac"],
+                    "peak_source": peak_src}
+    roofline.update({
+        "traffic": NCU_TRAFFIC_BYTES.get((mode, args.schedule, k_eff)) if L == 16384 else None,
+        "kernel": "strip_kernel<%s, %s, k=%d, 0>" % (mode, args.schedule, k_eff) if path_used == "STRIP"
+                  else "tiled_sweep_kernel<%s,0>" % mode,
+        "kernel_ms": kern_ms,
+        "kernel_ms_source": ("CUDA events around the %d equilibration launches inside the timed steps "
+                             "(mpr_get_run_timing)" % state["eq_launches"]) if in_step else "burst leg",
+        "kernel_ms_burst": kern_ms_burst, "sweeps_per_launch": k_eff,
+        "algorithmic_bytes_per_launch": ceil["hbm_algorithmic"]["bytes_per_launch"],
+        "state_bytes_per_launch": ceil["hbm_state_layout"]["bytes_per_launch"],
+        "hbm_peak_gb_s": peak, "hbm_peak_source": peak_src,
+        "ceilings": ceil,
+        "kernel_site_updates_per_s": 2.0 * state["n_free"] * k_eff / (kern_ms * 1e-3),
+    })
+
+    # ---- per-mode sweep rates (BASELINE.json: "per precision mode"), both schedules --------------------------------
     modes = {}
     if not args.skip_modes:
         for md, n_sw in (("DP", 10), ("SP", 10), ("SP_PRECISE", 30), ("SP_INTRINSIC", 30)):
             if md not in c.modes:
                 continue
-            gm = mpr.Mpr(d_values, d_mask, mode=md, seed=seed, device=dev)
-            gm.set_temperature(T_hat)
-            gm.sweep(3)
-            torch.cuda.synchronize(dev)
-            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            a.record()
-            gm.sweep(n_sw)
-            b.record()
-            torch.cuda.synchronize(dev)
-            t = a.elapsed_time(b) / n_sw
-            a.record()
-            _, e_m, se_m = gm.run(0, 5, want_pred=False)
-            b.record()
-            torch.cuda.synchronize(dev)
-            # same definitions as `roofline` above: every stored spin read and written once + the mask bits
-            md_bytes = stored * 2 * (16 if md == "DP" else 8) + 2 * stored / 8.0
-            modes[md] = {"ms_per_sweep": t, "site_updates_per_s": 2.0 * state["n_free"] / (t * 1e-3),
-                         "hbm_roofline_frac": md_bytes / (t * 1e-3) / 1e9 / peak,
-                         "ms_per_measurement_sweep": a.elapsed_time(b) / 5,
-                         # mean of 5 samples taken 3 + n_sw sweeps after the chain reset: NOT an equilibrium
-                         # value and not comparable between modes (n_sw differs); a plausibility figure only
-                         "e_unequilibrated_after_%d_sweeps" % (3 + n_sw): e_m}
-            gm.close()
+            entry = {}
+            for sched, k in (("R4", 1), ("SITE_FUSED", 2)):
+                t_l, t_meas = time_sweeps(md, "AUTO", sched, k, n_sw, warm=3)
+                cl = ceilings(md, t_l, k, sm_mhz)
+                entry[sched] = {"path": auto_path(md, sched), "sweeps_per_launch": k, "ms_per_sweep": t_l / k,
+                                "site_updates_per_s": 2.0 * state["n_free"] * k / (t_l * 1e-3),
+                                "ms_per_measurement_sweep": t_meas,
+                                "frac_hbm_algorithmic": cl["hbm_algorithmic"]["frac"],
+                                "frac_hbm_state_layout": cl["hbm_state_layout"]["frac"],
+                                "frac_fma_pipe": cl.get("fma_pipe", {}).get("frac")}
+            modes[md] = entry
 
     # ---- end to end through the C ABI with HOST buffers (mpr_predict_host) ---------------------
     e2e = None
@@ -344,15 +428,10 @@ def run_ours(args, rank, world, local_rank):
 
     cpu = None
     if rank == 0 and not args.skip_cpu_baseline:
-        o, nf, cores, n = cpu_sample(values, mask, T_hat, seed)
-        o.run(1, 0)
-        t0 = time.perf_counter()
-        o.run(CPU_EQ, CPU_MEAS)
-        dt = time.perf_counter() - t0
-        cpu = {"value": 2.0 * nf * (CPU_EQ + CPU_MEAS) / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
-               "sample": "top-left %dx%d window of the L=%d workload, run(%d,%d), T=T_hat, %.1f s" %
-                         (n, n, L, CPU_EQ, CPU_MEAS, dt)}
+        cpu, cpu_one = cpu_legs(values, mask, CPU_T[args.config], seed)
+        cpu["single_thread"] = cpu_one
 
+    state_gib = 2.0 * N * (16 if mode == "DP" else 8) / 2 ** 30
     if rank == 0:
         print(json.dumps({
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
@@ -360,8 +439,10 @@ def run_ours(args, rank, world, local_rank):
             "vs_baseline": None, "dtype": {"DP": "f64", "SP": "f64"}.get(mode, "f32"), "data": "synthetic",
             "config": {"workload": c.name, "L": L, "masked_fraction": c.f, "mode": mode, "n_eq": n_eq,
                        "n_meas": n_meas, "T_trials": state["trials"], "sweeps_per_step": state["sweeps"] // args.steps,
-                       "fused_sweeps": args.fused, "parallelism": "replicas x%d" % world,
-                       "l2": "state (%.1f GiB) larger than L2; no flush" % (stored * w / 2 ** 30)},
+                       "path": path_used, "schedule": args.schedule, "fused_sweeps": k_eff,
+                       "parallelism": "replicas x%d" % world,
+                       "l2": ("state (%.2f GiB) larger than the 126 MB L2; no flush" % (state_gib)) if state_gib * 2 ** 30 > 126e6
+                             else "state (%.1f MiB) is L2-resident by design of this config (BASELINE.json); no flush" % (state_gib * 1024)},
             "clocks": clk, "e2e": e2e, "gpu_launches": launches_total, "roofline": roofline,
             "cpu_baseline": cpu, "modes": modes, "T_hat": T_hat, "e_sample": state.get("e_sample"),
             "e_mean": state["e"], "e_stderr": state["se"], "mae": mae, "rmse": rmse,

@@ -64,14 +64,16 @@ typedef enum {
 typedef enum { MPR_DP = 0, MPR_SP = 1, MPR_SP_PRECISE = 2, MPR_SP_INTRINSIC = 3 } mpr_precision;
 
 /* Kernel paths.  All give bit-identical spin states (determinism contract).
- *   MPR_PATH_STRIP   (default) one launch per k <= 2 hybrid sweeps: every warp streams a column strip of
+ *   MPR_PATH_AUTO    (default) the path measured fastest for the mode, grid size and schedule: STRIP for
+ *                    MPR_SP_INTRINSIC at L >= 4096 and for the site-fused schedule, TILED otherwise.
+ *   MPR_PATH_STRIP   one launch per k <= 2 hybrid sweeps: every warp streams a column strip of
  *                    the grid through a private shared-memory ring fed by TMA and runs the colour
  *                    passes as a software pipeline down the rows (no barriers, no redundant rows).
  *   MPR_PATH_TILED   one launch per hybrid sweep group: TMA stages a tile + halo of both colour
  *                    planes in shared memory, all 4*k colour passes of k sweeps run there.
  *   MPR_PATH_PLAIN   one launch per colour pass on the global colour planes (reference path
  *                    for the self-consistency tests; also used for odd R8 quench passes).  */
-typedef enum { MPR_PATH_TILED = 0, MPR_PATH_PLAIN = 1, MPR_PATH_STRIP = 2 } mpr_path;
+typedef enum { MPR_PATH_TILED = 0, MPR_PATH_PLAIN = 1, MPR_PATH_STRIP = 2, MPR_PATH_AUTO = 3 } mpr_path;
 
 /* Order of the colour passes inside one hybrid sweep ("hybrid algorithm" -- the paper
  * leaves the order to its ref. [5]; both orders leave the conditional Boltzmann density invariant):
@@ -126,7 +128,7 @@ int mpr_set_seed(mpr_ctx* ctx, uint64_t seed);
 int mpr_set_temperature(mpr_ctx* ctx, double T);
 /* Number of quench double-passes of the R8 initialisation (default 32).  Resets the chain. */
 int mpr_set_quench(mpr_ctx* ctx, int n);
-/* Kernel path (default MPR_PATH_STRIP) and temporal-blocking depth 1 <= k <= 4 (hybrid sweeps
+/* Kernel path (default MPR_PATH_AUTO) and temporal-blocking depth 1 <= k <= 4 (hybrid sweeps
  * fused per launch, default 1; the STRIP path uses min(k, 2)).  Results do not depend on either. */
 int mpr_set_path(mpr_ctx* ctx, mpr_path path);
 int mpr_set_fused_sweeps(mpr_ctx* ctx, int k);

@@ -74,7 +74,7 @@ struct mpr_ctx {
   char* ws = nullptr;
   cudaStream_t stream = nullptr;
   int mode = MPR_DP;
-  int path = MPR_PATH_STRIP;
+  int path = MPR_PATH_AUTO;
   int schedule = MPR_SCHEDULE_R4;
   int fused = 1;
   int n_quench = 32;
@@ -352,6 +352,16 @@ int do_strip(mpr_ctx* c, int prog, int k, int measure, double* d_e) {
   }
 }
 
+// MPR_PATH_AUTO: the path measured fastest for the case at hand (B200, bench.py --path, profiles/): the STRIP
+// kernels in SP_INTRINSIC on grids large enough to give every warp a long run of rows, and for the site-fused
+// schedule (which the TILED kernels do not carry); the TILED kernels otherwise (double arithmetic and the
+// library sincosf / expf of SP_PRECISE need more registers per update chain than four interleaved chains leave).
+int eff_path(const mpr_ctx* c) {
+  if (c->path != MPR_PATH_AUTO) return c->path;
+  if (c->schedule == MPR_SCHEDULE_SITE_FUSED) return MPR_PATH_STRIP;
+  return (c->mode == MPR_SP_INTRINSIC && c->lo.g.L >= 4096) ? MPR_PATH_STRIP : MPR_PATH_TILED;
+}
+
 // R8: uniform initial spins, then n_quench x (quench colour 0, quench colour 1); everything
 // that belongs to the chain is cleared.
 int reset_chain(mpr_ctx* c, uint32_t trial) {
@@ -366,13 +376,14 @@ int reset_chain(mpr_ctx* c, uint32_t trial) {
   // quench double passes (colour 0, colour 1): the tiled kernel runs them 2 k at a time (k <= 2,
   // halo 4 k), an odd remainder goes through the plain kernels -- same moves, same order
   int left = c->n_quench;
-  if (c->path == MPR_PATH_TILED) {
+  const int path = eff_path(c);
+  if (path == MPR_PATH_TILED) {
     while (left >= 2) {
       const int k = left / 2 < 2 ? left / 2 : 2;
       TRY(do_tiled(c, k, kTiledQuench, nullptr));
       left -= 2 * k;
     }
-  } else if (c->path == MPR_PATH_STRIP) {
+  } else if (path == MPR_PATH_STRIP) {
     for (; left >= 2; left -= 2) TRY(do_strip(c, PROG_QUENCH, 2, 0, nullptr));     // two double passes per launch
   }
   for (; left > 0; --left) {
@@ -408,7 +419,8 @@ int hybrid_sweeps(mpr_ctx* c, int n, int measure, int first_slot) {
   if (n <= 0) return MPR_OK;
   if (!(c->T > 0.0)) return fail(c, MPR_ERR_NOT_READY, "temperature not set");
   TRY(ensure_chain(c));
-  if (c->path == MPR_PATH_PLAIN) {
+  const int path = eff_path(c);
+  if (path == MPR_PATH_PLAIN) {
     for (int i = 0; i < n; ++i) {
       const uint64_t sw = c->sweep + 1;
       if (c->schedule == MPR_SCHEDULE_SITE_FUSED) {      // R4b
@@ -432,14 +444,14 @@ int hybrid_sweeps(mpr_ctx* c, int n, int measure, int first_slot) {
     }
     return MPR_OK;
   }
-  if (c->path == MPR_PATH_TILED && c->schedule != MPR_SCHEDULE_R4)
+  if (path == MPR_PATH_TILED && c->schedule != MPR_SCHEDULE_R4)
     return fail(c, MPR_ERR_INVALID_ARG, "the site-fused schedule runs on the STRIP and PLAIN paths");
   int done = 0;
   while (done < n) {
     // measurement needs the state after every sweep: one sweep per launch there
     int k = measure ? 1 : (n - done < c->fused ? n - done : c->fused);
     double* d_e = measure ? c->dseries() + first_slot + done : nullptr;
-    if (c->path == MPR_PATH_STRIP) {
+    if (path == MPR_PATH_STRIP) {
       if (k > 2) k = 2;                                   // the strip pipeline carries at most two sweeps
       TRY(do_strip(c, c->schedule == MPR_SCHEDULE_SITE_FUSED ? PROG_FUSED : PROG_R4, k, measure, d_e));
     } else {
@@ -629,7 +641,7 @@ int mpr_set_quench(mpr_ctx* c, int n) {
   return MPR_OK;
 }
 int mpr_set_path(mpr_ctx* c, mpr_path path) {
-  if (!c || (path != MPR_PATH_TILED && path != MPR_PATH_PLAIN && path != MPR_PATH_STRIP))
+  if (!c || (path != MPR_PATH_TILED && path != MPR_PATH_PLAIN && path != MPR_PATH_STRIP && path != MPR_PATH_AUTO))
     return fail(c, MPR_ERR_INVALID_ARG, "bad path");
   c->path = path;
   return MPR_OK;

@@ -250,6 +250,24 @@ strip_kernel(const __grid_constant__ CUtensorMap tmap, typename Traits<MODE>::ve
             }
           }
 
+          // measuring launches: the accumulator words of the two rows that become final in this step are
+          // requested now and used at the end of the step (their latency hides behind the arithmetic)
+          double2 acc_pre[2];
+          if constexpr (MEASURE == 2) {
+#pragma unroll
+            for (int p = NS - 2; p < NS; ++p) {
+              const int col = p & 1, row = t - LAG * p;
+              const int rel = u - LAG * p;
+              const int mqk = (rel >= 0) ? 0 : (-rel + RB - 1) / RB;
+              const uint32_t mm = (cw[mqk] >> (4 * (rel + mqk * RB) + 2 * col)) & 3u;
+              const bool owned = lane_ok && (!EDGE || (row >= yb && row < ye));
+              acc_pre[p - (NS - 2)] = make_double2(0.0, 0.0);
+              if (owned && mm)
+                acc_pre[p - (NS - 2)] = *reinterpret_cast<const double2*>(
+                    ap - static_cast<long long>(LAG * p) * g.Wp + static_cast<long long>(col) * static_cast<long long>(g.plane));
+            }
+          }
+
           // ---- compute
           R o[NS][4];
 #pragma unroll
@@ -316,7 +334,7 @@ strip_kernel(const __grid_constant__ CUtensorMap tmap, typename Traits<MODE>::ve
                   const uint32_t mm = (cw[mqk] >> (4 * (rel + mqk * RB) + 2 * col)) & 3u;
                   if (mm) {
                     double* a = ap - static_cast<long long>(LAG * p) * g.Wp + static_cast<long long>(col) * static_cast<long long>(g.plane);
-                    double2 a2 = *reinterpret_cast<const double2*>(a);
+                    double2 a2 = acc_pre[p - (NS - 2)];
                     // from the spins AS STORED (SP: rounded to float), like the other paths
                     if (mm & 1u) a2.x += spin_angle<MODE>(R(out.ca), R(out.sa));
                     if (mm & 2u) a2.y += spin_angle<MODE>(R(out.cb), R(out.sb));

@@ -19,7 +19,7 @@ ERR_INVALID_ARG, ERR_NO_MEASURED, ERR_DEGENERATE_RANGE, ERR_NONFINITE = -1, -2, 
 ERR_WORKSPACE, ERR_NOT_READY, ERR_NO_ROOT, ERR_CUDA = -5, -6, -7, -8
 
 MODES = {"DP": 0, "SP": 1, "SP_PRECISE": 2, "SP_INTRINSIC": 3}
-PATHS = {"TILED": 0, "PLAIN": 1, "STRIP": 2}
+PATHS = {"TILED": 0, "PLAIN": 1, "STRIP": 2, "AUTO": 3}
 SCHEDULES = {"R4": 0, "SITE_FUSED": 1}
 PASS_KINDS = {"MET": 0, "OR": 1, "QUENCH": 2, "MO": 3}
 
