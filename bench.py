@@ -73,6 +73,11 @@ def parse():
     ap.add_argument("--skip-cpu-baseline", action="store_true")
     ap.add_argument("--skip-modes", action="store_true")
     ap.add_argument("--skip-e2e", action="store_true")
+    ap.add_argument("--matrix", action="store_true",
+                    help="the paper's experiment shape (PAPER.md:35-57): R_X = t_DDD / t_X for the eight (X_S X_E X_F) settings "
+                         "at L = 2^5 .. 2^12, f = 0.9, kappa = 0.2, and Delta MAAE_X over M mask realisations; one JSON line")
+    ap.add_argument("--matrix-masks", type=int, default=10, help="M, mask realisations per data set for Delta MAAE (paper: 100)")
+    ap.add_argument("--matrix-L", type=int, default=512, help="grid size of the Delta MAAE study")
     ap.add_argument("--microbench", action="store_true",
                     help="build and run tests/helpers/pipe_microbench.cu (pipe throughputs, L2 / HBM copy) and exit")
     return ap.parse_args()
@@ -452,6 +457,77 @@ def run_ours(args, rank, world, local_rank):
         dist.destroy_process_group()
 
 
+def run_matrix(args):
+    """PAPER.md:35 (eight precision settings), :39 / :47 (Fig. 1: R_X = t_DDD / t_X against L = 2^k, k = 5 .. 12, Gaussian
+    N(50, 10) data with exponential covariance, kappa = 0.2, 90 % removed), :55-57 (Fig. 2: Delta MAAE_X in % over M mask
+    realisations of one data set).  Synthetic stand-ins from inputs.make_problem (xi = 1 / kappa = 5)."""
+    import torch
+    from paper_1910_08448_b200 import inputs, mpr
+    dev = torch.device("cuda", 0)
+    n_eq, n_meas = 200, 50
+    out = {"triples": list(mpr.TRIPLES), "n_eq": n_eq, "n_meas": n_meas, "f": 0.9, "kappa": 0.2, "R_X": {}, "ms": {}}
+    for k in range(5, 13):
+        L = 2 ** k
+        values, mask, _ = inputs.make_problem(L, 5.0, 100 + k, 0.9, False)
+        dv, dm = torch.from_numpy(values).to(dev), torch.from_numpy(mask).to(dev)
+        g0 = mpr.Mpr(dv, dm, mode="DP", seed=7, device=dev)
+        T_hat, _, _ = g0.estimate_temperature()
+        g0.close()
+        ms = {}
+        for X in mpr.TRIPLES:
+            g = mpr.Mpr(dv, dm, seed=7, device=dev)
+            g.set_precision_triple(X)
+            g.set_temperature(T_hat)
+            g.run(20, 5, want_pred=False)
+            best = None
+            for _ in range(3):
+                a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                torch.cuda.synchronize(dev)
+                a.record()
+                g.run(n_eq, n_meas, want_pred=True)
+                b.record()
+                torch.cuda.synchronize(dev)
+                t = a.elapsed_time(b)
+                best = t if best is None or t < best else best
+            ms[X] = best
+            g.close()
+        out["ms"][str(L)] = ms
+        out["R_X"][str(L)] = {X: ms["DDD"] / ms[X] for X in mpr.TRIPLES}
+    # Delta MAAE_X: one data set, M masks; paired over the masks
+    L, M = args.matrix_L, args.matrix_masks
+    field_rng = np.random.default_rng(4242)
+    z = 50.0 + 10.0 * inputs.matern_field(L, 5.0, field_rng)
+    maes = {X: [] for X in mpr.TRIPLES}
+    for m in range(M):
+        rng = np.random.default_rng(9000 + m)
+        mask = np.zeros(L * L, dtype=np.uint8)
+        mask[rng.choice(L * L, size=round(0.9 * L * L), replace=False, shuffle=False)] = 1
+        mask = mask.reshape(L, L)
+        vals = np.where(mask == 1, np.nan, z)
+        dv, dm, dt = torch.from_numpy(vals).to(dev), torch.from_numpy(mask).to(dev), torch.from_numpy(z).to(dev)
+        g0 = mpr.Mpr(dv, dm, mode="DP", seed=11 + m, device=dev)
+        T_hat, _, _ = g0.estimate_temperature()
+        g0.close()
+        free = dm.bool()
+        for X in mpr.TRIPLES:
+            g = mpr.Mpr(dv, dm, seed=11 + m, device=dev)
+            g.set_precision_triple(X)
+            g.set_temperature(T_hat)
+            pred, _, _ = g.run(300, 100)
+            maes[X].append(float((pred - dt)[free].abs().mean()))
+            g.close()
+    ref = np.array(maes["DDD"])
+    out["delta_maae_pct"] = {}
+    for X in mpr.TRIPLES:
+        a = np.array(maes[X])
+        d = 100.0 * (a.mean() / ref.mean() - 1.0)
+        # error bar: standard error of the paired relative differences over the masks
+        se = 100.0 * float(np.std(a / ref - 1.0, ddof=1) / np.sqrt(M)) if M > 1 else None
+        out["delta_maae_pct"][X] = {"value": d, "stderr": se, "maae": float(a.mean())}
+    out["delta_maae_config"] = {"L": L, "M": M, "n_eq": 300, "n_meas": 100}
+    print(json.dumps({"matrix": out, "data": "synthetic"}))
+
+
 def run_microbench():
     """Measured per-SM pipe throughputs and copy bandwidths (JSON lines on stdout): the denominators of the
     "alu" ceilings, taken on the box the bench runs on."""
@@ -467,6 +543,9 @@ def main():
     args = parse()
     if args.microbench:
         run_microbench()
+        return
+    if args.matrix:
+        run_matrix(args)
         return
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))

@@ -60,8 +60,13 @@ typedef enum {
  *   MPR_SP            SSD  float storage of the spins, double arithmetic and functions
  *   MPR_SP_PRECISE    float storage and arithmetic, sinf/cosf/expf (not in the paper)
  *   MPR_SP_INTRINSIC  SSS  float storage and arithmetic, __sinf/__cosf/__expf
- * Energy sums are accumulated in double in every mode (R13).                              */
-typedef enum { MPR_DP = 0, MPR_SP = 1, MPR_SP_PRECISE = 2, MPR_SP_INTRINSIC = 3 } mpr_precision;
+ * Energy sums are accumulated in double in every mode (R13) unless X_E = S is asked for (below).
+ *   MPR_DS_INTRINSIC  D.S  double storage of the spins, float arithmetic with the intrinsics
+ * The paper's eight settings (X_S X_E X_F) = (spin storage, energy variable, functions), each D or S, are
+ * mpr_set_precision_triple("DDD" ... "SSS"): X_S, X_F select the mode (DD -> MPR_DP, SD -> MPR_SP,
+ * DS -> MPR_DS_INTRINSIC, SS -> MPR_SP_INTRINSIC), X_E = S makes the energy variable a float
+ * (mpr_set_energy_precision): every bond term and every partial sum of the energy reduction is then rounded to float. */
+typedef enum { MPR_DP = 0, MPR_SP = 1, MPR_SP_PRECISE = 2, MPR_SP_INTRINSIC = 3, MPR_DS_INTRINSIC = 4 } mpr_precision;
 
 /* Kernel paths.  All give bit-identical spin states (determinism contract).
  *   MPR_PATH_AUTO    (default) the path measured fastest for the mode, grid size and schedule: STRIP for
@@ -122,6 +127,10 @@ int mpr_set_stream(mpr_ctx* ctx, void* cuda_stream);
 
 /* Re-encodes the spins for `mode` and resets the chain (trial 0).                          */
 int mpr_set_precision(mpr_ctx* ctx, mpr_precision mode);
+/* The paper's (X_S X_E X_F) setting as three letters, e.g. "SDS"; see mpr_precision.  Resets the chain. */
+int mpr_set_precision_triple(mpr_ctx* ctx, const char* xs_xe_xf);
+/* X_E alone: 0 = energy sums in double (default, R13), 1 = float energy variable.  Does not touch the chain. */
+int mpr_set_energy_precision(mpr_ctx* ctx, int single);
 /* Philox key (R9).  Resets the chain.                                                      */
 int mpr_set_seed(mpr_ctx* ctx, uint64_t seed);
 /* Reduced temperature T > 0, bypassing the estimate.  Does not touch the chain.            */

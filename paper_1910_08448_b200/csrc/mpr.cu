@@ -47,6 +47,7 @@ Layout make_layout(int L) {
   lo.g.Wb = lo.g.Wm + kBitPadLeft + kBitPadRight;
   lo.g.Hb = L + kBitPadTop + kBitPadBot;
   lo.g.plane = static_cast<size_t>(L) * lo.g.Wp;
+  lo.g.energy_single = 0;
   size_t o = 0;
   const size_t state_bytes = 2 * lo.g.plane * sizeof(double2);
   lo.off_state[0] = o; o = align_up(o + state_bytes, 256);
@@ -221,7 +222,7 @@ template <int MODE> int plain_energy(mpr_ctx* c, double* d_out, bool as_e) {
   plain_energy_kernel<MODE><<<nblk, 256, 0, c->stream>>>(static_cast<const V*>(c->state(c->cur)), g, c->part());
   LAUNCH_OK(c);
   const double nb = 2.0 * g.L * (g.L - 1.0);
-  final_sum_kernel<<<1, 1024, 0, c->stream>>>(c->part(), nblk, as_e ? -kJ * 2.0 / nb : -kJ, d_out);
+  final_sum_kernel<<<1, 1024, 0, c->stream>>>(c->part(), nblk, as_e ? -kJ * 2.0 / nb : -kJ, d_out, g.energy_single);
   LAUNCH_OK(c);
   return MPR_OK;
 }
@@ -268,7 +269,7 @@ template <int MODE> int tiled_sweeps(mpr_ctx* c, int k, int measure, double* d_e
   c->cur = 1 - c->cur;
   if (measure == 1 || measure == 2) {
     const double nb = 2.0 * g.L * (g.L - 1.0);
-    final_sum_kernel<<<1, 1024, 0, c->stream>>>(c->part(), ntiles, -kJ * 2.0 / nb, d_e);
+    final_sum_kernel<<<1, 1024, 0, c->stream>>>(c->part(), ntiles, -kJ * 2.0 / nb, d_e, g.energy_single);
     LAUNCH_OK(c);
   }
   return MPR_OK;
@@ -284,13 +285,14 @@ template <int MODE> int strip_sweeps(mpr_ctx* c, int prog, int k, int measure, d
   StripArgs a{&c->strip, &c->tiled, g, c->cur, c->state(c->cur), c->state(1 - c->cur), {c->smask(1), c->smask(2)}, c->acc(), c->part(),
               c->slots(), &kc, static_cast<uint32_t>(c->sweep + 1), prog, k, measure, c->stream, &nblocks, kPartials};
   const int st = MODE == MODE_DP ? strip_launch_mode0(a) : MODE == MODE_SP ? strip_launch_mode1(a)
-                 : MODE == MODE_SP_PRECISE ? strip_launch_mode2(a) : strip_launch_mode3(a);
+                 : MODE == MODE_SP_PRECISE ? strip_launch_mode2(a) : MODE == MODE_DS ? strip_launch_mode4(a)
+                                           : strip_launch_mode3(a);
   if (st != 0) return fail(c, MPR_ERR_CUDA, std::string("strip launch: ") + tiled_error(st));
   c->launches += 1;
   c->cur = 1 - c->cur;
   if (measure == 1 || measure == 2) {
     const double nb = 2.0 * g.L * (g.L - 1.0);
-    final_sum_kernel<<<1, 1024, 0, c->stream>>>(c->part(), nblocks, -kJ * 2.0 / nb, d_e);
+    final_sum_kernel<<<1, 1024, 0, c->stream>>>(c->part(), nblocks, -kJ * 2.0 / nb, d_e, g.energy_single);
     LAUNCH_OK(c);
   }
   return MPR_OK;
@@ -307,6 +309,7 @@ int do_pass(mpr_ctx* c, int kind, int col, uint64_t sweep) {
     case MPR_DP: return plain_pass<MODE_DP>(c, kind, col, sweep);
     case MPR_SP: return plain_pass<MODE_SP>(c, kind, col, sweep);
     case MPR_SP_PRECISE: return plain_pass<MODE_SP_PRECISE>(c, kind, col, sweep);
+    case MPR_DS_INTRINSIC: return plain_pass<MODE_DS>(c, kind, col, sweep);
     default: return plain_pass<MODE_SP_INTRINSIC>(c, kind, col, sweep);
   }
 }
@@ -315,6 +318,7 @@ int do_init(mpr_ctx* c) {
     case MPR_DP: return init_chain<MODE_DP>(c);
     case MPR_SP: return init_chain<MODE_SP>(c);
     case MPR_SP_PRECISE: return init_chain<MODE_SP_PRECISE>(c);
+    case MPR_DS_INTRINSIC: return init_chain<MODE_DS>(c);
     default: return init_chain<MODE_SP_INTRINSIC>(c);
   }
 }
@@ -323,6 +327,7 @@ int do_energy(mpr_ctx* c, double* d_out, bool as_e) {
     case MPR_DP: return plain_energy<MODE_DP>(c, d_out, as_e);
     case MPR_SP: return plain_energy<MODE_SP>(c, d_out, as_e);
     case MPR_SP_PRECISE: return plain_energy<MODE_SP_PRECISE>(c, d_out, as_e);
+    case MPR_DS_INTRINSIC: return plain_energy<MODE_DS>(c, d_out, as_e);
     default: return plain_energy<MODE_SP_INTRINSIC>(c, d_out, as_e);
   }
 }
@@ -331,6 +336,7 @@ int do_accumulate(mpr_ctx* c) {
     case MPR_DP: return plain_accumulate<MODE_DP>(c);
     case MPR_SP: return plain_accumulate<MODE_SP>(c);
     case MPR_SP_PRECISE: return plain_accumulate<MODE_SP_PRECISE>(c);
+    case MPR_DS_INTRINSIC: return plain_accumulate<MODE_DS>(c);
     default: return plain_accumulate<MODE_SP_INTRINSIC>(c);
   }
 }
@@ -339,6 +345,7 @@ int do_tiled(mpr_ctx* c, int k, int measure, double* d_e) {
     case MPR_DP: return tiled_sweeps<MODE_DP>(c, k, measure, d_e);
     case MPR_SP: return tiled_sweeps<MODE_SP>(c, k, measure, d_e);
     case MPR_SP_PRECISE: return tiled_sweeps<MODE_SP_PRECISE>(c, k, measure, d_e);
+    case MPR_DS_INTRINSIC: return tiled_sweeps<MODE_DS>(c, k, measure, d_e);
     default: return tiled_sweeps<MODE_SP_INTRINSIC>(c, k, measure, d_e);
   }
 }
@@ -348,6 +355,7 @@ int do_strip(mpr_ctx* c, int prog, int k, int measure, double* d_e) {
     case MPR_DP: return strip_sweeps<MODE_DP>(c, prog, k, measure, d_e);
     case MPR_SP: return strip_sweeps<MODE_SP>(c, prog, k, measure, d_e);
     case MPR_SP_PRECISE: return strip_sweeps<MODE_SP_PRECISE>(c, prog, k, measure, d_e);
+    case MPR_DS_INTRINSIC: return strip_sweeps<MODE_DS>(c, prog, k, measure, d_e);
     default: return strip_sweeps<MODE_SP_INTRINSIC>(c, prog, k, measure, d_e);
   }
 }
@@ -618,10 +626,24 @@ void mpr_destroy(mpr_ctx* ctx) {
 }
 
 int mpr_set_precision(mpr_ctx* c, mpr_precision mode) {
-  if (!c || mode < MPR_DP || mode > MPR_SP_INTRINSIC) return fail(c, MPR_ERR_INVALID_ARG, "bad mode");
+  if (!c || mode < MPR_DP || mode > MPR_DS_INTRINSIC) return fail(c, MPR_ERR_INVALID_ARG, "bad mode");
   c->mode = mode;
   mark_stale(c);
   return MPR_OK;
+}
+int mpr_set_energy_precision(mpr_ctx* c, int single) {
+  if (!c || (single != 0 && single != 1)) return fail(c, MPR_ERR_INVALID_ARG, "energy precision: 0 (double) or 1 (single)");
+  c->lo.g.energy_single = single;     // only the measuring arithmetic changes: the chain is left alone
+  return MPR_OK;
+}
+int mpr_set_precision_triple(mpr_ctx* c, const char* xs_xe_xf) {
+  if (!c || !xs_xe_xf || std::strlen(xs_xe_xf) != 3) return fail(c, MPR_ERR_INVALID_ARG, "triple: three letters, D or S");
+  for (int i = 0; i < 3; ++i)
+    if (xs_xe_xf[i] != 'D' && xs_xe_xf[i] != 'S') return fail(c, MPR_ERR_INVALID_ARG, "triple: three letters, D or S");
+  const bool s_single = xs_xe_xf[0] == 'S', e_single = xs_xe_xf[1] == 'S', f_single = xs_xe_xf[2] == 'S';
+  const mpr_precision mode = f_single ? (s_single ? MPR_SP_INTRINSIC : MPR_DS_INTRINSIC) : (s_single ? MPR_SP : MPR_DP);
+  TRY(mpr_set_precision(c, mode));
+  return mpr_set_energy_precision(c, e_single ? 1 : 0);
 }
 int mpr_set_seed(mpr_ctx* c, uint64_t seed) {
   if (!c) return MPR_ERR_INVALID_ARG;
@@ -752,6 +774,7 @@ int mpr_get_state(mpr_ctx* c, double* d_phi) {
     case MPR_DP: return get_state<MODE_DP>(c, d_phi);
     case MPR_SP: return get_state<MODE_SP>(c, d_phi);
     case MPR_SP_PRECISE: return get_state<MODE_SP_PRECISE>(c, d_phi);
+    case MPR_DS_INTRINSIC: return get_state<MODE_DS>(c, d_phi);
     default: return get_state<MODE_SP_INTRINSIC>(c, d_phi);
   }
 }
@@ -762,6 +785,7 @@ int mpr_set_state(mpr_ctx* c, const double* d_phi) {
     case MPR_DP: return set_state<MODE_DP>(c, d_phi);
     case MPR_SP: return set_state<MODE_SP>(c, d_phi);
     case MPR_SP_PRECISE: return set_state<MODE_SP_PRECISE>(c, d_phi);
+    case MPR_DS_INTRINSIC: return set_state<MODE_DS>(c, d_phi);
     default: return set_state<MODE_SP_INTRINSIC>(c, d_phi);
   }
 }
@@ -775,7 +799,8 @@ int mpr_energy(mpr_ctx* c, double* H, double* e) {
   CUDA_OK(c, cudaStreamSynchronize(c->stream));
   const double nb = 2.0 * c->lo.g.L * (c->lo.g.L - 1.0);
   if (H) *H = h;
-  if (e) *e = 2.0 * h / nb;
+  if (e) *e = c->lo.g.energy_single ? static_cast<double>(2.0f * static_cast<float>(h) / static_cast<float>(nb))
+                                    : 2.0 * h / nb;
   return MPR_OK;
 }
 

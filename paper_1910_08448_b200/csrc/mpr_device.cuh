@@ -20,7 +20,7 @@
 
 namespace mpr {
 
-enum { MODE_DP = 0, MODE_SP = 1, MODE_SP_PRECISE = 2, MODE_SP_INTRINSIC = 3 };
+enum { MODE_DP = 0, MODE_SP = 1, MODE_SP_PRECISE = 2, MODE_SP_INTRINSIC = 3, MODE_DS = 4 };   // DS: double storage, float intrinsics (paper D.S)
 enum { PASS_INIT = 0, PASS_MET = 1 };  // Philox counter word 2 (R9)
 enum { KIND_MET = 0, KIND_OR = 1, KIND_QUENCH = 2, KIND_MO = 3 };   // MO: Metropolis then over-relaxation in one visit (R4b)
 
@@ -29,6 +29,7 @@ template <> struct Traits<MODE_DP>           { using real = double; using vec = 
 template <> struct Traits<MODE_SP>           { using real = double; using vec = float2;  };
 template <> struct Traits<MODE_SP_PRECISE>   { using real = float;  using vec = float2;  };
 template <> struct Traits<MODE_SP_INTRINSIC> { using real = float;  using vec = float2;  };
+template <> struct Traits<MODE_DS>           { using real = float;  using vec = double2; };
 
 // ---- Philox4x32-10 (Salmon et al., SC'11), restated.  counter (c0..c3), key (k0, k1).
 // R9: counter = (site, sweep, pass, trial), key = (seed lo, seed hi).
@@ -194,6 +195,9 @@ template <> struct Fn<MODE_SP_INTRINSIC> {
     return x < 0.0f ? 3.1415926535897931f - t : t;
   }
 };
+
+template <> struct Fn<MODE_DS> : Fn<MODE_SP_INTRINSIC> {};
+template <int MODE> struct IsIntrinsic { static constexpr bool value = MODE == MODE_SP_INTRINSIC || MODE == MODE_DS; };
 
 __device__ __forceinline__ double fma_(double a, double b, double c) { return fma(a, b, c); }
 __device__ __forceinline__ float fma_(float a, float b, float c) { return fmaf(a, b, c); }
@@ -377,7 +381,7 @@ __device__ __forceinline__ void met_update2(Two<typename Traits<MODE>::real> c, 
     un2(mul2(mdE, bc2(k.inv_T)), &xa, &xb);
     acc_a = R(u53(wa.a, wa.b)) < Fn<MODE>::exp_(xa);
     acc_b = R(u53(wb.a, wb.b)) < Fn<MODE>::exp_(xb);
-  } else if constexpr (MODE == MODE_SP_INTRINSIC) {
+  } else if constexpr (IsIntrinsic<MODE>::value) {
     R xa, xb;                                    // exp(-dE/T) 2^20 = ex2(-dE xscale + 20): one FFMA2 + 2 MUFU.EX2
     un2(fma2(mdE, bc2(k.xscale), bc2(R(20))), &xa, &xb);
     acc_a = acc_word(wa.a) < Fn<MODE>::ex2_(xa);

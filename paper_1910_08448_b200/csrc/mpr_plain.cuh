@@ -19,6 +19,7 @@ struct Geom {
   int L, Wp, Wm;
   int Wb, Hb;            // padded bitmap: words per row, rows per colour
   size_t plane;          // elements per colour plane = L * Wp
+  int energy_single;     // X_E of PAPER.md:35: 0 = energy sums in double (R13), 1 = the energy variable is a float
 };
 
 // The mask bitmaps are padded with zero words (kBitPadTop rows above, kBitPadBot below, kBitPadLeft
@@ -50,32 +51,41 @@ template <typename V> __device__ __forceinline__ void st_spin(V* base, long long
 }
 
 // ---- block reduction helpers (deterministic order) -------------------------------------
-__device__ __forceinline__ double warp_sum(double v) {
+// X_E = S ("the system specific energy ... as 32-bit single precision"): with `single` every partial
+// sum of the energy reduction is rounded to float, at every level -- thread, warp, block, grid.  energy_add is the
+// per-thread step; the running value is kept in a double variable that then only ever holds floats.
+__device__ __forceinline__ double sum_step(double a, double b, int single) {
+  return single ? static_cast<double>(static_cast<float>(a) + static_cast<float>(b)) : a + b;
+}
+__device__ __forceinline__ void energy_add(double& sum, double term, int single) { sum = sum_step(sum, term, single); }
+__device__ __forceinline__ double warp_sum(double v, int single = 0) {
 #pragma unroll
-  for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+  for (int o = 16; o > 0; o >>= 1) v = sum_step(v, __shfl_down_sync(0xffffffffu, v, o), single);
   return v;
 }
-__device__ __forceinline__ double block_sum(double v, double* sh /* >= 32 */) {
+__device__ __forceinline__ double block_sum(double v, double* sh /* >= 32 */, int single = 0) {
   const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, nw = (blockDim.x + 31) >> 5;
-  v = warp_sum(v);
+  v = warp_sum(v, single);
   __syncthreads();
   if (lane == 0) sh[w] = v;
   __syncthreads();
   double r = 0.0;
   if (w == 0) {
     r = lane < nw ? sh[lane] : 0.0;
-    r = warp_sum(r);
+    r = warp_sum(r, single);
   }
   return r;  // valid in thread 0
 }
 
 // out[0] = scale * sum(partials[0..n)), fixed order; one block.
-static __global__ void final_sum_kernel(const double* __restrict__ partials, int n, double scale, double* out) {
+static __global__ void final_sum_kernel(const double* __restrict__ partials, int n, double scale, double* out,
+                                        int single = 0) {
   __shared__ double sh[32];
   double v = 0.0;
-  for (int i = threadIdx.x; i < n; i += blockDim.x) v += partials[i];
-  v = block_sum(v, sh);
-  if (threadIdx.x == 0) out[0] = scale * v;
+  for (int i = threadIdx.x; i < n; i += blockDim.x) v = sum_step(v, partials[i], single);
+  v = block_sum(v, sh, single);
+  if (threadIdx.x == 0)
+    out[0] = single ? static_cast<double>(static_cast<float>(scale) * static_cast<float>(v)) : scale * v;
 }
 
 // ---- set-up ---------------------------------------------------------------------------------
@@ -201,8 +211,12 @@ __global__ void init_chain_kernel(const double* __restrict__ z, const uint8_t* _
     double sn, cs;
     sincos(0.5 * phi, &sn, &cs);
     if (sn < 0.0) sn = 0.0;
-    v.x = static_cast<decltype(v.x)>(cs);
-    v.y = static_cast<decltype(v.y)>(sn);
+    // through the arithmetic type of the mode first: with double storage and float arithmetic (MODE_DS) a stored spin
+    // must be a value the arithmetic can hand back unchanged, or the tiled kernels (which rewrite every site, moved or
+    // not) would round the measured spins on their first pass
+    using R = typename Traits<MODE>::real;
+    v.x = static_cast<decltype(v.x)>(static_cast<R>(cs));
+    v.y = static_cast<decltype(v.y)>(static_cast<R>(sn));
   }
   st_spin(state, static_cast<long long>(col) * g.plane + static_cast<long long>(y) * g.Wp + j, v);
 }
@@ -224,8 +238,9 @@ __global__ void set_state_kernel(const double* __restrict__ phi, Geom g, const u
   sincos(0.5 * p, &sn, &cs);
   if (sn < 0.0) { sn = 0.0; cs = cs < 0.0 ? -1.0 : 1.0; }
   V v;
-  v.x = static_cast<decltype(v.x)>(cs);
-  v.y = static_cast<decltype(v.y)>(sn);
+  using R = typename Traits<MODE>::real;
+  v.x = static_cast<decltype(v.x)>(static_cast<R>(cs));
+  v.y = static_cast<decltype(v.y)>(static_cast<R>(sn));
   st_spin(state, static_cast<long long>(col) * g.plane + static_cast<long long>(y) * g.Wp + j, v);
 }
 
@@ -329,10 +344,11 @@ plain_energy_kernel(const typename Traits<MODE>::vec* __restrict__ state, Geom g
       const V u = hu ? ld_spin(oth, j - g.Wp) : zero;
       const V d = hd ? ld_spin(oth, j + g.Wp) : zero;
       const V me = ld_spin(own, j);
-      sum += site_energy_term<R>(R(me.x), R(me.y), R(l.x), R(l.y), R(r.x), R(r.y), R(u.x), R(u.y), R(d.x), R(d.y));
+      energy_add(sum, site_energy_term<R>(R(me.x), R(me.y), R(l.x), R(l.y), R(r.x), R(r.y), R(u.x), R(u.y), R(d.x), R(d.y)),
+                 g.energy_single);
     }
   }
-  const double s = block_sum(sum, sh);
+  const double s = block_sum(sum, sh, g.energy_single);
   if (threadIdx.x == 0) part[blockIdx.x] = s;
 }
 

@@ -347,18 +347,18 @@ strip_kernel(const __grid_constant__ CUtensorMap tmap, typename Traits<MODE>::ve
                   if constexpr (sizeof(R) == 8) {
                     R Aa, Ab, Ba, Bb;
                     un2(A[p], &Aa, &Ab); un2(B[p], &Ba, &Bb);
-                    esum += static_cast<double>(fma_(R(out.ca), Aa, R(out.sa) * Ba));
-                    esum += static_cast<double>(fma_(R(out.cb), Ab, R(out.sb) * Bb));
+                    energy_add(esum, static_cast<double>(fma_(R(out.ca), Aa, R(out.sa) * Ba)), g.energy_single);
+                    energy_add(esum, static_cast<double>(fma_(R(out.cb), Ab, R(out.sb) * Bb)), g.energy_single);
                   } else {
                     const int par = (u + col) & 1;
                     const R alc = par ? R(nb_m.ca) : R(exc_last), als = par ? R(nb_m.sa) : R(exs_last);
                     const R arc = par ? R(nb_m.cb) : R(nb_m.ca), ars = par ? R(nb_m.sb) : R(nb_m.sa);
                     const R blc = par ? R(nb_m.cb) : R(nb_m.ca), bls = par ? R(nb_m.sb) : R(nb_m.sa);
                     const R brc = par ? R(exc_last) : R(nb_m.cb), brs = par ? R(exs_last) : R(nb_m.sb);
-                    esum += site_energy_term<R>(R(out.ca), R(out.sa), alc, als, arc, ars, R(nb_u.ca), R(nb_u.sa),
-                                                R(nb_d.ca), R(nb_d.sa));
-                    esum += site_energy_term<R>(R(out.cb), R(out.sb), blc, bls, brc, brs, R(nb_u.cb), R(nb_u.sb),
-                                                R(nb_d.cb), R(nb_d.sb));
+                    energy_add(esum, site_energy_term<R>(R(out.ca), R(out.sa), alc, als, arc, ars, R(nb_u.ca), R(nb_u.sa),
+                                                         R(nb_d.ca), R(nb_d.sa)), g.energy_single);
+                    energy_add(esum, site_energy_term<R>(R(out.cb), R(out.sb), blc, bls, brc, brs, R(nb_u.cb), R(nb_u.sb),
+                                                         R(nb_d.cb), R(nb_d.sb)), g.energy_single);
                   }
                 }
               }
@@ -388,7 +388,7 @@ strip_kernel(const __grid_constant__ CUtensorMap tmap, typename Traits<MODE>::ve
     }
   }
   if constexpr (MEASURE != 0) {
-    const double e = block_sum(esum, red);
+    const double e = block_sum(esum, red, g.energy_single);
     if (threadIdx.x == 0) part[blockIdx.x] = e;
   }
   if constexpr (PROG != PROG_QUENCH) {
@@ -435,7 +435,6 @@ inline cudaError_t strip_mask_build(const uint8_t* d_mask, const Geom& g, int hl
 // ---- host side -------------------------------------------------------------------------------
 struct StripPlan {
   int sm_count = 0;
-  bool attr_set[4] = {false, false, false, false};
   // tensor maps are encoded once per (state buffer, element width): the two buffers ping-pong
   CUtensorMap map[2][2];
   void* map_src[2][2] = {{nullptr, nullptr}, {nullptr, nullptr}};
@@ -579,5 +578,6 @@ int strip_launch_mode0(const StripArgs& a);
 int strip_launch_mode1(const StripArgs& a);
 int strip_launch_mode2(const StripArgs& a);
 int strip_launch_mode3(const StripArgs& a);
+int strip_launch_mode4(const StripArgs& a);
 
 }  // namespace mpr

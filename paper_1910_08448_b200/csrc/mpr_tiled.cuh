@@ -44,6 +44,7 @@ template <> struct TileCfg<MODE_DP>           { static constexpr int TH = 48, NT
 template <> struct TileCfg<MODE_SP>           { static constexpr int TH = 96, NT = 256, UNROLL = 2; static constexpr bool PAIR_SYNC = true; };
 template <> struct TileCfg<MODE_SP_PRECISE>   { static constexpr int TH = 96, NT = 512, UNROLL = 0; static constexpr bool PAIR_SYNC = true; };
 template <> struct TileCfg<MODE_SP_INTRINSIC> { static constexpr int TH = 96, NT = 384, UNROLL = 4; static constexpr bool PAIR_SYNC = false; };
+template <> struct TileCfg<MODE_DS>           { static constexpr int TH = 48, NT = 384, UNROLL = 4; static constexpr bool PAIR_SYNC = false; };
 
 inline int tiled_max_fused() { return 4; }
 
@@ -53,7 +54,7 @@ typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t,
 
 struct TiledPlan {
   EncodeTiledFn encode = nullptr;
-  bool attr_set[4] = {false, false, false, false};
+  bool attr_set[5] = {false, false, false, false, false};
 };
 
 enum { TILED_OK = 0, TILED_NO_DRIVER = 1, TILED_ENCODE = 2, TILED_ATTR = 3, TILED_LAUNCH = 4, TILED_TOO_MANY = 5 };
@@ -395,8 +396,10 @@ tiled_sweep_kernel(const __grid_constant__ CUtensorMap tmap, typename Traits<MOD
           const R arc = par ? R(mid.cb) : R(mid.ca), ars = par ? R(mid.sb) : R(mid.sa);
           const R blc = par ? R(mid.cb) : R(mid.ca), bls = par ? R(mid.sb) : R(mid.sa);
           const R brc = par ? exc : R(mid.cb), brs = par ? exs : R(mid.sb);
-          esum += site_energy_term<R>(R(u1.ca), R(u1.sa), alc, als, arc, ars, R(up.ca), R(up.sa), R(dn.ca), R(dn.sa));
-          esum += site_energy_term<R>(R(u1.cb), R(u1.sb), blc, bls, brc, brs, R(up.cb), R(up.sb), R(dn.cb), R(dn.sb));
+          energy_add(esum, site_energy_term<R>(R(u1.ca), R(u1.sa), alc, als, arc, ars, R(up.ca), R(up.sa), R(dn.ca), R(dn.sa)),
+                     g.energy_single);
+          energy_add(esum, site_energy_term<R>(R(u1.cb), R(u1.sb), blc, bls, brc, brs, R(up.cb), R(up.sb), R(dn.cb), R(dn.sb)),
+                     g.energy_single);
         }
         if constexpr (MEASURE == 2) {
 #pragma unroll
@@ -416,7 +419,7 @@ tiled_sweep_kernel(const __grid_constant__ CUtensorMap tmap, typename Traits<MOD
     }
   }
   if constexpr (MEASURE == 1 || MEASURE == 2) {
-    const double e = block_sum(esum, red);
+    const double e = block_sum(esum, red, g.energy_single);
     if (threadIdx.x == 0) part[blockIdx.x] = e;
   }
   const double a = block_sum(static_cast<double>(n_acc), red);

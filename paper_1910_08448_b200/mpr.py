@@ -18,7 +18,8 @@ MPR_OK = 0
 ERR_INVALID_ARG, ERR_NO_MEASURED, ERR_DEGENERATE_RANGE, ERR_NONFINITE = -1, -2, -3, -4
 ERR_WORKSPACE, ERR_NOT_READY, ERR_NO_ROOT, ERR_CUDA = -5, -6, -7, -8
 
-MODES = {"DP": 0, "SP": 1, "SP_PRECISE": 2, "SP_INTRINSIC": 3}
+MODES = {"DP": 0, "SP": 1, "SP_PRECISE": 2, "SP_INTRINSIC": 3, "DS_INTRINSIC": 4}
+TRIPLES = ("DDD", "DSD", "DDS", "SDD", "SDS", "DSS", "SSD", "SSS")      # PAPER.md:35, in Fig. 2's order after DDD
 PATHS = {"TILED": 0, "PLAIN": 1, "STRIP": 2, "AUTO": 3}
 SCHEDULES = {"R4": 0, "SITE_FUSED": 1}
 PASS_KINDS = {"MET": 0, "OR": 1, "QUENCH": 2, "MO": 3}
@@ -26,7 +27,8 @@ PASS_KINDS = {"MET": 0, "OR": 1, "QUENCH": 2, "MO": 3}
 # every symbol include/mpr.h declares
 SYMBOLS = [
     "mpr_workspace_bytes", "mpr_create", "mpr_destroy", "mpr_set_workspace", "mpr_set_stream",
-    "mpr_debug_series_stats", "mpr_debug_match_temperature", "mpr_debug_proposal_width", "mpr_set_precision", "mpr_set_seed",
+    "mpr_debug_series_stats", "mpr_debug_match_temperature", "mpr_debug_proposal_width", "mpr_set_precision",
+    "mpr_set_precision_triple", "mpr_set_energy_precision", "mpr_set_seed",
     "mpr_set_temperature", "mpr_set_quench", "mpr_set_path", "mpr_set_fused_sweeps", "mpr_set_schedule", "mpr_reset_chain",
     "mpr_estimate_temperature", "mpr_run", "mpr_sweep", "mpr_pass", "mpr_get_state", "mpr_set_state",
     "mpr_energy", "mpr_sample_energy", "mpr_get_counters", "mpr_get_run_timing", "mpr_get_energy_series",
@@ -75,6 +77,8 @@ def lib():
         "mpr_debug_series_stats": (C.c_int, [dp, i64, dp, dp]),
         "mpr_debug_match_temperature": (C.c_int, [C.c_double, TRIAL_FN, vp, dp, C.POINTER(C.c_int)]),
         "mpr_set_precision": (C.c_int, [vp, C.c_int]),
+        "mpr_set_precision_triple": (C.c_int, [vp, C.c_char_p]),
+        "mpr_set_energy_precision": (C.c_int, [vp, C.c_int]),
         "mpr_set_seed": (C.c_int, [vp, C.c_uint64]),
         "mpr_set_temperature": (C.c_int, [vp, C.c_double]),
         "mpr_set_quench": (C.c_int, [vp, C.c_int]),
@@ -190,6 +194,12 @@ class Mpr:
 
     def set_precision(self, mode):
         self._call(lib().mpr_set_precision, MODES[mode] if isinstance(mode, str) else int(mode))
+
+    def set_precision_triple(self, triple):
+        self._call(lib().mpr_set_precision_triple, triple.encode())
+
+    def set_energy_precision(self, single):
+        self._call(lib().mpr_set_energy_precision, 1 if single else 0)
 
     def set_seed(self, seed):
         self._call(lib().mpr_set_seed, int(seed))

@@ -196,7 +196,7 @@ NB4 = {(-1, 0): 1.3, (1, 0): 2.9, (0, -1): 0.4, (0, 1): 4.1}
 
 @pytest.mark.parametrize("T", [0.01, 0.1, 1.0])
 @pytest.mark.parametrize("path", ["TILED", "STRIP"])
-@pytest.mark.parametrize("mode", ["SP_PRECISE", "SP_INTRINSIC", "SP", "DP"])
+@pytest.mark.parametrize("mode", ["SP_PRECISE", "SP_INTRINSIC", "DS_INTRINSIC", "SP", "DP"])
 def test_interior_sites_sample_the_exact_conditional_density(mpr, mode, path, T):
     """39204 isolated free sites, each with the same four measured neighbours; after 60 hybrid sweeps, 26
     snapshots 6 sweeps apart: ~10^6 samples, chi^2 with 39 degrees of freedom against the exact density.
