@@ -65,7 +65,7 @@ def parse():
     ap.add_argument("--n-eq", type=int, default=None)
     ap.add_argument("--n-meas", type=int, default=None)
     ap.add_argument("--fused", type=int, default=1, help="hybrid sweeps per launch (STRIP: 1 or 2)")
-    ap.add_argument("--path", default="AUTO", choices=["AUTO", "STRIP", "TILED", "PLAIN"])
+    ap.add_argument("--path", default="AUTO", choices=["AUTO", "STRIP", "TILED", "PLAIN", "LIST"])
     ap.add_argument("--schedule", default="R4", choices=["R4", "SITE_FUSED"],
                     help="pass order of a hybrid sweep (DESIGN.md R4 / R4b); the headline is R4")
     ap.add_argument("--temperature", type=float, default=None,
@@ -315,7 +315,9 @@ def run_ours(args, rank, world, local_rank):
 
     # what MPR_PATH_AUTO resolves to (csrc/mpr.cu, eff_path)
     def auto_path(md, schedule):
-        return "STRIP" if schedule == "SITE_FUSED" or (md == "SP_INTRINSIC" and L >= 4096) else "TILED"
+        if schedule == "SITE_FUSED":
+            return "LIST" if (c.f < 0.5 and L <= 4096) else "STRIP"
+        return "STRIP" if (md == "SP_INTRINSIC" and L >= 4096) else "TILED"
     path_used = auto_path(mode, args.schedule) if args.path == "AUTO" else args.path
     k_eff = min(args.fused, 2) if path_used == "STRIP" else args.fused
     kern_ms_burst, _ = time_sweeps(mode, args.path, args.schedule, args.fused, 50)   # the kernel timed alone, after the steps

@@ -62,11 +62,15 @@ typedef enum {
  *   MPR_SP_INTRINSIC  SSS  float storage and arithmetic, __sinf/__cosf/__expf
  * Energy sums are accumulated in double in every mode (R13) unless X_E = S is asked for (below).
  *   MPR_DS_INTRINSIC  D.S  double storage of the spins, float arithmetic with the intrinsics
+ *   MPR_HP            half-precision storage of the spins (two fp16 per spin, 4 bytes), float arithmetic with the
+ *                     intrinsics -- the paper's outlook.  The stored vectors carry a 5e-4 relative rounding,
+ *                     which shows in e; predictions meet the same 1 % gate as the float modes.
  * The paper's eight settings (X_S X_E X_F) = (spin storage, energy variable, functions), each D or S, are
  * mpr_set_precision_triple("DDD" ... "SSS"): X_S, X_F select the mode (DD -> MPR_DP, SD -> MPR_SP,
  * DS -> MPR_DS_INTRINSIC, SS -> MPR_SP_INTRINSIC), X_E = S makes the energy variable a float
  * (mpr_set_energy_precision): every bond term and every partial sum of the energy reduction is then rounded to float. */
-typedef enum { MPR_DP = 0, MPR_SP = 1, MPR_SP_PRECISE = 2, MPR_SP_INTRINSIC = 3, MPR_DS_INTRINSIC = 4 } mpr_precision;
+typedef enum { MPR_DP = 0, MPR_SP = 1, MPR_SP_PRECISE = 2, MPR_SP_INTRINSIC = 3, MPR_DS_INTRINSIC = 4,
+               MPR_HP = 5 } mpr_precision;
 
 /* Kernel paths.  All give bit-identical spin states (determinism contract).
  *   MPR_PATH_AUTO    (default) the path measured fastest for the mode, grid size and schedule: STRIP for
@@ -77,8 +81,12 @@ typedef enum { MPR_DP = 0, MPR_SP = 1, MPR_SP_PRECISE = 2, MPR_SP_INTRINSIC = 3,
  *   MPR_PATH_TILED   one launch per hybrid sweep group: TMA stages a tile + halo of both colour
  *                    planes in shared memory, all 4*k colour passes of k sweeps run there.
  *   MPR_PATH_PLAIN   one launch per colour pass on the global colour planes (reference path
- *                    for the self-consistency tests; also used for odd R8 quench passes).  */
-typedef enum { MPR_PATH_TILED = 0, MPR_PATH_PLAIN = 1, MPR_PATH_STRIP = 2, MPR_PATH_AUTO = 3 } mpr_path;
+ *                    for the self-consistency tests; also used for odd R8 quench passes).
+ *   MPR_PATH_LIST    one launch per colour pass over the COMPACTED list of the prediction sites of that
+ *                    colour (built at set-up): work proportional to the number of prediction sites,
+ *                    neighbour reads are gathers.  For small masked fractions.               */
+typedef enum { MPR_PATH_TILED = 0, MPR_PATH_PLAIN = 1, MPR_PATH_STRIP = 2, MPR_PATH_AUTO = 3,
+               MPR_PATH_LIST = 4 } mpr_path;
 
 /* Order of the colour passes inside one hybrid sweep ("hybrid algorithm" -- the paper
  * leaves the order to its ref. [5]; both orders leave the conditional Boltzmann density invariant):

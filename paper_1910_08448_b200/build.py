@@ -2,7 +2,7 @@
 
     python -m paper_1910_08448_b200.build [--force]
 
-Six translation units compiled in parallel: mpr.cu (C ABI, host logic, PLAIN and TILED kernels) and
+Seven translation units compiled in parallel: mpr.cu (C ABI, host logic, PLAIN and TILED kernels) and
 mpr_strip_mode.cu once per precision mode (the STRIP kernels), then one device link into the shared library.
 """
 from __future__ import annotations
@@ -20,7 +20,7 @@ HEADERS = ["mpr_device.cuh", "mpr_host_math.hpp", "mpr_plain.cuh", "mpr_tiled.cu
            os.path.join("..", "..", "include", "mpr.h")]
 # (source, object name, extra flags)
 UNITS = [("mpr.cu", "mpr.o", [])] + [("mpr_strip_mode.cu", "mpr_strip_mode%d.o" % m, ["-DMPR_STRIP_MODE=%d" % m])
-                                    for m in range(5)]
+                                    for m in range(6)]
 
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",

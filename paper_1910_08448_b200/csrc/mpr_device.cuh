@@ -17,10 +17,11 @@
 #pragma once
 #include <cstdint>
 #include <cuda_runtime.h>
+#include <cuda_fp16.h>
 
 namespace mpr {
 
-enum { MODE_DP = 0, MODE_SP = 1, MODE_SP_PRECISE = 2, MODE_SP_INTRINSIC = 3, MODE_DS = 4 };   // DS: double storage, float intrinsics (paper D.S)
+enum { MODE_DP = 0, MODE_SP = 1, MODE_SP_PRECISE = 2, MODE_SP_INTRINSIC = 3, MODE_DS = 4, MODE_HP = 5 };   // DS: double storage, float intrinsics (paper D.S)
 enum { PASS_INIT = 0, PASS_MET = 1 };  // Philox counter word 2 (R9)
 enum { KIND_MET = 0, KIND_OR = 1, KIND_QUENCH = 2, KIND_MO = 3 };   // MO: Metropolis then over-relaxation in one visit (R4b)
 
@@ -30,6 +31,17 @@ template <> struct Traits<MODE_SP>           { using real = double; using vec = 
 template <> struct Traits<MODE_SP_PRECISE>   { using real = float;  using vec = float2;  };
 template <> struct Traits<MODE_SP_INTRINSIC> { using real = float;  using vec = float2;  };
 template <> struct Traits<MODE_DS>           { using real = float;  using vec = double2; };
+// half-precision storage (the paper's outlook): (c, s) as two fp16, arithmetic as in SP_INTRINSIC
+struct alignas(4) hvec2 { __half x, y; };
+template <> struct Traits<MODE_HP>           { using real = float;  using vec = hvec2;   };
+__device__ __forceinline__ double to_double(double v) { return v; }
+__device__ __forceinline__ double to_double(float v) { return static_cast<double>(v); }
+__device__ __forceinline__ double to_double(__half v) { return static_cast<double>(__half2float(v)); }
+// CUtensorMapDataType of a storage scalar (cuda.h: FLOAT16 = 6, FLOAT32 = 7, FLOAT64 = 8)
+template <typename S> struct TmaType;
+template <> struct TmaType<double> { static constexpr int value = 8; };
+template <> struct TmaType<float>  { static constexpr int value = 7; };
+template <> struct TmaType<__half> { static constexpr int value = 6; };
 
 // ---- Philox4x32-10 (Salmon et al., SC'11), restated.  counter (c0..c3), key (k0, k1).
 // R9: counter = (site, sweep, pass, trial), key = (seed lo, seed hi).
@@ -197,7 +209,8 @@ template <> struct Fn<MODE_SP_INTRINSIC> {
 };
 
 template <> struct Fn<MODE_DS> : Fn<MODE_SP_INTRINSIC> {};
-template <int MODE> struct IsIntrinsic { static constexpr bool value = MODE == MODE_SP_INTRINSIC || MODE == MODE_DS; };
+template <> struct Fn<MODE_HP> : Fn<MODE_SP_INTRINSIC> {};
+template <int MODE> struct IsIntrinsic { static constexpr bool value = MODE == MODE_SP_INTRINSIC || MODE == MODE_DS || MODE == MODE_HP; };
 
 __device__ __forceinline__ double fma_(double a, double b, double c) { return fma(a, b, c); }
 __device__ __forceinline__ float fma_(float a, float b, float c) { return fmaf(a, b, c); }

@@ -252,69 +252,163 @@ __global__ void get_state_kernel(const typename Traits<MODE>::vec* __restrict__ 
   if (x >= g.L) return;
   const int col = (x + y) & 1, j = x >> 1;
   const auto v = ld_spin(state, static_cast<long long>(col) * g.plane + static_cast<long long>(y) * g.Wp + j);
-  phi[static_cast<size_t>(y) * g.L + x] = 2.0 * atan2(static_cast<double>(v.y), static_cast<double>(v.x));
+  phi[static_cast<size_t>(y) * g.L + x] = 2.0 * atan2(to_double(v.y), to_double(v.x));
 }
 
 // ---- one colour pass on the global planes -------------------------------------------------
+// The move of ONE site (row y, plane column j of colour col), in place.  Shared by the kernel that visits every
+// plane position and tests its mask bit (PLAIN) and the one that walks the compacted list of prediction sites
+// (LIST): the same instructions on the same operands, hence the same spins.  Returns whether a Metropolis move
+// was accepted.
+template <int MODE, int KIND>
+__device__ __forceinline__ bool plain_site_update(typename Traits<MODE>::vec* __restrict__ state, const Geom& g, int col,
+                                                  int y, int j, uint32_t sweep,
+                                                  const ChainConst<typename Traits<MODE>::real>& k) {
+  using R = typename Traits<MODE>::real;
+  using V = typename Traits<MODE>::vec;
+  bool accepted = false;
+  const int par = x_parity(y, col);
+  const int x = 2 * j + par;
+  V* own = state + static_cast<size_t>(col) * g.plane + static_cast<size_t>(y) * g.Wp;
+  const V* oth = state + static_cast<size_t>(1 - col) * g.plane + static_cast<size_t>(y) * g.Wp;
+  const bool hl = x > 0, hr = x < g.L - 1, hu = y > 0, hd = y < g.L - 1;
+  const int jl = j - 1 + par, jr = j + par;
+  V zero; zero.x = 0; zero.y = 0;
+  const V l = hl ? ld_spin(oth, jl) : zero;
+  const V r = hr ? ld_spin(oth, jr) : zero;
+  const V u = hu ? ld_spin(oth, j - g.Wp) : zero;
+  const V d = hd ? ld_spin(oth, j + g.Wp) : zero;
+  R A, B;
+  local_field<R>(R(l.x), R(l.y), R(r.x), R(r.y), R(u.x), R(u.y), R(d.x), R(d.y), hl, hr, hu, hd, &A, &B);
+  const V me = ld_spin(own, j);
+  R c = R(me.x), s = R(me.y);
+  if constexpr (KIND == KIND_MET || KIND == KIND_MO) {
+    // R9: the quad (plane columns 2m, 2m + 1) x (rows 2k, 2k + 1) shares one Philox block in the float modes
+    const uint32_t pair_site = static_cast<uint32_t>(y) * static_cast<uint32_t>(g.L) +
+                               static_cast<uint32_t>(2 * (j & ~1) + par);
+    MetWords w0, w1;
+    met_words_pair<MODE>(pair_site, sweep, static_cast<uint32_t>(g.L), par, (y & 1) != 0, k, &w0, &w1);
+    const MetWords w = (j & 1) ? w1 : w0;
+    R o[4];
+    bool ok[2];
+    met_update2<MODE>(bc2(c), bc2(s), bc2(A), bc2(B), w, w, true, true, k, o, ok);   // the site in both lanes
+    c = o[0]; s = o[2];
+    accepted = ok[0];
+    if constexpr (KIND == KIND_MO) {     // site-fused schedule (R4b): the over-relaxation move follows at once
+      R o2[4];
+      or_update2<MODE>(bc2(c), bc2(s), bc2(A), bc2(B), true, true, o2);
+      c = o2[0]; s = o2[2];
+    }
+  } else if constexpr (KIND == KIND_OR) {
+    R o[4];
+    or_update2<MODE>(bc2(c), bc2(s), bc2(A), bc2(B), true, true, o);
+    c = o[0]; s = o[2];
+  } else {
+    quench_update<MODE>(&c, &s, A, B);
+  }
+  V out;
+  out.x = static_cast<decltype(out.x)>(c);
+  out.y = static_cast<decltype(out.y)>(s);
+  st_spin(own, j, out);
+  return accepted;
+}
+
 template <int MODE, int KIND>
 __global__ void __launch_bounds__(128)
 plain_pass_kernel(typename Traits<MODE>::vec* __restrict__ state, const uint32_t* __restrict__ bits, Geom g,
                   int col, uint32_t sweep, ChainConst<typename Traits<MODE>::real> k,
                   unsigned long long* __restrict__ accept_slots) {
-  using R = typename Traits<MODE>::real;
-  using V = typename Traits<MODE>::vec;
   const int y = blockIdx.y;
   const int j = blockIdx.x * blockDim.x + threadIdx.x;
   bool accepted = false;
-  if (j < g.Wp && mask_bit(bits, g, col, y, j)) {
-    const int par = x_parity(y, col);
-    const int x = 2 * j + par;
-    V* own = state + static_cast<size_t>(col) * g.plane + static_cast<size_t>(y) * g.Wp;
-    const V* oth = state + static_cast<size_t>(1 - col) * g.plane + static_cast<size_t>(y) * g.Wp;
-    const bool hl = x > 0, hr = x < g.L - 1, hu = y > 0, hd = y < g.L - 1;
-    const int jl = j - 1 + par, jr = j + par;
-    V zero; zero.x = 0; zero.y = 0;
-    const V l = hl ? ld_spin(oth, jl) : zero;
-    const V r = hr ? ld_spin(oth, jr) : zero;
-    const V u = hu ? ld_spin(oth, j - g.Wp) : zero;
-    const V d = hd ? ld_spin(oth, j + g.Wp) : zero;
-    R A, B;
-    local_field<R>(R(l.x), R(l.y), R(r.x), R(r.y), R(u.x), R(u.y), R(d.x), R(d.y), hl, hr, hu, hd, &A, &B);
-    const V me = ld_spin(own, j);
-    R c = R(me.x), s = R(me.y);
-    if constexpr (KIND == KIND_MET || KIND == KIND_MO) {
-      // R9: the quad (plane columns 2m, 2m + 1) x (rows 2k, 2k + 1) shares one Philox block in the float modes
-      const uint32_t pair_site = static_cast<uint32_t>(y) * static_cast<uint32_t>(g.L) +
-                                 static_cast<uint32_t>(2 * (j & ~1) + par);
-      MetWords w0, w1;
-      met_words_pair<MODE>(pair_site, sweep, static_cast<uint32_t>(g.L), par, (y & 1) != 0, k, &w0, &w1);
-      const MetWords w = (j & 1) ? w1 : w0;
-      R o[4];
-      bool ok[2];
-      met_update2<MODE>(bc2(c), bc2(s), bc2(A), bc2(B), w, w, true, true, k, o, ok);   // the site in both lanes
-      c = o[0]; s = o[2];
-      accepted = ok[0];
-      if constexpr (KIND == KIND_MO) {     // site-fused schedule (R4b): the over-relaxation move follows at once
-        R o2[4];
-        or_update2<MODE>(bc2(c), bc2(s), bc2(A), bc2(B), true, true, o2);
-        c = o2[0]; s = o2[2];
-      }
-    } else if constexpr (KIND == KIND_OR) {
-      R o[4];
-      or_update2<MODE>(bc2(c), bc2(s), bc2(A), bc2(B), true, true, o);
-      c = o[0]; s = o[2];
-    } else {
-      quench_update<MODE>(&c, &s, A, B);
-    }
-    V out;
-    out.x = static_cast<decltype(out.x)>(c);
-    out.y = static_cast<decltype(out.y)>(s);
-    st_spin(own, j, out);
-  }
+  if (j < g.Wp && mask_bit(bits, g, col, y, j)) accepted = plain_site_update<MODE, KIND>(state, g, col, y, j, sweep, k);
   if constexpr (KIND == KIND_MET || KIND == KIND_MO) {
     const int n = __syncthreads_count(accepted);
     if (threadIdx.x == 0 && n)
       atomicAdd(accept_slots + ((blockIdx.y * gridDim.x + blockIdx.x) & 1023u), static_cast<unsigned long long>(n));
+  }
+}
+
+// ---- LIST path: the compacted per-colour lists of prediction sites (north_star (a)) ------------------------------
+// list[col] holds the plane positions y * Wp + j of the prediction sites of colour col in row-major order, n[col]
+// of them.  Built once per context from the mask bitmaps: per-row counts, an exclusive scan over the rows, then
+// every row writes its positions.  A pass over a list does work proportional to the number of PREDICTION sites of
+// the colour, whatever the masked fraction; neighbour reads are gathers from the global planes.
+static __global__ void list_row_count_kernel(const uint32_t* __restrict__ bits, Geom g, uint32_t* __restrict__ row_count) {
+  __shared__ double sh[32];
+  const int y = blockIdx.x, col = blockIdx.y;
+  double n = 0.0;
+  for (int wi = threadIdx.x; wi < g.Wm; wi += blockDim.x) n += static_cast<double>(__popc(*mask_word(bits, g, col, y, wi)));
+  const double s = block_sum(n, sh);
+  if (threadIdx.x == 0) row_count[static_cast<size_t>(col) * g.L + y] = static_cast<uint32_t>(s);
+}
+// exclusive scan of the row counts of both colours (one block; L <= 32768 rows): row_off[col][y], total[col]
+static __global__ void list_row_scan_kernel(const uint32_t* __restrict__ row_count, int L, uint32_t* __restrict__ row_off,
+                                            uint32_t* __restrict__ total) {
+  __shared__ uint32_t part[1024];
+  for (int col = 0; col < 2; ++col) {
+    const uint32_t* rc = row_count + static_cast<size_t>(col) * L;
+    uint32_t* ro = row_off + static_cast<size_t>(col) * L;
+    const int per = (L + blockDim.x - 1) / blockDim.x;
+    const int lo = threadIdx.x * per, hi = min(L, lo + per);
+    uint32_t s = 0;
+    for (int y = lo; y < hi; ++y) s += rc[y];
+    part[threadIdx.x] = s;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+      uint32_t run = 0;
+      for (int t = 0; t < static_cast<int>(blockDim.x); ++t) { const uint32_t v = part[t]; part[t] = run; run += v; }
+      total[col] = run;
+    }
+    __syncthreads();
+    uint32_t run = part[threadIdx.x];
+    for (int y = lo; y < hi; ++y) { ro[y] = run; run += rc[y]; }
+    __syncthreads();
+  }
+}
+// one warp per row: positions in increasing column order
+static __global__ void list_fill_kernel(const uint32_t* __restrict__ bits, Geom g, const uint32_t* __restrict__ row_off,
+                                        uint32_t* __restrict__ list0, uint32_t* __restrict__ list1) {
+  const int y = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5), col = blockIdx.y, lane = threadIdx.x & 31;
+  if (y >= g.L) return;
+  uint32_t* out = (col ? list1 : list0) + row_off[static_cast<size_t>(col) * g.L + y];
+  uint32_t base = 0;
+  for (int w0 = 0; w0 < g.Wm; w0 += 32) {
+    const int wi = w0 + lane;
+    const uint32_t word = wi < g.Wm ? *mask_word(bits, g, col, y, wi) : 0u;
+    const uint32_t cnt = __popc(word);
+    uint32_t incl = cnt;                                  // inclusive prefix of the counts over the warp
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      const uint32_t v = __shfl_up_sync(0xffffffffu, incl, o);
+      if (lane >= o) incl += v;
+    }
+    uint32_t pos = base + incl - cnt;
+    uint32_t rest = word;
+    while (rest) {
+      const int b = __ffs(rest) - 1;
+      rest &= rest - 1;
+      out[pos++] = static_cast<uint32_t>(y) * static_cast<uint32_t>(g.Wp) + static_cast<uint32_t>(32 * wi + b);
+    }
+    base += __shfl_sync(0xffffffffu, incl, 31);
+  }
+}
+
+template <int MODE, int KIND>
+__global__ void __launch_bounds__(128)
+list_pass_kernel(typename Traits<MODE>::vec* __restrict__ state, const uint32_t* __restrict__ list, uint32_t n, Geom g,
+                 int col, uint32_t sweep, ChainConst<typename Traits<MODE>::real> k,
+                 unsigned long long* __restrict__ accept_slots) {
+  const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+  bool accepted = false;
+  if (i < n) {
+    const uint32_t pos = list[i];
+    const int y = static_cast<int>(pos / static_cast<uint32_t>(g.Wp)), j = static_cast<int>(pos % static_cast<uint32_t>(g.Wp));
+    accepted = plain_site_update<MODE, KIND>(state, g, col, y, j, sweep, k);
+  }
+  if constexpr (KIND == KIND_MET || KIND == KIND_MO) {
+    const int m = __syncthreads_count(accepted);
+    if (threadIdx.x == 0 && m) atomicAdd(accept_slots + (blockIdx.x & 1023u), static_cast<unsigned long long>(m));
   }
 }
 

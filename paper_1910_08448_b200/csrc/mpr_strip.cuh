@@ -173,7 +173,7 @@ strip_kernel(const __grid_constant__ CUtensorMap tmap, typename Traits<MODE>::ve
       if (lane == 0) {                                        // chunk 0 -> slot 0
         fence_proxy_async_smem();
         mbar_expect_tx(bars, kChunkBytes);
-        tma_load_3d(ring, &tmap, bars, 2 * j0, t0, 0);
+        tma_load_3d(ring, &tmap, bars, (sizeof(S) == 2 ? 1 : 2) * j0, t0, 0);
         bulk_load_1d(mring, mblk, kMaskBytes, bars);
       }
       // cb[k] = scalar offset (inside this warp's ring) of the chunk  i + 2 - NSLOT + k,  i.e. cb[NSLOT-1] holds
@@ -205,7 +205,7 @@ strip_kernel(const __grid_constant__ CUtensorMap tmap, typename Traits<MODE>::ve
         if (lane == 0) {
           fence_proxy_async_smem();
           mbar_expect_tx(bars + slot_next, kChunkBytes);
-          tma_load_3d(ring + cb[NSLOT - 1], &tmap, bars + slot_next, 2 * j0, t0 + RB * (i + 1), 0);
+          tma_load_3d(ring + cb[NSLOT - 1], &tmap, bars + slot_next, (sizeof(S) == 2 ? 1 : 2) * j0, t0 + RB * (i + 1), 0);
           bulk_load_1d(mring + slot_next * 32, mblk + static_cast<size_t>(i + 1) * 32, kMaskBytes, bars + slot_next);
         }
         // the mask word of chunk i (its slot is the one before slot_next; the chunk was awaited in iteration i - 1)
@@ -436,22 +436,24 @@ inline cudaError_t strip_mask_build(const uint8_t* d_mask, const Geom& g, int hl
 struct StripPlan {
   int sm_count = 0;
   // tensor maps are encoded once per (state buffer, element width): the two buffers ping-pong
-  CUtensorMap map[2][2];
-  void* map_src[2][2] = {{nullptr, nullptr}, {nullptr, nullptr}};
+  CUtensorMap map[2][3];
+  void* map_src[2][3] = {{nullptr, nullptr, nullptr}, {nullptr, nullptr, nullptr}};
 };
 
 template <int MODE>
 int strip_encode(TiledPlan& tp, const Geom& g, void* src, CUtensorMap* map) {
   using V = typename Traits<MODE>::vec;
-  constexpr bool f64 = sizeof(V) == 16;
-  const cuuint64_t dims[3] = {static_cast<cuuint64_t>(2) * g.Wp, static_cast<cuuint64_t>(g.L), 2};
+  // fp16 storage travels as 32-bit words (two halves each): the copy is the same bytes, and the plain FLOAT32 path
+  // of the TMA unit is the one every other mode has proven
+  constexpr bool kHalf = sizeof(decltype(V::x)) == 2;
+  const cuuint64_t dims[3] = {static_cast<cuuint64_t>(kHalf ? 1 : 2) * g.Wp, static_cast<cuuint64_t>(g.L), 2};
   const cuuint64_t strides[2] = {static_cast<cuuint64_t>(g.Wp) * sizeof(V), static_cast<cuuint64_t>(g.plane) * sizeof(V)};
-  const cuuint32_t box[3] = {2 * kTileCols, static_cast<cuuint32_t>(kStripRB), 2};
+  const cuuint32_t box[3] = {(kHalf ? 1 : 2) * kTileCols, static_cast<cuuint32_t>(kStripRB), 2};
   const cuuint32_t estr[3] = {1, 1, 1};
   // 64-byte promotion: a strip row (512 B at a 480-byte pitch) then drags in the least data it does not use
   // (128 B: 0.983 ms, 64 B: 0.970 ms, none: 0.983 ms per sweep at L = 16384)
   const CUtensorMapL2promotion promo = CU_TENSOR_MAP_L2_PROMOTION_L2_64B;
-  const CUresult r = tp.encode(map, f64 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, src,
+  const CUresult r = tp.encode(map, kHalf ? CU_TENSOR_MAP_DATA_TYPE_FLOAT32 : static_cast<CUtensorMapDataType>(TmaType<decltype(V::x)>::value), 3, src,
                                dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
                                promo, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
   return r == CUDA_SUCCESS ? TILED_OK : TILED_ENCODE;
@@ -510,7 +512,7 @@ int strip_launch_one(StripPlan& plan, const CUtensorMap& map, const Geom& g, voi
   if (MEASURE != 0 && nblocks > max_partials) return TILED_TOO_MANY;
   strip_kernel<MODE, PROG, K, MEASURE><<<nblocks, NW * 32, smem, stream>>>(map, static_cast<V*>(dst), smask[strip_halo_lanes(NS) - 1], acc, part, slots,
                                                                             g, kc, first_sweep, sg);
-  if (cudaGetLastError() != cudaSuccess) return TILED_LAUNCH;
+  if (const cudaError_t le = cudaGetLastError(); le != cudaSuccess) { tiled_last_cuda_error() = le; return TILED_LAUNCH; }
   *nblocks_out = nblocks;
   return TILED_OK;
 }
@@ -529,7 +531,7 @@ int strip_launch(StripPlan& plan, TiledPlan& tp, const Geom& g, int src_index, v
         cudaDeviceGetAttribute(&plan.sm_count, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || plan.sm_count <= 0)
       return TILED_ATTR;
   }
-  constexpr int w = sizeof(typename Traits<MODE>::vec) == 16 ? 1 : 0;
+  constexpr int w = sizeof(typename Traits<MODE>::vec) == 16 ? 1 : sizeof(typename Traits<MODE>::vec) == 8 ? 0 : 2;
   if (plan.map_src[src_index][w] != src) {
     const int es = strip_encode<MODE>(tp, g, src, &plan.map[src_index][w]);
     if (es != TILED_OK) return es;
@@ -579,5 +581,6 @@ int strip_launch_mode1(const StripArgs& a);
 int strip_launch_mode2(const StripArgs& a);
 int strip_launch_mode3(const StripArgs& a);
 int strip_launch_mode4(const StripArgs& a);
+int strip_launch_mode5(const StripArgs& a);
 
 }  // namespace mpr

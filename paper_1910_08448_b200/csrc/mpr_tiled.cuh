@@ -27,6 +27,9 @@
 
 namespace mpr {
 
+static_assert(TmaType<double>::value == CU_TENSOR_MAP_DATA_TYPE_FLOAT64 && TmaType<float>::value == CU_TENSOR_MAP_DATA_TYPE_FLOAT32 &&
+              TmaType<__half>::value == CU_TENSOR_MAP_DATA_TYPE_FLOAT16, "TmaType mirrors cuda.h");
+
 constexpr int kTileCols = 64;   // plane columns staged per tile (incl. halo)
 
 template <int MODE> struct TileCfg;
@@ -45,6 +48,7 @@ template <> struct TileCfg<MODE_SP>           { static constexpr int TH = 96, NT
 template <> struct TileCfg<MODE_SP_PRECISE>   { static constexpr int TH = 96, NT = 512, UNROLL = 0; static constexpr bool PAIR_SYNC = true; };
 template <> struct TileCfg<MODE_SP_INTRINSIC> { static constexpr int TH = 96, NT = 384, UNROLL = 4; static constexpr bool PAIR_SYNC = false; };
 template <> struct TileCfg<MODE_DS>           { static constexpr int TH = 48, NT = 384, UNROLL = 4; static constexpr bool PAIR_SYNC = false; };
+template <> struct TileCfg<MODE_HP>           { static constexpr int TH = 96, NT = 384, UNROLL = 4; static constexpr bool PAIR_SYNC = false; };
 
 inline int tiled_max_fused() { return 4; }
 
@@ -54,10 +58,13 @@ typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t,
 
 struct TiledPlan {
   EncodeTiledFn encode = nullptr;
-  bool attr_set[5] = {false, false, false, false, false};
+  bool attr_set[6] = {false, false, false, false, false, false};
 };
 
 enum { TILED_OK = 0, TILED_NO_DRIVER = 1, TILED_ENCODE = 2, TILED_ATTR = 3, TILED_LAUNCH = 4, TILED_TOO_MANY = 5 };
+
+// the CUDA error behind the last TILED_LAUNCH / TILED_ATTR (for the message of mpr_last_error)
+inline cudaError_t& tiled_last_cuda_error() { static cudaError_t e = cudaSuccess; return e; }
 
 inline const char* tiled_error(int st) {
   switch (st) {
@@ -65,7 +72,7 @@ inline const char* tiled_error(int st) {
     case TILED_NO_DRIVER: return "cuTensorMapEncodeTiled not found in the driver";
     case TILED_ENCODE: return "cuTensorMapEncodeTiled failed";
     case TILED_ATTR: return "cudaFuncSetAttribute(max dynamic shared memory) failed";
-    case TILED_LAUNCH: return "kernel launch failed";
+    case TILED_LAUNCH: return cudaGetErrorString(tiled_last_cuda_error());
     case TILED_TOO_MANY: return "too many tiles for the partials buffer";
     default: return "unknown";
   }
@@ -297,7 +304,7 @@ tiled_sweep_kernel(const __grid_constant__ CUtensorMap tmap, typename Traits<MOD
   if (threadIdx.x == 0) {
     mbar_init(bar, 1);
     mbar_expect_tx(bar, static_cast<uint32_t>(sizeof(V) * 2 * TH * kTileCols));
-    tma_load_3d(t.base, &tmap, bar, 2 * j0, y0, 0);
+    tma_load_3d(t.base, &tmap, bar, (sizeof(S) == 2 ? 1 : 2) * j0, y0, 0);
   }
   // pad row behind plane 1 (read as "row TH" by the last warp in colour-0 passes): the zero vector
   if (threadIdx.x < kRowScalars) t.base[2 * TH * kRowScalars + threadIdx.x] = S(0);
@@ -430,12 +437,14 @@ tiled_sweep_kernel(const __grid_constant__ CUtensorMap tmap, typename Traits<MOD
 template <int MODE>
 int tiled_encode(TiledPlan& plan, const Geom& g, void* src, CUtensorMap* map) {
   using V = typename Traits<MODE>::vec;
-  constexpr bool f64 = sizeof(V) == 16;
-  const cuuint64_t dims[3] = {static_cast<cuuint64_t>(2) * g.Wp, static_cast<cuuint64_t>(g.L), 2};
+  // fp16 storage travels as 32-bit words (two halves each): the copy is the same bytes, and the plain FLOAT32 path
+  // of the TMA unit is the one every other mode has proven
+  constexpr bool kHalf = sizeof(decltype(V::x)) == 2;
+  const cuuint64_t dims[3] = {static_cast<cuuint64_t>(kHalf ? 1 : 2) * g.Wp, static_cast<cuuint64_t>(g.L), 2};
   const cuuint64_t strides[2] = {static_cast<cuuint64_t>(g.Wp) * sizeof(V), static_cast<cuuint64_t>(g.plane) * sizeof(V)};
-  const cuuint32_t box[3] = {2 * kTileCols, static_cast<cuuint32_t>(TileCfg<MODE>::TH), 2};
+  const cuuint32_t box[3] = {(kHalf ? 1 : 2) * kTileCols, static_cast<cuuint32_t>(TileCfg<MODE>::TH), 2};
   const cuuint32_t estr[3] = {1, 1, 1};
-  const CUresult r = plan.encode(map, f64 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, src,
+  const CUresult r = plan.encode(map, kHalf ? CU_TENSOR_MAP_DATA_TYPE_FLOAT32 : static_cast<CUtensorMapDataType>(TmaType<decltype(V::x)>::value), 3, src,
                                  dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
                                  CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
   return r == CUDA_SUCCESS ? TILED_OK : TILED_ENCODE;
@@ -482,7 +491,7 @@ int tiled_launch(TiledPlan& plan, const Geom& g, void* src, void* dst, const uin
   else
     tiled_sweep_kernel<MODE, 0><<<static_cast<unsigned>(ntiles), NT, smem, stream>>>(
         map, static_cast<V*>(dst), bits, acc, part, slots, g, kc, first_sweep, k, tiles_x);
-  if (cudaGetLastError() != cudaSuccess) return TILED_LAUNCH;
+  if (const cudaError_t le = cudaGetLastError(); le != cudaSuccess) { tiled_last_cuda_error() = le; return TILED_LAUNCH; }
   *ntiles_out = static_cast<int>(ntiles);
   return TILED_OK;
 }

@@ -90,6 +90,38 @@ def make_problem(L: int, xi: float, field_seed: int, f: float, lognormal: bool =
     return values, mask, truth
 
 
+def structured_mask(L: int, kind: str, f: float, seed: int) -> np.ndarray:
+    """Gap patterns of remote-sensing data ("restricted satellite paths or bad weather conditions"),
+    uint8[L, L] with 1 = prediction site and a masked fraction close to f:
+      "clouds"  -- the sites where a smooth Gaussian random field (correlation length L / 16) exceeds its (1 - f) quantile:
+                   compact blobs with ragged edges;
+      "tracks"  -- everything EXCEPT diagonal swaths (the satellite paths) of equal width, one every L / 8 columns, whose
+                   width is set so that the swaths cover 1 - f of the grid."""
+    rng = np.random.default_rng(seed)
+    if kind == "clouds":
+        g = matern_field(L, max(2.0, L / 16.0), rng, nu=1.5)
+        thr = np.quantile(g, 1.0 - f)
+        return (g > thr).astype(np.uint8)
+    if kind == "tracks":
+        period = max(8, L // 8)
+        width = max(1, int(round((1.0 - f) * period)))
+        y, x = np.mgrid[0:L, 0:L]
+        phase = int(rng.integers(0, period))
+        seen = ((x + (y // 3) + phase) % period) < width          # swaths inclined by 1 : 3
+        return (~seen).astype(np.uint8)
+    raise ValueError(kind)
+
+
+def make_structured_problem(L: int, xi: float, field_seed: int, f: float, kind: str):
+    """make_problem with a structured gap pattern instead of uniformly scattered prediction sites."""
+    rng = np.random.default_rng(field_seed)
+    z = 50.0 + 10.0 * matern_field(L, xi, rng)
+    mask = structured_mask(L, kind, f, field_seed + 7919)
+    values = z.copy()
+    values[mask == 1] = np.nan
+    return values, mask, z
+
+
 def make_config(i: int):
     c = CONFIGS[i]
     return (c,) + make_problem(c.L, c.xi, c.field_seed, c.f, c.lognormal)

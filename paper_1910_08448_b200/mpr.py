@@ -18,9 +18,9 @@ MPR_OK = 0
 ERR_INVALID_ARG, ERR_NO_MEASURED, ERR_DEGENERATE_RANGE, ERR_NONFINITE = -1, -2, -3, -4
 ERR_WORKSPACE, ERR_NOT_READY, ERR_NO_ROOT, ERR_CUDA = -5, -6, -7, -8
 
-MODES = {"DP": 0, "SP": 1, "SP_PRECISE": 2, "SP_INTRINSIC": 3, "DS_INTRINSIC": 4}
+MODES = {"DP": 0, "SP": 1, "SP_PRECISE": 2, "SP_INTRINSIC": 3, "DS_INTRINSIC": 4, "HP": 5}
 TRIPLES = ("DDD", "DSD", "DDS", "SDD", "SDS", "DSS", "SSD", "SSS")      # PAPER.md:35, in Fig. 2's order after DDD
-PATHS = {"TILED": 0, "PLAIN": 1, "STRIP": 2, "AUTO": 3}
+PATHS = {"TILED": 0, "PLAIN": 1, "STRIP": 2, "AUTO": 3, "LIST": 4}
 SCHEDULES = {"R4": 0, "SITE_FUSED": 1}
 PASS_KINDS = {"MET": 0, "OR": 1, "QUENCH": 2, "MO": 3}
 
