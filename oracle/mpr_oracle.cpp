@@ -97,6 +97,7 @@ struct Oracle {
   uint64_t accepted = 0, attempted = 0;
   double T = -1.0;
   int n_quench = 32;            // R8
+  int schedule = 0;             // 0 = R4 (MET c0, MET c1, OR c0, OR c1), 1 = R4b site-fused (MET c0, OR c0, MET c1, OR c1)
   int threads = 1;
   long n_acc = 0;
   int est_trials = 0;
@@ -234,12 +235,22 @@ void quench_pass(Oracle& o, int c) {
 }
 
 // R4: one hybrid sweep = Metropolis colour 0, colour 1, then over-relaxation colour 0, 1.
+// R4b (site-fused order): the same four passes as MET c0, OR c0, MET c1, OR c1.  Both moves of a site read only the
+// other colour, so doing a colour's over-relaxation pass right after its Metropolis pass is the same as giving every
+// site of the colour its Metropolis move and at once its over-relaxation move -- which is how the CUDA path runs it.
 void hybrid_sweep(Oracle& o) {
   o.sweep += 1;
-  met_pass(o, 0, o.sweep);
-  met_pass(o, 1, o.sweep);
-  or_pass(o, 0);
-  or_pass(o, 1);
+  if (o.schedule == 0) {
+    met_pass(o, 0, o.sweep);
+    met_pass(o, 1, o.sweep);
+    or_pass(o, 0);
+    or_pass(o, 1);
+  } else {
+    met_pass(o, 0, o.sweep);
+    or_pass(o, 0);
+    met_pass(o, 1, o.sweep);
+    or_pass(o, 1);
+  }
 }
 
 void reset_chain(Oracle& o, uint32_t trial) {
@@ -512,6 +523,11 @@ int orc_configure(void* h, uint64_t seed, int n_quench) {
   o.seed = seed;
   o.n_quench = n_quench;
   reset_chain(o, 0);
+  return OK;
+}
+int orc_set_schedule(void* h, int schedule) {
+  if (schedule != 0 && schedule != 1) return ERR_INVALID_ARG;
+  static_cast<Oracle*>(h)->schedule = schedule;
   return OK;
 }
 int orc_set_threads(void* h, int n) {

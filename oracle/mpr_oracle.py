@@ -56,6 +56,7 @@ def lib():
             "orc_set_temperature": (C.c_int, [vp, C.c_double]),
             "orc_set_quench": (C.c_int, [vp, C.c_int]),
             "orc_set_threads": (C.c_int, [vp, C.c_int]),
+            "orc_set_schedule": (C.c_int, [vp, C.c_int]),
             "orc_threads_available": (C.c_int, []),
             "orc_reset_chain": (None, [vp, C.c_uint32]),
             "orc_init_random": (None, [vp, C.c_uint32]),
@@ -168,6 +169,10 @@ class Oracle:
 
     def set_quench(self, n):
         self._chk(lib().orc_set_quench(self.h, int(n)))
+
+    def set_schedule(self, schedule):
+        """"R4" (default) or "SITE_FUSED" (R4b): the order of the four colour passes of a hybrid sweep."""
+        self._chk(lib().orc_set_schedule(self.h, {"R4": 0, "SITE_FUSED": 1}[schedule]))
 
     def set_threads(self, n):
         self._chk(lib().orc_set_threads(self.h, int(n)))

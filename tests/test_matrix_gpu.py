@@ -187,3 +187,37 @@ def test_half_precision_storage(mpr, inputs):
     assert abs(res["HP"][0] - res["DP"][0]) <= 3e-5
     assert abs(res["HP"][1] / res["DP"][1] - 1.0) <= 0.01
     assert abs(res["HP"][2] / res["DP"][2] - 1.0) <= 0.01
+
+
+# --------------------------------------------------------------------------- site-fused schedule (R4b) vs the oracle
+@pytest.mark.parametrize("L,f,T", [(97, 0.9, 0.02), (250, 0.66, 0.3)])
+def test_site_fused_schedule_matches_oracle(mpr, oracle_mod, inputs, L, f, T):
+    """DP, pass order MET c0, OR c0, MET c1, OR c1 (the oracle's `SITE_FUSED` flag, pinned by the single-site and
+    two-site tests of tests/test_oracle_pins.py): identical decisions and |dphi| <= 1e-9 after 10 sweeps on the
+    PLAIN, LIST and STRIP paths (one and two sweeps per launch), then a measured run."""
+    values, mask, _ = inputs.make_problem(L, 8.0, 3, f, False)
+    o = oracle_mod.Oracle(values=values, mask=mask, seed=1000)
+    o.set_schedule("SITE_FUSED")
+    o.set_temperature(T)
+    o.hybrid_sweeps(10)
+    so, cnt_o = o.get_state(), o.counters()
+    pred_o, e_o, _ = o.run(3, 5)
+    for path, k in (("PLAIN", 1), ("LIST", 1), ("STRIP", 1), ("STRIP", 2)):
+        g = mpr.Mpr(values, mask, mode="DP", seed=1000)
+        g.set_path(path)
+        g.set_schedule("SITE_FUSED")
+        g.set_fused_sweeps(k)
+        g.set_temperature(T)
+        g.sweep(10)
+        assert float(np.max(np.abs(g.get_state().cpu().numpy() - so))) <= 1e-9, (path, k)
+        assert g.counters() == cnt_o, (path, k)
+        pred, e, _ = g.run(3, 5)
+        m1 = mask == 1
+        assert float(np.max(np.abs(pred.cpu().numpy()[m1] - pred_o[m1]))) <= 1e-8 * 100.0
+        assert abs(e - e_o) <= 1e-11
+        g.close()
+    # and it IS a different chain from R4 (same random numbers, other order)
+    g = mpr.Mpr(values, mask, mode="DP", seed=1000)
+    g.set_temperature(T)
+    g.sweep(10)
+    assert float(np.max(np.abs(g.get_state().cpu().numpy() - so))) > 1e-3

@@ -287,11 +287,12 @@ SITE_CASES = [
 ]
 
 
-@pytest.mark.parametrize("kind", [0, 1], ids=["metropolis", "hybrid"])
+@pytest.mark.parametrize("kind", [0, 1, 2], ids=["metropolis", "hybrid", "hybrid-site-fused"])
 @pytest.mark.parametrize("T", [0.01, 0.1, 1.0, 10.0])
 @pytest.mark.parametrize("case", [0, 1, 2], ids=["interior4", "corner2", "edge3"])
 def test_single_site_histogram(oracle_mod, kind, T, case):
-    """10^6 thinned draws at one free site with fixed neighbours vs p(phi) ~ exp(sum_j cos[q(phi-phi_j)]/T)."""
+    """10^6 thinned draws at one free site with fixed neighbours vs p(phi) ~ exp(sum_j cos[q(phi-phi_j)]/T).
+    kind 2 = hybrid sweeps in the site-fused pass order R4b (MET c0, OR c0, MET c1, OR c1)."""
     (x, y), nbrs = SITE_CASES[case]
     L = 3
     phi = np.full((L, L), 3.0)
@@ -303,8 +304,10 @@ def test_single_site_histogram(oracle_mod, kind, T, case):
     o.set_quench(0)
     o.set_seed(1234 + 17 * case + kind)
     o.set_temperature(T)
+    if kind == 2:
+        o.set_schedule("SITE_FUSED")
     thin = 8
-    tr = o.trace(1_000_000 * thin // 4, kind, [y * L + x])[:, 0]
+    tr = o.trace(1_000_000 * thin // 4, min(kind, 1), [y * L + x])[:, 0]
     samples = tr[1000::thin]
     chi2, p = chi2_against_density(samples, list(nbrs.values()), T)
     assert p > 1e-4, (chi2, p)
@@ -333,7 +336,11 @@ def test_histogram_detects_a_wrong_temperature(oracle_mod):
 
 
 # --------------------------------------------------------------------------- two free sites (T6)
-def test_two_free_sites_vs_quadrature(oracle_mod):
+@pytest.mark.parametrize("schedule", ["R4", "SITE_FUSED"])
+def test_two_free_sites_vs_quadrature(oracle_mod, schedule):
+    """Two neighbouring free sites (one of each colour) in a ring of fixed spins: the chain's means against a 2-D
+    quadrature of the Boltzmann weight.  In the site-fused order the over-relaxation move of site a uses site b
+    BEFORE b's Metropolis move of the same sweep: a wrong composition shows here."""
     rng = np.random.default_rng(8)
     L = 4
     phi = rng.uniform(0.5, 5.5, (L, L))
@@ -344,6 +351,7 @@ def test_two_free_sites_vs_quadrature(oracle_mod):
     o.set_quench(0)
     o.set_seed(4242)
     o.set_temperature(T)
+    o.set_schedule(schedule)
     tr = o.trace(800_000, 1, [1 * L + 1, 1 * L + 2])[2000:]
     # exact: p(a,b) ~ exp{[sum_fixed-nbrs cos(q(a-.)) + sum cos(q(b-.)) + cos(q(a-b))]/T}
     n = 1201
