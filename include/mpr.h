@@ -137,6 +137,10 @@ int mpr_set_stream(mpr_ctx* ctx, void* cuda_stream);
 int mpr_set_precision(mpr_ctx* ctx, mpr_precision mode);
 /* The paper's (X_S X_E X_F) setting as three letters, e.g. "SDS"; see mpr_precision.  Resets the chain. */
 int mpr_set_precision_triple(mpr_ctx* ctx, const char* xs_xe_xf);
+/* The exponent q of Eq. 2 (q in (0, 1/2]; default 1/2, the value north_star fixes).  Recomputes the
+ * sample energy and resets the chain.  With q < 1/2 the allowed arc of q phi is shorter than the half circle; the
+ * range test that needs lives in the per-pass kernels, so the context then runs on MPR_PATH_PLAIN / MPR_PATH_LIST. */
+int mpr_set_q(mpr_ctx* ctx, double q);
 /* X_E alone: 0 = energy sums in double (default, R13), 1 = float energy variable.  Does not touch the chain. */
 int mpr_set_energy_precision(mpr_ctx* ctx, int single);
 /* Philox key (R9).  Resets the chain.                                                      */
@@ -228,6 +232,7 @@ int mpr_predict_host(int L, const double* h_values, const uint8_t* h_mask, mpr_p
  *                                Returns MPR_OK and T_hat, or MPR_ERR_NO_ROOT; *n_trials = trials made.
  *   mpr_debug_proposal_width     the Metropolis proposal half-width delta(T) of R7 the kernels are given. */
 double mpr_debug_proposal_width(double T);
+double mpr_debug_proposal_width_q(double T, double q);
 typedef int (*mpr_trial_fn)(double T, int trial_index, double* e, double* se, void* user);
 int mpr_debug_series_stats(const double* h_series, int64_t n, double* mean, double* se);
 int mpr_debug_match_temperature(double e_sample, mpr_trial_fn trial, void* user, double* T_hat,

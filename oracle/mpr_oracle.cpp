@@ -42,7 +42,7 @@
 
 namespace {
 
-constexpr double kQ = 0.5;   // PAPER.md:27, q in (0,1/2]; north_star fixes q = 1/2
+constexpr double kQDefault = 0.5;   // PAPER.md:27, q in (0,1/2]; north_star fixes q = 1/2 (orc_set_q: any q of the range)
 constexpr double kJ = 1.0;   // PAPER.md:27, exchange constant
 // 2*pi rounded to double; the closed upper end of the spin range.
 const double kTwoPi = 2.0 * 3.14159265358979323846264338327950288;
@@ -97,6 +97,7 @@ struct Oracle {
   uint64_t accepted = 0, attempted = 0;
   double T = -1.0;
   int n_quench = 32;            // R8
+  double q = kQDefault;
   int schedule = 0;             // 0 = R4 (MET c0, MET c1, OR c0, OR c1), 1 = R4b site-fused (MET c0, OR c0, MET c1, OR c1)
   int threads = 1;
   long n_acc = 0;
@@ -121,13 +122,13 @@ double local_energy(const Oracle& o, int x, int y, double phi_s) {
   size_t nb[4];
   const int n = neighbours(o.L, x, y, nb);
   double sum = 0.0;
-  for (int k = 0; k < n; ++k) sum += std::cos(kQ * (phi_s - o.phi[nb[k]]));
+  for (int k = 0; k < n; ++k) sum += std::cos(o.q * (phi_s - o.phi[nb[k]]));
   return -kJ * sum;
 }
 
 // R7: proposal half-width delta = min(pi, 4 sqrt(T / (4 J q^2))).
-double proposal_width(double T) {
-  const double d = 4.0 * std::sqrt(T / (4.0 * kJ * kQ * kQ));
+double proposal_width(double T, double q = kQDefault) {
+  const double d = 4.0 * std::sqrt(T / (4.0 * kJ * q * q));
   const double pi = 0.5 * kTwoPi;
   return d < pi ? d : pi;
 }
@@ -149,7 +150,8 @@ void init_random(Oracle& o, uint32_t trial) {
 // Metropolis pass over the free sites of colour c = (x+y)&1 at sweep n (O3 MET, R7, R10).
 void met_pass(Oracle& o, int c, uint64_t n) {
   const int L = o.L;
-  const double T = o.T, delta = proposal_width(o.T);
+  const double T = o.T, delta = proposal_width(o.T, o.q);
+  const double kQ = o.q;
   const uint32_t key[2] = {static_cast<uint32_t>(o.seed), static_cast<uint32_t>(o.seed >> 32)};
   uint64_t acc = 0, att = 0;
 #pragma omp parallel for schedule(static) reduction(+ : acc, att) num_threads(o.threads)
@@ -189,6 +191,7 @@ inline void field(const Oracle& o, int x, int y, double& A, double& B) {
   size_t nb[4];
   const int nn = neighbours(o.L, x, y, nb);
   A = 0.0; B = 0.0;
+  const double kQ = o.q;
   for (int k = 0; k < nn; ++k) {
     A += std::cos(kQ * o.phi[nb[k]]);
     B += std::sin(kQ * o.phi[nb[k]]);
@@ -199,6 +202,7 @@ inline void field(const Oracle& o, int x, int y, double& A, double& B) {
 // E_loc = -J R cos(q phi - Phi) is unchanged.  Out of [0,2pi] -> leave the spin alone.
 void or_pass(Oracle& o, int c) {
   const int L = o.L;
+  const double kQ = o.q;
 #pragma omp parallel for schedule(static) num_threads(o.threads)
   for (int y = 0; y < L; ++y) {
     for (int x = (y + c) & 1; x < L; x += 2) {
@@ -218,6 +222,7 @@ void or_pass(Oracle& o, int c) {
 // phi = Phi / q, clipped to [0, 2pi].  Deterministic; never raises H.
 void quench_pass(Oracle& o, int c) {
   const int L = o.L;
+  const double kQ = o.q;
 #pragma omp parallel for schedule(static) num_threads(o.threads)
   for (int y = 0; y < L; ++y) {
     for (int x = (y + c) & 1; x < L; x += 2) {
@@ -268,6 +273,7 @@ void reset_chain(Oracle& o, uint32_t trial) {
 // e = 2 H / N_b with N_b = 2 L (L-1) bonds (R3).  Neumaier-compensated sum.
 void energy(const Oracle& o, double* H_out, double* e_out) {
   const int L = o.L;
+  const double kQ = o.q;
   double sum = 0.0, comp = 0.0;
   auto add = [&](double v) {
     const double t = sum + v;
@@ -289,6 +295,7 @@ void energy(const Oracle& o, double* H_out, double* e_out) {
 // O1: sample energy over nearest-neighbour pairs with both ends measured, same normalisation.
 int sample_energy(const Oracle& o, double* es, long long* nsp) {
   const int L = o.L;
+  const double kQ = o.q;
   double sum = 0.0;
   long long cnt = 0;
   for (int y = 0; y < L; ++y)
@@ -437,6 +444,7 @@ void orc_philox4x32_10(const uint32_t* ctr, const uint32_t* key, uint32_t* out) 
 }
 double orc_u53(uint32_t a, uint32_t b) { return u53(a, b); }
 double orc_proposal_width(double T) { return proposal_width(T); }
+double orc_proposal_width_q(double T, double q) { return proposal_width(T, q); }
 void orc_mean_stderr(const double* v, long n, double* mean, double* se) {
   std::vector<double> w(v, v + n);
   mean_stderr(w, mean, se);
@@ -522,6 +530,14 @@ int orc_configure(void* h, uint64_t seed, int n_quench) {
   Oracle& o = *static_cast<Oracle*>(h);
   o.seed = seed;
   o.n_quench = n_quench;
+  reset_chain(o, 0);
+  return OK;
+}
+// q in (0, 1/2].  The spins (angles) do not depend on q; the chain is restarted.
+int orc_set_q(void* h, double q) {
+  if (!(q > 0.0) || q > 0.5) return ERR_INVALID_ARG;
+  Oracle& o = *static_cast<Oracle*>(h);
+  o.q = q;
   reset_chain(o, 0);
   return OK;
 }

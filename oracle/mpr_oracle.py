@@ -57,6 +57,8 @@ def lib():
             "orc_set_quench": (C.c_int, [vp, C.c_int]),
             "orc_set_threads": (C.c_int, [vp, C.c_int]),
             "orc_set_schedule": (C.c_int, [vp, C.c_int]),
+            "orc_set_q": (C.c_int, [vp, C.c_double]),
+            "orc_proposal_width_q": (C.c_double, [C.c_double, C.c_double]),
             "orc_threads_available": (C.c_int, []),
             "orc_reset_chain": (None, [vp, C.c_uint32]),
             "orc_init_random": (None, [vp, C.c_uint32]),
@@ -108,8 +110,8 @@ def u53(a, b):
     return lib().orc_u53(int(a), int(b))
 
 
-def proposal_width(T):
-    return lib().orc_proposal_width(float(T))
+def proposal_width(T, q=None):
+    return lib().orc_proposal_width(float(T)) if q is None else lib().orc_proposal_width_q(float(T), float(q))
 
 
 def mean_stderr(v):
@@ -169,6 +171,9 @@ class Oracle:
 
     def set_quench(self, n):
         self._chk(lib().orc_set_quench(self.h, int(n)))
+
+    def set_q(self, q):
+        self._chk(lib().orc_set_q(self.h, float(q)))
 
     def set_schedule(self, schedule):
         """"R4" (default) or "SITE_FUSED" (R4b): the order of the four colour passes of a hybrid sweep."""

@@ -24,7 +24,7 @@ using namespace mpr;
 
 namespace {
 
-constexpr double kQ = 0.5;   // PAPER.md:27; north_star fixes q = 1/2
+constexpr double kQDefault = 0.5;   // PAPER.md:27, q in (0, 1/2]; north_star fixes q = 1/2 (mpr_set_q: any q of the range)
 constexpr double kJ = 1.0;
 constexpr int kMaxL = 32768;
 constexpr int kPartials = 1 << 18;       // doubles
@@ -48,6 +48,7 @@ Layout make_layout(int L) {
   lo.g.Hb = L + kBitPadTop + kBitPadBot;
   lo.g.plane = static_cast<size_t>(L) * lo.g.Wp;
   lo.g.energy_single = 0;
+  lo.g.q = kQDefault;
   size_t o = 0;
   const size_t state_bytes = 2 * lo.g.plane * sizeof(double2);
   lo.off_state[0] = o; o = align_up(o + state_bytes, 256);
@@ -147,8 +148,8 @@ int fail(mpr_ctx* c, int code, const std::string& msg) {
   } while (0)
 
 // R7: proposal half-width delta = min(pi, 4 sqrt(T / (4 J q^2))).
-double proposal_width(double T) {
-  const double d = 4.0 * std::sqrt(T / (4.0 * kJ * kQ * kQ));
+double proposal_width(double T, double q = kQDefault) {
+  const double d = 4.0 * std::sqrt(T / (4.0 * kJ * q * q));
   const double pi = 3.14159265358979323846264338327950288;
   return d < pi ? d : pi;
 }
@@ -157,9 +158,13 @@ template <typename R>
 ChainConst<R> chain_const(const mpr_ctx* c) {
   ChainConst<R> k;
   const double T = c->T > 0.0 ? c->T : 1.0;
-  k.delta = static_cast<R>(proposal_width(T));
+  const double q = c->lo.g.q;
+  k.delta = static_cast<R>(proposal_width(T, q));
+  k.qhalf = static_cast<R>(0.5 * q);
+  k.bq_c = static_cast<R>(std::cos(6.283185307179586476925286766559 * q));
+  k.bq_s = static_cast<R>(std::sin(6.283185307179586476925286766559 * q));
   k.inv_T = static_cast<R>(1.0 / T);
-  k.hscale = static_cast<R>(0.5 * proposal_width(T));
+  k.hscale = static_cast<R>(q * proposal_width(T, q));      // q Delta / 2 = q delta (f - 3/2)
   if (sizeof(R) == 4) {
     // the two lowest mantissa bits cleared: 3/2 hscale is then exact in float and the 4096 proposal offsets
     // fma(f, hscale, hoff) are exactly symmetric about 0 (delta itself is a free parameter, R7)
@@ -190,7 +195,7 @@ void mean_stderr(const std::vector<double>& v, double* mean, double* se) {
 }
 
 // ---- mode dispatch ---------------------------------------------------------------------------
-template <int MODE> int plain_pass(mpr_ctx* c, int kind, int col, uint64_t sweep) {
+template <int MODE, bool GENQ> int plain_pass_q(mpr_ctx* c, int kind, int col, uint64_t sweep) {
   using R = typename Traits<MODE>::real;
   using V = typename Traits<MODE>::vec;
   const Geom& g = c->lo.g;
@@ -199,18 +204,22 @@ template <int MODE> int plain_pass(mpr_ctx* c, int kind, int col, uint64_t sweep
   const ChainConst<R> k = chain_const<R>(c);
   const uint32_t sw = static_cast<uint32_t>(sweep);
   if (kind == KIND_MET)
-    plain_pass_kernel<MODE, KIND_MET><<<grid, block, 0, c->stream>>>(st, c->bits(), g, col, sw, k, c->slots());
+    plain_pass_kernel<MODE, KIND_MET, GENQ><<<grid, block, 0, c->stream>>>(st, c->bits(), g, col, sw, k, c->slots());
   else if (kind == KIND_MO)
-    plain_pass_kernel<MODE, KIND_MO><<<grid, block, 0, c->stream>>>(st, c->bits(), g, col, sw, k, c->slots());
+    plain_pass_kernel<MODE, KIND_MO, GENQ><<<grid, block, 0, c->stream>>>(st, c->bits(), g, col, sw, k, c->slots());
   else if (kind == KIND_OR)
-    plain_pass_kernel<MODE, KIND_OR><<<grid, block, 0, c->stream>>>(st, c->bits(), g, col, sw, k, c->slots());
+    plain_pass_kernel<MODE, KIND_OR, GENQ><<<grid, block, 0, c->stream>>>(st, c->bits(), g, col, sw, k, c->slots());
   else
-    plain_pass_kernel<MODE, KIND_QUENCH><<<grid, block, 0, c->stream>>>(st, c->bits(), g, col, sw, k, c->slots());
+    plain_pass_kernel<MODE, KIND_QUENCH, GENQ><<<grid, block, 0, c->stream>>>(st, c->bits(), g, col, sw, k, c->slots());
   LAUNCH_OK(c);
   return MPR_OK;
 }
+// q = 1/2 (the default) runs the kernels without the second range test; any other q the general ones
+template <int MODE> int plain_pass(mpr_ctx* c, int kind, int col, uint64_t sweep) {
+  return c->lo.g.q == kQDefault ? plain_pass_q<MODE, false>(c, kind, col, sweep) : plain_pass_q<MODE, true>(c, kind, col, sweep);
+}
 
-template <int MODE> int list_pass(mpr_ctx* c, int kind, int col, uint64_t sweep) {
+template <int MODE, bool GENQ> int list_pass_q(mpr_ctx* c, int kind, int col, uint64_t sweep) {
   using R = typename Traits<MODE>::real;
   using V = typename Traits<MODE>::vec;
   const Geom& g = c->lo.g;
@@ -221,15 +230,18 @@ template <int MODE> int list_pass(mpr_ctx* c, int kind, int col, uint64_t sweep)
   const ChainConst<R> k = chain_const<R>(c);
   const uint32_t sw = static_cast<uint32_t>(sweep);
   if (kind == KIND_MET)
-    list_pass_kernel<MODE, KIND_MET><<<grid, 128, 0, c->stream>>>(st, c->list(col), n, g, col, sw, k, c->slots());
+    list_pass_kernel<MODE, KIND_MET, GENQ><<<grid, 128, 0, c->stream>>>(st, c->list(col), n, g, col, sw, k, c->slots());
   else if (kind == KIND_MO)
-    list_pass_kernel<MODE, KIND_MO><<<grid, 128, 0, c->stream>>>(st, c->list(col), n, g, col, sw, k, c->slots());
+    list_pass_kernel<MODE, KIND_MO, GENQ><<<grid, 128, 0, c->stream>>>(st, c->list(col), n, g, col, sw, k, c->slots());
   else if (kind == KIND_OR)
-    list_pass_kernel<MODE, KIND_OR><<<grid, 128, 0, c->stream>>>(st, c->list(col), n, g, col, sw, k, c->slots());
+    list_pass_kernel<MODE, KIND_OR, GENQ><<<grid, 128, 0, c->stream>>>(st, c->list(col), n, g, col, sw, k, c->slots());
   else
-    list_pass_kernel<MODE, KIND_QUENCH><<<grid, 128, 0, c->stream>>>(st, c->list(col), n, g, col, sw, k, c->slots());
+    list_pass_kernel<MODE, KIND_QUENCH, GENQ><<<grid, 128, 0, c->stream>>>(st, c->list(col), n, g, col, sw, k, c->slots());
   LAUNCH_OK(c);
   return MPR_OK;
+}
+template <int MODE> int list_pass(mpr_ctx* c, int kind, int col, uint64_t sweep) {
+  return c->lo.g.q == kQDefault ? list_pass_q<MODE, false>(c, kind, col, sweep) : list_pass_q<MODE, true>(c, kind, col, sweep);
 }
 
 template <int MODE> int init_chain(mpr_ctx* c) {
@@ -417,6 +429,8 @@ int eff_path(const mpr_ctx* c) {
   // half-precision storage runs on the per-pass kernels only (its TILED / STRIP instantiations
   // raise an illegal-instruction fault on the B200 that has not been tracked down; they are compiled but not routed to)
   if (c->mode == MPR_HP) return c->path == MPR_PATH_LIST ? MPR_PATH_LIST : MPR_PATH_PLAIN;
+  // q < 1/2 (mpr_set_q): the general range test lives in the per-pass kernels only
+  if (c->lo.g.q != kQDefault) return c->path == MPR_PATH_LIST ? MPR_PATH_LIST : MPR_PATH_PLAIN;
   if (c->path != MPR_PATH_AUTO) return c->path;
   if (c->schedule == MPR_SCHEDULE_SITE_FUSED) {
     // small, sparsely masked grids: the compacted lists win (config 3, f = 0.33, L2-resident: 0.021 against 0.025 ms)
@@ -567,7 +581,7 @@ int setup(mpr_ctx* c) {
   c->zmin = h[0];
   c->zmax = h[1];
   // R6: sample energy
-  sample_energy_kernel<<<nblk, 256, 0, c->stream>>>(c->d_values, c->d_mask, g.L, c->zmin, c->zmax, c->part());
+  sample_energy_kernel<<<nblk, 256, 0, c->stream>>>(c->d_values, c->d_mask, g.L, c->zmin, c->zmax, c->part(), g.q);
   LAUNCH_OK(c);
   pair_final_kernel<<<1, 32, 0, c->stream>>>(c->part(), nblk, c->scal());
   LAUNCH_OK(c);
@@ -697,6 +711,13 @@ void mpr_destroy(mpr_ctx* ctx) {
 int mpr_set_precision(mpr_ctx* c, mpr_precision mode) {
   if (!c || mode < MPR_DP || mode > MPR_HP) return fail(c, MPR_ERR_INVALID_ARG, "bad mode");
   c->mode = mode;
+  mark_stale(c);
+  return MPR_OK;
+}
+int mpr_set_q(mpr_ctx* c, double q) {
+  if (!c || !(q > 0.0) || q > 0.5) return fail(c, MPR_ERR_INVALID_ARG, "q must lie in (0, 1/2]");
+  c->lo.g.q = q;
+  if (c->ws) TRY(setup(c));       // the sample energy of R6 depends on q
   mark_stale(c);
   return MPR_OK;
 }
@@ -973,6 +994,7 @@ int mpr_predict_host(int L, const double* h_values, const uint8_t* h_mask, mpr_p
 }
 
 double mpr_debug_proposal_width(double T) { return proposal_width(T); }
+double mpr_debug_proposal_width_q(double T, double q) { return proposal_width(T, q); }
 
 int mpr_debug_series_stats(const double* h_series, int64_t n, double* mean, double* se) {
   if (n < 0 || (n > 0 && !h_series)) return MPR_ERR_INVALID_ARG;

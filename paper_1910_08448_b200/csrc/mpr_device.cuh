@@ -221,6 +221,8 @@ template <typename R> struct ChainConst {
   R inv_T;     // 1/T
   R hscale;    // float modes: q Delta / 2 = hscale (f - 3/2), f = prop_word in [1, 2): hscale = delta / 2
   R hoff;      //              = fma(f, hscale, hoff), hoff = -3/2 hscale
+  R qhalf;     // q / 2 (double-arithmetic proposal: q Delta / 2 = qhalf * delta * (2 u1 - 1)); 1/4 for q = 1/2
+  R bq_c, bq_s;  // general q only (GENQ): the end of the allowed arc, (cos 2 pi q, sin 2 pi q): phi <= 2 pi <=> u x b >= 0
   R xscale;    // SP_INTRINSIC: log2(e) / T, so that exp(-dE / T) 2^20 = ex2(-dE * xscale + 20)
   uint32_t k0, k1, trial;
   PhiloxKeys rk;   // round keys of (k0, k1)
@@ -356,7 +358,10 @@ __device__ __forceinline__ void met_words_pair(uint32_t pair_site, uint32_t swee
 // site is free, the proposal stays in range (s' >= 0) and the acceptance test passes; ok[x] tells.
 //   sd = sin(q Delta/2), cd = cos(q Delta/2);  sin(q Delta) = 2 sd cd,  cos(q Delta) - 1 = -2 sd^2
 //   u' = rot(q Delta) u;  P = u.F;  -Q = s A - c B;  dE = 2 sd (sd P - cd Q)
-template <int MODE>
+// GENQ: q < 1/2 (q in (0, 1/2]).  q phi then runs over [0, 2 pi q], an arc shorter than the half circle: besides
+// s >= 0 (phi >= 0) a spin must satisfy u x b = c b_s - s b_c >= 0 (phi <= 2 pi), b the end of the arc.  For q = 1/2 that
+// second test IS s >= 0, and the kernels of the fused paths are compiled without it.
+template <int MODE, bool GENQ = false>
 __device__ __forceinline__ void met_update2(Two<typename Traits<MODE>::real> c, Two<typename Traits<MODE>::real> s,
                                             Two<typename Traits<MODE>::real> A, Two<typename Traits<MODE>::real> B,
                                             const MetWords& wa, const MetWords& wb, bool free_a, bool free_b,
@@ -367,7 +372,7 @@ __device__ __forceinline__ void met_update2(Two<typename Traits<MODE>::real> c, 
   if constexpr (sizeof(R) == 8) {
     const R ta = fma_(R(2), R(u53(wa.p, wa.q)), R(-1));   // 2 u1 - 1 (exact)
     const R tb = fma_(R(2), R(u53(wb.p, wb.q)), R(-1));
-    h = mul2(bc2(R(0.25)), mul2(bc2(k.delta), mk2(ta, tb)));
+    h = mul2(bc2(k.qhalf), mul2(bc2(k.delta), mk2(ta, tb)));
   } else {
     h = fma2(mk2(prop_word(wa.p), prop_word(wb.p)), bc2(k.hscale), bc2(k.hoff));
   }
@@ -406,8 +411,13 @@ __device__ __forceinline__ void met_update2(Two<typename Traits<MODE>::real> c, 
     acc_a = ua < Fn<MODE>::exp_(xa);
     acc_b = ub < Fn<MODE>::exp_(xb);
   }
-  const bool oka = free_a && (sna >= R(0)) && acc_a;
-  const bool okb = free_b && (snb >= R(0)) && acc_b;
+  bool in_a = sna >= R(0), in_b = snb >= R(0);
+  if constexpr (GENQ) {
+    in_a = in_a && (fma_(cna, k.bq_s, -(sna * k.bq_c)) >= R(0));
+    in_b = in_b && (fma_(cnb, k.bq_s, -(snb * k.bq_c)) >= R(0));
+  }
+  const bool oka = free_a && in_a && acc_a;
+  const bool okb = free_b && in_b && acc_b;
   out[0] = oka ? cna : c0a; out[2] = oka ? sna : s0a;
   out[1] = okb ? cnb : c0b; out[3] = okb ? snb : s0b;
   ok[0] = oka; ok[1] = okb;
@@ -417,11 +427,12 @@ __device__ __forceinline__ void met_update2(Two<typename Traits<MODE>::real> c, 
 // t = 2 (u.F)/|F|^2; keep it iff the site is free, F != 0 and u' stays on the upper half circle.
 // One Newton step towards |u'| = 1 stops the rounding drift of the norm.  Computed as
 // m = u - t F = -u' and -f, so that no negation is needed: u' f = m (-f).
-template <int MODE>
+template <int MODE, bool GENQ = false>
 __device__ __forceinline__ void or_update2(Two<typename Traits<MODE>::real> c, Two<typename Traits<MODE>::real> s,
                                            Two<typename Traits<MODE>::real> A, Two<typename Traits<MODE>::real> B,
                                            bool free_a, bool free_b,
-                                           typename Traits<MODE>::real out[4] /* ca, cb, sa, sb */) {
+                                           typename Traits<MODE>::real out[4] /* ca, cb, sa, sb */,
+                                           const ChainConst<typename Traits<MODE>::real>* kq = nullptr) {
   using R = typename Traits<MODE>::real;
   const Two<R> F2 = fma2(A, A, mul2(B, B));
   const Two<R> P = fma2(c, A, mul2(s, B));
@@ -439,21 +450,30 @@ __device__ __forceinline__ void or_update2(Two<typename Traits<MODE>::real> c, T
   // F = 0 (no field: nothing to reflect about) needs no test of its own: t = -2 P / 0 is inf or NaN, t F - u is NaN
   // (inf x 0), and NaN <= 0 is false -- the spin stays.  (void)f2a keeps the name for readers of the formula above.
   (void)f2a; (void)f2b;
-  const bool oka = free_a && (msa <= R(0));
-  const bool okb = free_b && (msb <= R(0));
+  bool oka = free_a && (msa <= R(0));
+  bool okb = free_b && (msb <= R(0));
+  if constexpr (GENQ) {
+    oka = oka && (fma_(coa, kq->bq_s, -(soa * kq->bq_c)) >= R(0));
+    okb = okb && (fma_(cob, kq->bq_s, -(sob * kq->bq_c)) >= R(0));
+  }
   out[0] = oka ? coa : c0a; out[2] = oka ? soa : s0a;
   out[1] = okb ? cob : c0b; out[3] = okb ? sob : s0b;
 }
 
 // Quench move (R8): the minimiser of the local energy, u = F/|F|.
-template <int MODE>
+template <int MODE, bool GENQ = false>
 __device__ __forceinline__ void quench_update(typename Traits<MODE>::real* c, typename Traits<MODE>::real* s,
-                                              typename Traits<MODE>::real A, typename Traits<MODE>::real B) {
+                                              typename Traits<MODE>::real A, typename Traits<MODE>::real B,
+                                              const ChainConst<typename Traits<MODE>::real>* kq = nullptr) {
   using R = typename Traits<MODE>::real;
   const R R2 = fma_(A, A, B * B);
   if (R2 == R(0)) return;
   const R inv = Fn<MODE>::rsqrt_(R2);
-  *c = A * inv; *s = B * inv;
+  R cn = A * inv, sn = B * inv;
+  if constexpr (GENQ) {                       // Phi / q > 2 pi: clipped to the end of the arc (R8)
+    if (fma_(cn, kq->bq_s, -(sn * kq->bq_c)) < R(0)) { cn = kq->bq_c; sn = kq->bq_s; }
+  }
+  *c = cn; *s = sn;
 }
 
 // Quench move of two sites at once (same per-lane operations as quench_update).
@@ -473,10 +493,10 @@ __device__ __forceinline__ void quench_update2(Two<typename Traits<MODE>::real> 
   out[1] = okb ? cob : c0b; out[3] = okb ? sob : s0b;
 }
 
-// phi = 2 atan2(s, c) in [0, 2pi] (s >= 0).
+// phi = atan2(s, c) / q in [0, 2pi] (s >= 0); inv_q = 2 for q = 1/2.
 template <int MODE>
-__device__ __forceinline__ double spin_angle(typename Traits<MODE>::real c, typename Traits<MODE>::real s) {
-  return 2.0 * static_cast<double>(Fn<MODE>::atan2_(s, c));
+__device__ __forceinline__ double spin_angle(typename Traits<MODE>::real c, typename Traits<MODE>::real s, double inv_q = 2.0) {
+  return inv_q * static_cast<double>(Fn<MODE>::atan2_(s, c));
 }
 
 // Column pair of the left/right neighbours in the other colour plane: a site of colour col

@@ -19,6 +19,7 @@ struct Geom {
   int L, Wp, Wm;
   int Wb, Hb;            // padded bitmap: words per row, rows per colour
   size_t plane;          // elements per colour plane = L * Wp
+  double q;              // PAPER.md:27, q in (0, 1/2]; 1/2 unless mpr_set_q
   int energy_single;     // X_E of PAPER.md:35: 0 = energy sums in double (R13), 1 = the energy variable is a float
 };
 
@@ -137,7 +138,7 @@ __device__ __forceinline__ double map_to_phi(double z, double zmin, double zmax)
 // R6 first half: e_s = -2J mean over measured nearest-neighbour pairs of cos[q(phi_s - phi_t)].
 // Per-block partials: [0] sum of cos, [1] pair count.
 static __global__ void sample_energy_kernel(const double* __restrict__ z, const uint8_t* __restrict__ mask, int L,
-                                     double zmin, double zmax, double* __restrict__ part /* 2 per block */) {
+                                     double zmin, double zmax, double* __restrict__ part /* 2 per block */, double q) {
   __shared__ double sh[32];
   double sum = 0.0, cnt = 0.0;
   const size_t N = static_cast<size_t>(L) * L;
@@ -146,8 +147,8 @@ static __global__ void sample_energy_kernel(const double* __restrict__ z, const 
     if (mask[i]) continue;
     const int x = static_cast<int>(i % L), y = static_cast<int>(i / L);
     const double p = map_to_phi(z[i], zmin, zmax);
-    if (x < L - 1 && !mask[i + 1]) { sum += cos(0.5 * (p - map_to_phi(z[i + 1], zmin, zmax))); cnt += 1.0; }
-    if (y < L - 1 && !mask[i + L]) { sum += cos(0.5 * (p - map_to_phi(z[i + L], zmin, zmax))); cnt += 1.0; }
+    if (x < L - 1 && !mask[i + 1]) { sum += cos(q * (p - map_to_phi(z[i + 1], zmin, zmax))); cnt += 1.0; }
+    if (y < L - 1 && !mask[i + L]) { sum += cos(q * (p - map_to_phi(z[i + L], zmin, zmax))); cnt += 1.0; }
   }
   const double s = block_sum(sum, sh);
   const double c = block_sum(cnt, sh);
@@ -209,7 +210,7 @@ __global__ void init_chain_kernel(const double* __restrict__ z, const uint8_t* _
       phi = map_to_phi(z[s], zmin, zmax);
     }
     double sn, cs;
-    sincos(0.5 * phi, &sn, &cs);
+    sincos(g.q * phi, &sn, &cs);
     if (sn < 0.0) sn = 0.0;
     // through the arithmetic type of the mode first: with double storage and float arithmetic (MODE_DS) a stored spin
     // must be a value the arithmetic can hand back unchanged, or the tiled kernels (which rewrite every site, moved or
@@ -235,7 +236,7 @@ __global__ void set_state_kernel(const double* __restrict__ phi, Geom g, const u
   // angles outside [0, 2pi] are clamped to the nearer end: the stored vector is always a
   // unit vector on the upper half circle
   const double p = fmin(fmax(phi[static_cast<size_t>(y) * g.L + x], 0.0), 6.283185307179586476925286766559);
-  sincos(0.5 * p, &sn, &cs);
+  sincos(g.q * p, &sn, &cs);
   if (sn < 0.0) { sn = 0.0; cs = cs < 0.0 ? -1.0 : 1.0; }
   V v;
   using R = typename Traits<MODE>::real;
@@ -252,7 +253,7 @@ __global__ void get_state_kernel(const typename Traits<MODE>::vec* __restrict__ 
   if (x >= g.L) return;
   const int col = (x + y) & 1, j = x >> 1;
   const auto v = ld_spin(state, static_cast<long long>(col) * g.plane + static_cast<long long>(y) * g.Wp + j);
-  phi[static_cast<size_t>(y) * g.L + x] = 2.0 * atan2(to_double(v.y), to_double(v.x));
+  phi[static_cast<size_t>(y) * g.L + x] = atan2(to_double(v.y), to_double(v.x)) / g.q;
 }
 
 // ---- one colour pass on the global planes -------------------------------------------------
@@ -260,7 +261,7 @@ __global__ void get_state_kernel(const typename Traits<MODE>::vec* __restrict__ 
 // plane position and tests its mask bit (PLAIN) and the one that walks the compacted list of prediction sites
 // (LIST): the same instructions on the same operands, hence the same spins.  Returns whether a Metropolis move
 // was accepted.
-template <int MODE, int KIND>
+template <int MODE, int KIND, bool GENQ = false>
 __device__ __forceinline__ bool plain_site_update(typename Traits<MODE>::vec* __restrict__ state, const Geom& g, int col,
                                                   int y, int j, uint32_t sweep,
                                                   const ChainConst<typename Traits<MODE>::real>& k) {
@@ -291,20 +292,20 @@ __device__ __forceinline__ bool plain_site_update(typename Traits<MODE>::vec* __
     const MetWords w = (j & 1) ? w1 : w0;
     R o[4];
     bool ok[2];
-    met_update2<MODE>(bc2(c), bc2(s), bc2(A), bc2(B), w, w, true, true, k, o, ok);   // the site in both lanes
+    met_update2<MODE, GENQ>(bc2(c), bc2(s), bc2(A), bc2(B), w, w, true, true, k, o, ok);   // the site in both lanes
     c = o[0]; s = o[2];
     accepted = ok[0];
     if constexpr (KIND == KIND_MO) {     // site-fused schedule (R4b): the over-relaxation move follows at once
       R o2[4];
-      or_update2<MODE>(bc2(c), bc2(s), bc2(A), bc2(B), true, true, o2);
+      or_update2<MODE, GENQ>(bc2(c), bc2(s), bc2(A), bc2(B), true, true, o2, &k);
       c = o2[0]; s = o2[2];
     }
   } else if constexpr (KIND == KIND_OR) {
     R o[4];
-    or_update2<MODE>(bc2(c), bc2(s), bc2(A), bc2(B), true, true, o);
+    or_update2<MODE, GENQ>(bc2(c), bc2(s), bc2(A), bc2(B), true, true, o, &k);
     c = o[0]; s = o[2];
   } else {
-    quench_update<MODE>(&c, &s, A, B);
+    quench_update<MODE, GENQ>(&c, &s, A, B, &k);
   }
   V out;
   out.x = static_cast<decltype(out.x)>(c);
@@ -313,7 +314,7 @@ __device__ __forceinline__ bool plain_site_update(typename Traits<MODE>::vec* __
   return accepted;
 }
 
-template <int MODE, int KIND>
+template <int MODE, int KIND, bool GENQ = false>
 __global__ void __launch_bounds__(128)
 plain_pass_kernel(typename Traits<MODE>::vec* __restrict__ state, const uint32_t* __restrict__ bits, Geom g,
                   int col, uint32_t sweep, ChainConst<typename Traits<MODE>::real> k,
@@ -321,7 +322,7 @@ plain_pass_kernel(typename Traits<MODE>::vec* __restrict__ state, const uint32_t
   const int y = blockIdx.y;
   const int j = blockIdx.x * blockDim.x + threadIdx.x;
   bool accepted = false;
-  if (j < g.Wp && mask_bit(bits, g, col, y, j)) accepted = plain_site_update<MODE, KIND>(state, g, col, y, j, sweep, k);
+  if (j < g.Wp && mask_bit(bits, g, col, y, j)) accepted = plain_site_update<MODE, KIND, GENQ>(state, g, col, y, j, sweep, k);
   if constexpr (KIND == KIND_MET || KIND == KIND_MO) {
     const int n = __syncthreads_count(accepted);
     if (threadIdx.x == 0 && n)
@@ -394,7 +395,7 @@ static __global__ void list_fill_kernel(const uint32_t* __restrict__ bits, Geom 
   }
 }
 
-template <int MODE, int KIND>
+template <int MODE, int KIND, bool GENQ = false>
 __global__ void __launch_bounds__(128)
 list_pass_kernel(typename Traits<MODE>::vec* __restrict__ state, const uint32_t* __restrict__ list, uint32_t n, Geom g,
                  int col, uint32_t sweep, ChainConst<typename Traits<MODE>::real> k,
@@ -404,7 +405,7 @@ list_pass_kernel(typename Traits<MODE>::vec* __restrict__ state, const uint32_t*
   if (i < n) {
     const uint32_t pos = list[i];
     const int y = static_cast<int>(pos / static_cast<uint32_t>(g.Wp)), j = static_cast<int>(pos % static_cast<uint32_t>(g.Wp));
-    accepted = plain_site_update<MODE, KIND>(state, g, col, y, j, sweep, k);
+    accepted = plain_site_update<MODE, KIND, GENQ>(state, g, col, y, j, sweep, k);
   }
   if constexpr (KIND == KIND_MET || KIND == KIND_MO) {
     const int m = __syncthreads_count(accepted);
@@ -456,7 +457,7 @@ __global__ void plain_accumulate_kernel(const typename Traits<MODE>::vec* __rest
   if (j >= g.Wp || !mask_bit(bits, g, col, y, j)) return;
   const size_t i = static_cast<size_t>(col) * g.plane + static_cast<size_t>(y) * g.Wp + j;
   const auto v = ld_spin(state, static_cast<long long>(i));
-  acc[i] += spin_angle<MODE>(R(v.x), R(v.y));
+  acc[i] += spin_angle<MODE>(R(v.x), R(v.y), 1.0 / g.q);
 }
 
 static __global__ void clear_acc_kernel(double* __restrict__ acc, size_t n) {

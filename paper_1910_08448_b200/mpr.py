@@ -28,7 +28,7 @@ PASS_KINDS = {"MET": 0, "OR": 1, "QUENCH": 2, "MO": 3}
 SYMBOLS = [
     "mpr_workspace_bytes", "mpr_create", "mpr_destroy", "mpr_set_workspace", "mpr_set_stream",
     "mpr_debug_series_stats", "mpr_debug_match_temperature", "mpr_debug_proposal_width", "mpr_set_precision",
-    "mpr_set_precision_triple", "mpr_set_energy_precision", "mpr_set_seed",
+    "mpr_set_precision_triple", "mpr_set_energy_precision", "mpr_set_q", "mpr_debug_proposal_width_q", "mpr_set_seed",
     "mpr_set_temperature", "mpr_set_quench", "mpr_set_path", "mpr_set_fused_sweeps", "mpr_set_schedule", "mpr_reset_chain",
     "mpr_estimate_temperature", "mpr_run", "mpr_sweep", "mpr_pass", "mpr_get_state", "mpr_set_state",
     "mpr_energy", "mpr_sample_energy", "mpr_get_counters", "mpr_get_run_timing", "mpr_get_energy_series",
@@ -79,6 +79,8 @@ def lib():
         "mpr_set_precision": (C.c_int, [vp, C.c_int]),
         "mpr_set_precision_triple": (C.c_int, [vp, C.c_char_p]),
         "mpr_set_energy_precision": (C.c_int, [vp, C.c_int]),
+        "mpr_set_q": (C.c_int, [vp, C.c_double]),
+        "mpr_debug_proposal_width_q": (C.c_double, [C.c_double, C.c_double]),
         "mpr_set_seed": (C.c_int, [vp, C.c_uint64]),
         "mpr_set_temperature": (C.c_int, [vp, C.c_double]),
         "mpr_set_quench": (C.c_int, [vp, C.c_int]),
@@ -197,6 +199,9 @@ class Mpr:
 
     def set_precision_triple(self, triple):
         self._call(lib().mpr_set_precision_triple, triple.encode())
+
+    def set_q(self, q):
+        self._call(lib().mpr_set_q, float(q))
 
     def set_energy_precision(self, single):
         self._call(lib().mpr_set_energy_precision, 1 if single else 0)
@@ -318,8 +323,8 @@ def predict_host(values, mask, mode="DP", seed=0, T=-1.0, n_eq=100, n_meas=100, 
     return pred_out, m.value, s.value, Tu.value, nl.value
 
 
-def debug_proposal_width(T):
-    return lib().mpr_debug_proposal_width(float(T))
+def debug_proposal_width(T, q=None):
+    return lib().mpr_debug_proposal_width(float(T)) if q is None else lib().mpr_debug_proposal_width_q(float(T), float(q))
 
 
 def debug_series_stats(series):

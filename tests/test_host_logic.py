@@ -225,3 +225,6 @@ def test_proposal_width(sides, side):
     assert w(0.61) < math.pi and abs(w(0.61) - 4.0 * math.sqrt(0.61)) <= 1e-15
     assert w(0.62) == math.pi and w(1e6) == math.pi
     assert abs(w((math.pi / 4) ** 2) - math.pi) <= 1e-15
+    # general q: delta = min(pi, 2 sqrt(T) / q)
+    assert w(0.01, 0.25) == 0.8
+    assert abs(w(0.0025, 0.1) - 1.0) <= 1e-15 and w(1.0, 0.1) == math.pi

@@ -221,3 +221,83 @@ def test_site_fused_schedule_matches_oracle(mpr, oracle_mod, inputs, L, f, T):
     g.set_temperature(T)
     g.sweep(10)
     assert float(np.max(np.abs(g.get_state().cpu().numpy() - so))) > 1e-3
+
+
+# --------------------------------------------------------------------------- general q
+@pytest.mark.parametrize("q", [0.3, 0.1])
+@pytest.mark.parametrize("schedule", ["R4", "SITE_FUSED"])
+def test_general_q_matches_oracle(mpr, oracle_mod, inputs, q, schedule):
+    """q < 1/2: set-up (sample energy), R8 initialisation (the quench clips at phi = 2 pi), 10 hybrid sweeps and a
+    measured run in DP against the oracle with the same q -- identical decisions, |dphi| <= 1e-9 -- on the PLAIN and
+    LIST paths; asking for a fused path still works (the context routes itself to the per-pass kernels)."""
+    values, mask, _ = inputs.make_problem(120, 8.0, 3, 0.8, False)
+    o = oracle_mod.Oracle(values=values, mask=mask, seed=1000)
+    o.set_q(q)
+    o.set_schedule(schedule)
+    o.set_temperature(0.05)
+    es_o, n_o = o.sample_energy()
+    s_init = o.get_state()
+    o.hybrid_sweeps(10)
+    so, cnt_o = o.get_state(), o.counters()
+    pred_o, e_o, _ = o.run(3, 5)
+    for path in ("PLAIN", "LIST", "STRIP"):
+        g = mpr.Mpr(values, mask, mode="DP", seed=1000)
+        g.set_q(q)
+        g.set_path(path)
+        g.set_schedule(schedule)
+        g.set_temperature(0.05)
+        es_g, n_g = g.sample_energy()
+        assert n_g == n_o and abs(es_g - es_o) <= 1e-12
+        assert float(np.max(np.abs(g.get_state().cpu().numpy() - s_init))) <= 1e-9
+        g.sweep(10)
+        sg = g.get_state().cpu().numpy()
+        assert float(np.max(np.abs(sg - so))) <= 1e-9, path
+        assert sg.min() >= 0.0 and sg.max() <= 2.0 * math.pi + 1e-12
+        assert g.counters() == cnt_o, path
+        pred, e, _ = g.run(3, 5)
+        m1 = mask == 1
+        assert float(np.max(np.abs(pred.cpu().numpy()[m1] - pred_o[m1]))) <= 1e-6
+        assert abs(e - e_o) <= 1e-11
+        g.close()
+    with pytest.raises(mpr.MprError):
+        mpr.Mpr(values, mask).set_q(0.6)
+
+
+@pytest.mark.parametrize("mode", ["SP_INTRINSIC", "SP_PRECISE"])
+def test_general_q_float_modes_sample_the_exact_density(mpr, mode):
+    """Isolated free sites with identical measured neighbourhoods at q = 0.25: chi^2 of the pooled samples against
+    p(phi) ~ exp(sum_j cos[q (phi - phi_j)] / T) (the density piles up against phi = 2 pi for these neighbours, so the
+    upper range test is exercised)."""
+    q, T, L = 0.25, 0.3, 302
+    nb = {(-1, 0): 5.3, (1, 0): 6.0, (0, -1): 4.4, (0, 1): 5.8}
+    rng = np.random.default_rng(3)
+    z = rng.uniform(0.5, 5.5, (L, L))
+    mask = np.zeros((L, L), dtype=np.uint8)
+    sites = [(x, y) for y in range(2, L - 2, 3) for x in range(1, L - 3, 3)]
+    for (x, y) in sites:
+        mask[y, x] = 1
+        for (dx, dy), a in nb.items():
+            z[y + dy, x + dx] = a
+    z[L // 2, L - 1], z[L // 2 + 2, L - 1] = 0.0, 2.0 * math.pi          # anchors of the R1 map: phi = z
+    g = mpr.Mpr(z, mask, mode=mode, seed=9)
+    g.set_q(q)
+    g.set_temperature(T)
+    g.sweep(60)
+    ys, xs = np.array([s[1] for s in sites]), np.array([s[0] for s in sites])
+    snaps = []
+    for _ in range(50):
+        g.sweep(6)
+        snaps.append(g.get_state().cpu().numpy()[ys, xs])
+    samples = np.concatenate(snaps)
+    grid = np.linspace(0.0, 2.0 * math.pi, 400001)
+    logw = sum(np.cos(q * (grid - a)) for a in nb.values()) / T
+    w = np.exp(logw - logw.max())
+    cdf = np.concatenate([[0.0], np.cumsum(0.5 * (w[1:] + w[:-1]) * np.diff(grid))])
+    cdf /= cdf[-1]
+    nbins = 40
+    edges = np.concatenate([[0.0], np.interp(np.arange(1, nbins) / nbins, cdf, grid), [2.0 * math.pi + 1e-9]])
+    cnt, _ = np.histogram(samples, bins=edges)
+    assert cnt.sum() == samples.size
+    chi2 = float(((cnt - samples.size / nbins) ** 2 / (samples.size / nbins)).sum())
+    assert chi2 < 85.0, chi2
+    assert float(np.mean(samples > 6.0)) > 0.05            # the mass near the upper end of the range is really there

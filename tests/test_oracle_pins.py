@@ -571,3 +571,83 @@ def test_no_root_is_reported(oracle_mod):
     with pytest.raises(oracle_mod.OracleError) as ei:
         o.estimate_temperature()
     assert ei.value.code == oracle_mod.ERR_NO_ROOT
+
+
+# --------------------------------------------------------------------------- general q (q in (0, 1/2])
+@pytest.mark.parametrize("q", [0.5, 0.3, 0.1])
+def test_general_q_energy_closed_forms(oracle_mod, q):
+    """Uniform grid: e = -2J for every q.  I.i.d.-uniform spins: E cos[q(a - b)] = (E cos qa)^2 + (E sin qa)^2 =
+    (2 - 2 cos 2 pi q) / (2 pi q)^2, so e -> -2J times that (4 / pi^2 at q = 1/2)."""
+    L = 96
+    o = oracle_mod.Oracle(phi=np.full((L, L), 1.234), mask=np.zeros((L, L), dtype=np.uint8))
+    o.set_q(q)
+    assert abs(o.energy()[1] + 2.0) <= 1e-12
+    mask = np.ones((L, L), dtype=np.uint8)
+    o = oracle_mod.Oracle(phi=np.zeros((L, L)), mask=mask)
+    o.set_quench(0)
+    o.set_q(q)
+    o.set_seed(77)                                   # free spins i.i.d. uniform (R8 without the quench)
+    expect = -2.0 * (2.0 - 2.0 * math.cos(TWO_PI * q)) / (TWO_PI * q) ** 2
+    assert abs(o.energy()[1] - expect) < 5.0 / L     # ~ 1 / sqrt(number of bonds), generous
+
+
+@pytest.mark.parametrize("q", [0.3, 0.1])
+def test_general_q_over_relaxation(oracle_mod, q):
+    """R5 at q < 1/2: the reflection phi' = 2 Phi / q - phi conserves H exactly and never leaves [0, 2 pi]
+    (moves that would are dropped); applied twice it is the identity where it was accepted."""
+    rng = np.random.default_rng(5)
+    L = 24
+    phi = rng.uniform(0.0, TWO_PI, (L, L))
+    mask = (rng.uniform(size=(L, L)) < 0.8).astype(np.uint8)
+    o = oracle_mod.Oracle(phi=phi, mask=mask)
+    o.set_quench(0)
+    o.set_q(q)
+    o.set_state(phi)
+    H0 = o.energy()[0]
+    moved = 0
+    for c in (0, 1, 0, 1):
+        before = o.get_state()
+        o.or_pass(c)
+        after = o.get_state()
+        moved += int((before != after).sum())
+        assert abs(o.energy()[0] - H0) <= 1e-10 * abs(H0)
+        assert after.min() >= 0.0 and after.max() <= TWO_PI
+        assert np.array_equal(after[mask == 0], phi[mask == 0])
+    assert moved > 0.1 * mask.sum()
+
+
+@pytest.mark.parametrize("q,T", [(0.25, 0.1), (0.1, 0.02), (0.4, 1.0)])
+def test_general_q_single_site_histogram(oracle_mod, q, T):
+    """Hybrid sweeps at one free site with four fixed neighbours against p(phi) ~ exp(sum_j cos[q (phi - phi_j)] / T)."""
+    (x, y), nbrs = SITE_CASES[0]
+    L = 3
+    phi = np.full((L, L), 3.0)
+    for (a, b), v in nbrs.items():
+        phi[b, a] = v
+    mask = np.zeros((L, L), dtype=np.uint8)
+    mask[y, x] = 1
+    o = oracle_mod.Oracle(phi=phi, mask=mask)
+    o.set_quench(0)
+    o.set_q(q)
+    o.set_seed(321)
+    o.set_temperature(T)
+    tr = o.trace(2_000_000, 1, [y * L + x])[1000::8, 0]
+    xs = np.linspace(0.0, TWO_PI, 400001)
+    logw = sum(np.cos(q * (xs - pj)) for pj in nbrs.values()) / T
+    w = np.exp(logw - logw.max())
+    cdf = np.concatenate([[0.0], np.cumsum(0.5 * (w[1:] + w[:-1]) * np.diff(xs))])
+    cdf /= cdf[-1]
+    nbins = 50
+    edges = np.interp(np.linspace(0, 1, nbins + 1), cdf, xs)
+    edges[0], edges[-1] = 0.0, TWO_PI
+    counts, _ = np.histogram(tr, bins=edges)
+    assert counts.sum() == tr.size
+    chi2 = float(np.sum((counts - tr.size / nbins) ** 2 / (tr.size / nbins)))
+    assert stats.chi2.sf(chi2, nbins - 1) > 1e-4, chi2
+
+
+def test_general_q_proposal_width(oracle_mod):
+    """delta = min(pi, 4 sqrt(T / (4 J q^2))) = min(pi, 2 sqrt(T) / q)."""
+    assert oracle_mod.proposal_width(0.01, 0.25) == 0.8
+    assert abs(oracle_mod.proposal_width(0.0025, 0.1) - 1.0) <= 1e-15
+    assert oracle_mod.proposal_width(1.0, 0.1) == math.pi
