@@ -315,8 +315,10 @@ def run_ours(args, rank, world, local_rank):
 
     # what MPR_PATH_AUTO resolves to (csrc/mpr.cu, eff_path)
     def auto_path(md, schedule):
-        if schedule == "SITE_FUSED":
+        if schedule == "SITE_FUSED" and md != "HP":
             return "LIST" if (c.f < 0.5 and L <= 4096) else "STRIP"
+        if md == "HP":
+            return "STRIP" if L >= 4096 else "PLAIN"
         return "STRIP" if (md == "SP_INTRINSIC" and L >= 4096) else "TILED"
     path_used = auto_path(mode, args.schedule) if args.path == "AUTO" else args.path
     k_eff = min(args.fused, 2) if path_used == "STRIP" else args.fused
@@ -332,7 +334,7 @@ def run_ours(args, rank, world, local_rank):
         """Ceilings of one sweep launch of k hybrid sweeps.  Bytes per SURVEY.md 8(d): every spin read once and written
         once per LAUNCH at the paper's storage width w (4 B in the float-storage modes: one 32-bit angle; 8 B in DP),
         plus the mask bits; `state_bytes` is what this library's layout moves (a unit vector per spin: 2 w)."""
-        w = 8 if md == "DP" else 4
+        w = 8 if md == "DP" else 2 if md == "HP" else 4
         alg_bytes = 2.0 * N * w + N / 8.0
         state_bytes = 2.0 * N * 2 * w + N / 8.0
         units = N / 2.0                                             # one unit = 2 sites of one colour and row
@@ -386,8 +388,8 @@ def run_ours(args, rank, world, local_rank):
     # ---- per-mode sweep rates (BASELINE.json: "per precision mode"), both schedules --------------------------------
     modes = {}
     if not args.skip_modes:
-        for md, n_sw in (("DP", 10), ("SP", 10), ("SP_PRECISE", 30), ("SP_INTRINSIC", 30)):
-            if md not in c.modes:
+        for md, n_sw in (("DP", 10), ("SP", 10), ("SP_PRECISE", 30), ("SP_INTRINSIC", 30), ("HP", 30)):
+            if md not in c.modes and not (md == "HP" and "SP_INTRINSIC" in c.modes):     # HP: the paper's outlook, beside SSS
                 continue
             entry = {}
             for sched, k in (("R4", 1), ("SITE_FUSED", 2)):

@@ -5,6 +5,7 @@
 
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <limits>
 #include <new>
@@ -426,11 +427,15 @@ int do_strip(mpr_ctx* c, int prog, int k, int measure, double* d_e) {
 // schedule (which the TILED kernels do not carry); the TILED kernels otherwise (double arithmetic and the
 // library sincosf / expf of SP_PRECISE need more registers per update chain than four interleaved chains leave).
 int eff_path(const mpr_ctx* c) {
-  // half-precision storage runs on the per-pass kernels only (its TILED / STRIP instantiations
-  // raise an illegal-instruction fault on the B200 that has not been tracked down; they are compiled but not routed to)
-  if (c->mode == MPR_HP) return c->path == MPR_PATH_LIST ? MPR_PATH_LIST : MPR_PATH_PLAIN;
   // q < 1/2 (mpr_set_q): the general range test lives in the per-pass kernels only
   if (c->lo.g.q != kQDefault) return c->path == MPR_PATH_LIST ? MPR_PATH_LIST : MPR_PATH_PLAIN;
+  // half-precision storage: the TILED kernel's tile origins (60 tx - 2 plane columns) are not 16-byte aligned at
+  // 4 bytes per column, which the TMA unit requires; the STRIP kernels carry two halo lanes for it and take over
+  if (c->mode == MPR_HP) {
+    if (c->path == MPR_PATH_PLAIN || c->path == MPR_PATH_LIST) return c->path;
+    if (c->path == MPR_PATH_AUTO && c->lo.g.L < 4096) return MPR_PATH_PLAIN;
+    return MPR_PATH_STRIP;
+  }
   if (c->path != MPR_PATH_AUTO) return c->path;
   if (c->schedule == MPR_SCHEDULE_SITE_FUSED) {
     // small, sparsely masked grids: the compacted lists win (config 3, f = 0.33, L2-resident: 0.021 against 0.025 ms)

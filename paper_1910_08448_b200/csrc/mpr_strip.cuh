@@ -53,6 +53,12 @@ template <int PROG, int K> struct StripProg {
 
 __host__ __device__ constexpr int strip_halo_lanes(int ns) { return (ns + 3) / 4; }            // stale lanes per side after ns stages
 __host__ __device__ constexpr int strip_interior_cols(int ns) { return kTileCols - 4 * strip_halo_lanes(ns); }
+// Halo lanes of a MODE: the TMA unit wants every box row to start on a 16-byte boundary.  The first plane column of
+// a strip is strip * (64 - 4 HL) - 2 HL; with 8 or 16 bytes per plane column (float / double storage) any HL does, with
+// the 4 bytes of fp16 storage the column must be a multiple of 4, i.e. HL even: HP strips carry two halo lanes per side.
+template <int MODE> __host__ __device__ constexpr int strip_mode_halo_lanes(int ns) {
+  return (sizeof(decltype(Traits<MODE>::vec::x)) == 2 && strip_halo_lanes(ns) < 2) ? 2 : strip_halo_lanes(ns);
+}
 __host__ __device__ constexpr int strip_slots(int ns) { return (2 * ns + 1 + kStripRB - 1) / kStripRB + 1; }
 __host__ __device__ constexpr int strip_lead_rows(int ns) { return (ns + kStripRB - 1) / kStripRB * kStripRB; }   // rows loaded above a segment
 
@@ -111,7 +117,7 @@ strip_kernel(const __grid_constant__ CUtensorMap tmap, typename Traits<MODE>::ve
   using S = decltype(V::x);
   using P = StripProg<PROG, K>;
   constexpr int NS = P::NS, NW = StripCfg<MODE, NS>::NW, RB = kStripRB, LAG = kStripLag;
-  constexpr int NSLOT = strip_slots(NS), HL = strip_halo_lanes(NS), IC = strip_interior_cols(NS);
+  constexpr int NSLOT = strip_slots(NS), HL = strip_mode_halo_lanes<MODE>(NS), IC = kTileCols - 4 * HL;
   constexpr int LEAD = strip_lead_rows(NS);
   constexpr int CHUNK = 2 * RB * kRowScalars;          // scalars per chunk: [plane][row][128]
   constexpr int PLANE = RB * kRowScalars;
@@ -240,8 +246,8 @@ strip_kernel(const __grid_constant__ CUtensorMap tmap, typename Traits<MODE>::ve
             const Unit<S> mid = *reinterpret_cast<const Unit<S>*>(at(1 - col, rel));
             const Unit<S> dn = *reinterpret_cast<const Unit<S>*>(at(1 - col, rel + 1));
             const Unit<S> me = *reinterpret_cast<const Unit<S>*>(own[p]);
-            const S exc = par ? __shfl_down_sync(0xffffffffu, mid.ca, 1) : __shfl_up_sync(0xffffffffu, mid.cb, 1);
-            const S exs = par ? __shfl_down_sync(0xffffffffu, mid.sa, 1) : __shfl_up_sync(0xffffffffu, mid.sb, 1);
+            const S exc = par ? lane_dn(mid.ca) : lane_up(mid.cb);
+            const S exs = par ? lane_dn(mid.sa) : lane_up(mid.sb);
             combine_fields<MODE>(par, up, mid, dn, exc, exs, &A[p], &B[p]);
             c[p] = mk2(R(me.ca), R(me.cb));
             s[p] = mk2(R(me.sa), R(me.sb));
@@ -465,9 +471,10 @@ int strip_encode(TiledPlan& tp, const Geom& g, void* src, CUtensorMap* map) {
 // Otherwise the rows of all strips are laid end to end and cut into equal quotas, whatever the strip boundaries.
 // Fewer warps than slots when a warp would get fewer than 8 rows (a warp pays LEAD + 2 (NS - 1) + 3 warm-up / drain
 // steps per segment whatever its quota).
-inline StripGeom strip_geometry(const Geom& g, int ns, int nw, int sm_count, int* nblocks) {
+inline StripGeom strip_geometry(const Geom& g, int ns, int hl, int nw, int sm_count, int* nblocks) {
   StripGeom sg;
-  const int ic = strip_interior_cols(ns);
+  (void)ns;
+  const int ic = kTileCols - 4 * hl;
   sg.n_strips = (g.Wp + ic - 1) / ic;
   const int L4 = (g.L + 3) / 4 * 4;
   const long long slots = static_cast<long long>(sm_count) * nw;
@@ -508,9 +515,10 @@ int strip_launch_one(StripPlan& plan, const CUtensorMap& map, const Geom& g, voi
     attr_done = true;
   }
   int nblocks = 0;
-  const StripGeom sg = strip_geometry(g, NS, NW, plan.sm_count, &nblocks);
+  constexpr int HL = strip_mode_halo_lanes<MODE>(NS);
+  const StripGeom sg = strip_geometry(g, NS, HL, NW, plan.sm_count, &nblocks);
   if (MEASURE != 0 && nblocks > max_partials) return TILED_TOO_MANY;
-  strip_kernel<MODE, PROG, K, MEASURE><<<nblocks, NW * 32, smem, stream>>>(map, static_cast<V*>(dst), smask[strip_halo_lanes(NS) - 1], acc, part, slots,
+  strip_kernel<MODE, PROG, K, MEASURE><<<nblocks, NW * 32, smem, stream>>>(map, static_cast<V*>(dst), smask[HL - 1], acc, part, slots,
                                                                             g, kc, first_sweep, sg);
   if (const cudaError_t le = cudaGetLastError(); le != cudaSuccess) { tiled_last_cuda_error() = le; return TILED_LAUNCH; }
   *nblocks_out = nblocks;

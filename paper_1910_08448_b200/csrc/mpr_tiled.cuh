@@ -117,6 +117,12 @@ __device__ __forceinline__ void tma_load_3d(void* dst, const CUtensorMap* map, u
       : "memory");
 }
 
+// neighbour exchange between adjacent lanes; fp16 values travel as floats (exact both ways)
+template <typename S> __device__ __forceinline__ S lane_dn(S v) { return __shfl_down_sync(0xffffffffu, v, 1); }
+template <typename S> __device__ __forceinline__ S lane_up(S v) { return __shfl_up_sync(0xffffffffu, v, 1); }
+template <> __device__ __forceinline__ __half lane_dn<__half>(__half v) { return __float2half_rn(__shfl_down_sync(0xffffffffu, __half2float(v), 1)); }
+template <> __device__ __forceinline__ __half lane_up<__half>(__half v) { return __float2half_rn(__shfl_up_sync(0xffffffffu, __half2float(v), 1)); }
+
 template <int MODE> constexpr size_t tile_smem_bytes() {
   return sizeof(typename Traits<MODE>::vec) * (2 * TileCfg<MODE>::TH + 1) * kTileCols   // spins + one pad row
          + 64;                                                                            // mbarrier
@@ -175,8 +181,8 @@ __device__ __forceinline__ int row_step(int par, decltype(Traits<MODE>::vec::x)*
                                         bool row_odd, const ChainConst<typename Traits<MODE>::real>& kc) {
   using R = typename Traits<MODE>::real;
   using S = decltype(Traits<MODE>::vec::x);
-  const S exc = par ? __shfl_down_sync(0xffffffffu, mid.ca, 1) : __shfl_up_sync(0xffffffffu, mid.cb, 1);
-  const S exs = par ? __shfl_down_sync(0xffffffffu, mid.sa, 1) : __shfl_up_sync(0xffffffffu, mid.sb, 1);
+  const S exc = par ? lane_dn(mid.ca) : lane_up(mid.cb);
+  const S exs = par ? lane_dn(mid.sa) : lane_up(mid.sb);
   Two<R> A, B;
   combine_fields<MODE>(par, up, mid, dn, exc, exs, &A, &B);
   const Unit<S> me = *reinterpret_cast<const Unit<S>*>(own);
