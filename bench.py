@@ -48,6 +48,12 @@ CPU_ONE_CROP, CPU_ONE_SWEEPS = 2048, 3         # one thread: top-left 2048^2 win
 # measured cost per warp instruction and scheduler (tests/helpers/pipe_microbench.cu, profiles/r02_microbench.md):
 #   IMAD.WIDE.U32 4.27 cycles (inside a Philox block), FADD2 / FMUL2 2.03, FFMA2 2.34 -> packed average 2.1
 ALG_FMA_CYCLES_PER_UNIT_SWEEP = 10 * 4.27 + (21 + 19) * 2.1       # = 126.7 scheduler cycles
+# Double-arithmetic modes (DP, SP): the FP64 pipe carries the moves.  Per unit and sweep 210 FP64-pipe instructions
+# (DFMA / DMUL / DADD / DSETP / I2F.F64: two Philox-to-double conversions and the branch-free sincos / exp polynomials of the
+# Metropolis move, the Newton-free reflection with one division of the over-relaxation move, the local fields; counted in the
+# SASS of the move functions: 857 in the eight unit-passes of tiled_sweep_kernel<DP, 0>), at the measured 3.28 cycles per
+# warp instruction and scheduler (DFMA 1.22 per clock and SM, profiles/r02_microbench.md).
+ALG_FP64_CYCLES_PER_UNIT_SWEEP = 210 * 3.28
 SMS, SCHEDULERS = 148, 4
 # dram__bytes_read.sum + dram__bytes_write.sum of one launch at L = 16384 from the committed `ncu --set full` captures
 # (profiles/); None for configurations not captured.
@@ -73,6 +79,7 @@ def parse():
     ap.add_argument("--skip-cpu-baseline", action="store_true")
     ap.add_argument("--skip-modes", action="store_true")
     ap.add_argument("--skip-e2e", action="store_true")
+    ap.add_argument("--skip-fused-leg", action="store_true", help="do not time the same step under the site-fused schedule")
     ap.add_argument("--matrix", action="store_true",
                     help="the paper's experiment shape (PAPER.md:35-57): R_X = t_DDD / t_X for the eight (X_S X_E X_F) settings "
                          "at L = 2^5 .. 2^12, f = 0.9, kappa = 0.2, and Delta MAAE_X over M mask realisations; one JSON line")
@@ -284,6 +291,40 @@ def run_ours(args, rank, world, local_rank):
         ms, 2.0 * state["n_free"] * state["sweeps"], state["launches"], world, device=dev)
     value = sharding.throughput(units_total, ms_max)
 
+    # ---- the same step under the site-fused schedule (R4b), two sweeps per launch: reported beside the headline ------
+    fused_leg = None
+    if args.schedule == "R4" and not args.skip_fused_leg and mode in ("SP_INTRINSIC", "HP"):
+        def fused_step():
+            gf = mpr.Mpr(d_values, d_mask, mode=mode, seed=seed, device=dev)
+            gf.set_schedule("SITE_FUSED")
+            gf.set_fused_sweeps(2)
+            if args.temperature is not None:
+                gf.set_temperature(args.temperature)
+                nt = 0
+            else:
+                _, _, nt = gf.estimate_temperature()
+            pf, ef, sef = gf.run(n_eq, n_meas)
+            ms_eq, n_l, n_sw = gf.run_timing()
+            gf.close()
+            return nt * 250 + n_eq + n_meas, pf, ef, sef, ms_eq, n_sw
+        fused_step()
+        barrier()
+        f0, f1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        f0.record()
+        sw_f, eq_ms_f, eq_sw_f = 0, 0.0, 0
+        for _ in range(args.steps):
+            n_sw_step, pred_f, e_f, se_f, ms_eq, n_sw = fused_step()
+            sw_f += n_sw_step
+            eq_ms_f += ms_eq
+            eq_sw_f += n_sw
+        f1.record()
+        barrier()
+        msf_max, units_f, _ = sharding.aggregate(f0.elapsed_time(f1), 2.0 * state["n_free"] * sw_f, 0, world, device=dev)
+        dfz = (pred_f - d_truth)[d_mask.bool()]
+        fused_leg = {"value": sharding.throughput(units_f, msf_max), "unit": UNIT, "ms_per_step": msf_max / args.steps,
+                     "schedule": "SITE_FUSED", "sweeps_per_launch": 2, "ms_per_sweep_in_step": eq_ms_f / max(eq_sw_f, 1),
+                     "e_mean": e_f, "e_stderr": se_f, "mae": float(dfz.abs().mean().item())}
+
     # prediction error of the last step (metric of PAPER.md Eq. 4; post-processing, not the path)
     m1 = d_mask.bool()
     diff = (state["pred"] - d_truth)[m1]
@@ -337,7 +378,8 @@ def run_ours(args, rank, world, local_rank):
         w = 8 if md == "DP" else 2 if md == "HP" else 4
         alg_bytes = 2.0 * N * w + N / 8.0
         state_bytes = 2.0 * N * 2 * w + N / 8.0
-        units = N / 2.0                                             # one unit = 2 sites of one colour and row
+        # one unit = 2 sites of one colour and row; the method's arithmetic is owed at the PREDICTION sites only
+        units = state["n_free"] / 2.0
         fma_cycles = units / 32.0 * k * ALG_FMA_CYCLES_PER_UNIT_SWEEP   # scheduler cycles on the FMA-heavy pipe
         fma_peak = SMS * SCHEDULERS * sm_mhz_used * 1e6             # scheduler cycles per second at the sampled clock
         t = ms_launch * 1e-3
@@ -347,7 +389,12 @@ def run_ours(args, rank, world, local_rank):
             "hbm_state_layout": {"bytes_per_launch": state_bytes, "achieved_gb_s": state_bytes / t / 1e9,
                                  "frac": state_bytes / t / 1e9 / peak, "lower_bound_ms": state_bytes / (peak * 1e9) * 1e3},
         }
-        if md in ("SP_INTRINSIC", "SP_PRECISE"):
+        if md in ("DP", "SP"):
+            cyc = units / 32.0 * k * ALG_FP64_CYCLES_PER_UNIT_SWEEP
+            out["fp64_pipe"] = {"cycles_per_launch": cyc, "achieved_cycles_per_s": cyc / t, "peak_cycles_per_s": fma_peak,
+                                "frac": cyc / t / fma_peak, "lower_bound_ms": cyc / fma_peak * 1e3, "sm_mhz": sm_mhz_used,
+                                "cycles_per_unit_sweep": ALG_FP64_CYCLES_PER_UNIT_SWEEP}
+        if md in ("SP_INTRINSIC", "SP_PRECISE", "HP"):
             out["fma_pipe"] = {"cycles_per_launch": fma_cycles, "achieved_cycles_per_s": fma_cycles / t,
                                "peak_cycles_per_s": fma_peak, "frac": fma_cycles / t / fma_peak,
                                "lower_bound_ms": fma_cycles / fma_peak * 1e3, "sm_mhz": sm_mhz_used,
@@ -356,12 +403,12 @@ def run_ours(args, rank, world, local_rank):
 
     ceil = ceilings(mode, kern_ms, k_eff, sm_mhz)
     # the binding ceiling = the one with the largest lower-bound time among those computed from ALGORITHMIC work
-    binding = "alu" if "fma_pipe" in ceil and ceil["fma_pipe"]["lower_bound_ms"] > ceil["hbm_algorithmic"]["lower_bound_ms"] \
-        else "hbm"
+    pipe_key = "fma_pipe" if "fma_pipe" in ceil else "fp64_pipe" if "fp64_pipe" in ceil else None
+    binding = "alu" if pipe_key and ceil[pipe_key]["lower_bound_ms"] > ceil["hbm_algorithmic"]["lower_bound_ms"] else "hbm"
     if binding == "alu":
-        fp = ceil["fma_pipe"]
+        fp = ceil[pipe_key]
         roofline = {"bound": "alu", "achieved": fp["achieved_cycles_per_s"], "peak": fp["peak_cycles_per_s"],
-                    "unit": "FMA-pipe scheduler cycles/s", "frac": fp["frac"],
+                    "unit": ("FMA-pipe" if pipe_key == "fma_pipe" else "FP64-pipe") + " scheduler cycles/s", "frac": fp["frac"],
                     "peak_source": "148 SMs x 4 schedulers x SM clock sampled during the timed steps (%.0f MHz); "
                                    "instruction costs measured by tests/helpers/pipe_microbench.cu "
                                    "(profiles/r02_microbench.md)" % sm_mhz,
@@ -400,7 +447,8 @@ def run_ours(args, rank, world, local_rank):
                                 "ms_per_measurement_sweep": t_meas,
                                 "frac_hbm_algorithmic": cl["hbm_algorithmic"]["frac"],
                                 "frac_hbm_state_layout": cl["hbm_state_layout"]["frac"],
-                                "frac_fma_pipe": cl.get("fma_pipe", {}).get("frac")}
+                                "frac_fma_pipe": cl.get("fma_pipe", {}).get("frac"),
+                                "frac_fp64_pipe": cl.get("fp64_pipe", {}).get("frac")}
             modes[md] = entry
 
     # ---- end to end through the C ABI with HOST buffers (mpr_predict_host) ---------------------
@@ -453,7 +501,7 @@ def run_ours(args, rank, world, local_rank):
                        "l2": ("state (%.2f GiB) larger than the 126 MB L2; no flush" % (state_gib)) if state_gib * 2 ** 30 > 126e6
                              else "state (%.1f MiB) is L2-resident by design of this config (BASELINE.json); no flush" % (state_gib * 1024)},
             "clocks": clk, "e2e": e2e, "gpu_launches": launches_total, "roofline": roofline,
-            "cpu_baseline": cpu, "modes": modes, "T_hat": T_hat, "e_sample": state.get("e_sample"),
+            "cpu_baseline": cpu, "modes": modes, "site_fused": fused_leg, "T_hat": T_hat, "e_sample": state.get("e_sample"),
             "e_mean": state["e"], "e_stderr": state["se"], "mae": mae, "rmse": rmse,
             "mae_of_sample_mean_predictor": base_mae, "input_generation_s": t_gen,
         }))
