@@ -68,9 +68,13 @@ __host__ __device__ constexpr int strip_lead_rows(int ns) { return (ns + kStripR
 // site-fused schedule, one sweep per launch: 12 warps 1.07 ms, 16 warps 0.78 ms per sweep; a 4-stage program
 // squeezed into 128 registers for 13 warps: 1.11 against 0.98 ms).  The ring of a warp is 16.5 KiB with float
 // storage and NS = 4, 33 KiB in DP.
-template <int MODE, int NS> struct StripCfg {
-  static constexpr int kRingBytes = strip_slots(NS) * (2 * kStripRB * 2 * kTileCols * static_cast<int>(sizeof(decltype(Traits<MODE>::vec::x))) + 128 + 8);
-  static constexpr int kFit = (216 * 1024) / kRingBytes;
+// Launches that accumulate phi (MEASURE == 2) add 2 KiB of accumulator staging per warp (kAccStageBytes) and may
+// fill the 227 KiB of a CTA to the last KiB: 12 warps for NS = 4, 15 for NS = 2 with float storage.
+constexpr int kAccStageBytes = 2 * 2 * 32 * 16;
+template <int MODE, int NS, int MEASURE = 0> struct StripCfg {
+  static constexpr int kRingBytes = strip_slots(NS) * (2 * kStripRB * 2 * kTileCols * static_cast<int>(sizeof(decltype(Traits<MODE>::vec::x))) + 128 + 8) +
+                                    (MEASURE == 2 ? kAccStageBytes : 0);
+  static constexpr int kFit = (MEASURE == 2 ? 232448 - 256 - 128 : 216 * 1024) / kRingBytes;
   static constexpr int kMax = (NS <= 2 && sizeof(typename Traits<MODE>::real) == 4) ? 16 : 12;
   static constexpr int NW = kFit < kMax ? kFit : kMax;
 };
@@ -93,12 +97,35 @@ constexpr int kStripMaskLead = 8;      // rows (two chunks) above the grid
 constexpr int kStripMaskTail = 32;     // rows below it
 __host__ __device__ constexpr int strip_mask_chunks(int L) { return ((L + 3) / 4 * 4 + kStripMaskLead + kStripMaskTail) / kStripRB; }
 
-template <int MODE, int NS> constexpr size_t strip_smem_bytes() {
+// Measuring launches that accumulate phi (MEASURE == 2) stage the accumulator words of the NEXT step through shared
+// memory (cp.async, two buffers of 2 rows x 32 lanes x 16 bytes per warp): a whole step hides the DRAM latency
+// without holding registers.
+template <int MODE, int NS, int MEASURE = 0> constexpr size_t strip_smem_bytes() {
   using S = decltype(Traits<MODE>::vec::x);
-  return static_cast<size_t>(StripCfg<MODE, NS>::NW) * strip_slots(NS) * (2 * kStripRB * kRowScalars * sizeof(S) + 128 + sizeof(uint64_t)) + 128;
+  return static_cast<size_t>(StripCfg<MODE, NS, MEASURE>::NW) *
+             (strip_slots(NS) * (2 * kStripRB * kRowScalars * sizeof(S) + 128 + sizeof(uint64_t)) + (MEASURE == 2 ? kAccStageBytes : 0)) + 128;
 }
 
 __device__ __forceinline__ void fence_proxy_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+// Arming a slot's mbarrier publishes nothing (the data arrives through complete_tx and the waiter acquires): the
+// default .release of mbarrier.arrive costs a MEMBAR.ALL.CTA that waits for the warp's global stores.
+__device__ __forceinline__ void mbar_expect_tx_relaxed(uint64_t* bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.relaxed.cta.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+// One lane of the (converged) warp; unlike `lane == 0` the compiler knows the branch is taken by one thread of a
+// uniform warp and issues the TMA instructions from uniform registers without a broadcast loop.
+__device__ __forceinline__ bool elect_one() {
+  uint32_t pred;
+  asm volatile("{\n.reg .pred p;\nelect.sync _|p, 0xffffffff;\nselp.u32 %0, 1, 0, p;\n}\n" : "=r"(pred));
+  return pred != 0u;
+}
+// 16-byte asynchronous copy global -> shared (SASS LDGSTS), skipped when `pred` is false; groups are per thread
+__device__ __forceinline__ void cp_async_16(void* dst_smem, const void* src, bool pred) {
+  asm volatile("{\n.reg .pred p;\nsetp.ne.b32 p, %2, 0;\n@p cp.async.cg.shared.global [%0], [%1], 16;\n}\n"
+               ::"r"(smem_u32(dst_smem)), "l"(src), "r"(static_cast<int>(pred)) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
 // 1-D bulk copy global -> shared, completion counted on an mbarrier (SASS UBLKCP)
 __device__ __forceinline__ void bulk_load_1d(void* dst, const void* src, uint32_t bytes, uint64_t* bar) {
   asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
@@ -107,7 +134,7 @@ __device__ __forceinline__ void bulk_load_1d(void* dst, const void* src, uint32_
 
 // MEASURE: 0 = none; 1 = + energy sample after the last stage; 2 = + accumulation of phi (R15)
 template <int MODE, int PROG, int K, int MEASURE>
-__global__ void __launch_bounds__(StripCfg<MODE, StripProg<PROG, K>::NS>::NW * 32, 1)
+__global__ void __launch_bounds__(StripCfg<MODE, StripProg<PROG, K>::NS, MEASURE>::NW * 32, 1)
 strip_kernel(const __grid_constant__ CUtensorMap tmap, typename Traits<MODE>::vec* __restrict__ dst,
              const uint32_t* __restrict__ smask, double* __restrict__ acc, double* __restrict__ part,
              unsigned long long* __restrict__ accept_slots, Geom g, ChainConst<typename Traits<MODE>::real> kc,
@@ -116,7 +143,7 @@ strip_kernel(const __grid_constant__ CUtensorMap tmap, typename Traits<MODE>::ve
   using V = typename Traits<MODE>::vec;
   using S = decltype(V::x);
   using P = StripProg<PROG, K>;
-  constexpr int NS = P::NS, NW = StripCfg<MODE, NS>::NW, RB = kStripRB, LAG = kStripLag;
+  constexpr int NS = P::NS, NW = StripCfg<MODE, NS, MEASURE>::NW, RB = kStripRB, LAG = kStripLag;
   constexpr int NSLOT = strip_slots(NS), HL = strip_mode_halo_lanes<MODE>(NS), IC = kTileCols - 4 * HL;
   constexpr int LEAD = strip_lead_rows(NS);
   constexpr int CHUNK = 2 * RB * kRowScalars;          // scalars per chunk: [plane][row][128]
@@ -136,9 +163,19 @@ strip_kernel(const __grid_constant__ CUtensorMap tmap, typename Traits<MODE>::ve
   unsigned char* const after_rings = smem_raw + static_cast<size_t>(NW) * NSLOT * CHUNK * sizeof(S);
   uint32_t* const mring = reinterpret_cast<uint32_t*>(after_rings) + warp * NSLOT * 32;          // 128 B of mask per slot
   uint64_t* const bars = reinterpret_cast<uint64_t*>(after_rings + static_cast<size_t>(NW) * NSLOT * kMaskBytes) + warp * NSLOT;
+  // accumulator staging (MEASURE == 2): [buffer = step parity][final stage 0 / 1][lane] double2
+  double2* const astage = reinterpret_cast<double2*>(after_rings + ((static_cast<size_t>(NW) * NSLOT * (kMaskBytes + sizeof(uint64_t)) + 15) & ~size_t(15))) +
+                          warp * (kAccStageBytes / 16) + lane;
+  (void)astage;
 
   int n_acc = 0;
+  // per-thread energy sum: X_E = D in `esum`, X_E = S (every partial sum a float) in `esum_f` -- the same values as
+  // energy_add gives, without its per-term conversions both ways
   double esum = 0.0;
+  float esum_f = 0.0f;
+  auto energy_term = [&](double term) {
+    if (g.energy_single) esum_f = esum_f + static_cast<float>(term); else esum = esum + term;
+  };
   const int wg = warp * static_cast<int>(gridDim.x) + static_cast<int>(blockIdx.x);
   if (wg < sg.n_warps) {
     if (lane == 0) {
@@ -176,9 +213,9 @@ strip_kernel(const __grid_constant__ CUtensorMap tmap, typename Traits<MODE>::ve
       __syncwarp();
       // this strip's mask blocks; block of the chunk whose first row is t0 + 4 c: index (t0 + lead) / 4 + c
       const uint32_t* const mblk = smask + (static_cast<size_t>(strip) * sg.n_mchunks + (t0 + kStripMaskLead) / RB) * 32;
-      if (lane == 0) {                                        // chunk 0 -> slot 0
+      if (elect_one()) {                                      // chunk 0 -> slot 0
         fence_proxy_async_smem();
-        mbar_expect_tx(bars, kChunkBytes);
+        mbar_expect_tx_relaxed(bars, kChunkBytes);
         tma_load_3d(ring, &tmap, bars, (sizeof(S) == 2 ? 1 : 2) * j0, t0, 0);
         bulk_load_1d(mring, mblk, kMaskBytes, bars);
       }
@@ -208,9 +245,9 @@ strip_kernel(const __grid_constant__ CUtensorMap tmap, typename Traits<MODE>::ve
         constexpr bool EDGE = decltype(edge_tag)::value;
         // prefetch chunk i + 1 into the slot whose old chunk (i + 1 - NSLOT) nobody reads any more
         __syncwarp();
-        if (lane == 0) {
+        if (elect_one()) {
           fence_proxy_async_smem();
-          mbar_expect_tx(bars + slot_next, kChunkBytes);
+          mbar_expect_tx_relaxed(bars + slot_next, kChunkBytes);
           tma_load_3d(ring + cb[NSLOT - 1], &tmap, bars + slot_next, (sizeof(S) == 2 ? 1 : 2) * j0, t0 + RB * (i + 1), 0);
           bulk_load_1d(mring + slot_next * 32, mblk + static_cast<size_t>(i + 1) * 32, kMaskBytes, bars + slot_next);
         }
@@ -256,22 +293,17 @@ strip_kernel(const __grid_constant__ CUtensorMap tmap, typename Traits<MODE>::ve
             }
           }
 
-          // measuring launches: the accumulator words of the two rows that become final in this step are
-          // requested now and used at the end of the step (their latency hides behind the arithmetic)
-          double2 acc_pre[2];
+          // measuring launches: the accumulator words of the two rows that become final in the NEXT step are requested
+          // now (cp.async into the other staging buffer); this step's words were requested one step ago
           if constexpr (MEASURE == 2) {
 #pragma unroll
             for (int p = NS - 2; p < NS; ++p) {
-              const int col = p & 1, row = t - LAG * p;
-              const int rel = u - LAG * p;
-              const int mqk = (rel >= 0) ? 0 : (-rel + RB - 1) / RB;
-              const uint32_t mm = (cw[mqk] >> (4 * (rel + mqk * RB) + 2 * col)) & 3u;
-              const bool owned = lane_ok && (!EDGE || (row >= yb && row < ye));
-              acc_pre[p - (NS - 2)] = make_double2(0.0, 0.0);
-              if (owned && mm)
-                acc_pre[p - (NS - 2)] = *reinterpret_cast<const double2*>(
-                    ap - static_cast<long long>(LAG * p) * g.Wp + static_cast<long long>(col) * static_cast<long long>(g.plane));
+              const int col = p & 1, row_next = t + 1 - LAG * p;
+              cp_async_16(astage + (((u + 1) & 1) * 2 + (p - (NS - 2))) * 32,
+                          ap + static_cast<long long>(1 - LAG * p) * g.Wp + static_cast<long long>(col) * static_cast<long long>(g.plane),
+                          lane_ok && row_next >= yb && row_next < ye);
             }
+            cp_async_commit();
           }
 
           // ---- compute
@@ -329,7 +361,8 @@ strip_kernel(const __grid_constant__ CUtensorMap tmap, typename Traits<MODE>::ve
             Unit<S> out;
             out.ca = static_cast<S>(o[p][0]); out.cb = static_cast<S>(o[p][1]);
             out.sa = static_cast<S>(o[p][2]); out.sb = static_cast<S>(o[p][3]);
-            if (!EDGE || n >= LAG * p) *reinterpret_cast<Unit<S>*>(own[p]) = out;       // rows above t0 do not exist
+            // rows above t0 do not exist; nobody reads the ring copy of the last stage's row (it is final: global only)
+            if (p < NS - 1 && (!EDGE || n >= LAG * p)) *reinterpret_cast<Unit<S>*>(own[p]) = out;
             if (p >= NS - 2) {                                                            // last stage of this colour
               const bool owned = lane_ok && (!EDGE || (row >= yb && row < ye));
               if (owned) {
@@ -340,7 +373,8 @@ strip_kernel(const __grid_constant__ CUtensorMap tmap, typename Traits<MODE>::ve
                   const uint32_t mm = (cw[mqk] >> (4 * (rel + mqk * RB) + 2 * col)) & 3u;
                   if (mm) {
                     double* a = ap - static_cast<long long>(LAG * p) * g.Wp + static_cast<long long>(col) * static_cast<long long>(g.plane);
-                    double2 a2 = acc_pre[p - (NS - 2)];
+                    cp_async_wait<1>();                       // everything but the group of the next step has landed
+                    double2 a2 = astage[((u & 1) * 2 + (p - (NS - 2))) * 32];
                     // from the spins AS STORED (SP: rounded to float), like the other paths
                     if (mm & 1u) a2.x += spin_angle<MODE>(R(out.ca), R(out.sa));
                     if (mm & 2u) a2.y += spin_angle<MODE>(R(out.cb), R(out.sb));
@@ -353,18 +387,18 @@ strip_kernel(const __grid_constant__ CUtensorMap tmap, typename Traits<MODE>::ve
                   if constexpr (sizeof(R) == 8) {
                     R Aa, Ab, Ba, Bb;
                     un2(A[p], &Aa, &Ab); un2(B[p], &Ba, &Bb);
-                    energy_add(esum, static_cast<double>(fma_(R(out.ca), Aa, R(out.sa) * Ba)), g.energy_single);
-                    energy_add(esum, static_cast<double>(fma_(R(out.cb), Ab, R(out.sb) * Bb)), g.energy_single);
+                    energy_term(static_cast<double>(fma_(R(out.ca), Aa, R(out.sa) * Ba)));
+                    energy_term(static_cast<double>(fma_(R(out.cb), Ab, R(out.sb) * Bb)));
                   } else {
                     const int par = (u + col) & 1;
                     const R alc = par ? R(nb_m.ca) : R(exc_last), als = par ? R(nb_m.sa) : R(exs_last);
                     const R arc = par ? R(nb_m.cb) : R(nb_m.ca), ars = par ? R(nb_m.sb) : R(nb_m.sa);
                     const R blc = par ? R(nb_m.cb) : R(nb_m.ca), bls = par ? R(nb_m.sb) : R(nb_m.sa);
                     const R brc = par ? R(exc_last) : R(nb_m.cb), brs = par ? R(exs_last) : R(nb_m.sb);
-                    energy_add(esum, site_energy_term<R>(R(out.ca), R(out.sa), alc, als, arc, ars, R(nb_u.ca), R(nb_u.sa),
-                                                         R(nb_d.ca), R(nb_d.sa)), g.energy_single);
-                    energy_add(esum, site_energy_term<R>(R(out.cb), R(out.sb), blc, bls, brc, brs, R(nb_u.cb), R(nb_u.sb),
-                                                         R(nb_d.cb), R(nb_d.sb)), g.energy_single);
+                    energy_term(site_energy_term<R>(R(out.ca), R(out.sa), alc, als, arc, ars, R(nb_u.ca), R(nb_u.sa),
+                                                         R(nb_d.ca), R(nb_d.sa)));
+                    energy_term(site_energy_term<R>(R(out.cb), R(out.sb), blc, bls, brc, brs, R(nb_u.cb), R(nb_u.sb),
+                                                         R(nb_d.cb), R(nb_d.sb)));
                   }
                 }
               }
@@ -394,7 +428,7 @@ strip_kernel(const __grid_constant__ CUtensorMap tmap, typename Traits<MODE>::ve
     }
   }
   if constexpr (MEASURE != 0) {
-    const double e = block_sum(esum, red, g.energy_single);
+    const double e = block_sum(g.energy_single ? static_cast<double>(esum_f) : esum, red, g.energy_single);
     if (threadIdx.x == 0) part[blockIdx.x] = e;
   }
   if constexpr (PROG != PROG_QUENCH) {
@@ -505,8 +539,9 @@ int strip_launch_one(StripPlan& plan, const CUtensorMap& map, const Geom& g, voi
                      double* part, unsigned long long* slots, const ChainConst<typename Traits<MODE>::real>& kc,
                      uint32_t first_sweep, cudaStream_t stream, int* nblocks_out, long long max_partials) {
   using V = typename Traits<MODE>::vec;
-  constexpr int NS = StripProg<PROG, K>::NS, NW = StripCfg<MODE, NS>::NW;
-  constexpr size_t smem = strip_smem_bytes<MODE, NS>();
+  constexpr int NS = StripProg<PROG, K>::NS, NW = StripCfg<MODE, NS, MEASURE>::NW;
+  constexpr size_t smem = strip_smem_bytes<MODE, NS, MEASURE>();
+  static_assert(smem <= 232448 - 256, "dynamic + static shared memory of one CTA");
   static bool attr_done = false;
   if (!attr_done) {
     if (cudaFuncSetAttribute(strip_kernel<MODE, PROG, K, MEASURE>, cudaFuncAttributeMaxDynamicSharedMemorySize,
