@@ -347,12 +347,14 @@ def run_ours(args, rank, world, local_rank):
         k1.record()
         torch.cuda.synchronize(dev)
         ms_launch = k0.elapsed_time(k1) / n_launch
+        gk.run(0, 2, want_pred=False)      # first use of the measuring kernel (lazy module load) stays outside
+        torch.cuda.synchronize(dev)
         k0.record()
-        gk.run(0, 5, want_pred=False)
+        gk.run(0, 10, want_pred=False)
         k1.record()
         torch.cuda.synchronize(dev)
         gk.close()
-        return ms_launch, k0.elapsed_time(k1) / 5
+        return ms_launch, k0.elapsed_time(k1) / 10
 
     # what MPR_PATH_AUTO resolves to (csrc/mpr.cu, eff_path)
     def auto_path(md, schedule):

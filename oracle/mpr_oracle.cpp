@@ -84,7 +84,8 @@ double u53(uint32_t a, uint32_t b) {
 }
 
 struct Oracle {
-  int L = 0;
+  int L = 0;                    // columns (x)
+  int H = 0;                    // rows (y); == L unless the grid is rectangular (orc_create_rect)
   std::vector<double> z;        // input values, row-major s = y*L + x
   std::vector<uint8_t> mask;    // 1 = prediction ("free") site, 0 = measured
   std::vector<double> phi;      // spins
@@ -103,24 +104,24 @@ struct Oracle {
   long n_acc = 0;
   int est_trials = 0;
 
-  size_t N() const { return static_cast<size_t>(L) * L; }
+  size_t N() const { return static_cast<size_t>(L) * H; }
 };
 
 // Neighbour list of (x,y) in the fixed order left, right, up, down; open boundaries (R2).
-inline int neighbours(int L, int x, int y, size_t nb[4]) {
+inline int neighbours(int L, int H, int x, int y, size_t nb[4]) {
   int n = 0;
   const size_t s = static_cast<size_t>(y) * L + x;
   if (x > 0)     nb[n++] = s - 1;
   if (x < L - 1) nb[n++] = s + 1;
   if (y > 0)     nb[n++] = s - L;
-  if (y < L - 1) nb[n++] = s + L;
+  if (y < H - 1) nb[n++] = s + L;
   return n;
 }
 
 // E_loc(phi_s) = -J sum_j cos(q (phi_s - phi_j))  (the part of Eq. 2 that contains site s)
 double local_energy(const Oracle& o, int x, int y, double phi_s) {
   size_t nb[4];
-  const int n = neighbours(o.L, x, y, nb);
+  const int n = neighbours(o.L, o.H, x, y, nb);
   double sum = 0.0;
   for (int k = 0; k < n; ++k) sum += std::cos(o.q * (phi_s - o.phi[nb[k]]));
   return -kJ * sum;
@@ -155,7 +156,7 @@ void met_pass(Oracle& o, int c, uint64_t n) {
   const uint32_t key[2] = {static_cast<uint32_t>(o.seed), static_cast<uint32_t>(o.seed >> 32)};
   uint64_t acc = 0, att = 0;
 #pragma omp parallel for schedule(static) reduction(+ : acc, att) num_threads(o.threads)
-  for (int y = 0; y < L; ++y) {
+  for (int y = 0; y < o.H; ++y) {
     for (int x = (y + c) & 1; x < L; x += 2) {
       const size_t s = static_cast<size_t>(y) * L + x;
       if (!o.mask[s]) continue;
@@ -169,7 +170,7 @@ void met_pass(Oracle& o, int c, uint64_t n) {
       const double phi_new = phi_old + delta * (2.0 * u1 - 1.0);
       if (phi_new < 0.0 || phi_new > kTwoPi) continue;            // outside [0,2pi]: reject
       size_t nb[4];
-      const int nn = neighbours(L, x, y, nb);
+      const int nn = neighbours(L, o.H, x, y, nb);
       double diff = 0.0;
       for (int k = 0; k < nn; ++k) {
         const double pj = o.phi[nb[k]];
@@ -189,7 +190,7 @@ void met_pass(Oracle& o, int c, uint64_t n) {
 // Neighbour field of a site: A = sum_j cos(q phi_j), B = sum_j sin(q phi_j).
 inline void field(const Oracle& o, int x, int y, double& A, double& B) {
   size_t nb[4];
-  const int nn = neighbours(o.L, x, y, nb);
+  const int nn = neighbours(o.L, o.H, x, y, nb);
   A = 0.0; B = 0.0;
   const double kQ = o.q;
   for (int k = 0; k < nn; ++k) {
@@ -204,7 +205,7 @@ void or_pass(Oracle& o, int c) {
   const int L = o.L;
   const double kQ = o.q;
 #pragma omp parallel for schedule(static) num_threads(o.threads)
-  for (int y = 0; y < L; ++y) {
+  for (int y = 0; y < o.H; ++y) {
     for (int x = (y + c) & 1; x < L; x += 2) {
       const size_t s = static_cast<size_t>(y) * L + x;
       if (!o.mask[s]) continue;
@@ -224,7 +225,7 @@ void quench_pass(Oracle& o, int c) {
   const int L = o.L;
   const double kQ = o.q;
 #pragma omp parallel for schedule(static) num_threads(o.threads)
-  for (int y = 0; y < L; ++y) {
+  for (int y = 0; y < o.H; ++y) {
     for (int x = (y + c) & 1; x < L; x += 2) {
       const size_t s = static_cast<size_t>(y) * L + x;
       if (!o.mask[s]) continue;
@@ -270,7 +271,7 @@ void reset_chain(Oracle& o, uint32_t trial) {
 }
 
 // H = -J sum over right and down bonds of cos(q (phi_s - phi_t)), open boundaries;
-// e = 2 H / N_b with N_b = 2 L (L-1) bonds (R3).  Neumaier-compensated sum.
+// e = 2 H / N_b with N_b = Lx (Ly - 1) + Ly (Lx - 1) bonds, 2 L (L-1) on the paper's square grid (R3).  Neumaier-compensated sum.
 void energy(const Oracle& o, double* H_out, double* e_out) {
   const int L = o.L;
   const double kQ = o.q;
@@ -280,14 +281,14 @@ void energy(const Oracle& o, double* H_out, double* e_out) {
     if (std::fabs(sum) >= std::fabs(v)) comp += (sum - t) + v; else comp += (v - t) + sum;
     sum = t;
   };
-  for (int y = 0; y < L; ++y)
+  for (int y = 0; y < o.H; ++y)
     for (int x = 0; x < L; ++x) {
       const size_t s = static_cast<size_t>(y) * L + x;
       if (x < L - 1) add(std::cos(kQ * (o.phi[s] - o.phi[s + 1])));
-      if (y < L - 1) add(std::cos(kQ * (o.phi[s] - o.phi[s + L])));
+      if (y < o.H - 1) add(std::cos(kQ * (o.phi[s] - o.phi[s + L])));
     }
   const double H = -kJ * (sum + comp);
-  const double nb = 2.0 * L * (L - 1.0);
+  const double nb = static_cast<double>(L) * (o.H - 1.0) + static_cast<double>(o.H) * (L - 1.0);   // 2 L (L - 1) on a square grid
   if (H_out) *H_out = H;
   if (e_out) *e_out = 2.0 * H / nb;
 }
@@ -298,12 +299,12 @@ int sample_energy(const Oracle& o, double* es, long long* nsp) {
   const double kQ = o.q;
   double sum = 0.0;
   long long cnt = 0;
-  for (int y = 0; y < L; ++y)
+  for (int y = 0; y < o.H; ++y)
     for (int x = 0; x < L; ++x) {
       const size_t s = static_cast<size_t>(y) * L + x;
       if (o.mask[s]) continue;
       if (x < L - 1 && !o.mask[s + 1]) { sum += std::cos(kQ * (o.phi[s] - o.phi[s + 1])); ++cnt; }
-      if (y < L - 1 && !o.mask[s + L]) { sum += std::cos(kQ * (o.phi[s] - o.phi[s + L])); ++cnt; }
+      if (y < o.H - 1 && !o.mask[s + L]) { sum += std::cos(kQ * (o.phi[s] - o.phi[s + L])); ++cnt; }
     }
   if (nsp) *nsp = cnt;
   if (cnt == 0) return ERR_NO_MEASURED;
@@ -452,21 +453,29 @@ void orc_mean_stderr(const double* v, long n, double* mean, double* se) {
 
 // O0 (R1): phi = 2pi (z - zmin)/(zmax - zmin), min/max over the measured sample.
 // mask[s] = 1 -> prediction site (value never read).  Returns a handle or null + status.
-static void* create_impl(int L, const double* values, const uint8_t* mask, int* status, bool reset);
+static void* create_impl(int L, int H, const double* values, const uint8_t* mask, int* status, bool reset);
 void* orc_create(int L, const double* values, const uint8_t* mask, int* status) {
-  return create_impl(L, values, mask, status, true);
+  return create_impl(L, L, values, mask, status, true);
+}
+// Rectangular grid of Lx columns and Ly rows (row-major, s = y Lx + x): nothing in the method depends on the
+// grid being square (nearest neighbours on a regular grid); only the bond count of R3 changes.
+void* orc_create_rect(int Lx, int Ly, const double* values, const uint8_t* mask, int* status) {
+  return create_impl(Lx, Ly, values, mask, status, true);
+}
+void* orc_create_rect_deferred(int Lx, int Ly, const double* values, const uint8_t* mask, int* status) {
+  return create_impl(Lx, Ly, values, mask, status, false);
 }
 // Same map, but the chain is NOT initialised: the caller sets threads / seed / quench count first and
 // then calls orc_configure, so that a large grid pays for one R8 initialisation (on all threads)
 // instead of three single-threaded ones.
 void* orc_create_deferred(int L, const double* values, const uint8_t* mask, int* status) {
-  return create_impl(L, values, mask, status, false);
+  return create_impl(L, L, values, mask, status, false);
 }
-static void* create_impl(int L, const double* values, const uint8_t* mask, int* status, bool reset) {
+static void* create_impl(int L, int H, const double* values, const uint8_t* mask, int* status, bool reset) {
   auto fail = [&](int code) -> void* { if (status) *status = code; return nullptr; };
-  if (L < 2 || !values || !mask) return fail(ERR_INVALID_ARG);
+  if (L < 1 || H < 1 || static_cast<long long>(L) * H < 2 || (L == H && L < 2) || !values || !mask) return fail(ERR_INVALID_ARG);
   Oracle* o = new Oracle;
-  o->L = L;
+  o->L = L; o->H = H;
   const size_t N = o->N();
   o->z.assign(values, values + N);
   o->mask.assign(mask, mask + N);
@@ -492,10 +501,15 @@ static void* create_impl(int L, const double* values, const uint8_t* mask, int* 
 }
 
 // Pins only: take the spins as given (identity map, zmin = 0, zmax = 2pi); no chain reset.
+void* orc_create_from_phi_rect(int L, int H, const double* phi, const uint8_t* mask);
 void* orc_create_from_phi(int L, const double* phi, const uint8_t* mask) {
-  if (L < 2 || !phi || !mask) return nullptr;
+  if (L < 2) return nullptr;
+  return orc_create_from_phi_rect(L, L, phi, mask);
+}
+void* orc_create_from_phi_rect(int L, int H, const double* phi, const uint8_t* mask) {
+  if (L < 1 || H < 1 || static_cast<long long>(L) * H < 2 || !phi || !mask) return nullptr;
   Oracle* o = new Oracle;
-  o->L = L;
+  o->L = L; o->H = H;
   const size_t N = o->N();
   o->z.assign(phi, phi + N);
   o->mask.assign(mask, mask + N);

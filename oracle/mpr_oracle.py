@@ -51,6 +51,9 @@ def lib():
             "orc_create_deferred": (vp, [C.c_int, dp, u8p, C.POINTER(C.c_int)]),
             "orc_configure": (C.c_int, [vp, C.c_uint64, C.c_int]),
             "orc_create_from_phi": (vp, [C.c_int, dp, u8p]),
+            "orc_create_rect": (vp, [C.c_int, C.c_int, dp, u8p, C.POINTER(C.c_int)]),
+            "orc_create_rect_deferred": (vp, [C.c_int, C.c_int, dp, u8p, C.POINTER(C.c_int)]),
+            "orc_create_from_phi_rect": (vp, [C.c_int, C.c_int, dp, u8p]),
             "orc_destroy": (None, [vp]),
             "orc_set_seed": (C.c_int, [vp, C.c_uint64]),
             "orc_set_temperature": (C.c_int, [vp, C.c_double]),
@@ -129,19 +132,23 @@ class Oracle:
         (seed, n_quench) (orc_create_deferred + orc_configure) instead of once per setter."""
         L_ = lib()
         mask = np.ascontiguousarray(mask, dtype=np.uint8)
-        self.L = int(mask.shape[0])
-        assert mask.shape == (self.L, self.L)
+        # mask.shape = (Ly rows, Lx columns); L is kept as the name of the size of a square grid
+        self.Ly, self.Lx = int(mask.shape[0]), int(mask.shape[1])
+        self.L = self.Ly if self.Ly == self.Lx else None
+        self.shape = (self.Ly, self.Lx)
         self.mask = mask
         if phi is not None:
             phi = np.ascontiguousarray(phi, dtype=np.float64)
-            self.h = L_.orc_create_from_phi(self.L, _dp(phi), mask.ctypes.data_as(C.POINTER(C.c_uint8)))
+            assert phi.shape == self.shape
+            self.h = L_.orc_create_from_phi_rect(self.Lx, self.Ly, _dp(phi), mask.ctypes.data_as(C.POINTER(C.c_uint8)))
             if not self.h:
                 raise OracleError(ERR_INVALID_ARG)
         else:
             values = np.ascontiguousarray(values, dtype=np.float64)
             st = C.c_int()
-            create = L_.orc_create if n_quench is None else L_.orc_create_deferred
-            self.h = create(self.L, _dp(values), mask.ctypes.data_as(C.POINTER(C.c_uint8)), C.byref(st))
+            assert values.shape == self.shape
+            create = L_.orc_create_rect if n_quench is None else L_.orc_create_rect_deferred
+            self.h = create(self.Lx, self.Ly, _dp(values), mask.ctypes.data_as(C.POINTER(C.c_uint8)), C.byref(st))
             if not self.h:
                 raise OracleError(st.value)
             if n_quench is not None:
@@ -231,13 +238,13 @@ class Oracle:
         return lib().orc_local_energy(self.h, int(x), int(y), float(phi_s))
 
     def get_state(self):
-        out = np.empty((self.L, self.L), dtype=np.float64)
+        out = np.empty(self.shape, dtype=np.float64)
         lib().orc_get_state(self.h, _dp(out))
         return out
 
     def set_state(self, phi):
         phi = np.ascontiguousarray(phi, dtype=np.float64)
-        assert phi.shape == (self.L, self.L)
+        assert phi.shape == self.shape
         lib().orc_set_state(self.h, _dp(phi))
 
     def counters(self):
@@ -246,7 +253,7 @@ class Oracle:
         return a.value, b.value, c.value
 
     def run(self, n_eq, n_meas):
-        pred = np.empty((self.L, self.L), dtype=np.float64)
+        pred = np.empty(self.shape, dtype=np.float64)
         m, s = C.c_double(), C.c_double()
         self._chk(lib().orc_run(self.h, int(n_eq), int(n_meas), _dp(pred), C.byref(m), C.byref(s)))
         return pred, m.value, s.value

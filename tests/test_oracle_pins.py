@@ -651,3 +651,117 @@ def test_general_q_proposal_width(oracle_mod):
     assert oracle_mod.proposal_width(0.01, 0.25) == 0.8
     assert abs(oracle_mod.proposal_width(0.0025, 0.1) - 1.0) <= 1e-15
     assert oracle_mod.proposal_width(1.0, 0.1) == math.pi
+
+
+# --------------------------------------------------------------------------- rectangular grids
+def brute_force_H_rect(phi):
+    """All pairs at Manhattan distance 1 on a (Ly, Lx) array -- no index arithmetic shared with the oracle."""
+    Ly, Lx = phi.shape
+    pts = [(x, y) for y in range(Ly) for x in range(Lx)]
+    H = 0.0
+    for i, (xa, ya) in enumerate(pts):
+        for (xb, yb) in pts[i + 1:]:
+            if abs(xa - xb) + abs(ya - yb) == 1:
+                H -= math.cos(Q * (phi[ya, xa] - phi[yb, xb]))
+    return H
+
+
+@pytest.mark.parametrize("shape", [(3, 5), (5, 3), (1, 7), (7, 1), (2, 9), (6, 4)])
+def test_rect_energy_vs_brute_force_and_transpose(oracle_mod, shape):
+    """H on a rectangular grid = brute force over all unit-distance pairs; e = 2H / N_b with
+    N_b = Lx (Ly - 1) + Ly (Lx - 1); the transposed field on the transposed grid has the same H (a row / column
+    mix-up in the neighbour arithmetic breaks one of the three)."""
+    Ly, Lx = shape
+    rng = np.random.default_rng(100 * Ly + Lx)
+    phi = rng.uniform(0, TWO_PI, (Ly, Lx))
+    zero = np.zeros((Ly, Lx), dtype=np.uint8)
+    o = oracle_mod.Oracle(phi=phi, mask=zero)
+    H, e = o.energy()
+    Hb = brute_force_H_rect(phi)
+    nb = Lx * (Ly - 1) + Ly * (Lx - 1)
+    assert abs(H - Hb) < 1e-12 * max(1.0, abs(Hb))
+    assert abs(e - 2.0 * Hb / nb) < 1e-13
+    ot = oracle_mod.Oracle(phi=np.ascontiguousarray(phi.T), mask=np.ascontiguousarray(zero.T))
+    assert abs(ot.energy()[0] - H) < 1e-12 * max(1.0, abs(H))
+    # aligned spins: every bond contributes -J, e = -2 whatever the shape
+    oa = oracle_mod.Oracle(phi=np.full((Ly, Lx), 1.25), mask=zero)
+    Ha, ea = oa.energy()
+    assert abs(Ha + nb) < 1e-12 and abs(ea + 2.0) < 1e-14
+    # local energy of every site = its part of H (sum over sites counts every bond twice)
+    tot = sum(o.local_energy(x, y, phi[y, x]) for y in range(Ly) for x in range(Lx))
+    assert abs(tot - 2.0 * Hb) < 1e-11
+
+
+def test_rect_sample_energy_counts_measured_pairs_only(oracle_mod):
+    Ly, Lx = 4, 7
+    rng = np.random.default_rng(5)
+    z = rng.uniform(0.0, TWO_PI, (Ly, Lx))
+    mask = (rng.uniform(size=(Ly, Lx)) < 0.4).astype(np.uint8)
+    mask[0, 0] = 0; mask[0, 1] = 0
+    z[0, 0], z[0, 1] = 0.0, TWO_PI          # pins the range, so that phi = z
+    z[mask == 1] = np.nan                    # never read
+    o = oracle_mod.Oracle(values=z, mask=mask)
+    es, n = o.sample_energy()
+    s, cnt = 0.0, 0
+    for y in range(Ly):
+        for x in range(Lx):
+            for (dx, dy) in ((1, 0), (0, 1)):
+                xx, yy = x + dx, y + dy
+                if xx < Lx and yy < Ly and not mask[y, x] and not mask[yy, xx]:
+                    s += math.cos(Q * (z[y, x] - z[yy, xx])); cnt += 1
+    assert n == cnt and abs(es + 2.0 * s / cnt) < 1e-13
+
+
+RECT_SITE_CASES = [
+    # (shape (Ly, Lx), free site (x, y), neighbour phis {(x, y): phi}) -- the free site has a DOWN neighbour in a row
+    # index >= Lx (tall grid) or a RIGHT neighbour in a column index >= Ly (wide grid): a test of y against Lx or of
+    # x against Ly drops it
+    ((5, 2), (0, 3), {(1, 3): 0.7, (0, 2): 2.9, (0, 4): 5.1}),
+    ((2, 6), (4, 1), {(3, 1): 1.3, (5, 1): 3.3, (4, 0): 0.2}),
+    ((4, 3), (1, 2), {(0, 2): 1.0, (2, 2): 2.5, (1, 1): 4.0, (1, 3): 0.3}),
+]
+
+
+@pytest.mark.parametrize("schedule", ["R4", "SITE_FUSED"])
+@pytest.mark.parametrize("case", [0, 1, 2], ids=["tall-edge3", "wide-edge3", "tall-interior4"])
+def test_rect_single_site_histogram(oracle_mod, case, schedule):
+    """The conditional density of one free site of a rectangular grid, hybrid sweeps, against the exact density."""
+    (Ly, Lx), (x, y), nbrs = RECT_SITE_CASES[case]
+    T = 0.1
+    phi = np.full((Ly, Lx), 3.0)
+    for (a, b), v in nbrs.items():
+        phi[b, a] = v
+    mask = np.zeros((Ly, Lx), dtype=np.uint8)
+    mask[y, x] = 1
+    o = oracle_mod.Oracle(phi=phi, mask=mask)
+    o.set_quench(0)
+    o.set_seed(4321 + case)
+    o.set_temperature(T)
+    o.set_schedule(schedule)
+    thin = 8
+    tr = o.trace(400_000 * thin // 4, 1, [y * Lx + x])[:, 0]
+    chi2, p = chi2_against_density(tr[1000::thin], list(nbrs.values()), T)
+    assert p > 1e-4, (chi2, p)
+    st = o.get_state()
+    for (a, b), v in nbrs.items():
+        assert st[b, a] == v
+
+
+def test_rect_chain_equals_square_chain_on_embedded_block(oracle_mod):
+    """A rectangular problem is the same Markov chain as the square problem that contains it as a block walled off by
+    measured sites -- but for the site indices the random numbers are keyed on.  What is index-free: a 1 x n chain
+    of free sites between two measured ends at T -> 0 relaxes (quench passes) to the linear interpolation of the
+    two end angles, the minimiser of sum cos[(phi_i - phi_i+1)/2], in a row and in a column alike."""
+    n = 9
+    for shape in ((1, n), (n, 1)):
+        phi = np.zeros(shape); mask = np.ones(shape, dtype=np.uint8)
+        flat_phi, flat_mask = phi.reshape(-1), mask.reshape(-1)
+        flat_phi[0], flat_phi[-1] = 1.0, 3.0
+        flat_mask[0] = flat_mask[-1] = 0
+        o = oracle_mod.Oracle(phi=phi, mask=mask)
+        o.set_seed(3)
+        o.init_random(0)
+        for _ in range(4000):
+            o.quench_pass(0); o.quench_pass(1)
+        st = o.get_state().reshape(-1)
+        assert np.allclose(st, np.linspace(1.0, 3.0, n), atol=1e-6), st
