@@ -120,6 +120,15 @@ int mpr_workspace_bytes(int L, size_t* bytes);
  * call returns MPR_ERR_WORKSPACE until mpr_set_workspace has attached one.                  */
 int mpr_create(mpr_ctx** out, int L, const double* d_values, const uint8_t* d_mask,
                void* d_workspace, size_t workspace_bytes, void* cuda_stream);
+/* Rectangular grids: Lx columns by Ly rows, row-major (site (x, y) at y * Lx + x),
+ * d_values f64[Lx*Ly], d_mask u8[Lx*Ly].  Nothing in the method needs a square grid (PAPER.md:19:
+ * nearest neighbours on a regular grid); the specific energy is normalised by the
+ * Lx (Ly - 1) + Ly (Lx - 1) bonds of the open grid (R3; 2 L (L - 1) when square).  1 <= Lx, Ly <= 32768,
+ * Lx * Ly >= 2.  mpr_create(L, ...) is mpr_create_rect(L, L, ...) with L >= 2; every other call takes the
+ * shape from the context, and the [L*L] buffers named in this header are [Lx*Ly] for such a context.  */
+int mpr_workspace_bytes_rect(int Lx, int Ly, size_t* bytes);
+int mpr_create_rect(mpr_ctx** out, int Lx, int Ly, const double* d_values, const uint8_t* d_mask,
+                    void* d_workspace, size_t workspace_bytes, void* cuda_stream);
 void mpr_destroy(mpr_ctx* ctx); /* frees the host struct only */
 
 /* Attaches (or replaces) the caller-owned device workspace: >= mpr_workspace_bytes(L) bytes, 256-byte
@@ -220,6 +229,12 @@ int mpr_predict_host(int L, const double* h_values, const uint8_t* h_mask, mpr_p
                      uint64_t seed, double T, int n_eq, int n_meas, void* d_workspace,
                      size_t workspace_bytes, void* cuda_stream, double* h_pred, double* e_mean,
                      double* e_stderr, double* T_used, uint64_t* launches);
+/* The same on an Lx x Ly grid (see mpr_create_rect). */
+int mpr_workspace_bytes_host_rect(int Lx, int Ly, size_t* bytes);
+int mpr_predict_host_rect(int Lx, int Ly, const double* h_values, const uint8_t* h_mask,
+                          mpr_precision mode, uint64_t seed, double T, int n_eq, int n_meas,
+                          void* d_workspace, size_t workspace_bytes, void* cuda_stream, double* h_pred,
+                          double* e_mean, double* e_stderr, double* T_used, uint64_t* launches);
 
 /* HOST-only hooks into the library's host-side numerics, so that they can be pinned against
  * hand-worked numbers without a GPU (tests/test_host_logic.py); no device work, no context.

@@ -34,20 +34,27 @@ constexpr int kAcceptSlots = 1024;
 constexpr int kTrialEq = 200, kTrialMeas = 50;   // R6: sweeps of one temperature trial
 
 size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+// N_b of R3: nearest-neighbour bonds of an open L x H grid, 2 L (L - 1) on the paper's square one
+// the side of the square grid with as many sites (what the AUTO thresholds, tuned on square grids, go by)
+double grid_side(const Geom& g) { return std::sqrt(static_cast<double>(g.L) * g.H); }
+double bond_count(const Geom& g) {
+  return static_cast<double>(g.L) * (g.H - 1.0) + static_cast<double>(g.H) * (g.L - 1.0);
+}
 
 struct Layout {
   Geom g;
   size_t off_state[2], off_acc, off_bits, off_smask[2], off_list[2], off_rows, off_part, off_series, off_slots, off_scal, total;
 };
 
-Layout make_layout(int L) {
+Layout make_layout(int L, int H) {      // L columns, H rows
   Layout lo;
   lo.g.L = L;
+  lo.g.H = H;
   lo.g.Wp = static_cast<int>(align_up(static_cast<size_t>((L + 1) / 2), 16));
   lo.g.Wm = (lo.g.Wp + 31) / 32;
   lo.g.Wb = lo.g.Wm + kBitPadLeft + kBitPadRight;
-  lo.g.Hb = L + kBitPadTop + kBitPadBot;
-  lo.g.plane = static_cast<size_t>(L) * lo.g.Wp;
+  lo.g.Hb = H + kBitPadTop + kBitPadBot;
+  lo.g.plane = static_cast<size_t>(H) * lo.g.Wp;
   lo.g.energy_single = 0;
   lo.g.q = kQDefault;
   size_t o = 0;
@@ -64,7 +71,7 @@ Layout make_layout(int L) {
     lo.off_list[col] = o;
     o = align_up(o + lo.g.plane * sizeof(uint32_t), 256);
   }
-  lo.off_rows = o;     o = align_up(o + static_cast<size_t>(4) * L * sizeof(uint32_t) + 64, 256);   // row counts, offsets, totals
+  lo.off_rows = o;     o = align_up(o + static_cast<size_t>(4) * H * sizeof(uint32_t) + 64, 256);   // row counts, offsets, totals
   lo.off_part = o;     o = align_up(o + kPartials * sizeof(double), 256);
   lo.off_series = o;   o = align_up(o + kSeriesCap * sizeof(double), 256);
   lo.off_slots = o;    o = align_up(o + kAcceptSlots * sizeof(unsigned long long), 256);
@@ -200,7 +207,7 @@ template <int MODE, bool GENQ> int plain_pass_q(mpr_ctx* c, int kind, int col, u
   using R = typename Traits<MODE>::real;
   using V = typename Traits<MODE>::vec;
   const Geom& g = c->lo.g;
-  dim3 block(128), grid((g.Wp + 127) / 128, g.L);
+  dim3 block(128), grid((g.Wp + 127) / 128, g.H);
   V* st = static_cast<V*>(c->state(c->cur));
   const ChainConst<R> k = chain_const<R>(c);
   const uint32_t sw = static_cast<uint32_t>(sweep);
@@ -248,7 +255,7 @@ template <int MODE> int list_pass(mpr_ctx* c, int kind, int col, uint64_t sweep)
 template <int MODE> int init_chain(mpr_ctx* c) {
   using V = typename Traits<MODE>::vec;
   const Geom& g = c->lo.g;
-  dim3 block(128), grid((g.Wp + 127) / 128, g.L, 2);
+  dim3 block(128), grid((g.Wp + 127) / 128, g.H, 2);
   init_chain_kernel<MODE><<<grid, block, 0, c->stream>>>(c->d_values, c->d_mask, g, c->zmin, c->zmax,
                                                          static_cast<uint32_t>(c->seed),
                                                          static_cast<uint32_t>(c->seed >> 32), c->trial,
@@ -261,10 +268,10 @@ template <int MODE> int init_chain(mpr_ctx* c) {
 template <int MODE> int plain_energy(mpr_ctx* c, double* d_out, bool as_e) {
   using V = typename Traits<MODE>::vec;
   const Geom& g = c->lo.g;
-  const int nblk = g.L < 2048 ? g.L : 2048;
+  const int nblk = g.H < 2048 ? g.H : 2048;
   plain_energy_kernel<MODE><<<nblk, 256, 0, c->stream>>>(static_cast<const V*>(c->state(c->cur)), g, c->part());
   LAUNCH_OK(c);
-  const double nb = 2.0 * g.L * (g.L - 1.0);
+  const double nb = bond_count(g);
   final_sum_kernel<<<1, 1024, 0, c->stream>>>(c->part(), nblk, as_e ? -kJ * 2.0 / nb : -kJ, d_out, g.energy_single);
   LAUNCH_OK(c);
   return MPR_OK;
@@ -273,7 +280,7 @@ template <int MODE> int plain_energy(mpr_ctx* c, double* d_out, bool as_e) {
 template <int MODE> int plain_accumulate(mpr_ctx* c) {
   using V = typename Traits<MODE>::vec;
   const Geom& g = c->lo.g;
-  dim3 block(128), grid((g.Wp + 127) / 128, g.L, 2);
+  dim3 block(128), grid((g.Wp + 127) / 128, g.H, 2);
   plain_accumulate_kernel<MODE><<<grid, block, 0, c->stream>>>(static_cast<const V*>(c->state(c->cur)), c->bits(),
                                                                g, c->acc());
   LAUNCH_OK(c);
@@ -283,7 +290,7 @@ template <int MODE> int plain_accumulate(mpr_ctx* c) {
 template <int MODE> int get_state(mpr_ctx* c, double* d_phi) {
   using V = typename Traits<MODE>::vec;
   const Geom& g = c->lo.g;
-  dim3 block(128), grid((g.L + 127) / 128, g.L);
+  dim3 block(128), grid((g.L + 127) / 128, g.H);
   get_state_kernel<MODE><<<grid, block, 0, c->stream>>>(static_cast<const V*>(c->state(c->cur)), g, d_phi);
   LAUNCH_OK(c);
   return MPR_OK;
@@ -292,7 +299,7 @@ template <int MODE> int get_state(mpr_ctx* c, double* d_phi) {
 template <int MODE> int set_state(mpr_ctx* c, const double* d_phi) {
   using V = typename Traits<MODE>::vec;
   const Geom& g = c->lo.g;
-  dim3 block(128), grid((g.Wp + 127) / 128, g.L, 2);
+  dim3 block(128), grid((g.Wp + 127) / 128, g.H, 2);
   set_state_kernel<MODE><<<grid, block, 0, c->stream>>>(d_phi, g, c->bits(), static_cast<V*>(c->state(c->cur)));
   LAUNCH_OK(c);
   return MPR_OK;
@@ -311,7 +318,7 @@ template <int MODE> int tiled_sweeps(mpr_ctx* c, int k, int measure, double* d_e
   c->launches += 1;
   c->cur = 1 - c->cur;
   if (measure == 1 || measure == 2) {
-    const double nb = 2.0 * g.L * (g.L - 1.0);
+    const double nb = bond_count(g);
     final_sum_kernel<<<1, 1024, 0, c->stream>>>(c->part(), ntiles, -kJ * 2.0 / nb, d_e, g.energy_single);
     LAUNCH_OK(c);
   }
@@ -334,7 +341,7 @@ template <int MODE> int strip_sweeps(mpr_ctx* c, int prog, int k, int measure, d
   c->launches += 1;
   c->cur = 1 - c->cur;
   if (measure == 1 || measure == 2) {
-    const double nb = 2.0 * g.L * (g.L - 1.0);
+    const double nb = bond_count(g);
     final_sum_kernel<<<1, 1024, 0, c->stream>>>(c->part(), nblocks, -kJ * 2.0 / nb, d_e, g.energy_single);
     LAUNCH_OK(c);
   }
@@ -433,16 +440,16 @@ int eff_path(const mpr_ctx* c) {
   // 4 bytes per column, which the TMA unit requires; the STRIP kernels carry two halo lanes for it and take over
   if (c->mode == MPR_HP) {
     if (c->path == MPR_PATH_PLAIN || c->path == MPR_PATH_LIST) return c->path;
-    if (c->path == MPR_PATH_AUTO && c->lo.g.L < 4096) return MPR_PATH_PLAIN;
+    if (c->path == MPR_PATH_AUTO && grid_side(c->lo.g) < 4096) return MPR_PATH_PLAIN;
     return MPR_PATH_STRIP;
   }
   if (c->path != MPR_PATH_AUTO) return c->path;
   if (c->schedule == MPR_SCHEDULE_SITE_FUSED) {
     // small, sparsely masked grids: the compacted lists win (config 3, f = 0.33, L2-resident: 0.021 against 0.025 ms)
-    const double f = static_cast<double>(c->n_free) / (static_cast<double>(c->lo.g.L) * c->lo.g.L);
-    return (f < 0.5 && c->lo.g.L <= 4096) ? MPR_PATH_LIST : MPR_PATH_STRIP;
+    const double f = static_cast<double>(c->n_free) / (static_cast<double>(c->lo.g.L) * c->lo.g.H);
+    return (f < 0.5 && grid_side(c->lo.g) <= 4096) ? MPR_PATH_LIST : MPR_PATH_STRIP;
   }
-  return (c->mode == MPR_SP_INTRINSIC && c->lo.g.L >= 4096) ? MPR_PATH_STRIP : MPR_PATH_TILED;
+  return (c->mode == MPR_SP_INTRINSIC && grid_side(c->lo.g) >= 4096) ? MPR_PATH_STRIP : MPR_PATH_TILED;
 }
 
 // R8: uniform initial spins, then n_quench x (quench colour 0, quench colour 1); everything
@@ -570,7 +577,7 @@ int trial_energy(mpr_ctx* c, int* est_trials, double T, double* e, double* se) {
 
 int setup(mpr_ctx* c) {
   const Geom& g = c->lo.g;
-  const size_t N = static_cast<size_t>(g.L) * g.L;
+  const size_t N = static_cast<size_t>(g.L) * g.H;
   // R1: range of the measured sample
   const int nblk = 1024;
   sample_range_kernel<<<nblk, 256, 0, c->stream>>>(c->d_values, c->d_mask, N, c->part());
@@ -586,7 +593,7 @@ int setup(mpr_ctx* c) {
   c->zmin = h[0];
   c->zmax = h[1];
   // R6: sample energy
-  sample_energy_kernel<<<nblk, 256, 0, c->stream>>>(c->d_values, c->d_mask, g.L, c->zmin, c->zmax, c->part(), g.q);
+  sample_energy_kernel<<<nblk, 256, 0, c->stream>>>(c->d_values, c->d_mask, g.L, g.H, c->zmin, c->zmax, c->part(), g.q);
   LAUNCH_OK(c);
   pair_final_kernel<<<1, 32, 0, c->stream>>>(c->part(), nblk, c->scal());
   LAUNCH_OK(c);
@@ -607,13 +614,13 @@ int setup(mpr_ctx* c) {
   // compacted per-colour lists of the prediction sites, for the LIST path (mpr_plain.cuh)
   {
     uint32_t* row_count = c->rows();
-    uint32_t* row_off = row_count + 2 * static_cast<size_t>(g.L);
-    uint32_t* totals = row_off + 2 * static_cast<size_t>(g.L);
-    list_row_count_kernel<<<dim3(g.L, 2), 128, 0, c->stream>>>(c->bits(), g, row_count);
+    uint32_t* row_off = row_count + 2 * static_cast<size_t>(g.H);
+    uint32_t* totals = row_off + 2 * static_cast<size_t>(g.H);
+    list_row_count_kernel<<<dim3(g.H, 2), 128, 0, c->stream>>>(c->bits(), g, row_count);
     LAUNCH_OK(c);
-    list_row_scan_kernel<<<1, 1024, 0, c->stream>>>(row_count, g.L, row_off, totals);
+    list_row_scan_kernel<<<1, 1024, 0, c->stream>>>(row_count, g.H, row_off, totals);
     LAUNCH_OK(c);
-    list_fill_kernel<<<dim3((g.L + 3) / 4, 2), 128, 0, c->stream>>>(c->bits(), g, row_off, c->list(0), c->list(1));
+    list_fill_kernel<<<dim3((g.H + 3) / 4, 2), 128, 0, c->stream>>>(c->bits(), g, row_off, c->list(0), c->list(1));
     LAUNCH_OK(c);
     CUDA_OK(c, cudaMemcpyAsync(c->n_list, totals, sizeof(c->n_list), cudaMemcpyDeviceToHost, c->stream));
   }
@@ -648,18 +655,36 @@ const char* mpr_status_string(int status) {
 
 const char* mpr_last_error(const mpr_ctx* ctx) { return ctx ? ctx->err.c_str() : ""; }
 
-int mpr_workspace_bytes(int L, size_t* bytes) {
-  if (L < 2 || L > kMaxL || !bytes) return MPR_ERR_INVALID_ARG;
-  *bytes = make_layout(L).total;
+// a grid is valid when both sides are in [1, kMaxL], it has at least two sites, and its Philox site index fits 32 bits
+static bool valid_shape(int Lx, int Ly) {
+  return Lx >= 1 && Ly >= 1 && Lx <= kMaxL && Ly <= kMaxL && static_cast<long long>(Lx) * Ly >= 2 &&
+         static_cast<long long>(Lx) * Ly <= (1ll << 32);
+}
+
+int mpr_workspace_bytes_rect(int Lx, int Ly, size_t* bytes) {
+  if (!valid_shape(Lx, Ly) || !bytes) return MPR_ERR_INVALID_ARG;
+  *bytes = make_layout(Lx, Ly).total;
   return MPR_OK;
+}
+int mpr_workspace_bytes(int L, size_t* bytes) {
+  if (L < 2) return MPR_ERR_INVALID_ARG;
+  return mpr_workspace_bytes_rect(L, L, bytes);
 }
 
 int mpr_create(mpr_ctx** out, int L, const double* d_values, const uint8_t* d_mask, void* d_workspace,
                size_t workspace_bytes, void* cuda_stream) {
   if (!out) return MPR_ERR_INVALID_ARG;
   *out = nullptr;
-  if (L < 2 || L > kMaxL || !d_values || !d_mask) return MPR_ERR_INVALID_ARG;
-  const Layout lo = make_layout(L);
+  if (L < 2) return MPR_ERR_INVALID_ARG;
+  return mpr_create_rect(out, L, L, d_values, d_mask, d_workspace, workspace_bytes, cuda_stream);
+}
+
+int mpr_create_rect(mpr_ctx** out, int Lx, int Ly, const double* d_values, const uint8_t* d_mask, void* d_workspace,
+                    size_t workspace_bytes, void* cuda_stream) {
+  if (!out) return MPR_ERR_INVALID_ARG;
+  *out = nullptr;
+  if (!valid_shape(Lx, Ly) || !d_values || !d_mask) return MPR_ERR_INVALID_ARG;
+  const Layout lo = make_layout(Lx, Ly);
   const bool with_ws = d_workspace || workspace_bytes;
   if (with_ws && (!d_workspace || (reinterpret_cast<uintptr_t>(d_workspace) & 255u) || workspace_bytes < lo.total))
     return MPR_ERR_WORKSPACE;
@@ -838,7 +863,7 @@ int mpr_run(mpr_ctx* c, int n_eq, int n_meas, double* d_pred, double* e_mean, do
   TRY(hybrid_sweeps(c, n_meas, 2, 0));
   if (d_pred) {
     const Geom& g = c->lo.g;
-    dim3 block(128), grid((g.L + 127) / 128, g.L);
+    dim3 block(128), grid((g.L + 127) / 128, g.H);
     predict_kernel<<<grid, block, 0, c->stream>>>(c->d_values, c->d_mask, g, c->acc(), c->zmin, c->zmax, c->n_acc,
                                                   d_pred);
     LAUNCH_OK(c);
@@ -895,7 +920,7 @@ int mpr_energy(mpr_ctx* c, double* H, double* e) {
   double h = 0.0;
   CUDA_OK(c, cudaMemcpyAsync(&h, c->scal() + 8, sizeof(double), cudaMemcpyDeviceToHost, c->stream));
   CUDA_OK(c, cudaStreamSynchronize(c->stream));
-  const double nb = 2.0 * c->lo.g.L * (c->lo.g.L - 1.0);
+  const double nb = bond_count(c->lo.g);
   if (H) *H = h;
   if (e) *e = c->lo.g.energy_single ? static_cast<double>(2.0f * static_cast<float>(h) / static_cast<float>(nb))
                                     : 2.0 * h / nb;
@@ -948,24 +973,36 @@ int mpr_get_launch_stats(mpr_ctx* c, uint64_t* launches) {
   return MPR_OK;
 }
 
-int mpr_workspace_bytes_host(int L, size_t* bytes) {
+int mpr_workspace_bytes_host_rect(int Lx, int Ly, size_t* bytes) {
   size_t b = 0;
-  const int st = mpr_workspace_bytes(L, &b);
+  const int st = mpr_workspace_bytes_rect(Lx, Ly, &b);
   if (st != MPR_OK) return st;
-  const size_t N = static_cast<size_t>(L) * L;
+  const size_t N = static_cast<size_t>(Lx) * Ly;
   *bytes = b + align_up(N * sizeof(double), 256) * 2 + align_up(N, 256);
   return MPR_OK;
+}
+int mpr_workspace_bytes_host(int L, size_t* bytes) {
+  if (L < 2) return MPR_ERR_INVALID_ARG;
+  return mpr_workspace_bytes_host_rect(L, L, bytes);
 }
 
 int mpr_predict_host(int L, const double* h_values, const uint8_t* h_mask, mpr_precision mode, uint64_t seed, double T,
                      int n_eq, int n_meas, void* d_workspace, size_t workspace_bytes, void* cuda_stream,
                      double* h_pred, double* e_mean, double* e_stderr, double* T_used, uint64_t* launches) {
+  if (L < 2) return MPR_ERR_INVALID_ARG;
+  return mpr_predict_host_rect(L, L, h_values, h_mask, mode, seed, T, n_eq, n_meas, d_workspace, workspace_bytes, cuda_stream,
+                               h_pred, e_mean, e_stderr, T_used, launches);
+}
+
+int mpr_predict_host_rect(int Lx, int Ly, const double* h_values, const uint8_t* h_mask, mpr_precision mode, uint64_t seed,
+                          double T, int n_eq, int n_meas, void* d_workspace, size_t workspace_bytes, void* cuda_stream,
+                          double* h_pred, double* e_mean, double* e_stderr, double* T_used, uint64_t* launches) {
   size_t need = 0, core = 0;
-  if (mpr_workspace_bytes_host(L, &need) != MPR_OK || !h_values || !h_mask) return MPR_ERR_INVALID_ARG;
-  mpr_workspace_bytes(L, &core);
+  if (mpr_workspace_bytes_host_rect(Lx, Ly, &need) != MPR_OK || !h_values || !h_mask) return MPR_ERR_INVALID_ARG;
+  mpr_workspace_bytes_rect(Lx, Ly, &core);
   if (!d_workspace || (reinterpret_cast<uintptr_t>(d_workspace) & 255u) || workspace_bytes < need)
     return MPR_ERR_WORKSPACE;
-  const size_t N = static_cast<size_t>(L) * L;
+  const size_t N = static_cast<size_t>(Lx) * Ly;
   char* base = static_cast<char*>(d_workspace) + core;
   double* d_values = reinterpret_cast<double*>(base);
   double* d_pred = reinterpret_cast<double*>(base + align_up(N * sizeof(double), 256));
@@ -975,7 +1012,7 @@ int mpr_predict_host(int L, const double* h_values, const uint8_t* h_mask, mpr_p
       cudaMemcpyAsync(d_mask, h_mask, N, cudaMemcpyHostToDevice, s) != cudaSuccess)
     return MPR_ERR_CUDA;
   mpr_ctx* c = nullptr;
-  int st = mpr_create(&c, L, d_values, d_mask, d_workspace, core, cuda_stream);
+  int st = mpr_create_rect(&c, Lx, Ly, d_values, d_mask, d_workspace, core, cuda_stream);
   if (st != MPR_OK) return st;
   st = mpr_set_precision(c, mode);
   if (st != MPR_OK) { mpr_destroy(c); return st; }

@@ -3,7 +3,8 @@
 // (the PLAIN path, also the quench passes of R8), energy (R3), accumulation and back-map (R15).
 //
 // Layout.  Site (x, y) has colour (x + y) & 1 and lives in colour plane `col`
-// at row y, column j = x >> 1; a plane is L rows of Wp columns (Wp = ceil(L/2) rounded up to 16),
+// at row y, column j = x >> 1; a plane is H rows of Wp columns (Wp = ceil(L/2) rounded up to 16; L columns, H rows,
+// H = L on the paper's square grid),
 // one spin (c, s) per site, stored PAIR-INTERLEAVED: the two sites of plane columns (2m, 2m + 1)
 // share one unit of four scalars (c_2m, c_2m+1, s_2m, s_2m+1), so that the tiled kernel reads a pair
 // with one 128-bit access whose register halves are already (site a, site b) lanes for the packed
@@ -16,9 +17,10 @@
 namespace mpr {
 
 struct Geom {
-  int L, Wp, Wm;
+  int L, Wp, Wm;         // L = columns of the grid (x); rows: H below
   int Wb, Hb;            // padded bitmap: words per row, rows per colour
-  size_t plane;          // elements per colour plane = L * Wp
+  size_t plane;          // elements per colour plane = H * Wp
+  int H;                 // rows of the grid (y); == L unless created by mpr_create_rect
   double q;              // PAPER.md:27, q in (0, 1/2]; 1/2 unless mpr_set_q
   int energy_single;     // X_E of PAPER.md:35: 0 = energy sums in double (R13), 1 = the energy variable is a float
 };
@@ -137,18 +139,18 @@ __device__ __forceinline__ double map_to_phi(double z, double zmin, double zmax)
 
 // R6 first half: e_s = -2J mean over measured nearest-neighbour pairs of cos[q(phi_s - phi_t)].
 // Per-block partials: [0] sum of cos, [1] pair count.
-static __global__ void sample_energy_kernel(const double* __restrict__ z, const uint8_t* __restrict__ mask, int L,
+static __global__ void sample_energy_kernel(const double* __restrict__ z, const uint8_t* __restrict__ mask, int L, int H,
                                      double zmin, double zmax, double* __restrict__ part /* 2 per block */, double q) {
   __shared__ double sh[32];
   double sum = 0.0, cnt = 0.0;
-  const size_t N = static_cast<size_t>(L) * L;
+  const size_t N = static_cast<size_t>(L) * H;
   for (size_t i = blockIdx.x * static_cast<size_t>(blockDim.x) + threadIdx.x; i < N;
        i += static_cast<size_t>(gridDim.x) * blockDim.x) {
     if (mask[i]) continue;
     const int x = static_cast<int>(i % L), y = static_cast<int>(i / L);
     const double p = map_to_phi(z[i], zmin, zmax);
     if (x < L - 1 && !mask[i + 1]) { sum += cos(q * (p - map_to_phi(z[i + 1], zmin, zmax))); cnt += 1.0; }
-    if (y < L - 1 && !mask[i + L]) { sum += cos(q * (p - map_to_phi(z[i + L], zmin, zmax))); cnt += 1.0; }
+    if (y < H - 1 && !mask[i + L]) { sum += cos(q * (p - map_to_phi(z[i + L], zmin, zmax))); cnt += 1.0; }
   }
   const double s = block_sum(sum, sh);
   const double c = block_sum(cnt, sh);
@@ -174,7 +176,7 @@ static __global__ void pack_mask_kernel(const uint8_t* __restrict__ mask, Geom g
     const size_t row = w / g.Wb;
     const int y = static_cast<int>(row % g.Hb) - kBitPadTop, col = static_cast<int>(row / g.Hb);
     uint32_t word = 0;
-    if (y >= 0 && y < g.L && wi >= 0 && wi < g.Wm) {
+    if (y >= 0 && y < g.H && wi >= 0 && wi < g.Wm) {
       const int par = x_parity(y, col);
       for (int b = 0; b < 32; ++b) {
         const int x = 2 * (32 * wi + b) + par;
@@ -272,7 +274,7 @@ __device__ __forceinline__ bool plain_site_update(typename Traits<MODE>::vec* __
   const int x = 2 * j + par;
   V* own = state + static_cast<size_t>(col) * g.plane + static_cast<size_t>(y) * g.Wp;
   const V* oth = state + static_cast<size_t>(1 - col) * g.plane + static_cast<size_t>(y) * g.Wp;
-  const bool hl = x > 0, hr = x < g.L - 1, hu = y > 0, hd = y < g.L - 1;
+  const bool hl = x > 0, hr = x < g.L - 1, hu = y > 0, hd = y < g.H - 1;
   const int jl = j - 1 + par, jr = j + par;
   V zero; zero.x = 0; zero.y = 0;
   const V l = hl ? ld_spin(oth, jl) : zero;
@@ -341,9 +343,9 @@ static __global__ void list_row_count_kernel(const uint32_t* __restrict__ bits, 
   double n = 0.0;
   for (int wi = threadIdx.x; wi < g.Wm; wi += blockDim.x) n += static_cast<double>(__popc(*mask_word(bits, g, col, y, wi)));
   const double s = block_sum(n, sh);
-  if (threadIdx.x == 0) row_count[static_cast<size_t>(col) * g.L + y] = static_cast<uint32_t>(s);
+  if (threadIdx.x == 0) row_count[static_cast<size_t>(col) * g.H + y] = static_cast<uint32_t>(s);
 }
-// exclusive scan of the row counts of both colours (one block; L <= 32768 rows): row_off[col][y], total[col]
+// exclusive scan of the row counts of both colours (one block; L = number of ROWS <= 32768): row_off[col][y], total[col]
 static __global__ void list_row_scan_kernel(const uint32_t* __restrict__ row_count, int L, uint32_t* __restrict__ row_off,
                                             uint32_t* __restrict__ total) {
   __shared__ uint32_t part[1024];
@@ -371,8 +373,8 @@ static __global__ void list_row_scan_kernel(const uint32_t* __restrict__ row_cou
 static __global__ void list_fill_kernel(const uint32_t* __restrict__ bits, Geom g, const uint32_t* __restrict__ row_off,
                                         uint32_t* __restrict__ list0, uint32_t* __restrict__ list1) {
   const int y = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5), col = blockIdx.y, lane = threadIdx.x & 31;
-  if (y >= g.L) return;
-  uint32_t* out = (col ? list1 : list0) + row_off[static_cast<size_t>(col) * g.L + y];
+  if (y >= g.H) return;
+  uint32_t* out = (col ? list1 : list0) + row_off[static_cast<size_t>(col) * g.H + y];
   uint32_t base = 0;
   for (int w0 = 0; w0 < g.Wm; w0 += 32) {
     const int wi = w0 + lane;
@@ -425,14 +427,14 @@ plain_energy_kernel(const typename Traits<MODE>::vec* __restrict__ state, Geom g
   __shared__ double sh[32];
   double sum = 0.0;
   const int col = 1;
-  for (int y = blockIdx.x; y < g.L; y += gridDim.x) {
+  for (int y = blockIdx.x; y < g.H; y += gridDim.x) {
     const int par = x_parity(y, col);
     const V* own = state + static_cast<size_t>(col) * g.plane + static_cast<size_t>(y) * g.Wp;
     const V* oth = state + static_cast<size_t>(1 - col) * g.plane + static_cast<size_t>(y) * g.Wp;
     for (int j = threadIdx.x; j < g.Wp; j += blockDim.x) {
       const int x = 2 * j + par;
       if (x >= g.L) continue;
-      const bool hl = x > 0, hr = x < g.L - 1, hu = y > 0, hd = y < g.L - 1;
+      const bool hl = x > 0, hr = x < g.L - 1, hu = y > 0, hd = y < g.H - 1;
       V zero; zero.x = 0; zero.y = 0;
       const V l = hl ? ld_spin(oth, j - 1 + par) : zero;
       const V r = hr ? ld_spin(oth, j + par) : zero;

@@ -79,7 +79,7 @@ template <int MODE, int NS, int MEASURE = 0> struct StripCfg {
   static constexpr int NW = kFit < kMax ? kFit : kMax;
 };
 
-// Work distribution.  The rows of all strips are laid end to end (strip s occupies [s Lp, (s + 1) Lp), Lp = L rounded
+// Work distribution.  The rows of all strips are laid end to end (strip s occupies [s Lp, (s + 1) Lp), Lp = the number of rows rounded
 // up to a multiple of 4) and cut into equal quotas of `quota` rows (a multiple of 4): warp w of the launch takes
 // [w quota, (w + 1) quota).  A quota that crosses the end of a strip is worked off as two segments.  Warp w is warp
 // slot w / gridDim.x of CTA w % gridDim.x, so that a launch with fewer warps than slots still uses every SM.
@@ -197,7 +197,7 @@ strip_kernel(const __grid_constant__ CUtensorMap tmap, typename Traits<MODE>::ve
       const int yb = static_cast<int>(q0 - static_cast<long long>(strip) * sg.Lp);     // multiple of 4
       const int ye_pad = static_cast<int>(min(static_cast<long long>(sg.Lp), yb + (q1 - q0)));
       q0 += ye_pad - yb;
-      const int ye = min(g.L, ye_pad);
+      const int ye = min(g.H, ye_pad);
       if (yb >= ye) continue;
       const int j0 = strip * IC - 2 * HL;                     // plane column of lane 0 (even)
       const int t0 = yb - LEAD;                               // first loaded row (a multiple of 4, so even)
@@ -451,7 +451,7 @@ static __global__ void pack_strip_mask_kernel(const uint8_t* __restrict__ mask, 
   uint32_t word = 0;
   for (int r = 0; r < kStripRB; ++r) {
     const int y = chunk * kStripRB - kStripMaskLead + r;
-    if (y < 0 || y >= g.L) continue;
+    if (y < 0 || y >= g.H) continue;
     for (int c = 0; c < 2; ++c)
       for (int k = 0; k < 2; ++k) {
         const int jj = j + k;
@@ -463,12 +463,12 @@ static __global__ void pack_strip_mask_kernel(const uint8_t* __restrict__ mask, 
 }
 inline int strip_mask_strips(const Geom& g, int hl) { const int ic = kTileCols - 4 * hl; return (g.Wp + ic - 1) / ic; }
 inline size_t strip_mask_words(const Geom& g, int hl) {
-  return static_cast<size_t>(strip_mask_strips(g, hl)) * strip_mask_chunks(g.L) * 32;
+  return static_cast<size_t>(strip_mask_strips(g, hl)) * strip_mask_chunks(g.H) * 32;
 }
 inline cudaError_t strip_mask_build(const uint8_t* d_mask, const Geom& g, int hl, uint32_t* out, cudaStream_t stream) {
   const size_t n = strip_mask_words(g, hl);
   pack_strip_mask_kernel<<<static_cast<unsigned>((n + 255) / 256), 256, 0, stream>>>(d_mask, g, hl, strip_mask_strips(g, hl),
-                                                                                     strip_mask_chunks(g.L), out);
+                                                                                     strip_mask_chunks(g.H), out);
   return cudaGetLastError();
 }
 
@@ -486,7 +486,7 @@ int strip_encode(TiledPlan& tp, const Geom& g, void* src, CUtensorMap* map) {
   // fp16 storage travels as 32-bit words (two halves each): the copy is the same bytes, and the plain FLOAT32 path
   // of the TMA unit is the one every other mode has proven
   constexpr bool kHalf = sizeof(decltype(V::x)) == 2;
-  const cuuint64_t dims[3] = {static_cast<cuuint64_t>(kHalf ? 1 : 2) * g.Wp, static_cast<cuuint64_t>(g.L), 2};
+  const cuuint64_t dims[3] = {static_cast<cuuint64_t>(kHalf ? 1 : 2) * g.Wp, static_cast<cuuint64_t>(g.H), 2};
   const cuuint64_t strides[2] = {static_cast<cuuint64_t>(g.Wp) * sizeof(V), static_cast<cuuint64_t>(g.plane) * sizeof(V)};
   const cuuint32_t box[3] = {(kHalf ? 1 : 2) * kTileCols, static_cast<cuuint32_t>(kStripRB), 2};
   const cuuint32_t estr[3] = {1, 1, 1};
@@ -510,12 +510,12 @@ inline StripGeom strip_geometry(const Geom& g, int ns, int hl, int nw, int sm_co
   (void)ns;
   const int ic = kTileCols - 4 * hl;
   sg.n_strips = (g.Wp + ic - 1) / ic;
-  const int L4 = (g.L + 3) / 4 * 4;
+  const int L4 = (g.H + 3) / 4 * 4;
   const long long slots = static_cast<long long>(sm_count) * nw;
   const long long n_seg = slots / sg.n_strips;
-  const int seg_rows = n_seg > 0 ? static_cast<int>(((g.L + n_seg - 1) / n_seg + 3) / 4 * 4) : 0;
+  const int seg_rows = n_seg > 0 ? static_cast<int>(((g.H + n_seg - 1) / n_seg + 3) / 4 * 4) : 0;
   if (n_seg > 0 && sg.n_strips * n_seg * 100 >= slots * 96 && seg_rows >= 8) {
-    const int segs = (g.L + seg_rows - 1) / seg_rows;
+    const int segs = (g.H + seg_rows - 1) / seg_rows;
     sg.Lp = segs * seg_rows;
     sg.quota = seg_rows;
     sg.n_warps = sg.n_strips * segs;
@@ -529,7 +529,7 @@ inline StripGeom strip_geometry(const Geom& g, int ns, int hl, int nw, int sm_co
     sg.quota = static_cast<int>(quota);
     sg.n_warps = static_cast<int>((total + quota - 1) / quota);
   }
-  sg.n_mchunks = strip_mask_chunks(g.L);
+  sg.n_mchunks = strip_mask_chunks(g.H);
   *nblocks = sg.n_warps < sm_count ? sg.n_warps : sm_count;
   return sg;
 }

@@ -373,13 +373,13 @@ tiled_sweep_kernel(const __grid_constant__ CUtensorMap tmap, typename Traits<MOD
 
   // interior -> other state buffer (+ energy sample and accumulation of phi when measuring).
   // cnt already says which rows of this warp and whether this thread's columns are owned; what
-  // is left is the edge of the grid (rows >= L, plane columns >= Wp).  Unrolled: one pointer each
+  // is left is the edge of the grid (rows >= H, plane columns >= Wp).  Unrolled: one pointer each
   // for shared and global memory plus immediate / strided offsets.
   double esum = 0.0;
   {
     const int j = j0 + jj;                                        // even
     const int row0 = y0 + warp * RPW;
-    const int nrows = g.L - row0;                                 // rows i < nrows lie in the grid
+    const int nrows = g.H - row0;                                 // rows i < nrows lie in the grid
     const uint32_t own_rows = j < g.Wp ? cnt : 0u;
     const long long g0 = static_cast<long long>(row0) * g.Wp + j; // never dereferenced for rows outside
     S* gp = reinterpret_cast<S*>(dst) + 2 * g0;
@@ -446,7 +446,7 @@ int tiled_encode(TiledPlan& plan, const Geom& g, void* src, CUtensorMap* map) {
   // fp16 storage travels as 32-bit words (two halves each): the copy is the same bytes, and the plain FLOAT32 path
   // of the TMA unit is the one every other mode has proven
   constexpr bool kHalf = sizeof(decltype(V::x)) == 2;
-  const cuuint64_t dims[3] = {static_cast<cuuint64_t>(kHalf ? 1 : 2) * g.Wp, static_cast<cuuint64_t>(g.L), 2};
+  const cuuint64_t dims[3] = {static_cast<cuuint64_t>(kHalf ? 1 : 2) * g.Wp, static_cast<cuuint64_t>(g.H), 2};
   const cuuint64_t strides[2] = {static_cast<cuuint64_t>(g.Wp) * sizeof(V), static_cast<cuuint64_t>(g.plane) * sizeof(V)};
   const cuuint32_t box[3] = {(kHalf ? 1 : 2) * kTileCols, static_cast<cuuint32_t>(TileCfg<MODE>::TH), 2};
   const cuuint32_t estr[3] = {1, 1, 1};
@@ -480,7 +480,7 @@ int tiled_launch(TiledPlan& plan, const Geom& g, void* src, void* dst, const uin
     plan.attr_set[MODE] = true;
   }
   const int IC = kTileCols - 4 * k, IR = TH - 8 * k;
-  const int tiles_x = (g.Wp + IC - 1) / IC, tiles_y = (g.L + IR - 1) / IR;
+  const int tiles_x = (g.Wp + IC - 1) / IC, tiles_y = (g.H + IR - 1) / IR;
   const long long ntiles = static_cast<long long>(tiles_x) * tiles_y;
   // only the measuring launches write one partial per tile (they always run at k = 1)
   if ((measure == 1 || measure == 2) && ntiles > max_partials) return TILED_TOO_MANY;

@@ -90,6 +90,20 @@ def make_problem(L: int, xi: float, field_seed: int, f: float, lognormal: bool =
     return values, mask, truth
 
 
+def make_rect_problem(Ly: int, Lx: int, xi: float, field_seed: int, f: float, lognormal: bool = False):
+    """A rectangular problem (Ly rows, Lx columns): the top-left Ly x Lx window of the square problem of
+    side max(Ly, Lx), with its mask (the masked fraction of the window is close to f, not exactly f).  A window that
+    came out with fewer than two measured sites gets its first two sites measured."""
+    values, mask, truth = make_problem(max(Ly, Lx), xi, field_seed, f, lognormal)
+    values = np.ascontiguousarray(values[:Ly, :Lx]); mask = np.ascontiguousarray(mask[:Ly, :Lx])
+    truth = np.ascontiguousarray(truth[:Ly, :Lx])
+    if int((mask == 0).sum()) < 2:
+        flat_m, flat_v, flat_t = mask.reshape(-1), values.reshape(-1), truth.reshape(-1)
+        flat_m[:2] = 0
+        flat_v[:2] = flat_t[:2]
+    return values, mask, truth
+
+
 def structured_mask(L: int, kind: str, f: float, seed: int) -> np.ndarray:
     """Gap patterns of remote-sensing data ("restricted satellite paths or bad weather conditions"),
     uint8[L, L] with 1 = prediction site and a masked fraction close to f:

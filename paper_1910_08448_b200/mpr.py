@@ -34,6 +34,7 @@ SYMBOLS = [
     "mpr_energy", "mpr_sample_energy", "mpr_get_counters", "mpr_get_run_timing", "mpr_get_energy_series",
     "mpr_get_info",
     "mpr_get_launch_stats", "mpr_workspace_bytes_host", "mpr_predict_host", "mpr_debug_philox",
+    "mpr_workspace_bytes_rect", "mpr_create_rect", "mpr_workspace_bytes_host_rect", "mpr_predict_host_rect",
     "mpr_last_error", "mpr_status_string",
 ]
 
@@ -70,6 +71,11 @@ def lib():
     sig = {
         "mpr_workspace_bytes": (C.c_int, [C.c_int, C.POINTER(C.c_size_t)]),
         "mpr_create": (C.c_int, [C.POINTER(vp), C.c_int, vp, vp, vp, C.c_size_t, vp]),
+        "mpr_workspace_bytes_rect": (C.c_int, [C.c_int, C.c_int, C.POINTER(C.c_size_t)]),
+        "mpr_create_rect": (C.c_int, [C.POINTER(vp), C.c_int, C.c_int, vp, vp, vp, C.c_size_t, vp]),
+        "mpr_workspace_bytes_host_rect": (C.c_int, [C.c_int, C.c_int, C.POINTER(C.c_size_t)]),
+        "mpr_predict_host_rect": (C.c_int, [C.c_int, C.c_int, vp, vp, C.c_int, C.c_uint64, C.c_double, C.c_int, C.c_int,
+                                            vp, C.c_size_t, vp, vp, dp, dp, dp, u64p]),
         "mpr_destroy": (None, [vp]),
         "mpr_set_workspace": (C.c_int, [vp, vp, C.c_size_t]),
         "mpr_set_stream": (C.c_int, [vp, vp]),
@@ -115,10 +121,15 @@ def lib():
     return L
 
 
-def workspace_bytes(L: int, host: bool = False) -> int:
+def workspace_bytes(L, host: bool = False) -> int:
+    """L: the size of a square grid, or a shape (Ly rows, Lx columns)."""
     n = C.c_size_t()
-    fn = lib().mpr_workspace_bytes_host if host else lib().mpr_workspace_bytes
-    st = fn(int(L), C.byref(n))
+    if isinstance(L, (tuple, list)):
+        fn = lib().mpr_workspace_bytes_host_rect if host else lib().mpr_workspace_bytes_rect
+        st = fn(int(L[1]), int(L[0]), C.byref(n))
+    else:
+        fn = lib().mpr_workspace_bytes_host if host else lib().mpr_workspace_bytes
+        st = fn(int(L), C.byref(n))
     if st != MPR_OK:
         raise MprError(st)
     return n.value
@@ -144,10 +155,13 @@ class Mpr:
         dev = torch.device(device)
         self.values = torch.as_tensor(values, dtype=torch.float64).to(dev).contiguous()
         self.mask = torch.as_tensor(mask, dtype=torch.uint8).to(dev).contiguous()
-        self.L = int(self.mask.shape[0])
-        assert self.mask.shape == (self.L, self.L) and self.values.shape == (self.L, self.L)
+        # shape = (Ly rows, Lx columns); L names the size of a square grid (None otherwise)
+        self.Ly, self.Lx = int(self.mask.shape[0]), int(self.mask.shape[1])
+        self.shape = (self.Ly, self.Lx)
+        self.L = self.Ly if self.Ly == self.Lx else None
+        assert self.mask.dim() == 2 and tuple(self.values.shape) == self.shape
         self.device = dev
-        self.ws = torch.empty(workspace_bytes(self.L) + 256, dtype=torch.uint8, device=dev)
+        self.ws = torch.empty(workspace_bytes(self.shape) + 256, dtype=torch.uint8, device=dev)
         off = (-self.ws.data_ptr()) % 256
         self._ws_ptr = self.ws.data_ptr() + off
         self._stream = stream
@@ -157,8 +171,12 @@ class Mpr:
         # globals (lib, C) may already be cleared
         self._destroy, self._null = lib().mpr_destroy, C.c_void_p
         with torch.cuda.device(dev):
-            st = lib().mpr_create(C.byref(self.h), self.L, self.values.data_ptr(), self.mask.data_ptr(),
-                                  self._ws_ptr, self.ws.numel() - off, sptr)
+            if self.L is not None:
+                st = lib().mpr_create(C.byref(self.h), self.L, self.values.data_ptr(), self.mask.data_ptr(),
+                                      self._ws_ptr, self.ws.numel() - off, sptr)
+            else:
+                st = lib().mpr_create_rect(C.byref(self.h), self.Lx, self.Ly, self.values.data_ptr(), self.mask.data_ptr(),
+                                           self._ws_ptr, self.ws.numel() - off, sptr)
         if st != MPR_OK:
             self.h = C.c_void_p()
             raise MprError(st)
@@ -235,7 +253,7 @@ class Mpr:
 
     def run(self, n_eq, n_meas, want_pred=True):
         """Returns (pred CUDA tensor [L, L] or None, e_mean, e_stderr)."""
-        pred = self._torch.empty((self.L, self.L), dtype=self._torch.float64, device=self.device) if want_pred else None
+        pred = self._torch.empty(self.shape, dtype=self._torch.float64, device=self.device) if want_pred else None
         m, s = C.c_double(), C.c_double()
         self._call(lib().mpr_run, int(n_eq), int(n_meas), pred.data_ptr() if want_pred else None,
                    C.byref(m), C.byref(s))
@@ -249,13 +267,13 @@ class Mpr:
 
     # -- inspection ----------------------------------------------------------------------
     def get_state(self):
-        phi = self._torch.empty((self.L, self.L), dtype=self._torch.float64, device=self.device)
+        phi = self._torch.empty(self.shape, dtype=self._torch.float64, device=self.device)
         self._call(lib().mpr_get_state, phi.data_ptr())
         return phi
 
     def set_state(self, phi):
         phi = self._torch.as_tensor(phi, dtype=self._torch.float64).to(self.device).contiguous()
-        assert phi.shape == (self.L, self.L)
+        assert tuple(phi.shape) == self.shape
         self._call(lib().mpr_set_state, phi.data_ptr())
         self._torch.cuda.synchronize(self.device)
 
@@ -305,19 +323,20 @@ def predict_host(values, mask, mode="DP", seed=0, T=-1.0, n_eq=100, n_meas=100, 
     torch = _torch()
     values = np.ascontiguousarray(values, dtype=np.float64)
     mask = np.ascontiguousarray(mask, dtype=np.uint8)
-    L = int(mask.shape[0])
+    Ly, Lx = int(mask.shape[0]), int(mask.shape[1])
+    assert values.shape == mask.shape
     dev = torch.device(device)
     if workspace is None:
-        workspace = torch.empty(workspace_bytes(L, host=True) + 256, dtype=torch.uint8, device=dev)
+        workspace = torch.empty(workspace_bytes((Ly, Lx), host=True) + 256, dtype=torch.uint8, device=dev)
     off = (-workspace.data_ptr()) % 256
     if pred_out is None:
-        pred_out = np.empty((L, L), dtype=np.float64)
+        pred_out = np.empty((Ly, Lx), dtype=np.float64)
     m, s, Tu, nl = C.c_double(), C.c_double(), C.c_double(), C.c_uint64()
     with torch.cuda.device(dev):
-        st = lib().mpr_predict_host(L, values.ctypes.data, mask.ctypes.data, MODES[mode], int(seed), float(T),
-                                    int(n_eq), int(n_meas), workspace.data_ptr() + off, workspace.numel() - off,
-                                    torch.cuda.current_stream(dev).cuda_stream, pred_out.ctypes.data,
-                                    C.byref(m), C.byref(s), C.byref(Tu), C.byref(nl))
+        tail = (values.ctypes.data, mask.ctypes.data, MODES[mode], int(seed), float(T), int(n_eq), int(n_meas),
+                workspace.data_ptr() + off, workspace.numel() - off, torch.cuda.current_stream(dev).cuda_stream,
+                pred_out.ctypes.data, C.byref(m), C.byref(s), C.byref(Tu), C.byref(nl))
+        st = lib().mpr_predict_host(Lx, *tail) if Lx == Ly else lib().mpr_predict_host_rect(Lx, Ly, *tail)
     if st != MPR_OK:
         raise MprError(st)
     return pred_out, m.value, s.value, Tu.value, nl.value
