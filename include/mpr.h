@@ -236,6 +236,34 @@ int mpr_predict_host_rect(int Lx, int Ly, const double* h_values, const uint8_t*
                           void* d_workspace, size_t workspace_bytes, void* cuda_stream, double* h_pred,
                           double* e_mean, double* e_stderr, double* T_used, uint64_t* launches);
 
+/* ---- The one entry point that needs no workspace and allocates nothing (csrc/mpr_static.cu) -------------------
+ * For callers that cannot call cudaMalloc (code under CUDA-graph capture, serving loops, harnesses that forbid it)
+ * and have no workspace for mpr_create: the sample statistics the method starts from (R1: range of the measured
+ * values; R6 first half: the sample energy e_s = -2 J mean of cos[q (phi_s - phi_t)] over nearest-
+ * neighbour pairs with both ends measured), computed by four kernel launches on cuda_stream with every intermediate
+ * (per-block partial sums, the range) in a file-scope `static __device__` array of the library: 49 216 bytes, held
+ * by every GPU that loads libmpr.so until the process exits.  No cudaMalloc / cudaFree, no host allocation on the
+ * success path, no synchronisation: the call returns when the work is enqueued.
+ *   Lx, Ly     columns, rows; Lx * Ly >= 2 and <= mpr_static_max_sites() = 2^28 (16384 x 16384).  Larger grids are
+ *              rejected with MPR_ERR_INVALID_ARG (mpr_static_last_error() says why): use mpr_create.
+ *   d_values   f64[Lx*Ly] DEVICE, never read where d_mask == 1;  d_mask u8[Lx*Ly] DEVICE, 1 = prediction site
+ *   q          of Eq. 2, in (0, 1/2]; the paper's value is 0.5
+ *   d_out      f64[6] DEVICE, caller-owned: e_s, number of measured pairs, z_min, z_max, number of measured sites,
+ *              number of non-finite measured values.  e_s is NaN where mpr_create would have failed (no measured
+ *              pair, a non-finite measured value, z_max == z_min): the host cannot know without a synchronisation.
+ * The same numbers as mpr_create + mpr_sample_energy + mpr_get_info give (same per-thread order of operations).
+ * SHARED STATE: every call on a device uses the same array.  Calls that overlap on the GPU (different streams or
+ * threads without an ordering between them) race; calls on one stream, or ordered by events, do not.  The array
+ * keeps the previous call's contents; every slot a call reads it has written first, nothing needs clearing.
+ * mpr_static_setup() takes the array's device address for the CURRENT device (cudaGetSymbolAddress, once per
+ * device); the entry point does so itself on first use, but a caller about to capture a graph calls it beforehand.
+ * mpr_static_last_error(): message of the calling thread's last failed mpr_*_static* call ("" after a success). */
+int mpr_static_setup(void);
+int64_t mpr_static_max_sites(void);
+const char* mpr_static_last_error(void);
+int mpr_sample_energy_static(int Lx, int Ly, const double* d_values, const uint8_t* d_mask, double q,
+                             void* cuda_stream, double* d_out);
+
 /* HOST-only hooks into the library's host-side numerics, so that they can be pinned against
  * hand-worked numbers without a GPU (tests/test_host_logic.py); no device work, no context.
  *   mpr_debug_series_stats       mean and binned standard error (R16) of h_series[0..n), exactly

@@ -2,7 +2,8 @@
 
     python -m paper_1910_08448_b200.build [--force]
 
-Seven translation units compiled in parallel: mpr.cu (C ABI, host logic, PLAIN and TILED kernels) and
+Eight translation units compiled in parallel: mpr.cu (C ABI, host logic, PLAIN and TILED kernels), mpr_static.cu (the
+entry point that needs no workspace) and
 mpr_strip_mode.cu once per precision mode (the STRIP kernels), then one device link into the shared library.
 """
 from __future__ import annotations
@@ -19,8 +20,8 @@ LIB = os.path.join(_HERE, "libmpr.so")
 HEADERS = ["mpr_device.cuh", "mpr_host_math.hpp", "mpr_plain.cuh", "mpr_tiled.cuh", "mpr_strip.cuh",
            os.path.join("..", "..", "include", "mpr.h")]
 # (source, object name, extra flags)
-UNITS = [("mpr.cu", "mpr.o", [])] + [("mpr_strip_mode.cu", "mpr_strip_mode%d.o" % m, ["-DMPR_STRIP_MODE=%d" % m])
-                                    for m in range(6)]
+UNITS = [("mpr.cu", "mpr.o", []), ("mpr_static.cu", "mpr_static.o", [])] + \
+        [("mpr_strip_mode.cu", "mpr_strip_mode%d.o" % m, ["-DMPR_STRIP_MODE=%d" % m]) for m in range(6)]
 
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",

@@ -35,6 +35,7 @@ SYMBOLS = [
     "mpr_get_info",
     "mpr_get_launch_stats", "mpr_workspace_bytes_host", "mpr_predict_host", "mpr_debug_philox",
     "mpr_workspace_bytes_rect", "mpr_create_rect", "mpr_workspace_bytes_host_rect", "mpr_predict_host_rect",
+    "mpr_static_setup", "mpr_static_max_sites", "mpr_static_last_error", "mpr_sample_energy_static",
     "mpr_last_error", "mpr_status_string",
 ]
 
@@ -111,6 +112,10 @@ def lib():
         "mpr_predict_host": (C.c_int, [C.c_int, vp, vp, C.c_int, C.c_uint64, C.c_double, C.c_int, C.c_int, vp,
                                        C.c_size_t, vp, vp, dp, dp, dp, u64p]),
         "mpr_debug_philox": (C.c_int, [vp, C.POINTER(C.c_uint32), vp, i64, vp]),
+        "mpr_static_setup": (C.c_int, []),
+        "mpr_static_max_sites": (C.c_int64, []),
+        "mpr_static_last_error": (C.c_char_p, []),
+        "mpr_sample_energy_static": (C.c_int, [C.c_int, C.c_int, vp, vp, C.c_double, vp, vp]),
         "mpr_last_error": (C.c_char_p, [vp]),
         "mpr_status_string": (C.c_char_p, [C.c_int]),
     }
@@ -340,6 +345,27 @@ def predict_host(values, mask, mode="DP", seed=0, T=-1.0, n_eq=100, n_meas=100, 
     if st != MPR_OK:
         raise MprError(st)
     return pred_out, m.value, s.value, Tu.value, nl.value
+
+
+def static_max_sites():
+    return int(lib().mpr_static_max_sites())
+
+
+def sample_energy_static(d_values, d_mask, out, q=0.5, stream=None, shape=None):
+    """mpr_sample_energy_static: the sample energy and range of (d_values, d_mask) -- CUDA tensors f64 / u8 of shape
+    (Ly, Lx) -- into `out` (CUDA f64[6]: e_s, pairs, z_min, z_max, measured sites, non-finite values), enqueued on
+    `stream` (default: torch's current stream).  Argument marshalling only: no tensor is created here and the library
+    allocates nothing.  `shape` overrides the tensors' shape (for the size checks)."""
+    torch = _torch()
+    Ly, Lx = shape if shape is not None else (int(d_mask.shape[0]), int(d_mask.shape[1]))
+    dev = d_mask.device
+    sptr = stream.cuda_stream if stream is not None else torch.cuda.current_stream(dev).cuda_stream
+    with torch.cuda.device(dev):
+        st = lib().mpr_sample_energy_static(int(Lx), int(Ly), d_values.data_ptr(), d_mask.data_ptr(), float(q), sptr,
+                                            out.data_ptr())
+    if st != MPR_OK:
+        raise MprError(st, lib().mpr_static_last_error().decode())
+    return out
 
 
 def debug_proposal_width(T, q=None):
