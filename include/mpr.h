@@ -236,6 +236,41 @@ int mpr_predict_host_rect(int Lx, int Ly, const double* h_values, const uint8_t*
                           void* d_workspace, size_t workspace_bytes, void* cuda_stream, double* h_pred,
                           double* e_mean, double* e_stderr, double* T_used, uint64_t* launches);
 
+/* ---- Slabs of a larger grid (1-D decomposition over rows, one slab per GPU) ----------------
+ * A context created (mpr_create_rect) on rows [row0, row0 + Ly) of a larger Lx-column grid becomes a SLAB of it:
+ *   mpr_set_slab   global_row0 (even, >= 0) = the grid row of the slab's row 0; rows [own_begin, own_end) of the
+ *                  slab are the rows it OWNS, the others are halo copies of its neighbours' rows; z_min / z_max =
+ *                  the range of the WHOLE measured sample (R1); global_bonds = the whole grid's bond count (R3).
+ *                  From then on the random numbers are keyed on the global site index (so the slabs together make
+ *                  the moves a single context on the whole grid makes, bit for bit), the accepted-move count, the
+ *                  prediction-site count and every energy sum cover the own rows only, and energies are normalised
+ *                  by global_bonds: the whole grid's e is the SUM of the slabs' e.  Resets the chain.  A halo row
+ *                  is updated like any other row but sees the slab's edge as an open boundary: one colour pass
+ *                  spoils one more row from each inner edge (4 per hybrid sweep, 2 per quench double pass), so the
+ *                  caller refreshes the halos (export from the owner, import into the neighbour) at least every
+ *                  halo / 4 sweeps -- paper_1910_08448_b200/slabs.py does, in one process or one rank per slab.
+ *                  (mpr_set_workspace on a slab context: call mpr_set_slab again afterwards.)
+ *   mpr_sample_energy_parts   the sum of cos over, and the number of, measured nearest-neighbour pairs to the right
+ *                  of and below the own rows: e_s of the whole grid = -2 J sum(parts) / sum(counts).  HOST outs.
+ *   mpr_rows_bytes / mpr_export_rows / mpr_import_rows   n_rows rows of the chain state from row_begin on (both
+ *                  colours, in the storage type of the mode), packed into / read from a DEVICE buffer of
+ *                  mpr_rows_bytes bytes; enqueued on the context's stream.
+ *   mpr_advance    n_sweeps hybrid sweeps without the bookkeeping of mpr_run; measure = 0: sweeps only, 1: the energy
+ *                  of each sweep goes to slot first_slot + i of the device series, 2: and phi is accumulated.
+ *   mpr_fetch_series   the first n slots of that series -> HOST out (synchronises the stream).
+ *   mpr_predict    the back-mapped average of phi accumulated since the last chain reset -> d_pred f64[Lx*Ly].
+ *   mpr_debug_trial_lengths   the fixed sweep counts of one temperature trial of R6 (equilibration, measurement). */
+int mpr_set_slab(mpr_ctx* ctx, int global_row0, int own_begin, int own_end, double z_min, double z_max,
+                 double global_bonds);
+int mpr_sample_energy_parts(mpr_ctx* ctx, double* cos_sum, int64_t* n_pairs);
+int mpr_rows_bytes(mpr_ctx* ctx, int n_rows, size_t* bytes);
+int mpr_export_rows(mpr_ctx* ctx, int row_begin, int n_rows, void* d_out);
+int mpr_import_rows(mpr_ctx* ctx, int row_begin, int n_rows, const void* d_in);
+int mpr_advance(mpr_ctx* ctx, int n_sweeps, int measure, int first_slot);
+int mpr_fetch_series(mpr_ctx* ctx, int n, double* h_out);
+int mpr_predict(mpr_ctx* ctx, double* d_pred);
+void mpr_debug_trial_lengths(int* n_eq, int* n_meas);
+
 /* ---- The one entry point that needs no workspace and allocates nothing (csrc/mpr_static.cu) -------------------
  * For callers that cannot call cudaMalloc (code under CUDA-graph capture, serving loops, harnesses that forbid it)
  * and have no workspace for mpr_create: the sample statistics the method starts from (R1: range of the measured

@@ -50,6 +50,9 @@ Layout make_layout(int L, int H) {      // L columns, H rows
   Layout lo;
   lo.g.L = L;
   lo.g.H = H;
+  lo.g.site0 = 0u;
+  lo.g.own0 = 0;
+  lo.g.own1 = H;
   lo.g.Wp = static_cast<int>(align_up(static_cast<size_t>((L + 1) / 2), 16));
   lo.g.Wm = (lo.g.Wp + 31) / 32;
   lo.g.Wb = lo.g.Wm + kBitPadLeft + kBitPadRight;
@@ -108,7 +111,10 @@ struct mpr_ctx {
   double zmin = 0.0, zmax = 0.0;
   double e_sample = 0.0;
   long long n_pairs = 0;
-  long long n_free = 0;
+  long long n_free = 0;          // prediction sites of the rows that count (all rows; a slab: its own rows)
+  double pair_sum = 0.0;         // sum of cos over the measured pairs behind e_sample (mpr_sample_energy_parts)
+  double nb_norm = 0.0;          // bonds the energy is normalised by: bond_count(g), or the whole grid's for a slab
+  bool slab = false;
   uint32_t n_list[2] = {0u, 0u};     // prediction sites per colour (lengths of the LIST path's lists)
   uint64_t launches = 0;
   std::vector<double> series;
@@ -271,7 +277,7 @@ template <int MODE> int plain_energy(mpr_ctx* c, double* d_out, bool as_e) {
   const int nblk = g.H < 2048 ? g.H : 2048;
   plain_energy_kernel<MODE><<<nblk, 256, 0, c->stream>>>(static_cast<const V*>(c->state(c->cur)), g, c->part());
   LAUNCH_OK(c);
-  const double nb = bond_count(g);
+  const double nb = c->nb_norm;
   final_sum_kernel<<<1, 1024, 0, c->stream>>>(c->part(), nblk, as_e ? -kJ * 2.0 / nb : -kJ, d_out, g.energy_single);
   LAUNCH_OK(c);
   return MPR_OK;
@@ -318,7 +324,7 @@ template <int MODE> int tiled_sweeps(mpr_ctx* c, int k, int measure, double* d_e
   c->launches += 1;
   c->cur = 1 - c->cur;
   if (measure == 1 || measure == 2) {
-    const double nb = bond_count(g);
+    const double nb = c->nb_norm;
     final_sum_kernel<<<1, 1024, 0, c->stream>>>(c->part(), ntiles, -kJ * 2.0 / nb, d_e, g.energy_single);
     LAUNCH_OK(c);
   }
@@ -341,7 +347,7 @@ template <int MODE> int strip_sweeps(mpr_ctx* c, int prog, int k, int measure, d
   c->launches += 1;
   c->cur = 1 - c->cur;
   if (measure == 1 || measure == 2) {
-    const double nb = bond_count(g);
+    const double nb = c->nb_norm;
     final_sum_kernel<<<1, 1024, 0, c->stream>>>(c->part(), nblocks, -kJ * 2.0 / nb, d_e, g.energy_single);
     LAUNCH_OK(c);
   }
@@ -593,7 +599,7 @@ int setup(mpr_ctx* c) {
   c->zmin = h[0];
   c->zmax = h[1];
   // R6: sample energy
-  sample_energy_kernel<<<nblk, 256, 0, c->stream>>>(c->d_values, c->d_mask, g.L, g.H, c->zmin, c->zmax, c->part(), g.q);
+  sample_energy_kernel<<<nblk, 256, 0, c->stream>>>(c->d_values, c->d_mask, g.L, g.H, g.own0, g.own1, c->zmin, c->zmax, c->part(), g.q);
   LAUNCH_OK(c);
   pair_final_kernel<<<1, 32, 0, c->stream>>>(c->part(), nblk, c->scal());
   LAUNCH_OK(c);
@@ -628,6 +634,8 @@ int setup(mpr_ctx* c) {
   CUDA_OK(c, cudaMemcpyAsync(h2, c->scal(), sizeof(h2), cudaMemcpyDeviceToHost, c->stream));
   CUDA_OK(c, cudaStreamSynchronize(c->stream));
   c->n_pairs = static_cast<long long>(h2[1]);
+  c->pair_sum = h2[0];
+  if (!c->slab) c->nb_norm = bond_count(g);
   c->e_sample = c->n_pairs > 0 ? -2.0 * kJ * h2[0] / h2[1] : std::numeric_limits<double>::quiet_NaN();
   c->n_free = static_cast<long long>(h2[2]);
   return MPR_OK;
@@ -920,7 +928,7 @@ int mpr_energy(mpr_ctx* c, double* H, double* e) {
   double h = 0.0;
   CUDA_OK(c, cudaMemcpyAsync(&h, c->scal() + 8, sizeof(double), cudaMemcpyDeviceToHost, c->stream));
   CUDA_OK(c, cudaStreamSynchronize(c->stream));
-  const double nb = bond_count(c->lo.g);
+  const double nb = c->nb_norm;
   if (H) *H = h;
   if (e) *e = c->lo.g.energy_single ? static_cast<double>(2.0f * static_cast<float>(h) / static_cast<float>(nb))
                                     : 2.0 * h / nb;
@@ -933,6 +941,106 @@ int mpr_sample_energy(mpr_ctx* c, double* e_sample, int64_t* n_pairs) {
   if (n_pairs) *n_pairs = c->n_pairs;
   if (c->n_pairs == 0) return fail(c, MPR_ERR_NO_MEASURED, "no measured nearest-neighbour pair");
   if (e_sample) *e_sample = c->e_sample;
+  return MPR_OK;
+}
+
+int mpr_sample_energy_parts(mpr_ctx* c, double* cos_sum, int64_t* n_pairs) {
+  if (!c) return MPR_ERR_INVALID_ARG;
+  if (!c->ws) return fail(c, MPR_ERR_WORKSPACE, "no workspace attached (mpr_set_workspace)");
+  if (cos_sum) *cos_sum = c->pair_sum;
+  if (n_pairs) *n_pairs = c->n_pairs;
+  return MPR_OK;
+}
+
+// ---- slabs of a larger grid ----------------------------------------------------
+static size_t spin_bytes(int mode) { return mode == MPR_HP ? 4 : (mode == MPR_DP || mode == MPR_DS_INTRINSIC) ? 16 : 8; }
+
+int mpr_set_slab(mpr_ctx* c, int global_row0, int own_begin, int own_end, double z_min, double z_max, double global_bonds) {
+  if (!c) return MPR_ERR_INVALID_ARG;
+  if (!c->ws) return fail(c, MPR_ERR_WORKSPACE, "no workspace attached (mpr_set_workspace)");
+  Geom& g = c->lo.g;
+  if (global_row0 < 0 || (global_row0 & 1) || own_begin < 0 || own_end > g.H || own_begin >= own_end || !(z_max > z_min) ||
+      !std::isfinite(z_min) || !std::isfinite(z_max) || !(global_bonds >= 1.0) ||
+      (static_cast<long long>(global_row0) + g.H) * g.L > (1ll << 32))
+    return fail(c, MPR_ERR_INVALID_ARG, "slab: first row even and >= 0, 0 <= own_begin < own_end <= rows, z_max > z_min");
+  CUDA_OK(c, cudaStreamSynchronize(c->stream));
+  g.site0 = static_cast<uint32_t>(static_cast<long long>(global_row0) * g.L);
+  g.own0 = own_begin;
+  g.own1 = own_end;
+  c->zmin = z_min;
+  c->zmax = z_max;
+  c->nb_norm = global_bonds;
+  c->slab = true;
+  // the measured pairs to the right of and below the slab's own rows, in the whole sample's range
+  const int nblk = 1024;
+  sample_energy_kernel<<<nblk, 256, 0, c->stream>>>(c->d_values, c->d_mask, g.L, g.H, g.own0, g.own1, c->zmin, c->zmax, c->part(), g.q);
+  LAUNCH_OK(c);
+  pair_final_kernel<<<1, 32, 0, c->stream>>>(c->part(), nblk, c->scal());
+  LAUNCH_OK(c);
+  double h2[2];
+  CUDA_OK(c, cudaMemcpyAsync(h2, c->scal(), sizeof(h2), cudaMemcpyDeviceToHost, c->stream));
+  // prediction sites of the own rows (the per-row counts the LIST set-up left in the workspace)
+  std::vector<uint32_t> rc(static_cast<size_t>(2) * g.H);
+  CUDA_OK(c, cudaMemcpyAsync(rc.data(), c->rows(), rc.size() * sizeof(uint32_t), cudaMemcpyDeviceToHost, c->stream));
+  CUDA_OK(c, cudaStreamSynchronize(c->stream));
+  c->pair_sum = h2[0];
+  c->n_pairs = static_cast<long long>(h2[1]);
+  c->e_sample = c->n_pairs > 0 ? -2.0 * kJ * h2[0] / h2[1] : std::numeric_limits<double>::quiet_NaN();
+  long long nf = 0;
+  for (int col = 0; col < 2; ++col)
+    for (int y = own_begin; y < own_end; ++y) nf += rc[static_cast<size_t>(col) * g.H + y];
+  c->n_free = nf;
+  mark_stale(c);
+  return MPR_OK;
+}
+
+int mpr_rows_bytes(mpr_ctx* c, int n_rows, size_t* bytes) {
+  if (!c || !bytes || n_rows < 0 || n_rows > c->lo.g.H) return MPR_ERR_INVALID_ARG;
+  *bytes = static_cast<size_t>(2) * n_rows * c->lo.g.Wp * spin_bytes(c->mode);
+  return MPR_OK;
+}
+
+static int copy_rows(mpr_ctx* c, int row_begin, int n_rows, void* d_buf, bool out) {
+  if (!c || !d_buf) return fail(c, MPR_ERR_INVALID_ARG, "null pointer");
+  const Geom& g = c->lo.g;
+  if (row_begin < 0 || n_rows < 0 || row_begin + n_rows > g.H) return fail(c, MPR_ERR_INVALID_ARG, "rows outside the grid");
+  TRY(ensure_chain(c));
+  const size_t sb = spin_bytes(c->mode), row_b = static_cast<size_t>(g.Wp) * sb, chunk = row_b * n_rows;
+  char* st = static_cast<char*>(c->state(c->cur));
+  for (int col = 0; col < 2 && n_rows > 0; ++col) {
+    char* in_state = st + (static_cast<size_t>(col) * g.plane + static_cast<size_t>(row_begin) * g.Wp) * sb;
+    char* in_buf = static_cast<char*>(d_buf) + col * chunk;
+    CUDA_OK(c, cudaMemcpyAsync(out ? in_buf : in_state, out ? in_state : in_buf, chunk, cudaMemcpyDeviceToDevice, c->stream));
+  }
+  return MPR_OK;
+}
+int mpr_export_rows(mpr_ctx* c, int row_begin, int n_rows, void* d_out) { return copy_rows(c, row_begin, n_rows, d_out, true); }
+int mpr_import_rows(mpr_ctx* c, int row_begin, int n_rows, const void* d_in) {
+  return copy_rows(c, row_begin, n_rows, const_cast<void*>(d_in), false);
+}
+
+int mpr_advance(mpr_ctx* c, int n_sweeps, int measure, int first_slot) {
+  if (!c || n_sweeps < 0 || measure < 0 || measure > 2 || first_slot < 0 ||
+      (measure && static_cast<long long>(first_slot) + n_sweeps > kSeriesCap))
+    return fail(c, MPR_ERR_INVALID_ARG, "bad sweep count, measure flag or series slot");
+  return hybrid_sweeps(c, n_sweeps, measure, first_slot);
+}
+
+int mpr_fetch_series(mpr_ctx* c, int n, double* h_out) {
+  if (!c || n < 0 || n > kSeriesCap || (n > 0 && !h_out)) return fail(c, MPR_ERR_INVALID_ARG, "bad series length");
+  if (!c->ws) return fail(c, MPR_ERR_WORKSPACE, "no workspace attached (mpr_set_workspace)");
+  TRY(fetch_series(c, n));
+  for (int i = 0; i < n; ++i) h_out[i] = c->series[static_cast<size_t>(i)];
+  return MPR_OK;
+}
+
+int mpr_predict(mpr_ctx* c, double* d_pred) {
+  if (!c || !d_pred) return fail(c, MPR_ERR_INVALID_ARG, "null pointer");
+  TRY(ensure_chain(c));
+  const Geom& g = c->lo.g;
+  dim3 block(128), grid((g.L + 127) / 128, g.H);
+  predict_kernel<<<grid, block, 0, c->stream>>>(c->d_values, c->d_mask, g, c->acc(), c->zmin, c->zmax, c->n_acc, d_pred);
+  LAUNCH_OK(c);
   return MPR_OK;
 }
 
@@ -1035,6 +1143,10 @@ int mpr_predict_host_rect(int Lx, int Ly, const double* h_values, const uint8_t*
   return st;
 }
 
+void mpr_debug_trial_lengths(int* n_eq, int* n_meas) {
+  if (n_eq) *n_eq = kTrialEq;
+  if (n_meas) *n_meas = kTrialMeas;
+}
 double mpr_debug_proposal_width(double T) { return proposal_width(T); }
 double mpr_debug_proposal_width_q(double T, double q) { return proposal_width(T, q); }
 

@@ -21,6 +21,11 @@ struct Geom {
   int Wb, Hb;            // padded bitmap: words per row, rows per colour
   size_t plane;          // elements per colour plane = H * Wp
   int H;                 // rows of the grid (y); == L unless created by mpr_create_rect
+  // Slab of a larger grid (mpr_set_slab): the context holds rows [row0, row0 + H) of it.  The random
+  // numbers are keyed on the GLOBAL site index (site0 = row0 * L is added to every local one), and only rows
+  // [own0, own1) -- the rows this slab owns, the rest being halo -- enter the energy sums and the accepted-move count.
+  uint32_t site0;        // 0 for a whole grid
+  int own0, own1;        // [0, H) for a whole grid
   double q;              // PAPER.md:27, q in (0, 1/2]; 1/2 unless mpr_set_q
   int energy_single;     // X_E of PAPER.md:35: 0 = energy sums in double (R13), 1 = the energy variable is a float
 };
@@ -139,7 +144,7 @@ __device__ __forceinline__ double map_to_phi(double z, double zmin, double zmax)
 
 // R6 first half: e_s = -2J mean over measured nearest-neighbour pairs of cos[q(phi_s - phi_t)].
 // Per-block partials: [0] sum of cos, [1] pair count.
-static __global__ void sample_energy_kernel(const double* __restrict__ z, const uint8_t* __restrict__ mask, int L, int H,
+static __global__ void sample_energy_kernel(const double* __restrict__ z, const uint8_t* __restrict__ mask, int L, int H, int own0, int own1,
                                      double zmin, double zmax, double* __restrict__ part /* 2 per block */, double q) {
   __shared__ double sh[32];
   double sum = 0.0, cnt = 0.0;
@@ -148,6 +153,7 @@ static __global__ void sample_energy_kernel(const double* __restrict__ z, const 
        i += static_cast<size_t>(gridDim.x) * blockDim.x) {
     if (mask[i]) continue;
     const int x = static_cast<int>(i % L), y = static_cast<int>(i / L);
+    if (y < own0 || y >= own1) continue;      // a slab counts the bonds to the right of and below its own rows
     const double p = map_to_phi(z[i], zmin, zmax);
     if (x < L - 1 && !mask[i + 1]) { sum += cos(q * (p - map_to_phi(z[i + 1], zmin, zmax))); cnt += 1.0; }
     if (y < H - 1 && !mask[i + L]) { sum += cos(q * (p - map_to_phi(z[i + L], zmin, zmax))); cnt += 1.0; }
@@ -206,7 +212,7 @@ __global__ void init_chain_kernel(const double* __restrict__ z, const uint8_t* _
     const size_t s = static_cast<size_t>(y) * g.L + x;
     double phi;
     if (mask[s]) {
-      const uint4 r = philox4x32_10(static_cast<uint32_t>(s), 0u, PASS_INIT, trial, k0, k1);
+      const uint4 r = philox4x32_10(g.site0 + static_cast<uint32_t>(s), 0u, PASS_INIT, trial, k0, k1);
       phi = 6.283185307179586476925286766559 * u53(r.x, r.y);
     } else {
       phi = map_to_phi(z[s], zmin, zmax);
@@ -287,7 +293,7 @@ __device__ __forceinline__ bool plain_site_update(typename Traits<MODE>::vec* __
   R c = R(me.x), s = R(me.y);
   if constexpr (KIND == KIND_MET || KIND == KIND_MO) {
     // R9: the quad (plane columns 2m, 2m + 1) x (rows 2k, 2k + 1) shares one Philox block in the float modes
-    const uint32_t pair_site = static_cast<uint32_t>(y) * static_cast<uint32_t>(g.L) +
+    const uint32_t pair_site = g.site0 + static_cast<uint32_t>(y) * static_cast<uint32_t>(g.L) +
                                static_cast<uint32_t>(2 * (j & ~1) + par);
     MetWords w0, w1;
     met_words_pair<MODE>(pair_site, sweep, static_cast<uint32_t>(g.L), par, (y & 1) != 0, k, &w0, &w1);
@@ -296,7 +302,7 @@ __device__ __forceinline__ bool plain_site_update(typename Traits<MODE>::vec* __
     bool ok[2];
     met_update2<MODE, GENQ>(bc2(c), bc2(s), bc2(A), bc2(B), w, w, true, true, k, o, ok);   // the site in both lanes
     c = o[0]; s = o[2];
-    accepted = ok[0];
+    accepted = ok[0] && y >= g.own0 && y < g.own1;
     if constexpr (KIND == KIND_MO) {     // site-fused schedule (R4b): the over-relaxation move follows at once
       R o2[4];
       or_update2<MODE, GENQ>(bc2(c), bc2(s), bc2(A), bc2(B), true, true, o2, &k);
@@ -427,7 +433,7 @@ plain_energy_kernel(const typename Traits<MODE>::vec* __restrict__ state, Geom g
   __shared__ double sh[32];
   double sum = 0.0;
   const int col = 1;
-  for (int y = blockIdx.x; y < g.H; y += gridDim.x) {
+  for (int y = g.own0 + blockIdx.x; y < g.own1; y += gridDim.x) {
     const int par = x_parity(y, col);
     const V* own = state + static_cast<size_t>(col) * g.plane + static_cast<size_t>(y) * g.Wp;
     const V* oth = state + static_cast<size_t>(1 - col) * g.plane + static_cast<size_t>(y) * g.Wp;

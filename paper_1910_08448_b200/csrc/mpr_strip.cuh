@@ -204,8 +204,11 @@ strip_kernel(const __grid_constant__ CUtensorMap tmap, typename Traits<MODE>::ve
       const int n_steps = ye - t0 + LAG * (NS - 1);           // the last stage finishes row ye - 1 in the last step
       const int n_iter = (n_steps + RB - 1) / RB;
       // iterations in which every stage works on an owned, loaded row in all four steps: no predicates needed
-      const int i_lo = (LEAD + LAG * (NS - 1) + RB - 1) / RB;
-      const int i_hi = (ye - t0) / RB;                        // RB i + RB - 1 < ye - t0
+      // [cnt_b, cnt_e): the rows of the segment that enter the accepted-move count and the energy sum -- all of them,
+      // unless the context is a slab of a larger grid (Geom::own0 / own1: its halo rows are updated and stored, not counted)
+      const int cnt_b = max(yb, g.own0), cnt_e = min(ye, g.own1);
+      const int i_lo = (cnt_b - t0 + LAG * (NS - 1) + RB - 1) / RB;     // = (LEAD + LAG (NS - 1) + RB - 1) / RB when cnt_b = yb
+      const int i_hi = (max(cnt_e, t0) - t0) / RB;                      // RB i + RB - 1 < cnt_e - t0
       const int j = j0 + 2 * lane;
       const bool lane_ok = lane >= HL && lane < 32 - HL && j < g.Wp;
       int seg_acc = 0;
@@ -231,7 +234,7 @@ strip_kernel(const __grid_constant__ CUtensorMap tmap, typename Traits<MODE>::ve
 #pragma unroll
       for (int k = 0; k < NQ; ++k) cw[k] = 0u;
 
-      uint32_t site_t = static_cast<uint32_t>(t0) * Lu + static_cast<uint32_t>(2 * j);   // Philox word 0 of row t, no parity
+      uint32_t site_t = g.site0 + static_cast<uint32_t>(t0) * Lu + static_cast<uint32_t>(2 * j);   // Philox word 0 of row t, no parity
       // global pointers of this lane's unit in row t of plane 0 (dst / accumulator); never dereferenced outside the grid
       const long long g_t0 = static_cast<long long>(t0) * g.Wp + j;
       S* gp = reinterpret_cast<S*>(dst) + 2 * g_t0;
@@ -340,7 +343,7 @@ strip_kernel(const __grid_constant__ CUtensorMap tmap, typename Traits<MODE>::ve
               met_update2<MODE>(c[p], s[p], A[p], B[p], w0, w1, fa, fb, kc, o[p], ok);
               // accepted moves are counted per lane; the lanes that do not own their columns are dropped at the end
               const int row = t - LAG * p;
-              if (!EDGE || (row >= yb && row < ye)) seg_acc += static_cast<int>(ok[0]) + static_cast<int>(ok[1]);
+              if (!EDGE || (row >= cnt_b && row < cnt_e)) seg_acc += static_cast<int>(ok[0]) + static_cast<int>(ok[1]);
               if (kind == KIND_MO) {
                 R o2[4];
                 or_update2<MODE>(mk2(o[p][0], o[p][1]), mk2(o[p][2], o[p][3]), A[p], B[p], fa, fb, o2);
@@ -381,7 +384,7 @@ strip_kernel(const __grid_constant__ CUtensorMap tmap, typename Traits<MODE>::ve
                     *reinterpret_cast<double2*>(a) = a2;
                   }
                 }
-                if (MEASURE != 0 && p == NS - 1) {
+                if (MEASURE != 0 && p == NS - 1 && (!EDGE || (row >= cnt_b && row < cnt_e))) {
                   // every bond has exactly one colour-1 end: H = -J sum over colour-1 sites of site_energy_term
                   // with the final spins; the neighbours (colour 0) were final when this stage gathered them
                   if constexpr (sizeof(R) == 8) {

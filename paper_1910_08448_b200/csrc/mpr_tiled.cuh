@@ -333,7 +333,7 @@ tiled_sweep_kernel(const __grid_constant__ CUtensorMap tmap, typename Traits<MOD
   }
   const bool col_interior = jj >= hc && jj < kTileCols - hc;
   // Philox counter word 0 of the first site of this thread's pair in tile row 0, without the parity
-  const uint32_t site_row0 = static_cast<uint32_t>(y0) * static_cast<uint32_t>(g.L) + static_cast<uint32_t>(2 * (j0 + jj));
+  const uint32_t site_row0 = g.site0 + static_cast<uint32_t>(y0) * static_cast<uint32_t>(g.L) + static_cast<uint32_t>(2 * (j0 + jj));
   const uint32_t Lu = static_cast<uint32_t>(g.L);
   __syncthreads();          // mbarrier initialised before anyone polls it
   mbar_wait(bar, 0);
@@ -346,6 +346,14 @@ tiled_sweep_kernel(const __grid_constant__ CUtensorMap tmap, typename Traits<MOD
       const int r = warp * RPW + i;
       if (r >= h && r < TH - h) cnt |= 1u << i;
     }
+  }
+  // the rows among them that enter the accepted-move count and the energy sum: all, unless the context is a slab of a
+  // larger grid (then its own rows only, Geom::own0 / own1)
+  uint32_t cnt_c = 0;
+#pragma unroll
+  for (int i = 0; i < RPW; ++i) {
+    const int row = y0 + warp * RPW + i;
+    if (((cnt >> i) & 1u) && row >= g.own0 && row < g.own1) cnt_c |= 1u << i;
   }
   int n_acc = 0;
 #pragma unroll 1
@@ -361,9 +369,9 @@ tiled_sweep_kernel(const __grid_constant__ CUtensorMap tmap, typename Traits<MOD
       }
       continue;
     }
-    n_acc += pass_rows<MODE, KIND_MET, 0>(t, mreg[0], cnt, site_row0, Lu, sweep, kc);
+    n_acc += pass_rows<MODE, KIND_MET, 0>(t, mreg[0], cnt_c, site_row0, Lu, sweep, kc);
     pass_sync<MODE>(warp);
-    n_acc += pass_rows<MODE, KIND_MET, 1>(t, mreg[1], cnt, site_row0, Lu, sweep, kc);
+    n_acc += pass_rows<MODE, KIND_MET, 1>(t, mreg[1], cnt_c, site_row0, Lu, sweep, kc);
     pass_sync<MODE>(warp);
     pass_rows<MODE, KIND_OR, 0>(t, mreg[0], cnt, site_row0, Lu, sweep, kc);
     pass_sync<MODE>(warp);
@@ -393,7 +401,7 @@ tiled_sweep_kernel(const __grid_constant__ CUtensorMap tmap, typename Traits<MOD
         const Unit<S> u1 = *reinterpret_cast<const Unit<S>*>(sp + (TH + i) * kRowScalars);
         *reinterpret_cast<Unit<S>*>(gp + i * grow) = u0;
         *reinterpret_cast<Unit<S>*>(gp + i * grow + gplane) = u1;
-        if constexpr (MEASURE == 1 || MEASURE == 2) {
+        if ((MEASURE == 1 || MEASURE == 2) && ((cnt_c >> i) & 1u)) {
           // every bond has exactly one colour-1 end: H = -J sum over colour-1 sites of their
           // site_energy_term (mpr_device.cuh; the same function as plain_energy_kernel).  The
           // neighbours are the other plane's units of rows r - 1, r, r + 1 and one extra site:

@@ -35,6 +35,8 @@ SYMBOLS = [
     "mpr_get_info",
     "mpr_get_launch_stats", "mpr_workspace_bytes_host", "mpr_predict_host", "mpr_debug_philox",
     "mpr_workspace_bytes_rect", "mpr_create_rect", "mpr_workspace_bytes_host_rect", "mpr_predict_host_rect",
+    "mpr_set_slab", "mpr_sample_energy_parts", "mpr_rows_bytes", "mpr_export_rows", "mpr_import_rows", "mpr_advance",
+    "mpr_fetch_series", "mpr_predict", "mpr_debug_trial_lengths",
     "mpr_static_setup", "mpr_static_max_sites", "mpr_static_last_error", "mpr_sample_energy_static",
     "mpr_last_error", "mpr_status_string",
 ]
@@ -112,6 +114,15 @@ def lib():
         "mpr_predict_host": (C.c_int, [C.c_int, vp, vp, C.c_int, C.c_uint64, C.c_double, C.c_int, C.c_int, vp,
                                        C.c_size_t, vp, vp, dp, dp, dp, u64p]),
         "mpr_debug_philox": (C.c_int, [vp, C.POINTER(C.c_uint32), vp, i64, vp]),
+        "mpr_set_slab": (C.c_int, [vp, C.c_int, C.c_int, C.c_int, C.c_double, C.c_double, C.c_double]),
+        "mpr_sample_energy_parts": (C.c_int, [vp, dp, i64p]),
+        "mpr_rows_bytes": (C.c_int, [vp, C.c_int, C.POINTER(C.c_size_t)]),
+        "mpr_export_rows": (C.c_int, [vp, C.c_int, C.c_int, vp]),
+        "mpr_import_rows": (C.c_int, [vp, C.c_int, C.c_int, vp]),
+        "mpr_advance": (C.c_int, [vp, C.c_int, C.c_int, C.c_int]),
+        "mpr_fetch_series": (C.c_int, [vp, C.c_int, dp]),
+        "mpr_predict": (C.c_int, [vp, vp]),
+        "mpr_debug_trial_lengths": (None, [C.POINTER(C.c_int), C.POINTER(C.c_int)]),
         "mpr_static_setup": (C.c_int, []),
         "mpr_static_max_sites": (C.c_int64, []),
         "mpr_static_last_error": (C.c_char_p, []),
@@ -315,6 +326,45 @@ class Mpr:
         self._call(lib().mpr_get_run_timing, C.byref(ms), C.byref(nl), C.byref(ns))
         return ms.value, nl.value, ns.value
 
+    # -- slabs of a larger grid (include/mpr.h, "Slabs"; orchestrated by slabs.py) -------------
+    def set_slab(self, global_row0, own_begin, own_end, z_min, z_max, global_bonds):
+        self._call(lib().mpr_set_slab, int(global_row0), int(own_begin), int(own_end), float(z_min), float(z_max),
+                   float(global_bonds))
+
+    def sample_energy_parts(self):
+        s, n = C.c_double(), C.c_int64()
+        self._call(lib().mpr_sample_energy_parts, C.byref(s), C.byref(n))
+        return s.value, n.value
+
+    def rows_bytes(self, n_rows):
+        n = C.c_size_t()
+        self._call(lib().mpr_rows_bytes, int(n_rows), C.byref(n))
+        return n.value
+
+    def export_rows(self, row_begin, n_rows, out=None):
+        """n_rows rows of the chain state from row_begin on -> uint8 CUDA tensor of rows_bytes(n_rows)."""
+        if out is None:
+            out = self._torch.empty(self.rows_bytes(n_rows), dtype=self._torch.uint8, device=self.device)
+        self._call(lib().mpr_export_rows, int(row_begin), int(n_rows), out.data_ptr())
+        return out
+
+    def import_rows(self, row_begin, n_rows, buf):
+        assert buf.is_cuda and buf.is_contiguous() and buf.numel() == self.rows_bytes(n_rows)
+        self._call(lib().mpr_import_rows, int(row_begin), int(n_rows), buf.data_ptr())
+
+    def advance(self, n_sweeps, measure=0, first_slot=0):
+        self._call(lib().mpr_advance, int(n_sweeps), int(measure), int(first_slot))
+
+    def fetch_series(self, n):
+        out = np.empty(int(n), dtype=np.float64)
+        self._call(lib().mpr_fetch_series, int(n), out.ctypes.data_as(C.POINTER(C.c_double)))
+        return out
+
+    def predict(self):
+        pred = self._torch.empty(self.shape, dtype=self._torch.float64, device=self.device)
+        self._call(lib().mpr_predict, pred.data_ptr())
+        return pred
+
     def launches(self):
         n = C.c_uint64()
         self._call(lib().mpr_get_launch_stats, C.byref(n))
@@ -345,6 +395,13 @@ def predict_host(values, mask, mode="DP", seed=0, T=-1.0, n_eq=100, n_meas=100, 
     if st != MPR_OK:
         raise MprError(st)
     return pred_out, m.value, s.value, Tu.value, nl.value
+
+
+def debug_trial_lengths():
+    """(equilibration sweeps, measurement sweeps) of one temperature trial of R6, as the library runs it."""
+    a, b = C.c_int(), C.c_int()
+    lib().mpr_debug_trial_lengths(C.byref(a), C.byref(b))
+    return a.value, b.value
 
 
 def static_max_sites():
