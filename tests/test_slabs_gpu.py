@@ -1,0 +1,114 @@
+"""Slab decomposition (paper_1910_08448_b200/slabs.py, include/mpr.h "Slabs") on ONE GPU: G slab contexts
+worked off in turn with halo refreshes must reproduce the single-context run on the whole grid bit for bit (spins,
+accepted moves, prediction) and its energies up to the order of the final sums; in DP they match the oracle like the
+single context does."""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+PHI_TOL = 1e-9
+
+
+@pytest.fixture(scope="module")
+def mpr():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    from paper_1910_08448_b200 import build, mpr as m
+    build.build()
+    m.lib()
+    return m
+
+
+@pytest.fixture(scope="module")
+def inputs():
+    from paper_1910_08448_b200 import inputs as i
+    return i
+
+
+@pytest.fixture(scope="module")
+def slabs():
+    from paper_1910_08448_b200 import slabs as s
+    return s
+
+
+def whole(mpr, values, mask, mode, seed, path, schedule, T, n_eq, n_meas):
+    g = mpr.Mpr(values, mask, mode=mode, seed=seed)
+    g.set_path(path); g.set_schedule(schedule); g.set_temperature(T)
+    pred, e, se = g.run(n_eq, n_meas)
+    out = (g.get_state().cpu().numpy(), g.counters()[0], g.series(), pred.cpu().numpy(), e, se, g.sample_energy(), g.info())
+    g.close()
+    return out
+
+
+@pytest.mark.parametrize("mode,path,schedule", [("DP", "PLAIN", "R4"), ("DP", "TILED", "R4"), ("DP", "STRIP", "SITE_FUSED"),
+                                                ("SP_INTRINSIC", "STRIP", "R4"), ("SP_INTRINSIC", "TILED", "R4"),
+                                                ("SP_INTRINSIC", "LIST", "SITE_FUSED"), ("SP", "STRIP", "R4"),
+                                                ("HP", "STRIP", "R4")])
+@pytest.mark.parametrize("count,halo", [(1, 8), (2, 4), (3, 8), (5, 12)])
+def test_slabs_reproduce_the_single_context(mpr, inputs, slabs, mode, path, schedule, count, halo):
+    Ly, Lx = 190, 141
+    values, mask, _ = inputs.make_rect_problem(Ly, Lx, 7.0, 51, 0.7)
+    T, n_eq, n_meas = 0.04, 7, 6
+    st_w, acc_w, series_w, pred_w, e_w, se_w, (es_w, np_w), info_w = whole(mpr, values, mask, mode, 77, path, schedule, T, n_eq, n_meas)
+    ss = slabs.make_slab_set(values, mask, count, halo=halo, mode=mode, seed=77, path=path, schedule=schedule)
+    assert (ss.z_min, ss.z_max) == (info_w["z_min"], info_w["z_max"]) and ss.n_free == info_w["n_free"]
+    assert ss.n_pairs == np_w and abs(ss.e_sample - es_w) <= 1e-12 * abs(es_w)
+    ss.set_temperature(T)
+    ss.reset_chain(0)
+    series, e, se = ss.run(n_eq, n_meas)
+    assert np.array_equal(ss.state(), st_w)                      # every spin, bit for bit
+    assert ss.accepted() == acc_w
+    tol = 1e-12 if mode != "HP" else 1e-12
+    assert np.max(np.abs(series - np.asarray(series_w))) <= tol * 2.0, (series, series_w)
+    assert abs(e - e_w) <= 2e-12 and abs(se - se_w) <= 2e-12
+    pw, ps = np.nan_to_num(pred_w, nan=-1.0), np.nan_to_num(ss.prediction(), nan=-1.0)
+    assert np.array_equal(ps, pw)
+
+
+def test_slabs_dp_match_the_oracle(mpr, oracle_mod, inputs, slabs):
+    Ly, Lx = 120, 97
+    values, mask, _ = inputs.make_rect_problem(Ly, Lx, 6.0, 52, 0.8)
+    o = oracle_mod.Oracle(values=values, mask=mask, seed=5)
+    o.set_temperature(0.06)
+    ss = slabs.make_slab_set(values, mask, 3, halo=8, mode="DP", seed=5, path="STRIP")
+    ss.set_temperature(0.06)
+    ss.reset_chain(0)
+    pred_o, e_o, se_o = o.run(9, 8)
+    series, e, se = ss.run(9, 8)
+    assert np.max(np.abs(ss.state() - o.get_state())) <= PHI_TOL
+    assert ss.accepted() == o.counters()[0]
+    assert abs(e - e_o) <= 1e-11 and abs(se - se_o) <= 1e-11
+    zr = o.zrange()
+    assert np.max(np.abs(ss.prediction() - pred_o)) <= 1e-9 * (zr[1] - zr[0])
+
+
+def test_slabs_temperature_matching(mpr, inputs, slabs):
+    """R6 over slabs: every trial chain runs on all slabs, the energies are the summed parts."""
+    Ly, Lx = 96, 96
+    values, mask, _ = inputs.make_rect_problem(Ly, Lx, 8.0, 53, 0.66)
+    g = mpr.Mpr(values, mask, mode="DP", seed=9)
+    T_w = g.estimate_temperature()[0]
+    g.close()
+    ss = slabs.make_slab_set(values, mask, 2, halo=8, mode="DP", seed=9)
+    T_s = ss.estimate_temperature()
+    assert abs(T_s - T_w) <= 1e-9 * T_w
+    assert ss.exchanges > 0
+
+
+def test_slab_argument_checks(mpr, inputs, slabs):
+    values, mask, _ = inputs.make_rect_problem(40, 33, 5.0, 54, 0.5)
+    g = mpr.Mpr(values, mask)
+    for args in [(1, 0, 40, 0.0, 1.0, 100.0), (0, 5, 5, 0.0, 1.0, 100.0), (0, 0, 41, 0.0, 1.0, 100.0), (0, 0, 40, 1.0, 1.0, 100.0),
+                 (-2, 0, 40, 0.0, 1.0, 100.0)]:
+        with pytest.raises(mpr.MprError) as ei:
+            g.set_slab(*args)
+        assert ei.value.code == mpr.ERR_INVALID_ARG
+    with pytest.raises(ValueError):
+        slabs.plan_slabs(40, 4, 12)
+    with pytest.raises(ValueError):
+        slabs.plan_slabs(40, 2, 6)
+    plans = slabs.plan_slabs(101, 4, 8)
+    assert plans[0].own_begin_g == 0 and plans[-1].own_end_g == 101
+    assert all(p.own_begin_g % 2 == 0 and p.row0_g % 2 == 0 for p in plans)
+    assert all(a.own_end_g == b.own_begin_g for a, b in zip(plans, plans[1:]))
