@@ -251,6 +251,7 @@ class SlabSet:
     def __init__(self, plans, slabs, n_cols, transport, n_quench=32, trial_lengths=(200, 50), stats=None, match=None):
         self.plans, self.slabs, self.transport = plans, slabs, transport
         self.halo = plans[0].halo
+        self.sweeps_per_exchange = self.halo // 4        # a hybrid sweep spoils 4 halo rows
         self.n_cols = n_cols
         self.n_quench = n_quench
         self.trial_lengths = trial_lengths
@@ -305,7 +306,7 @@ class SlabSet:
 
     def sweep(self, n):
         """n hybrid sweeps, halo / 4 at a time."""
-        k = self.halo // 4
+        k = self.sweeps_per_exchange
         done = 0
         while done < n:
             m = min(k, n - done)
@@ -320,7 +321,7 @@ class SlabSet:
         # one sweep per call (each has its own series slot); the halos last halo / 4 sweeps.  The energy of a sweep is
         # exact although the innermost halo row is then partly stale: a bond is counted at its colour-1 end, and the
         # colour-0 sites of that row -- the only halo sites an owned colour-1 site is bonded to -- go stale one pass later
-        k = self.halo // 4
+        k = self.sweeps_per_exchange
         for i in range(n):
             for s in self.slabs.values():
                 s.advance(1, 2 if accumulate else 1, i)
