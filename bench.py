@@ -85,6 +85,11 @@ def parse():
                          "at L = 2^5 .. 2^12, f = 0.9, kappa = 0.2, and Delta MAAE_X over M mask realisations; one JSON line")
     ap.add_argument("--matrix-masks", type=int, default=10, help="M, mask realisations per data set for Delta MAAE (paper: 100)")
     ap.add_argument("--matrix-L", type=int, default=512, help="grid size of the Delta MAAE study")
+    ap.add_argument("--slabs", type=int, default=0,
+                    help="opt-in, SURVEY 8(e): ONE problem cut into row slabs (strong scaling).  Under torchrun: one slab per "
+                         "rank, halo rows over NCCL.  On one GPU: --slabs G works the G slabs off in turn (what the exchange "
+                         "schedule and the redundant halo rows cost; checked against the single-context run)")
+    ap.add_argument("--halo", type=int, default=8, help="halo rows of a slab (a multiple of 4; exchange every halo / 4 sweeps)")
     ap.add_argument("--microbench", action="store_true",
                     help="build and run tests/helpers/pipe_microbench.cu (pipe throughputs, L2 / HBM copy) and exit")
     return ap.parse_args()
@@ -593,6 +598,89 @@ def run_microbench():
         subprocess.run([exe], check=True)
 
 
+def run_slabs(args, rank, world, local_rank):
+    """One problem (rank 0's seeds) on slabs: temperature matching + run(n_eq, n_meas) over all slabs."""
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+    from paper_1910_08448_b200 import inputs, mpr, slabs
+    dev = torch.device("cuda", local_rank)
+    torch.cuda.set_device(dev)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    c = inputs.CONFIGS[args.config]
+    n_eq = c.n_eq if args.n_eq is None else args.n_eq
+    n_meas = c.n_meas if args.n_meas is None else args.n_meas
+    values, mask, truth = inputs.make_problem(c.L, c.xi, c.field_seed, c.f, c.lognormal)
+    count = world if world > 1 else max(1, args.slabs)
+    transport = slabs.DistTransport() if world > 1 else None
+    ss = slabs.make_slab_set(values, mask, count, halo=args.halo, mode=args.mode, seed=c.mpr_seed, device=str(dev),
+                             path=args.path, schedule=args.schedule, transport=transport)
+
+    def sync():
+        torch.cuda.synchronize(dev)
+        if world > 1:
+            dist.barrier()
+
+    def step():
+        if args.temperature is not None:
+            ss.set_temperature(args.temperature)
+            ss.reset_chain(0)
+            nt = 0
+        else:
+            ss.estimate_temperature()
+            nt = ss.n_trials
+        _, e, se = ss.run(n_eq, n_meas)
+        return nt * sum(ss.trial_lengths) + n_eq + n_meas, e, se
+
+    for _ in range(args.warmup):
+        step()
+    sync()
+    clocks = ClockSampler(local_rank)
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    ev0.record()
+    sweeps = 0
+    for _ in range(args.steps):
+        n, e, se = step()
+        sweeps += n
+    ev1.record()
+    sync()
+    clk = clocks.stop()
+    ms = ev0.elapsed_time(ev1)
+    if world > 1:
+        t = torch.tensor([ms], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+    # prediction error over the own rows of this process's slabs, summed over the ranks
+    err = np.zeros(2)
+    for i, sl in ss.slabs.items():
+        p = sl.plan
+        pr, tr, mk = sl.own_prediction(), truth[p.own_begin_g:p.own_end_g], mask[p.own_begin_g:p.own_end_g] == 1
+        err += [np.abs(pr - tr)[mk].sum(), mk.sum()]
+    err = ss.transport.reduce_sum([err])
+    check = None
+    if world == 1 and count > 1 and args.temperature is not None:
+        g = mpr.Mpr(values, mask, mode=args.mode, seed=c.mpr_seed, device=dev)
+        g.set_path(args.path); g.set_schedule(args.schedule); g.set_temperature(args.temperature)
+        g.run(n_eq, n_meas)
+        check = bool(np.array_equal(g.get_state().cpu().numpy(), ss.state()))
+        g.close()
+    if rank == 0:
+        print(json.dumps({
+            "metric": METRIC, "value": 2.0 * ss.n_free * sweeps / (ms * 1e-3), "unit": UNIT, "n_gpus": world,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
+            "scaling": "strong", "vs_baseline": None, "dtype": "f64" if args.mode == "DP" else "f32", "data": "synthetic",
+            "config": {"workload": "config%d_L%d" % (args.config, c.L), "L": c.L, "masked_fraction": c.f, "mode": args.mode,
+                       "n_eq": n_eq, "n_meas": n_meas, "parallelism": "slabs x%d%s" % (count, "" if world > 1 else " on one GPU, in turn"),
+                       "halo_rows": args.halo, "sweeps_per_exchange": ss.sweeps_per_exchange,
+                       "l2": "state larger than the 126 MB L2; no flush" if c.L >= 4096 else "L2-resident state"},
+            "clocks": clk, "T_hat": ss.T, "e_mean": e, "e_stderr": se, "mae": float(err[0] / max(err[1], 1.0)),
+            "exchanges": ss.exchanges, "identical_to_single_context": check,
+        }))
+    if world > 1:
+        dist.destroy_process_group()
+
+
 def main():
     args = parse()
     if args.microbench:
@@ -606,6 +694,8 @@ def main():
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
     if args.impl == "reference":
         run_reference(args, rank, world)
+    elif args.slabs:
+        run_slabs(args, rank, world, local_rank)
     else:
         run_ours(args, rank, world, local_rank)
 

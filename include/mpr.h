@@ -257,6 +257,7 @@ int mpr_predict_host_rect(int Lx, int Ly, const double* h_values, const uint8_t*
  *                  mpr_rows_bytes bytes; enqueued on the context's stream.
  *   mpr_advance    n_sweeps hybrid sweeps without the bookkeeping of mpr_run; measure = 0: sweeps only, 1: the energy
  *                  of each sweep goes to slot first_slot + i of the device series, 2: and phi is accumulated.
+ *   mpr_quench     n quench double passes (R8: colour 0, colour 1) on the chain as it is, by the kernels of the path.
  *   mpr_fetch_series   the first n slots of that series -> HOST out (synchronises the stream).
  *   mpr_predict    the back-mapped average of phi accumulated since the last chain reset -> d_pred f64[Lx*Ly].
  *   mpr_debug_trial_lengths   the fixed sweep counts of one temperature trial of R6 (equilibration, measurement). */
@@ -267,6 +268,7 @@ int mpr_rows_bytes(mpr_ctx* ctx, int n_rows, size_t* bytes);
 int mpr_export_rows(mpr_ctx* ctx, int row_begin, int n_rows, void* d_out);
 int mpr_import_rows(mpr_ctx* ctx, int row_begin, int n_rows, const void* d_in);
 int mpr_advance(mpr_ctx* ctx, int n_sweeps, int measure, int first_slot);
+int mpr_quench(mpr_ctx* ctx, int n_double_passes);
 int mpr_fetch_series(mpr_ctx* ctx, int n, double* h_out);
 int mpr_predict(mpr_ctx* ctx, double* d_pred);
 void mpr_debug_trial_lengths(int* n_eq, int* n_meas);

@@ -458,20 +458,9 @@ int eff_path(const mpr_ctx* c) {
   return (c->mode == MPR_SP_INTRINSIC && grid_side(c->lo.g) >= 4096) ? MPR_PATH_STRIP : MPR_PATH_TILED;
 }
 
-// R8: uniform initial spins, then n_quench x (quench colour 0, quench colour 1); everything
-// that belongs to the chain is cleared.
-int reset_chain(mpr_ctx* c, uint32_t trial) {
-  if (!c->ws) return fail(c, MPR_ERR_WORKSPACE, "no workspace attached (mpr_set_workspace)");
-  c->stale = false;
-  c->trial = trial;
-  c->sweep = 0;
-  c->attempted = 0;
-  c->n_acc = 0;
-  c->series.clear();
-  TRY(do_init(c));
-  // quench double passes (colour 0, colour 1): the tiled kernel runs them 2 k at a time (k <= 2,
-  // halo 4 k), an odd remainder goes through the plain kernels -- same moves, same order
-  int left = c->n_quench;
+// `left` quench double passes (colour 0, colour 1): the tiled kernel runs them 2 k at a time (k <= 2,
+// halo 4 k), the strip kernel two per launch, an odd remainder goes through the plain kernels -- same moves, same order
+int quench_passes(mpr_ctx* c, int left) {
   const int path = eff_path(c);
   if (path == MPR_PATH_TILED) {
     while (left >= 2) {
@@ -486,6 +475,21 @@ int reset_chain(mpr_ctx* c, uint32_t trial) {
     TRY(do_pass(c, KIND_QUENCH, 0, 0));
     TRY(do_pass(c, KIND_QUENCH, 1, 0));
   }
+  return MPR_OK;
+}
+
+// R8: uniform initial spins, then n_quench x (quench colour 0, quench colour 1); everything
+// that belongs to the chain is cleared.
+int reset_chain(mpr_ctx* c, uint32_t trial) {
+  if (!c->ws) return fail(c, MPR_ERR_WORKSPACE, "no workspace attached (mpr_set_workspace)");
+  c->stale = false;
+  c->trial = trial;
+  c->sweep = 0;
+  c->attempted = 0;
+  c->n_acc = 0;
+  c->series.clear();
+  TRY(do_init(c));
+  TRY(quench_passes(c, c->n_quench));
   CUDA_OK(c, cudaMemsetAsync(c->slots(), 0, kAcceptSlots * sizeof(unsigned long long), c->stream));
   const size_t n = 2 * c->lo.g.plane;
   clear_acc_kernel<<<1184, 256, 0, c->stream>>>(c->acc(), n);
@@ -1024,6 +1028,12 @@ int mpr_advance(mpr_ctx* c, int n_sweeps, int measure, int first_slot) {
       (measure && static_cast<long long>(first_slot) + n_sweeps > kSeriesCap))
     return fail(c, MPR_ERR_INVALID_ARG, "bad sweep count, measure flag or series slot");
   return hybrid_sweeps(c, n_sweeps, measure, first_slot);
+}
+
+int mpr_quench(mpr_ctx* c, int n_double_passes) {
+  if (!c || n_double_passes < 0) return fail(c, MPR_ERR_INVALID_ARG, "negative pass count");
+  TRY(ensure_chain(c));
+  return quench_passes(c, n_double_passes);
 }
 
 int mpr_fetch_series(mpr_ctx* c, int n, double* h_out) {

@@ -36,7 +36,7 @@ SYMBOLS = [
     "mpr_get_launch_stats", "mpr_workspace_bytes_host", "mpr_predict_host", "mpr_debug_philox",
     "mpr_workspace_bytes_rect", "mpr_create_rect", "mpr_workspace_bytes_host_rect", "mpr_predict_host_rect",
     "mpr_set_slab", "mpr_sample_energy_parts", "mpr_rows_bytes", "mpr_export_rows", "mpr_import_rows", "mpr_advance",
-    "mpr_fetch_series", "mpr_predict", "mpr_debug_trial_lengths",
+    "mpr_fetch_series", "mpr_predict", "mpr_debug_trial_lengths", "mpr_quench",
     "mpr_static_setup", "mpr_static_max_sites", "mpr_static_last_error", "mpr_sample_energy_static",
     "mpr_last_error", "mpr_status_string",
 ]
@@ -121,6 +121,7 @@ def lib():
         "mpr_import_rows": (C.c_int, [vp, C.c_int, C.c_int, vp]),
         "mpr_advance": (C.c_int, [vp, C.c_int, C.c_int, C.c_int]),
         "mpr_fetch_series": (C.c_int, [vp, C.c_int, dp]),
+        "mpr_quench": (C.c_int, [vp, C.c_int]),
         "mpr_predict": (C.c_int, [vp, vp]),
         "mpr_debug_trial_lengths": (None, [C.POINTER(C.c_int), C.POINTER(C.c_int)]),
         "mpr_static_setup": (C.c_int, []),
@@ -354,6 +355,9 @@ class Mpr:
 
     def advance(self, n_sweeps, measure=0, first_slot=0):
         self._call(lib().mpr_advance, int(n_sweeps), int(measure), int(first_slot))
+
+    def quench(self, n_double_passes):
+        self._call(lib().mpr_quench, int(n_double_passes))
 
     def fetch_series(self, n):
         out = np.empty(int(n), dtype=np.float64)

@@ -203,9 +203,8 @@ class MprSlab:
     def reset_chain(self, trial):
         self.ctx.reset_chain(trial)
 
-    def quench_double_pass(self):
-        self.ctx.pass_("QUENCH", 0)
-        self.ctx.pass_("QUENCH", 1)
+    def quench(self, n_double_passes):
+        self.ctx.quench(n_double_passes)
 
     def advance(self, n, measure=0, first_slot=0):
         self.ctx.advance(n, measure, first_slot)
@@ -296,12 +295,13 @@ class SlabSet:
         then n_quench double passes; one double pass spoils 2 halo rows."""
         for s in self.slabs.values():
             s.reset_chain(trial)
-        per = self.halo // 2
-        for i in range(self.n_quench):
+        per, done = self.halo // 2, 0
+        while done < self.n_quench:
+            m = min(per, self.n_quench - done)
             for s in self.slabs.values():
-                s.quench_double_pass()
-            if (i + 1) % per == 0 or i + 1 == self.n_quench:
-                self.exchange()
+                s.quench(m)
+            self.exchange()
+            done += m
         self.sweeps = 0
 
     def sweep(self, n):

@@ -79,9 +79,10 @@ class ToySlab:
         self._accepted += int((upd & self.own & (new % 2 == 0)).sum())
         self.state = np.where(upd, new, s)
 
-    def quench_double_pass(self):
-        self._pass(0, 11)
-        self._pass(1, 11)
+    def quench(self, n_double_passes):
+        for _ in range(n_double_passes):
+            self._pass(0, 11)
+            self._pass(1, 11)
 
     def advance(self, n, measure=0, first_slot=0):
         for i in range(n):

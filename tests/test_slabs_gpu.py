@@ -112,3 +112,22 @@ def test_slab_argument_checks(mpr, inputs, slabs):
     assert plans[0].own_begin_g == 0 and plans[-1].own_end_g == 101
     assert all(p.own_begin_g % 2 == 0 and p.row0_g % 2 == 0 for p in plans)
     assert all(a.own_end_g == b.own_begin_g for a, b in zip(plans, plans[1:]))
+
+
+def test_slabs_at_a_strip_kernel_size(mpr, inputs, slabs):
+    """L = 4096 (where MPR_PATH_AUTO picks the strip kernels), 3 slabs of unequal height, the library's 32 quench passes
+    by the strip quench kernel with halo refreshes in between."""
+    L = 4096
+    values, mask, _ = inputs.make_problem(L, 64.0, 55, 0.9)
+    g = mpr.Mpr(values, mask, mode="SP_INTRINSIC", seed=8)
+    g.set_temperature(0.002)
+    pred_w, e_w, se_w = g.run(6, 4)
+    st_w, acc_w = g.get_state().cpu().numpy(), g.counters()[0]
+    g.close()
+    ss = slabs.make_slab_set(values, mask, 3, halo=8, mode="SP_INTRINSIC", seed=8)
+    ss.set_temperature(0.002)
+    ss.reset_chain(0)
+    series, e, se = ss.run(6, 4)
+    assert np.array_equal(ss.state(), st_w) and ss.accepted() == acc_w
+    assert abs(e - e_w) <= 2e-12
+    assert np.array_equal(np.nan_to_num(ss.prediction(), nan=-1.0), np.nan_to_num(pred_w.cpu().numpy(), nan=-1.0))
