@@ -48,12 +48,14 @@ CPU_ONE_CROP, CPU_ONE_SWEEPS = 2048, 3         # one thread: top-left 2048^2 win
 # measured cost per warp instruction and scheduler (tests/helpers/pipe_microbench.cu, profiles/r02_microbench.md):
 #   IMAD.WIDE.U32 4.27 cycles (inside a Philox block), FADD2 / FMUL2 2.03, FFMA2 2.34 -> packed average 2.1
 ALG_FMA_CYCLES_PER_UNIT_SWEEP = 10 * 4.27 + (21 + 19) * 2.1       # = 126.7 scheduler cycles
-# Double-arithmetic modes (DP, SP): the FP64 pipe carries the moves.  Per unit and sweep 210 FP64-pipe instructions
-# (DFMA / DMUL / DADD / DSETP / I2F.F64: two Philox-to-double conversions and the branch-free sincos / exp polynomials of the
-# Metropolis move, the Newton-free reflection with one division of the over-relaxation move, the local fields; counted in the
-# SASS of the move functions: 857 in the eight unit-passes of tiled_sweep_kernel<DP, 0>), at the measured 3.28 cycles per
-# warp instruction and scheduler (DFMA 1.22 per clock and SM, profiles/r02_microbench.md).
-ALG_FP64_CYCLES_PER_UNIT_SWEEP = 210 * 3.28
+# Double-arithmetic modes (DP, SP): the FP64 pipe carries the moves.  Per unit (two sites) and sweep 160 FP64-pipe
+# instructions at the temperatures of configs 3-5 (DFMA / DMUL / DADD / DSETP / conversions; per site: Metropolis 37 -- local
+# field 6, proposal from two Philox words 5, sin / cos of the half-angle with the 4 + 4 Taylor coefficients that delta needs
+# there 11 (19 with all 8 + 8 at T > 0.04), rotation, difference and energy 12, decision filter 2, range test 1; the double
+# exponential is only evaluated when the float filter cannot decide, ~3e-5 of the moves -- and over-relaxation 43 with its
+# one division), at the measured 3.28 cycles per warp instruction and scheduler (DFMA 1.22 per clock and SM,
+# profiles/r02_microbench.md).  Until the decision filter the count was 210.
+ALG_FP64_CYCLES_PER_UNIT_SWEEP = 160 * 3.28
 SMS, SCHEDULERS = 148, 4
 # dram__bytes_read.sum + dram__bytes_write.sum of one launch at L = 16384 from the committed `ncu --set full` captures
 # (profiles/); None for configurations not captured.

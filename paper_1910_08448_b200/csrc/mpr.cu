@@ -191,6 +191,7 @@ ChainConst<R> chain_const(const mpr_ctx* c) {
   }
   k.hoff = static_cast<R>(-1.5) * k.hscale;
   k.xscale = static_cast<R>(1.4426950408889634074 / T);
+  k.sc_terms = sincos_terms_for(0.5 * q * proposal_width(T, q));      // |q Delta / 2| <= q delta / 2
   k.k0 = static_cast<uint32_t>(c->seed);
   k.k1 = static_cast<uint32_t>(c->seed >> 32);
   k.trial = c->trial;

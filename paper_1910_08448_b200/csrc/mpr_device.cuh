@@ -116,15 +116,29 @@ static __constant__ double kExpC[12] = {1.0 / 2.0, 1.0 / 6.0, 1.0 / 24.0, 1.0 / 
                                  1.0 / 40320.0, 1.0 / 362880.0, 1.0 / 3628800.0, 1.0 / 39916800.0,
                                  1.0 / 479001600.0, 1.0 / 6227020800.0};
 
-// sin and cos of x, |x| <= pi/4 (no range reduction: the caller guarantees the range)
-__device__ __forceinline__ void sincos_quarter(double x, double* s, double* c) {
+// sin and cos of x, |x| <= pi/4 (no range reduction: the caller guarantees the range), from the first NC coefficients
+template <int NC>
+__device__ __forceinline__ void sincos_taylor(double x, double* s, double* c) {
   const double z = x * x;
-  double ps = kSinC[7], pc = kCosC[7];
+  double ps = kSinC[NC - 1], pc = kCosC[NC - 1];
 #pragma unroll
-  for (int i = 6; i >= 0; --i) { ps = fma(ps, z, kSinC[i]); pc = fma(pc, z, kCosC[i]); }
+  for (int i = NC - 2; i >= 0; --i) { ps = fma(ps, z, kSinC[i]); pc = fma(pc, z, kCosC[i]); }
   *s = fma(x * z, ps, x);        // x + x^3 (S1 + S2 z + ...)
   *c = fma(z, pc, 1.0);          // 1 + z (C1 + C2 z + ...)
 }
+__device__ __forceinline__ void sincos_quarter(double x, double* s, double* c) { sincos_taylor<8>(x, s, c); }
+// The proposal half-angle is bounded by q delta / 2, which shrinks with sqrt(T) (R7): at the temperatures the method
+// infers (1e-3 .. 1e-1) most of the 8 + 8 coefficients above multiply powers of x below half an ulp.  `terms` (4, 6 or 8;
+// the same for every thread of a launch, chosen on the host by sincos_terms_for) selects a shorter Horner chain whose
+// truncation error is still below 2^-54 relative:
+//   4 coefficients (sin to x^9, cos to x^8):   |x| <= 0.10   (x^10 / 10! < 2.8e-17, x^11 / 11! < 2.6e-19 x)
+//   6 coefficients (sin to x^13, cos to x^12): |x| <= 0.40   (x^14 / 14! < 3.1e-17, x^15 / 15! < 8.3e-19 x)
+__device__ __forceinline__ void sincos_quarter_terms(double x, int terms, double* s, double* c) {
+  if (terms == 4) sincos_taylor<4>(x, s, c);
+  else if (terms == 6) sincos_taylor<6>(x, s, c);
+  else sincos_taylor<8>(x, s, c);
+}
+inline int sincos_terms_for(double max_abs_x) { return max_abs_x <= 0.10 ? 4 : max_abs_x <= 0.40 ? 6 : 8; }
 
 // exp(min(y, 0)): for y >= 0 the result is exactly 1, which exceeds every u2 in [0, 1) -- the same
 // decision as "accept if dE <= 0".  y = k ln 2 + r, |r| <= ln 2 / 2; 2^k is applied as two exact
@@ -146,6 +160,32 @@ __device__ __forceinline__ double exp_nonpos(double y) {
   p = p * __hiloint2double((k1 + 1023) << 20, 0);
   p = p * __hiloint2double((k2 + 1023) << 20, 0);
   return y < -745.2 ? 0.0 : p;
+}
+
+// The Metropolis decision of the double-arithmetic modes, u2 < exp(min(x, 0)) with x = -dE/T and u2 = u53(wa, wb), taken
+// EXACTLY as the double evaluation takes it, but without evaluating the double exponential unless it matters:
+//   * 2^y, y = x log2 e, from one MUFU.EX2 in float: ef = 2^y (1 + d), |d| < 6e-6 for y >= -120 (argument rounding
+//     |y| 2^-24 ln 2 <= 5e-6, ex2.approx 2^-22);
+//   * u2 bracketed by its top 24 bits: u_lo <= u2 < u_hi = u_lo + 2^-24, both exact floats;
+//   * u_hi <= ef (1 - 2^-15)  =>  u2 < exp(x): accept;   u_lo >= ef (1 + 2^-15)  =>  u2 > exp(x): reject;
+//     y < -120: exp(x) < 2^-119 < 2^-24 <= u_lo unless u_lo = 0: reject;
+//   * anything else (probability ~3e-5 per move; also NaN) falls through to the double evaluation, out of line.
+// The decision is the one `u53(wa, wb) < exp_nonpos(x)` gives, always; what is saved is the ~25 FP64-pipe
+// instructions of exp_nonpos and u53 per move, a fifth of the FP64 work of a DP / SP hybrid sweep (the FP64 pipe is
+// what binds those modes on B200).
+static __device__ __noinline__ bool metropolis_accept_slow(uint32_t wa, uint32_t wb, double x) {
+  return u53(wa, wb) < exp_nonpos(x);
+}
+__device__ __forceinline__ bool metropolis_accept_exact(uint32_t wa, uint32_t wb, double mdE, double inv_T, double log2e_over_T) {
+  const float yf = __double2float_rn(mdE * log2e_over_T);
+  float ef;
+  asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(ef) : "f"(yf));
+  const float u_lo = static_cast<float>(wa >> 8) * 5.9604644775390625e-08f;      // k 2^-24, exact
+  const float u_hi = u_lo + 5.9604644775390625e-08f;                            // (k + 1) 2^-24, exact
+  const bool in_range = yf >= -120.0f, tiny = yf < -120.0f;                      // NaN: neither
+  if (in_range && u_hi <= ef * 0.999969482421875f) return true;                  // 1 - 2^-15
+  if ((in_range && u_lo >= ef * 1.000030517578125f) || (tiny && u_lo > 0.0f)) return false;   // 1 + 2^-15
+  return metropolis_accept_slow(wa, wb, mdE * inv_T);
 }
 
 // ---- function-precision policies (X_F) -----------------------------------
@@ -223,8 +263,9 @@ template <typename R> struct ChainConst {
   R hoff;      //              = fma(f, hscale, hoff), hoff = -3/2 hscale
   R qhalf;     // q / 2 (double-arithmetic proposal: q Delta / 2 = qhalf * delta * (2 u1 - 1)); 1/4 for q = 1/2
   R bq_c, bq_s;  // general q only (GENQ): the end of the allowed arc, (cos 2 pi q, sin 2 pi q): phi <= 2 pi <=> u x b >= 0
-  R xscale;    // SP_INTRINSIC: log2(e) / T, so that exp(-dE / T) 2^20 = ex2(-dE * xscale + 20)
+  R xscale;    // log2(e) / T.  SP_INTRINSIC: exp(-dE / T) 2^20 = ex2(-dE * xscale + 20); double modes: metropolis_accept_exact
   uint32_t k0, k1, trial;
+  int sc_terms;    // double modes: Taylor coefficients the proposal's sin / cos need at this delta (sincos_quarter_terms)
   PhiloxKeys rk;   // round keys of (k0, k1)
 };
 
@@ -378,8 +419,13 @@ __device__ __forceinline__ void met_update2(Two<typename Traits<MODE>::real> c, 
   }
   R ha, hb, sda, cda, sdb, cdb;
   un2(h, &ha, &hb);
-  Fn<MODE>::sincos_(ha, &sda, &cda);
-  Fn<MODE>::sincos_(hb, &sdb, &cdb);
+  if constexpr (sizeof(R) == 8) {
+    sincos_quarter_terms(ha, k.sc_terms, &sda, &cda);
+    sincos_quarter_terms(hb, k.sc_terms, &sdb, &cdb);
+  } else {
+    Fn<MODE>::sincos_(ha, &sda, &cda);
+    Fn<MODE>::sincos_(hb, &sdb, &cdb);
+  }
   const Two<R> sd = mk2(sda, sdb), cd = mk2(cda, cdb);
   const Two<R> ts = add2(sd, sd);                // 2 sd
   const Two<R> nts = mul2(sd, bc2(R(-2)));       // -2 sd
@@ -395,10 +441,10 @@ __device__ __forceinline__ void met_update2(Two<typename Traits<MODE>::real> c, 
   un2(c, &c0a, &c0b); un2(s, &s0a, &s0b); un2(cn, &cna, &cnb); un2(sn, &sna, &snb);
   bool acc_a, acc_b;
   if constexpr (sizeof(R) == 8) {
-    R xa, xb;
-    un2(mul2(mdE, bc2(k.inv_T)), &xa, &xb);
-    acc_a = R(u53(wa.a, wa.b)) < Fn<MODE>::exp_(xa);
-    acc_b = R(u53(wb.a, wb.b)) < Fn<MODE>::exp_(xb);
+    R ea, eb;
+    un2(mdE, &ea, &eb);
+    acc_a = metropolis_accept_exact(wa.a, wa.b, ea, k.inv_T, k.xscale);
+    acc_b = metropolis_accept_exact(wb.a, wb.b, eb, k.inv_T, k.xscale);
   } else if constexpr (IsIntrinsic<MODE>::value) {
     R xa, xb;                                    // exp(-dE/T) 2^20 = ex2(-dE xscale + 20): one FFMA2 + 2 MUFU.EX2
     un2(fma2(mdE, bc2(k.xscale), bc2(R(20))), &xa, &xb);

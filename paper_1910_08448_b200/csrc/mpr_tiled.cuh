@@ -40,7 +40,8 @@ template <int MODE> struct TileCfg;
 // (at its 80-register cap the barrier ids spill, and its barrier waits were already covered by the
 // second resident CTA), so that mode keeps __syncthreads.
 // UNROLL: rows of a warp per iteration of the pass loop (0 = all RPW rows).  Even, so the row
-// parities stay compile-time.  Double arithmetic: 2 keeps the code within the registers.  Float
+// parities stay compile-time.  Double arithmetic: 2 (measured again after the Metropolis decision filter freed
+// registers: DP 6 rows 3.67 -> 4.31 ms, SP 4 rows 2.98 -> 3.00 ms).  Float
 // arithmetic, A/B at 1965 MHz, ms per sweep, full unroll -> 4: SP_INTRINSIC 1.2266 -> 1.2199 (and half
 // the code), SP_PRECISE 1.570 -> 1.630, so only SP_INTRINSIC takes 4.
 template <> struct TileCfg<MODE_DP>           { static constexpr int TH = 48, NT = 256, UNROLL = 2; static constexpr bool PAIR_SYNC = true; };
