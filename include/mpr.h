@@ -324,6 +324,13 @@ int mpr_debug_match_temperature(double e_sample, mpr_trial_fn trial, void* user,
 int mpr_debug_philox(const uint32_t* d_ctr, const uint32_t key[2], uint32_t* d_out, int64_t n,
                      void* cuda_stream);
 
+/* The Metropolis decision of the double-arithmetic modes (float filter, double evaluation only when the
+ * filter cannot decide) next to the plain double evaluation u2 < exp(min(-dE/T, 0)), on the DEVICE, for n moves:
+ *   d_words u32[2n] (the two Philox words of u2), d_mdE f64[n] (-dE), T; d_out u8[n]: bit 0 = filtered decision,
+ *   bit 1 = plain decision, bit 2 = the filter decided alone.  Tests require bit 0 == bit 1 on adversarial inputs.  */
+int mpr_debug_accept(const uint32_t* d_words, const double* d_mdE, double T, uint8_t* d_out, int64_t n,
+                     void* cuda_stream);
+
 const char* mpr_last_error(const mpr_ctx* ctx);
 const char* mpr_status_string(int status);
 

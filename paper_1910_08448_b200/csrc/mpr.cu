@@ -1191,4 +1191,12 @@ int mpr_debug_philox(const uint32_t* d_ctr, const uint32_t key[2], uint32_t* d_o
   return cudaGetLastError() == cudaSuccess ? MPR_OK : MPR_ERR_CUDA;
 }
 
+int mpr_debug_accept(const uint32_t* d_words, const double* d_mdE, double T, uint8_t* d_out, int64_t n, void* cuda_stream) {
+  if (!d_words || !d_mdE || !d_out || n < 0 || !(T > 0.0)) return MPR_ERR_INVALID_ARG;
+  if (n == 0) return MPR_OK;
+  accept_debug_kernel<<<static_cast<unsigned>((n + 255) / 256), 256, 0, static_cast<cudaStream_t>(cuda_stream)>>>(
+      d_words, d_mdE, T, d_out, n);
+  return cudaGetLastError() == cudaSuccess ? MPR_OK : MPR_ERR_CUDA;
+}
+
 }  // extern "C"

@@ -176,7 +176,9 @@ __device__ __forceinline__ double exp_nonpos(double y) {
 static __device__ __noinline__ bool metropolis_accept_slow(uint32_t wa, uint32_t wb, double x) {
   return u53(wa, wb) < exp_nonpos(x);
 }
-__device__ __forceinline__ bool metropolis_accept_exact(uint32_t wa, uint32_t wb, double mdE, double inv_T, double log2e_over_T) {
+// `fast` (tests only): set to false when the decision went through the double evaluation
+__device__ __forceinline__ bool metropolis_accept_exact(uint32_t wa, uint32_t wb, double mdE, double inv_T, double log2e_over_T,
+                                                        bool* fast = nullptr) {
   const float yf = __double2float_rn(mdE * log2e_over_T);
   float ef;
   asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(ef) : "f"(yf));
@@ -185,6 +187,7 @@ __device__ __forceinline__ bool metropolis_accept_exact(uint32_t wa, uint32_t wb
   const bool in_range = yf >= -120.0f, tiny = yf < -120.0f;                      // NaN: neither
   if (in_range && u_hi <= ef * 0.999969482421875f) return true;                  // 1 - 2^-15
   if ((in_range && u_lo >= ef * 1.000030517578125f) || (tiny && u_lo > 0.0f)) return false;   // 1 + 2^-15
+  if (fast) *fast = false;
   return metropolis_accept_slow(wa, wb, mdE * inv_T);
 }
 

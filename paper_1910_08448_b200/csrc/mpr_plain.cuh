@@ -498,4 +498,17 @@ static __global__ void philox_debug_kernel(const uint32_t* __restrict__ ctr, uin
   out[4 * i] = r.x; out[4 * i + 1] = r.y; out[4 * i + 2] = r.z; out[4 * i + 3] = r.w;
 }
 
+// out[i]: bit 0 = decision of metropolis_accept_exact, bit 1 = decision of the plain double evaluation
+// u53(wa, wb) < exp_nonpos(mdE / T), bit 2 = the float filter decided alone
+static __global__ void accept_debug_kernel(const uint32_t* __restrict__ w, const double* __restrict__ mdE, double T,
+                                           uint8_t* __restrict__ out, long long n) {
+  const long long i = blockIdx.x * static_cast<long long>(blockDim.x) + threadIdx.x;
+  if (i >= n) return;
+  const double inv_T = 1.0 / T, xs = 1.4426950408889634074 / T;
+  bool fast = true;
+  const bool a = metropolis_accept_exact(w[2 * i], w[2 * i + 1], mdE[i], inv_T, xs, &fast);
+  const bool b = u53(w[2 * i], w[2 * i + 1]) < exp_nonpos(mdE[i] * inv_T);
+  out[i] = static_cast<uint8_t>((a ? 1 : 0) | (b ? 2 : 0) | (fast ? 4 : 0));
+}
+
 }  // namespace mpr

@@ -37,6 +37,7 @@ SYMBOLS = [
     "mpr_workspace_bytes_rect", "mpr_create_rect", "mpr_workspace_bytes_host_rect", "mpr_predict_host_rect",
     "mpr_set_slab", "mpr_sample_energy_parts", "mpr_rows_bytes", "mpr_export_rows", "mpr_import_rows", "mpr_advance",
     "mpr_fetch_series", "mpr_predict", "mpr_debug_trial_lengths", "mpr_quench",
+    "mpr_debug_accept",
     "mpr_static_setup", "mpr_static_max_sites", "mpr_static_last_error", "mpr_sample_energy_static",
     "mpr_last_error", "mpr_status_string",
 ]
@@ -124,6 +125,7 @@ def lib():
         "mpr_quench": (C.c_int, [vp, C.c_int]),
         "mpr_predict": (C.c_int, [vp, vp]),
         "mpr_debug_trial_lengths": (None, [C.POINTER(C.c_int), C.POINTER(C.c_int)]),
+        "mpr_debug_accept": (C.c_int, [vp, vp, C.c_double, vp, i64, vp]),
         "mpr_static_setup": (C.c_int, []),
         "mpr_static_max_sites": (C.c_int64, []),
         "mpr_static_last_error": (C.c_char_p, []),
@@ -461,6 +463,24 @@ def debug_match_temperature(e_sample, energy_of_T):
         raise err
     assert n.value == len(asked)
     return T.value, asked
+
+
+def debug_accept(words, mdE, T, device="cuda:0"):
+    """mpr_debug_accept: words uint32 [n, 2], mdE float64 [n] -> uint8 [n] (bit 0 filtered, bit 1 plain, bit 2 fast)."""
+    torch = _torch()
+    dev = torch.device(device)
+    words = np.ascontiguousarray(words, dtype=np.uint32).reshape(-1, 2)
+    mdE = np.ascontiguousarray(mdE, dtype=np.float64).reshape(-1)
+    assert words.shape[0] == mdE.shape[0]
+    d_w = torch.from_numpy(words.view(np.int32)).to(dev)
+    d_e = torch.from_numpy(mdE).to(dev)
+    out = torch.empty(mdE.shape[0], dtype=torch.uint8, device=dev)
+    with torch.cuda.device(dev):
+        st = lib().mpr_debug_accept(d_w.data_ptr(), d_e.data_ptr(), float(T), out.data_ptr(), mdE.shape[0],
+                                    torch.cuda.current_stream(dev).cuda_stream)
+    if st != MPR_OK:
+        raise MprError(st)
+    return out.cpu().numpy()
 
 
 def debug_philox(ctr, key, device="cuda:0"):

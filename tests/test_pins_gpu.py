@@ -320,3 +320,40 @@ def test_pass_synchronisation_long_stress(mpr, inputs, mode):
     for key, (st, cnt) in out.items():
         assert cnt == ref[1], (mode, key)
         assert torch.equal(st, ref[0]), (mode, key, int((st != ref[0]).sum()))
+
+
+def test_metropolis_decision_filter_is_exact(mpr):
+    """the double-arithmetic modes decide u2 < exp(-dE/T) through a float filter and evaluate the double
+    exponential only when the filter cannot decide.  On random moves and on moves built to sit on the edge -- u2 within a
+    few ulps, 2^-24 .. 2^-12 relative, of exp(x); x around the -120 log 2 cut of the filter, at the underflow of exp, at 0
+    and above; u2 = 0 and u2 = 1 - 2^-53; NaN -- the filtered decision equals the plain double one, and on ordinary moves
+    the filter decides alone all but ~1e-4 of the time."""
+    rng = np.random.default_rng(12)
+    T = 0.37
+
+    def words_of(u):                       # the two Philox words whose u53 is floor(u 2^53) 2^-53
+        k = np.floor(np.clip(u, 0.0, 1.0 - 2.0 ** -53) * 2.0 ** 53).astype(np.uint64)
+        hi, lo = (k >> np.uint64(26)).astype(np.uint64), (k & np.uint64((1 << 26) - 1)).astype(np.uint64)
+        return np.stack([(hi << np.uint64(5)).astype(np.uint32), (lo << np.uint64(6)).astype(np.uint32)], axis=1)
+
+    n = 1 << 20
+    x = np.concatenate([-rng.exponential(2.0, n), rng.uniform(-800.0, 5.0, n), rng.uniform(-84.0, -82.0, n),
+                        rng.uniform(-1e-6, 1e-6, n)])
+    u = rng.uniform(size=x.size)
+    # edge cases: u at exp(x) (1 + eps) for eps from a few ulps to the width of the filter's margin and beyond
+    xe = -rng.exponential(3.0, n)
+    eps = rng.choice([-1, 1], n) * 2.0 ** rng.uniform(-53, -10, n)
+    ue = np.exp(xe) * (1.0 + eps)
+    xs = np.array([0.0, -0.0, 1e-300, -1e-300, 3.0, -745.1, -745.3, -1e4, np.nan, -83.17, -83.18, -83.2, -120 * math.log(2.0)])
+    us = np.array([0.0, 1.0 - 2.0 ** -53, 2.0 ** -24, 2.0 ** -25, 0.5])
+    xg, ug = np.meshgrid(xs, us)
+    X = np.concatenate([x, xe, xg.ravel()])
+    U = np.concatenate([u, ue, ug.ravel()])
+    out = mpr.debug_accept(words_of(U), X * T, T)          # -dE = x T
+    filtered, plain, fast = out & 1, (out >> 1) & 1, (out >> 2) & 1
+    assert np.array_equal(filtered, plain)
+    # the plain device decision is itself the textbook one wherever double rounding cannot matter
+    clear = np.abs(U[: x.size] - np.exp(np.minimum(X[: x.size], 0.0))) > 1e-9
+    assert np.array_equal(plain[: x.size][clear], (U[: x.size] < np.exp(np.minimum(X[: x.size], 0.0)))[clear].astype(np.uint8))
+    assert 1.0 - fast[:n].mean() < 3e-4                    # ordinary moves: the filter decides alone
+    assert fast[x.size: x.size + n].mean() < 0.9           # the edge cases do reach the double evaluation
