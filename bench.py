@@ -72,7 +72,8 @@ def parse():
     ap.add_argument("--mode", default="SP_INTRINSIC")
     ap.add_argument("--n-eq", type=int, default=None)
     ap.add_argument("--n-meas", type=int, default=None)
-    ap.add_argument("--fused", type=int, default=1, help="hybrid sweeps per launch (STRIP: 1 or 2)")
+    ap.add_argument("--fused", type=int, default=0,
+                    help="hybrid sweeps per launch; 0 = the library's choice (several on small grids, 1 at the headline size)")
     ap.add_argument("--path", default="AUTO", choices=["AUTO", "STRIP", "TILED", "PLAIN", "LIST"])
     ap.add_argument("--schedule", default="R4", choices=["R4", "SITE_FUSED"],
                     help="pass order of a hybrid sweep (DESIGN.md R4 / R4b); the headline is R4")
@@ -371,8 +372,17 @@ def run_ours(args, rank, world, local_rank):
             return "STRIP" if L >= 4096 else "PLAIN"
         return "STRIP" if (md == "SP_INTRINSIC" and L >= 4096) else "TILED"
     path_used = auto_path(mode, args.schedule) if args.path == "AUTO" else args.path
-    k_eff = min(args.fused, 2) if path_used == "STRIP" else args.fused
-    kern_ms_burst, _ = time_sweeps(mode, args.path, args.schedule, args.fused, 50)   # the kernel timed alone, after the steps
+
+    # what mpr_set_fused_sweeps(0) resolves to (csrc/mpr.cu, auto_fused)
+    def auto_fused(md, path):
+        if path != "TILED":
+            return 1
+        if md in ("DP", "SP"):
+            return 4 if L <= 256 else 2 if L <= 512 else 1
+        return 4 if L <= 512 else 2 if L <= 1536 else 1
+    k_lib = args.fused or auto_fused(mode, path_used)
+    k_eff = min(k_lib, 2) if path_used == "STRIP" else k_lib
+    kern_ms_burst, _ = time_sweeps(mode, args.path, args.schedule, k_lib, 50)   # the kernel timed alone, after the steps
     # the in-step figure (sustained clocks) is the one the ceilings use; the burst leg stands in only when the steps had
     # no equilibration sweeps
     in_step = state["eq_launches"] > 0
@@ -448,7 +458,7 @@ def run_ours(args, rank, world, local_rank):
             if md not in c.modes and not (md == "HP" and "SP_INTRINSIC" in c.modes):     # HP: the paper's outlook, beside SSS
                 continue
             entry = {}
-            for sched, k in (("R4", 1), ("SITE_FUSED", 2)):
+            for sched, k in (("R4", auto_fused(md, auto_path(md, "R4"))), ("SITE_FUSED", 2)):
                 t_l, t_meas = time_sweeps(md, "AUTO", sched, k, n_sw, warm=3)
                 cl = ceilings(md, t_l, k, sm_mhz)
                 entry[sched] = {"path": auto_path(md, sched), "sweeps_per_launch": k, "ms_per_sweep": t_l / k,

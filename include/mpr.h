@@ -158,8 +158,9 @@ int mpr_set_seed(mpr_ctx* ctx, uint64_t seed);
 int mpr_set_temperature(mpr_ctx* ctx, double T);
 /* Number of quench double-passes of the R8 initialisation (default 32).  Resets the chain. */
 int mpr_set_quench(mpr_ctx* ctx, int n);
-/* Kernel path (default MPR_PATH_AUTO) and temporal-blocking depth 1 <= k <= 4 (hybrid sweeps
- * fused per launch, default 1; the STRIP path uses min(k, 2)).  Results do not depend on either. */
+/* Kernel path (default MPR_PATH_AUTO) and temporal-blocking depth 0 <= k <= 4 (hybrid sweeps
+ * fused per launch; 0, the default, lets the library choose: several per launch on small grids, where a launch is
+ * latency-bound, one otherwise; the STRIP path uses min(k, 2)).  Results do not depend on either. */
 int mpr_set_path(mpr_ctx* ctx, mpr_path path);
 int mpr_set_fused_sweeps(mpr_ctx* ctx, int k);
 /* Pass order of a hybrid sweep (see mpr_schedule).  Does not touch the chain.               */

@@ -94,7 +94,7 @@ struct mpr_ctx {
   int mode = MPR_DP;
   int path = MPR_PATH_AUTO;
   int schedule = MPR_SCHEDULE_R4;
-  int fused = 1;
+  int fused = 0;               // hybrid sweeps per launch; 0 = chosen by auto_fused()
   int n_quench = 32;
   uint64_t seed = 0;
   uint32_t trial = 0;
@@ -513,6 +513,20 @@ int ensure_chain(mpr_ctx* c) {
   return c->stale ? reset_chain(c, 0) : MPR_OK;
 }
 
+// Hybrid sweeps per launch when the caller has not fixed them (mpr_set_fused_sweeps(0), the default).  Small grids are
+// bound by the latency of a launch whose few tiles each run their passes back to back, so several sweeps per launch
+// (halo 4 k) pay until the redundant halo work outweighs it.  Measured on B200, tiled kernel, us per sweep at
+// k = 1 / 2 / 4 -- float arithmetic: L = 64: 10.3 / 8.2 / 7.2, 512: 12.3 / 8.7 / 7.2, 1024: 12.3 / 9.2 / 12.3,
+// 1536: 18.5 / 14.4 / 18.0, 2048: 24.8 / 26.2 / 29.0; double arithmetic: 256: 20.5 / 17.8 / 16.4, 512: 20.5 / 17.8 / 22.6,
+// 1024: 28.7 / 35.9 / 50.1.  The result does not depend on k.
+int auto_fused(const mpr_ctx* c, int path) {
+  if (path != MPR_PATH_TILED) return 1;
+  const double side = grid_side(c->lo.g);
+  const bool dbl = c->mode == MPR_DP || c->mode == MPR_SP;
+  if (dbl) return side <= 256.0 ? 4 : side <= 512.0 ? 2 : 1;
+  return side <= 512.0 ? 4 : side <= 1536.0 ? 2 : 1;
+}
+
 // measure: 0 = sweeps only, 1 = + energy sample per sweep, 2 = + accumulation of phi.
 // n hybrid sweeps (R4); with `measure`, each is followed by the energy sample into
 // dseries[first_slot + i] and the accumulation of phi.
@@ -547,10 +561,11 @@ int hybrid_sweeps(mpr_ctx* c, int n, int measure, int first_slot) {
   }
   if (path == MPR_PATH_TILED && c->schedule != MPR_SCHEDULE_R4)
     return fail(c, MPR_ERR_INVALID_ARG, "the site-fused schedule runs on the STRIP and PLAIN paths");
+  const int fused = c->fused > 0 ? c->fused : auto_fused(c, path);
   int done = 0;
   while (done < n) {
     // measurement needs the state after every sweep: one sweep per launch there
-    int k = measure ? 1 : (n - done < c->fused ? n - done : c->fused);
+    int k = measure ? 1 : (n - done < fused ? n - done : fused);
     double* d_e = measure ? c->dseries() + first_slot + done : nullptr;
     if (path == MPR_PATH_STRIP) {
       if (k > 2) k = 2;                                   // the strip pipeline carries at most two sweeps
@@ -809,7 +824,7 @@ int mpr_set_schedule(mpr_ctx* c, mpr_schedule schedule) {
   return MPR_OK;
 }
 int mpr_set_fused_sweeps(mpr_ctx* c, int k) {
-  if (!c || k < 1 || k > tiled_max_fused()) return fail(c, MPR_ERR_INVALID_ARG, "fused depth out of range");
+  if (!c || k < 0 || k > tiled_max_fused()) return fail(c, MPR_ERR_INVALID_ARG, "fused depth out of range");
   c->fused = k;
   return MPR_OK;
 }

@@ -93,7 +93,8 @@ def test_error_paths(mpr, inputs):
         g.set_temperature(0.0)
     assert ei.value.code == mpr.ERR_INVALID_ARG
     with pytest.raises(mpr.MprError):
-        g.set_fused_sweeps(0)
+        g.set_fused_sweeps(5)
+    g.set_fused_sweeps(0)                        # 0 = the library's choice
 
 
 # --------------------------------------------------------------------------- DP parity, pass by pass
@@ -234,7 +235,10 @@ def test_run_timing_reports_the_equilibration_launches(mpr, inputs):
     g.set_path("TILED")
     g.run(20, 3)
     ms, launches, sweeps = g.run_timing()
-    assert (launches, sweeps) == (20, 20) and 0.0 < ms < 1000.0       # tiled, one sweep per launch
+    assert (launches, sweeps) == (5, 20) and 0.0 < ms < 1000.0        # the library's choice at L = 300: 4 sweeps per launch
+    g.set_fused_sweeps(1)
+    g.run(20, 3)
+    assert g.run_timing()[1:] == (20, 20)                               # tiled, one sweep per launch
     g.set_fused_sweeps(4)
     g.run(18, 2)
     ms4, launches4, sweeps4 = g.run_timing()
