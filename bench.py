@@ -59,7 +59,9 @@ ALG_FP64_CYCLES_PER_UNIT_SWEEP = 160 * 3.28
 SMS, SCHEDULERS = 148, 4
 # dram__bytes_read.sum + dram__bytes_write.sum of one launch at L = 16384 from the committed `ncu --set full` captures
 # (profiles/); None for configurations not captured.
-NCU_TRAFFIC_BYTES = {("SP_INTRINSIC", "R4", 1): 2.957e9 + 2.117e9}
+NCU_TRAFFIC_BYTES = {("SP_INTRINSIC", "R4", 1): 2.671e9 + 2.116e9,           # profiles/r02v_ncu_full.md
+                     ("SP_INTRINSIC", "SITE_FUSED", 2): 2.678e9 + 2.119e9,   # profiles/r02s_ncu_full_strip.md
+                     ("DP", "R4", 1): 4.330e9 + 4.246e9}                     # profiles/r02w_ncu_dp.md
 
 
 def parse():
