@@ -95,6 +95,9 @@ def parse():
                          "rank, halo rows over NCCL.  On one GPU: --slabs G works the G slabs off in turn (what the exchange "
                          "schedule and the redundant halo rows cost; checked against the single-context run)")
     ap.add_argument("--halo", type=int, default=8, help="halo rows of a slab (a multiple of 4; exchange every halo / 4 sweeps)")
+    ap.add_argument("--peer", action="store_true",
+                    help="with --slabs on one GPU: peer mode (mpr_set_peers) -- every strip launch writes its edge rows straight "
+                         "into the neighbours' halos, no copy launches; halo 4")
     ap.add_argument("--microbench", action="store_true",
                     help="build and run tests/helpers/pipe_microbench.cu (pipe throughputs, L2 / HBM copy) and exit")
     return ap.parse_args()
@@ -628,8 +631,9 @@ def run_slabs(args, rank, world, local_rank):
     values, mask, truth = inputs.make_problem(c.L, c.xi, c.field_seed, c.f, c.lognormal)
     count = world if world > 1 else max(1, args.slabs)
     transport = slabs.DistTransport() if world > 1 else None
-    ss = slabs.make_slab_set(values, mask, count, halo=args.halo, mode=args.mode, seed=c.mpr_seed, device=str(dev),
-                             path=args.path, schedule=args.schedule, transport=transport)
+    peer = args.peer and world == 1
+    ss = slabs.make_slab_set(values, mask, count, halo=4 if peer else args.halo, mode=args.mode, seed=c.mpr_seed, device=str(dev),
+                             path="STRIP" if peer else args.path, schedule=args.schedule, transport=transport, peer=peer)
 
     def sync():
         torch.cuda.synchronize(dev)
@@ -675,7 +679,7 @@ def run_slabs(args, rank, world, local_rank):
     check = None
     if world == 1 and count > 1 and args.temperature is not None:
         g = mpr.Mpr(values, mask, mode=args.mode, seed=c.mpr_seed, device=dev)
-        g.set_path(args.path); g.set_schedule(args.schedule); g.set_temperature(args.temperature)
+        g.set_path("STRIP" if peer else args.path); g.set_schedule(args.schedule); g.set_temperature(args.temperature)
         g.run(n_eq, n_meas)
         check = bool(np.array_equal(g.get_state().cpu().numpy(), ss.state()))
         g.close()
@@ -686,7 +690,8 @@ def run_slabs(args, rank, world, local_rank):
             "scaling": "strong", "vs_baseline": None, "dtype": "f64" if args.mode == "DP" else "f32", "data": "synthetic",
             "config": {"workload": "config%d_L%d" % (args.config, c.L), "L": c.L, "masked_fraction": c.f, "mode": args.mode,
                        "n_eq": n_eq, "n_meas": n_meas, "parallelism": "slabs x%d%s" % (count, "" if world > 1 else " on one GPU, in turn"),
-                       "halo_rows": args.halo, "sweeps_per_exchange": ss.sweeps_per_exchange,
+                       "halo_rows": ss.halo, "sweeps_per_exchange": ss.sweeps_per_exchange,
+                       "exchange": "in-kernel peer stores" if peer else "export / import copies between launches",
                        "l2": "state larger than the 126 MB L2; no flush" if c.L >= 4096 else "L2-resident state"},
             "clocks": clk, "T_hat": ss.T, "e_mean": e, "e_stderr": se, "mae": float(err[0] / max(err[1], 1.0)),
             "exchanges": ss.exchanges, "identical_to_single_context": check,

@@ -251,6 +251,17 @@ int mpr_predict_host_rect(int Lx, int Ly, const double* h_values, const uint8_t*
  *                  caller refreshes the halos (export from the owner, import into the neighbour) at least every
  *                  halo / 4 sweeps -- paper_1910_08448_b200/slabs.py does, in one process or one rank per slab.
  *                  (mpr_set_workspace on a slab context: call mpr_set_slab again afterwards.)
+ *   mpr_set_peers  PEER MODE: instead of export / import between launches, every STRIP launch of a slab stores the 4 own
+ *                  rows next to each inner edge straight into the halo rows of the neighbour's destination buffer
+ *                  (peer memory: on one GPU another pointer, between GPUs of one process a store over NVLink once peer
+ *                  access is enabled) and its own buffer receives its halo rows the same way -- compute and exchange in
+ *                  ONE kernel, no copy launch.  up / down = the contexts of the slabs above / below (null at the ends of
+ *                  the grid; both null leaves peer mode).  Requirements: slabs of the same grid, mode and stream, halo
+ *                  of exactly 4 rows, >= 8 own rows, q = 1/2; every slab makes the same sequence of calls, one launch
+ *                  each in turn (a launch finds the neighbour's buffer by the number of launches both have made);
+ *                  one sweep per launch, quench double passes two per launch.  With the slabs on different streams or
+ *                  devices the caller orders launch n + 1 of a slab after launch n of its neighbours (events); on one
+ *                  stream the stream does.  Resets the chain.
  *   mpr_sample_energy_parts   the sum of cos over, and the number of, measured nearest-neighbour pairs to the right
  *                  of and below the own rows: e_s of the whole grid = -2 J sum(parts) / sum(counts).  HOST outs.
  *   mpr_rows_bytes / mpr_export_rows / mpr_import_rows   n_rows rows of the chain state from row_begin on (both
@@ -264,6 +275,7 @@ int mpr_predict_host_rect(int Lx, int Ly, const double* h_values, const uint8_t*
  *   mpr_debug_trial_lengths   the fixed sweep counts of one temperature trial of R6 (equilibration, measurement). */
 int mpr_set_slab(mpr_ctx* ctx, int global_row0, int own_begin, int own_end, double z_min, double z_max,
                  double global_bonds);
+int mpr_set_peers(mpr_ctx* ctx, mpr_ctx* up, mpr_ctx* down);
 int mpr_sample_energy_parts(mpr_ctx* ctx, double* cos_sum, int64_t* n_pairs);
 int mpr_rows_bytes(mpr_ctx* ctx, int n_rows, size_t* bytes);
 int mpr_export_rows(mpr_ctx* ctx, int row_begin, int n_rows, void* d_out);

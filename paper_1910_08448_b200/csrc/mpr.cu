@@ -53,6 +53,10 @@ Layout make_layout(int L, int H) {      // L columns, H rows
   lo.g.site0 = 0u;
   lo.g.own0 = 0;
   lo.g.own1 = H;
+  lo.g.peer_rows = 0;
+  lo.g.peer_dst[0] = lo.g.peer_dst[1] = nullptr;
+  lo.g.peer_plane[0] = lo.g.peer_plane[1] = 0;
+  lo.g.peer_row_off[0] = lo.g.peer_row_off[1] = 0;
   lo.g.Wp = static_cast<int>(align_up(static_cast<size_t>((L + 1) / 2), 16));
   lo.g.Wm = (lo.g.Wp + 31) / 32;
   lo.g.Wb = lo.g.Wm + kBitPadLeft + kBitPadRight;
@@ -115,6 +119,11 @@ struct mpr_ctx {
   double pair_sum = 0.0;         // sum of cos over the measured pairs behind e_sample (mpr_sample_energy_parts)
   double nb_norm = 0.0;          // bonds the energy is normalised by: bond_count(g), or the whole grid's for a slab
   bool slab = false;
+  // peer mode (mpr_set_peers): the neighbour slabs' contexts (same process) and the number of strip launches made so
+  // far, by which a launch finds the buffer its neighbour's launch of the same number writes
+  mpr_ctx* peer[2] = {nullptr, nullptr};
+  int slab_row0 = 0;           // global row of local row 0 (mpr_set_slab)
+  long long strip_epoch = 0;
   uint32_t n_list[2] = {0u, 0u};     // prediction sites per colour (lengths of the LIST path's lists)
   uint64_t launches = 0;
   std::vector<double> series;
@@ -336,7 +345,22 @@ template <int MODE> int tiled_sweeps(mpr_ctx* c, int k, int measure, double* d_e
 // passes (PROG_QUENCH, k = 2); `measure` as in tiled_sweeps.
 template <int MODE> int strip_sweeps(mpr_ctx* c, int prog, int k, int measure, double* d_e) {
   using R = typename Traits<MODE>::real;
-  const Geom& g = c->lo.g;
+  Geom g = c->lo.g;
+  if (g.peer_rows) {
+    // the buffer the neighbour's launch number `strip_epoch` writes: the other one if it has not been launched yet,
+    // its current one if it already has
+    for (int d = 0; d < 2; ++d) {
+      const mpr_ctx* p = c->peer[d];
+      g.peer_dst[d] = nullptr;
+      if (!p) continue;
+      if (p->strip_epoch != c->strip_epoch && p->strip_epoch != c->strip_epoch + 1)
+        return fail(c, MPR_ERR_INVALID_ARG, "peer mode: the slabs are out of step (every slab makes the same calls in turn)");
+      if (p->mode != c->mode || !p->ws) return fail(c, MPR_ERR_INVALID_ARG, "peer mode: neighbour in another mode or without workspace");
+      g.peer_dst[d] = p->state(p->strip_epoch == c->strip_epoch ? 1 - p->cur : p->cur);
+      g.peer_plane[d] = static_cast<long long>(p->lo.g.plane);
+      g.peer_row_off[d] = c->slab_row0 - p->slab_row0;
+    }
+  }
   const ChainConst<R> kc = chain_const<R>(c);
   int nblocks = 0;
   StripArgs a{&c->strip, &c->tiled, g, c->cur, c->state(c->cur), c->state(1 - c->cur), {c->smask(1), c->smask(2)}, c->acc(), c->part(),
@@ -347,6 +371,7 @@ template <int MODE> int strip_sweeps(mpr_ctx* c, int prog, int k, int measure, d
   if (st != 0) return fail(c, MPR_ERR_CUDA, std::string("strip launch: ") + tiled_error(st));
   c->launches += 1;
   c->cur = 1 - c->cur;
+  c->strip_epoch += 1;
   if (measure == 1 || measure == 2) {
     const double nb = c->nb_norm;
     final_sum_kernel<<<1, 1024, 0, c->stream>>>(c->part(), nblocks, -kJ * 2.0 / nb, d_e, g.energy_single);
@@ -441,6 +466,7 @@ int do_strip(mpr_ctx* c, int prog, int k, int measure, double* d_e) {
 // schedule (which the TILED kernels do not carry); the TILED kernels otherwise (double arithmetic and the
 // library sincosf / expf of SP_PRECISE need more registers per update chain than four interleaved chains leave).
 int eff_path(const mpr_ctx* c) {
+  if (c->lo.g.peer_rows) return MPR_PATH_STRIP;      // peer mode lives in the strip kernels (mpr_set_peers checks the rest)
   // q < 1/2 (mpr_set_q): the general range test lives in the per-pass kernels only
   if (c->lo.g.q != kQDefault) return c->path == MPR_PATH_LIST ? MPR_PATH_LIST : MPR_PATH_PLAIN;
   // half-precision storage: the TILED kernel's tile origins (60 tx - 2 plane columns) are not 16-byte aligned at
@@ -463,6 +489,8 @@ int eff_path(const mpr_ctx* c) {
 // halo 4 k), the strip kernel two per launch, an odd remainder goes through the plain kernels -- same moves, same order
 int quench_passes(mpr_ctx* c, int left) {
   const int path = eff_path(c);
+  if (c->lo.g.peer_rows && (left & 1))
+    return fail(c, MPR_ERR_INVALID_ARG, "peer mode: quench double passes come two per launch (an even number)");
   if (path == MPR_PATH_TILED) {
     while (left >= 2) {
       const int k = left / 2 < 2 ? left / 2 : 2;
@@ -569,6 +597,7 @@ int hybrid_sweeps(mpr_ctx* c, int n, int measure, int first_slot) {
     double* d_e = measure ? c->dseries() + first_slot + done : nullptr;
     if (path == MPR_PATH_STRIP) {
       if (k > 2) k = 2;                                   // the strip pipeline carries at most two sweeps
+      if (c->lo.g.peer_rows) k = 1;                       // peer mode: the halo lasts one sweep, refreshed by every launch
       TRY(do_strip(c, c->schedule == MPR_SCHEDULE_SITE_FUSED ? PROG_FUSED : PROG_R4, k, measure, d_e));
     } else {
       TRY(do_tiled(c, k, measure, d_e));
@@ -984,6 +1013,7 @@ int mpr_set_slab(mpr_ctx* c, int global_row0, int own_begin, int own_end, double
       (static_cast<long long>(global_row0) + g.H) * g.L > (1ll << 32))
     return fail(c, MPR_ERR_INVALID_ARG, "slab: first row even and >= 0, 0 <= own_begin < own_end <= rows, z_max > z_min");
   CUDA_OK(c, cudaStreamSynchronize(c->stream));
+  c->slab_row0 = global_row0;
   g.site0 = static_cast<uint32_t>(static_cast<long long>(global_row0) * g.L);
   g.own0 = own_begin;
   g.own1 = own_end;
@@ -1010,6 +1040,41 @@ int mpr_set_slab(mpr_ctx* c, int global_row0, int own_begin, int own_end, double
   for (int col = 0; col < 2; ++col)
     for (int y = own_begin; y < own_end; ++y) nf += rc[static_cast<size_t>(col) * g.H + y];
   c->n_free = nf;
+  mark_stale(c);
+  return MPR_OK;
+}
+
+int mpr_set_peers(mpr_ctx* c, mpr_ctx* up, mpr_ctx* down) {
+  if (!c) return MPR_ERR_INVALID_ARG;
+  Geom& g = c->lo.g;
+  if (!up && !down) {                       // leave peer mode
+    g.peer_rows = 0;
+    c->peer[0] = c->peer[1] = nullptr;
+    return MPR_OK;
+  }
+  if (!c->slab) return fail(c, MPR_ERR_INVALID_ARG, "peer mode: mpr_set_slab first");
+  if (g.q != kQDefault) return fail(c, MPR_ERR_INVALID_ARG, "peer mode runs on the strip kernels: q = 1/2 only");
+  constexpr int kPeerRows = 4;              // one launch (a hybrid sweep, or two quench double passes) spoils 4 halo rows
+  mpr_ctx* ps[2] = {up, down};
+  for (int d = 0; d < 2; ++d) {
+    const mpr_ctx* p = ps[d];
+    if (!p) continue;
+    if (p == c || !p->slab || p->lo.g.L != g.L || p->mode != c->mode || p->stream != c->stream)
+      return fail(c, MPR_ERR_INVALID_ARG, "peer mode: neighbours are slabs of the same grid, mode and stream");
+    // the neighbour's halo must be exactly the rows this slab sends: kPeerRows rows beyond its own rows, on my side
+    const int my_first = c->slab_row0 + g.own0, my_last = c->slab_row0 + g.own1;         // global own rows [first, last)
+    const int p_first = p->slab_row0 + p->lo.g.own0, p_last = p->slab_row0 + p->lo.g.own1;
+    const bool ok = d == 0 ? (p_last == my_first && p->lo.g.H - p->lo.g.own1 == kPeerRows && g.own0 == kPeerRows)
+                           : (p_first == my_last && p->lo.g.own0 == kPeerRows && g.H - g.own1 == kPeerRows);
+    if (!ok) return fail(c, MPR_ERR_INVALID_ARG, "peer mode: adjacent slabs with a halo of exactly 4 rows");
+  }
+  if ((!up && g.own0 != 0) || (!down && g.own1 != g.H))
+    return fail(c, MPR_ERR_INVALID_ARG, "peer mode: a slab with halo rows on a side needs the neighbour of that side");
+  if (g.own1 - g.own0 < 2 * kPeerRows) return fail(c, MPR_ERR_INVALID_ARG, "peer mode: a slab owns at least 8 rows");
+  c->peer[0] = up;
+  c->peer[1] = down;
+  g.peer_rows = kPeerRows;
+  c->strip_epoch = 0;
   mark_stale(c);
   return MPR_OK;
 }

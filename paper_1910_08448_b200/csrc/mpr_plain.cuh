@@ -26,6 +26,15 @@ struct Geom {
   // [own0, own1) -- the rows this slab owns, the rest being halo -- enter the energy sums and the accepted-move count.
   uint32_t site0;        // 0 for a whole grid
   int own0, own1;        // [0, H) for a whole grid
+  // Peer mode of a slab (mpr_set_peers; STRIP kernels only): a launch stores its OWN rows only, and the `peer_rows`
+  // own rows next to each inner edge ALSO straight into the halo rows of the neighbour slab's destination buffer --
+  // peer memory; on one GPU just another pointer, between GPUs a store over NVLink -- so that no copy launch follows.
+  // peer_dst[d] (d = 0: the slab above, 1: below; null = none) is the neighbour's destination state buffer of this
+  // launch, peer_plane[d] its plane size in units, peer_row_off[d] = (neighbour's local row) - (this slab's local row).
+  int peer_rows;         // 0: not in peer mode
+  void* peer_dst[2];
+  long long peer_plane[2];
+  int peer_row_off[2];
   double q;              // PAPER.md:27, q in (0, 1/2]; 1/2 unless mpr_set_q
   int energy_single;     // X_E of PAPER.md:35: 0 = energy sums in double (R13), 1 = the energy variable is a float
 };

@@ -207,8 +207,12 @@ strip_kernel(const __grid_constant__ CUtensorMap tmap, typename Traits<MODE>::ve
       // [cnt_b, cnt_e): the rows of the segment that enter the accepted-move count and the energy sum -- all of them,
       // unless the context is a slab of a larger grid (Geom::own0 / own1: its halo rows are updated and stored, not counted)
       const int cnt_b = max(yb, g.own0), cnt_e = min(ye, g.own1);
-      const int i_lo = (cnt_b - t0 + LAG * (NS - 1) + RB - 1) / RB;     // = (LEAD + LAG (NS - 1) + RB - 1) / RB when cnt_b = yb
-      const int i_hi = (max(cnt_e, t0) - t0) / RB;                      // RB i + RB - 1 < cnt_e - t0
+      // peer mode (Geom::peer_rows > 0): the own rows next to an inner edge are also stored into the neighbour slab; they
+      // are left to the predicated iterations too.  [st_b, st_e): the rows this launch stores into its own buffer.
+      const int fast_b = cnt_b + (g.peer_dst[0] ? g.peer_rows : 0), fast_e = cnt_e - (g.peer_dst[1] ? g.peer_rows : 0);
+      const int st_b = g.peer_rows ? cnt_b : yb, st_e = g.peer_rows ? cnt_e : ye;
+      const int i_lo = (fast_b - t0 + LAG * (NS - 1) + RB - 1) / RB;    // = (LEAD + LAG (NS - 1) + RB - 1) / RB when fast_b = yb
+      const int i_hi = (max(fast_e, t0) - t0) / RB;                     // RB i + RB - 1 < fast_e - t0
       const int j = j0 + 2 * lane;
       const bool lane_ok = lane >= HL && lane < 32 - HL && j < g.Wp;
       int seg_acc = 0;
@@ -367,9 +371,18 @@ strip_kernel(const __grid_constant__ CUtensorMap tmap, typename Traits<MODE>::ve
             // rows above t0 do not exist; nobody reads the ring copy of the last stage's row (it is final: global only)
             if (p < NS - 1 && (!EDGE || n >= LAG * p)) *reinterpret_cast<Unit<S>*>(own[p]) = out;
             if (p >= NS - 2) {                                                            // last stage of this colour
-              const bool owned = lane_ok && (!EDGE || (row >= yb && row < ye));
+              const bool owned = lane_ok && (!EDGE || (row >= st_b && row < st_e));
               if (owned) {
                 *reinterpret_cast<Unit<S>*>(gp - (LAG * p) * grow + col * gplane) = out;
+                if (EDGE && g.peer_rows) {       // peer mode: the rows next to an inner edge go to the neighbour's halo as well
+#pragma unroll
+                  for (int d = 0; d < 2; ++d) {
+                    const bool send = d == 0 ? row < g.own0 + g.peer_rows : row >= g.own1 - g.peer_rows;
+                    if (send && g.peer_dst[d])
+                      *reinterpret_cast<Unit<S>*>(reinterpret_cast<S*>(g.peer_dst[d]) +
+                          2 * (static_cast<long long>(row + g.peer_row_off[d]) * g.Wp + j + col * g.peer_plane[d])) = out;
+                  }
+                }
                 if (MEASURE == 2) {
                   const int rel = u - LAG * p;
                   const int mqk = (rel >= 0) ? 0 : (-rel + RB - 1) / RB;

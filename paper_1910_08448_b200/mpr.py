@@ -35,7 +35,7 @@ SYMBOLS = [
     "mpr_get_info",
     "mpr_get_launch_stats", "mpr_workspace_bytes_host", "mpr_predict_host", "mpr_debug_philox",
     "mpr_workspace_bytes_rect", "mpr_create_rect", "mpr_workspace_bytes_host_rect", "mpr_predict_host_rect",
-    "mpr_set_slab", "mpr_sample_energy_parts", "mpr_rows_bytes", "mpr_export_rows", "mpr_import_rows", "mpr_advance",
+    "mpr_set_slab", "mpr_set_peers", "mpr_sample_energy_parts", "mpr_rows_bytes", "mpr_export_rows", "mpr_import_rows", "mpr_advance",
     "mpr_fetch_series", "mpr_predict", "mpr_debug_trial_lengths", "mpr_quench",
     "mpr_debug_accept",
     "mpr_static_setup", "mpr_static_max_sites", "mpr_static_last_error", "mpr_sample_energy_static",
@@ -117,6 +117,7 @@ def lib():
         "mpr_debug_philox": (C.c_int, [vp, C.POINTER(C.c_uint32), vp, i64, vp]),
         "mpr_set_slab": (C.c_int, [vp, C.c_int, C.c_int, C.c_int, C.c_double, C.c_double, C.c_double]),
         "mpr_sample_energy_parts": (C.c_int, [vp, dp, i64p]),
+        "mpr_set_peers": (C.c_int, [vp, vp, vp]),
         "mpr_rows_bytes": (C.c_int, [vp, C.c_int, C.POINTER(C.c_size_t)]),
         "mpr_export_rows": (C.c_int, [vp, C.c_int, C.c_int, vp]),
         "mpr_import_rows": (C.c_int, [vp, C.c_int, C.c_int, vp]),
@@ -333,6 +334,10 @@ class Mpr:
     def set_slab(self, global_row0, own_begin, own_end, z_min, z_max, global_bonds):
         self._call(lib().mpr_set_slab, int(global_row0), int(own_begin), int(own_end), float(z_min), float(z_max),
                    float(global_bonds))
+
+    def set_peers(self, up, down):
+        """Peer mode (mpr_set_peers): up / down = the Mpr objects of the slabs above / below, or None."""
+        self._call(lib().mpr_set_peers, up.h if up is not None else None, down.h if down is not None else None)
 
     def sample_energy_parts(self):
         s, n = C.c_double(), C.c_int64()

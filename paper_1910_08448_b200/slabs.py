@@ -191,6 +191,9 @@ class MprSlab:
         p = self.plan
         self.ctx.set_slab(p.row0_g, p.own_begin, p.own_end, z_min, z_max, global_bonds)
 
+    def set_peers(self, up, down):
+        self.ctx.set_peers(up.ctx if up is not None else None, down.ctx if down is not None else None)
+
     def sample_energy_parts(self):
         return self.ctx.sample_energy_parts()
 
@@ -247,10 +250,16 @@ class SlabSet:
     The last three are the library's own host routines (no GPU needed); they are arguments so that this module
     imports nothing of the method."""
 
-    def __init__(self, plans, slabs, n_cols, transport, n_quench=32, trial_lengths=(200, 50), stats=None, match=None):
+    def __init__(self, plans, slabs, n_cols, transport, n_quench=32, trial_lengths=(200, 50), stats=None, match=None,
+                 peer=False):
         self.plans, self.slabs, self.transport = plans, slabs, transport
         self.halo = plans[0].halo
         self.sweeps_per_exchange = self.halo // 4        # a hybrid sweep spoils 4 halo rows
+        # peer mode (mpr_set_peers): every launch writes its edge rows straight into the neighbours' halos -- no exchange
+        # step at all; needs all slabs in this process, a halo of 4 rows and an even number of quench double passes
+        self.peer = bool(peer)
+        if self.peer and (self.halo != 4 or len(slabs) != len(plans) or n_quench % 2):
+            raise ValueError("peer mode: all slabs in one process, halo 4, even n_quench")
         self.n_cols = n_cols
         self.n_quench = n_quench
         self.trial_lengths = trial_lengths
@@ -269,6 +278,9 @@ class SlabSet:
         self.n_pairs = int(round(parts[1]))
         self.e_sample = -2.0 * parts[0] / parts[1] if parts[1] > 0 else float("nan")
         self.n_free = int(round(transport.reduce_sum([np.array([s.n_free()], dtype=np.float64) for s in slabs.values()])[0]))
+        if self.peer:
+            for i, s in slabs.items():
+                s.set_peers(slabs.get(i - 1), slabs.get(i + 1))
 
     def moves(self):
         """The rows that travel in one refresh: every slab sends the `halo` own rows next to each inner edge."""
@@ -281,7 +293,7 @@ class SlabSet:
         return out
 
     def exchange(self):
-        if len(self.plans) > 1:
+        if len(self.plans) > 1 and not self.peer:
             self.transport.transfer(self.slabs, self.moves())
             self.exchanges += 1
 
@@ -372,7 +384,7 @@ class SlabSet:
 
 
 def make_slab_set(values, mask, count, halo=8, mode="DP", seed=0, device="cuda:0", path="AUTO", schedule="R4",
-                  transport=None, n_quench=32):
+                  transport=None, n_quench=32, peer=False):
     """The CUDA path on `count` slabs.  transport None: all slabs in this process on `device`; a DistTransport: this rank
     builds slab number transport.rank only (count = world size)."""
     from . import mpr
@@ -382,4 +394,4 @@ def make_slab_set(values, mask, count, halo=8, mode="DP", seed=0, device="cuda:0
     mine = [p for p in plans if transport.owner(p.index) == transport.rank]
     slabs = {p.index: MprSlab(p, values, mask, mode=mode, seed=seed, device=device, path=path, schedule=schedule) for p in mine}
     return SlabSet(plans, slabs, int(mask.shape[1]), transport, n_quench=n_quench, trial_lengths=mpr.debug_trial_lengths(),
-                   stats=mpr.debug_series_stats, match=mpr.debug_match_temperature)
+                   stats=mpr.debug_series_stats, match=mpr.debug_match_temperature, peer=peer)

@@ -131,3 +131,42 @@ def test_slabs_at_a_strip_kernel_size(mpr, inputs, slabs):
     assert np.array_equal(ss.state(), st_w) and ss.accepted() == acc_w
     assert abs(e - e_w) <= 2e-12
     assert np.array_equal(np.nan_to_num(ss.prediction(), nan=-1.0), np.nan_to_num(pred_w.cpu().numpy(), nan=-1.0))
+
+
+@pytest.mark.parametrize("mode,schedule", [("SP_INTRINSIC", "R4"), ("SP_INTRINSIC", "SITE_FUSED"), ("DP", "R4"), ("HP", "R4")])
+@pytest.mark.parametrize("count", [2, 3, 4])
+def test_peer_mode_reproduces_the_single_context(mpr, inputs, slabs, mode, schedule, count):
+    """mpr_set_peers: every strip launch writes its 4 edge rows straight into the neighbours' halo rows (peer memory) and
+    stores its own rows only -- no export / import launches at all.  Same result as the single context, bit for bit."""
+    Ly, Lx = 190, 141
+    values, mask, _ = inputs.make_rect_problem(Ly, Lx, 7.0, 56, 0.7)
+    T, n_eq, n_meas = 0.04, 7, 6
+    st_w, acc_w, series_w, pred_w, e_w, se_w, _, _ = whole(mpr, values, mask, mode, 78, "STRIP", schedule, T, n_eq, n_meas)
+    ss = slabs.make_slab_set(values, mask, count, halo=4, mode=mode, seed=78, path="STRIP", schedule=schedule, peer=True)
+    ss.set_temperature(T)
+    ss.reset_chain(0)
+    launches0 = sum(s.ctx.launches() for s in ss.slabs.values())
+    series, e, se = ss.run(n_eq, n_meas)
+    # one strip launch per slab and sweep, plus the energy reduction of each measuring sweep: nothing else ran
+    assert sum(s.ctx.launches() for s in ss.slabs.values()) - launches0 == count * (n_eq + 2 * n_meas)
+    assert ss.exchanges == 0
+    assert np.array_equal(ss.state(), st_w) and ss.accepted() == acc_w
+    assert np.max(np.abs(series - np.asarray(series_w))) <= 2e-12 and abs(e - e_w) <= 2e-12
+    assert np.array_equal(np.nan_to_num(ss.prediction(), nan=-1.0), np.nan_to_num(pred_w, nan=-1.0))
+
+
+def test_peer_mode_temperature_matching_and_checks(mpr, inputs, slabs):
+    values, mask, _ = inputs.make_rect_problem(96, 96, 8.0, 53, 0.66)
+    g = mpr.Mpr(values, mask, mode="DP", seed=9)
+    g.set_path("STRIP")
+    T_w = g.estimate_temperature()[0]
+    ss = slabs.make_slab_set(values, mask, 2, halo=4, mode="DP", seed=9, path="STRIP", peer=True)
+    assert abs(ss.estimate_temperature() - T_w) <= 1e-9 * T_w and ss.exchanges == 0
+    with pytest.raises(ValueError):
+        slabs.make_slab_set(values, mask, 2, halo=8, mode="DP", seed=9, peer=True)
+    # a context that is not a slab, or a neighbour that does not fit, is refused
+    with pytest.raises(mpr.MprError):
+        g.set_peers(None, ss.slabs[0].ctx)
+    with pytest.raises(mpr.MprError):
+        ss.slabs[0].ctx.set_peers(ss.slabs[1].ctx, None)       # slab 1 lies below slab 0, not above
+    g.close()
