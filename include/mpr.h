@@ -259,9 +259,9 @@ int mpr_predict_host_rect(int Lx, int Ly, const double* h_values, const uint8_t*
  *                  the grid; both null leaves peer mode).  Requirements: slabs of the same grid, mode and stream, halo
  *                  of exactly 4 rows, >= 8 own rows, q = 1/2; every slab makes the same sequence of calls, one launch
  *                  each in turn (a launch finds the neighbour's buffer by the number of launches both have made);
- *                  one sweep per launch, quench double passes two per launch.  With the slabs on different streams or
- *                  devices the caller orders launch n + 1 of a slab after launch n of its neighbours (events); on one
- *                  stream the stream does.  Resets the chain.
+ *                  one sweep per launch, quench double passes two per launch.  Launch n + 1 of a slab must follow launch
+ *                  n of its neighbours: this version requires all slabs on ONE stream, whose order gives exactly that
+ *                  (slabs on several devices would need peer access and an event per launch: not built).  Resets the chain.
  *   mpr_sample_energy_parts   the sum of cos over, and the number of, measured nearest-neighbour pairs to the right
  *                  of and below the own rows: e_s of the whole grid = -2 J sum(parts) / sum(counts).  HOST outs.
  *   mpr_rows_bytes / mpr_export_rows / mpr_import_rows   n_rows rows of the chain state from row_begin on (both
