@@ -357,3 +357,49 @@ def test_metropolis_decision_filter_is_exact(mpr):
     assert np.array_equal(plain[: x.size][clear], (U[: x.size] < np.exp(np.minimum(X[: x.size], 0.0)))[clear].astype(np.uint8))
     assert 1.0 - fast[:n].mean() < 3e-4                    # ordinary moves: the filter decides alone
     assert fast[x.size: x.size + n].mean() < 0.9           # the edge cases do reach the double evaluation
+
+
+@pytest.mark.parametrize("path", ["PLAIN", "LIST", "TILED", "STRIP"])
+@pytest.mark.parametrize("mode", ["DP", "SP_INTRINSIC"])
+def test_nothing_to_predict(mpr, path, mode):
+    """The empty problem: every site measured.  Every path runs (no zero-sized launch), nothing moves, no move is
+    attempted, the chain energy is the sample energy, the prediction is the input."""
+    L = 70
+    rng = np.random.default_rng(4)
+    z = rng.normal(50.0, 10.0, (L, L))
+    g = mpr.Mpr(z, np.zeros((L, L), dtype=np.uint8), mode=mode, seed=1)
+    g.set_path(path)
+    g.set_temperature(0.1)
+    st0 = g.get_state().cpu().numpy()
+    pred, e, se = g.run(3, 4)
+    assert np.array_equal(g.get_state().cpu().numpy(), st0)
+    assert g.counters() == (0, 0, 7)
+    es, n_pairs = g.sample_energy()
+    assert n_pairs == 2 * L * (L - 1) and abs(e - es) <= (1e-12 if mode == "DP" else 2e-6) and se <= 1e-12
+    assert np.array_equal(pred.cpu().numpy(), z)
+    for sched in ("SITE_FUSED",):
+        if path != "TILED":
+            g.set_schedule(sched)
+            g.sweep(2)
+            assert np.array_equal(g.get_state().cpu().numpy(), st0)
+    g.close()
+
+
+def test_one_prediction_site(mpr, oracle_mod):
+    """The smallest non-empty problem on every path: one free site in a corner of a grid that is not a multiple of anything."""
+    L = 67
+    rng = np.random.default_rng(6)
+    z = rng.normal(50.0, 10.0, (L, L))
+    mask = np.zeros((L, L), dtype=np.uint8)
+    mask[L - 1, L - 1] = 1
+    o = oracle_mod.Oracle(values=z, mask=mask, seed=3)
+    o.set_temperature(0.2)
+    o.hybrid_sweeps(25)
+    for path in ("PLAIN", "LIST", "TILED", "STRIP"):
+        g = mpr.Mpr(z, mask, seed=3)
+        g.set_path(path)
+        g.set_temperature(0.2)
+        g.sweep(25)
+        assert np.max(np.abs(g.get_state().cpu().numpy() - o.get_state())) <= 1e-9, path
+        assert g.counters() == o.counters(), path
+        g.close()
