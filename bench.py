@@ -648,12 +648,23 @@ def run_slabs(args, rank, world, local_rank):
         else:
             ss.estimate_temperature()
             nt = ss.n_trials
-        _, e, se = ss.run(n_eq, n_meas)
+        # the equilibration sweeps timed by themselves (all slabs, exchanges included), then the measuring sweeps
+        q0, q1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        q0.record()
+        ss.sweep(n_eq)
+        q1.record()
+        _, e, se = ss.run(0, n_meas)
+        torch.cuda.synchronize(dev)
+        eq["ms"] += q0.elapsed_time(q1)
+        eq["sweeps"] += n_eq
         return nt * sum(ss.trial_lengths) + n_eq + n_meas, e, se
+
+    eq = {"ms": 0.0, "sweeps": 0}
 
     for _ in range(args.warmup):
         step()
     sync()
+    eq.update(ms=0.0, sweeps=0)
     clocks = ClockSampler(local_rank)
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     ev0.record()
@@ -695,6 +706,7 @@ def run_slabs(args, rank, world, local_rank):
                        "l2": "state larger than the 126 MB L2; no flush" if c.L >= 4096 else "L2-resident state"},
             "clocks": clk, "T_hat": ss.T, "e_mean": e, "e_stderr": se, "mae": float(err[0] / max(err[1], 1.0)),
             "exchanges": ss.exchanges, "identical_to_single_context": check,
+            "ms_per_equilibration_sweep": eq["ms"] / max(eq["sweeps"], 1),
         }))
     if world > 1:
         dist.destroy_process_group()
