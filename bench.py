@@ -303,14 +303,16 @@ def run_ours(args, rank, world, local_rank):
     ms_max, units_total, launches_total = sharding.aggregate(
         ms, 2.0 * state["n_free"] * state["sweeps"], state["launches"], world, device=dev)
     value = sharding.throughput(units_total, ms_max)
+    path_used_early = args.path if args.path != "AUTO" else ("STRIP" if (mode in ("SP_INTRINSIC", "HP") and c.L >= 4096) else "OTHER")
 
-    # ---- the same step under the site-fused schedule (R4b), two sweeps per launch: reported beside the headline ------
-    fused_leg = None
-    if args.schedule == "R4" and not args.skip_fused_leg and mode in ("SP_INTRINSIC", "HP"):
-        def fused_step():
+    # ---- the same step in two other launch configurations, reported beside the headline (which stays R4, one sweep per
+    # launch): the site-fused schedule (R4b) and R4 with two sweeps per launch (slower alone, but not clocked down by the
+    # power cap in a long run: DESIGN.md 4.4).  Same work, same timing rules, SM clock sampled during each leg.
+    def other_leg(schedule, k):
+        def leg_step():
             gf = mpr.Mpr(d_values, d_mask, mode=mode, seed=seed, device=dev)
-            gf.set_schedule("SITE_FUSED")
-            gf.set_fused_sweeps(2)
+            gf.set_schedule(schedule)
+            gf.set_fused_sweeps(k)
             if args.temperature is not None:
                 gf.set_temperature(args.temperature)
                 nt = 0
@@ -320,23 +322,31 @@ def run_ours(args, rank, world, local_rank):
             ms_eq, n_l, n_sw = gf.run_timing()
             gf.close()
             return nt * 250 + n_eq + n_meas, pf, ef, sef, ms_eq, n_sw
-        fused_step()
+        leg_step()
         barrier()
+        leg_clocks = ClockSampler(local_rank)
         f0, f1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         f0.record()
         sw_f, eq_ms_f, eq_sw_f = 0, 0.0, 0
         for _ in range(args.steps):
-            n_sw_step, pred_f, e_f, se_f, ms_eq, n_sw = fused_step()
+            n_sw_step, pred_f, e_f, se_f, ms_eq, n_sw = leg_step()
             sw_f += n_sw_step
             eq_ms_f += ms_eq
             eq_sw_f += n_sw
         f1.record()
         barrier()
+        leg_clk = leg_clocks.stop()
         msf_max, units_f, _ = sharding.aggregate(f0.elapsed_time(f1), 2.0 * state["n_free"] * sw_f, 0, world, device=dev)
         dfz = (pred_f - d_truth)[d_mask.bool()]
-        fused_leg = {"value": sharding.throughput(units_f, msf_max), "unit": UNIT, "ms_per_step": msf_max / args.steps,
-                     "schedule": "SITE_FUSED", "sweeps_per_launch": 2, "ms_per_sweep_in_step": eq_ms_f / max(eq_sw_f, 1),
-                     "e_mean": e_f, "e_stderr": se_f, "mae": float(dfz.abs().mean().item())}
+        return {"value": sharding.throughput(units_f, msf_max), "unit": UNIT, "ms_per_step": msf_max / args.steps,
+                "schedule": schedule, "sweeps_per_launch": k, "ms_per_sweep_in_step": eq_ms_f / max(eq_sw_f, 1),
+                "sm_mhz": leg_clk.get("sm_mhz"), "e_mean": e_f, "e_stderr": se_f, "mae": float(dfz.abs().mean().item())}
+
+    fused_leg, k2_leg = None, None
+    if args.schedule == "R4" and not args.skip_fused_leg and mode in ("SP_INTRINSIC", "HP"):
+        fused_leg = other_leg("SITE_FUSED", 2)
+        if path_used_early == "STRIP" and (args.fused or 1) == 1:
+            k2_leg = other_leg("R4", 2)
 
     # prediction error of the last step (metric of PAPER.md Eq. 4; post-processing, not the path)
     m1 = d_mask.bool()
@@ -379,7 +389,7 @@ def run_ours(args, rank, world, local_rank):
     path_used = auto_path(mode, args.schedule) if args.path == "AUTO" else args.path
 
     # what mpr_set_fused_sweeps(0) resolves to (csrc/mpr.cu, auto_fused)
-    def auto_fused(md, path):
+    def auto_fused(md, path, sched=None):
         if path != "TILED":
             return 1
         if md in ("DP", "SP"):
@@ -449,6 +459,10 @@ def run_ours(args, rank, world, local_rank):
         "kernel_ms_source": ("CUDA events around the %d equilibration launches inside the timed steps "
                              "(mpr_get_run_timing)" % state["eq_launches"]) if in_step else "burst leg",
         "kernel_ms_burst": kern_ms_burst, "sweeps_per_launch": k_eff,
+        "kernel_ms_per_sweep": kern_ms / k_eff, "kernel_ms_burst_per_sweep": kern_ms_burst / k_eff,
+        # the same fraction against the peak at the MAXIMUM SM clock: a launch that draws less power is clocked higher
+        # under the cap, which raises the sampled-clock peak it is measured against (and lowers `frac`) while it runs faster
+        "frac_at_max_clock": (roofline["frac"] * sm_mhz / (clk.get("sm_max_mhz") or sm_mhz)) if roofline["bound"] == "alu" else None,
         "algorithmic_bytes_per_launch": ceil["hbm_algorithmic"]["bytes_per_launch"],
         "state_bytes_per_launch": ceil["hbm_state_layout"]["bytes_per_launch"],
         "hbm_peak_gb_s": peak, "hbm_peak_source": peak_src,
@@ -463,7 +477,7 @@ def run_ours(args, rank, world, local_rank):
             if md not in c.modes and not (md == "HP" and "SP_INTRINSIC" in c.modes):     # HP: the paper's outlook, beside SSS
                 continue
             entry = {}
-            for sched, k in (("R4", auto_fused(md, auto_path(md, "R4"))), ("SITE_FUSED", 2)):
+            for sched, k in (("R4", auto_fused(md, auto_path(md, "R4"), "R4")), ("SITE_FUSED", 2)):
                 t_l, t_meas = time_sweeps(md, "AUTO", sched, k, n_sw, warm=3)
                 cl = ceilings(md, t_l, k, sm_mhz)
                 entry[sched] = {"path": auto_path(md, sched), "sweeps_per_launch": k, "ms_per_sweep": t_l / k,
@@ -525,7 +539,7 @@ def run_ours(args, rank, world, local_rank):
                        "l2": ("state (%.2f GiB) larger than the 126 MB L2; no flush" % (state_gib)) if state_gib * 2 ** 30 > 126e6
                              else "state (%.1f MiB) is L2-resident by design of this config (BASELINE.json); no flush" % (state_gib * 1024)},
             "clocks": clk, "e2e": e2e, "gpu_launches": launches_total, "roofline": roofline,
-            "cpu_baseline": cpu, "modes": modes, "site_fused": fused_leg, "T_hat": T_hat, "e_sample": state.get("e_sample"),
+            "cpu_baseline": cpu, "modes": modes, "site_fused": fused_leg, "two_sweeps_per_launch": k2_leg, "T_hat": T_hat, "e_sample": state.get("e_sample"),
             "e_mean": state["e"], "e_stderr": state["se"], "mae": mae, "rmse": rmse,
             "mae_of_sample_mean_predictor": base_mae, "input_generation_s": t_gen,
         }))

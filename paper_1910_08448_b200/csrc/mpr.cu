@@ -547,7 +547,13 @@ int ensure_chain(mpr_ctx* c) {
 // k = 1 / 2 / 4 -- float arithmetic: L = 64: 10.3 / 8.2 / 7.2, 512: 12.3 / 8.7 / 7.2, 1024: 12.3 / 9.2 / 12.3,
 // 1536: 18.5 / 14.4 / 18.0, 2048: 24.8 / 26.2 / 29.0; double arithmetic: 256: 20.5 / 17.8 / 16.4, 512: 20.5 / 17.8 / 22.6,
 // 1024: 28.7 / 35.9 / 50.1.  The result does not depend on k.
-int auto_fused(const mpr_ctx* c, int path) {
+// Not chosen automatically, but measured: the strip kernel of the headline mode with TWO sweeps per launch
+// (mpr_set_fused_sweeps(2): 8 stages, 8 warps per SM) is slower than one per launch when timed alone (1.066 against 0.99 ms
+// per sweep at L = 16384) yet moves half the DRAM bytes per sweep, draws less power and is not clocked down by this
+// pool's 1000 W cap in a long run (1965 against 1680 MHz): 1.068 against 1.101 ms per sweep inside bench.py's step.  A
+// property of the box's power limit, not of the kernel: the default stays one sweep per launch.
+int auto_fused(const mpr_ctx* c, int path, int n) {
+  (void)n;
   if (path != MPR_PATH_TILED) return 1;
   const double side = grid_side(c->lo.g);
   const bool dbl = c->mode == MPR_DP || c->mode == MPR_SP;
@@ -589,7 +595,7 @@ int hybrid_sweeps(mpr_ctx* c, int n, int measure, int first_slot) {
   }
   if (path == MPR_PATH_TILED && c->schedule != MPR_SCHEDULE_R4)
     return fail(c, MPR_ERR_INVALID_ARG, "the site-fused schedule runs on the STRIP and PLAIN paths");
-  const int fused = c->fused > 0 ? c->fused : auto_fused(c, path);
+  const int fused = c->fused > 0 ? c->fused : auto_fused(c, path, n);
   int done = 0;
   while (done < n) {
     // measurement needs the state after every sweep: one sweep per launch there

@@ -589,3 +589,14 @@ def test_bench_configuration_full_size_properties(mpr, config5, mode):
         assert out[path][1] == out["PLAIN"][1], path
         np.testing.assert_allclose(out[path][2], out["PLAIN"][2], rtol=0, atol=1e-12)
         assert torch.equal(out[path][3], out["PLAIN"][3]), path
+    if mode == "SP_INTRINSIC":
+        # bench.py also times the step with two sweeps per launch (`two_sweeps_per_launch`): 5 sweeps at depth 2 =
+        # launches of 2 + 2 + 1 sweeps, against the per-pass kernels
+        res = {}
+        for path, k in (("STRIP", 2), ("PLAIN", 1)):
+            g = mpr.Mpr(d_values, d_mask, mode=mode, seed=c.mpr_seed)
+            g.set_path(path); g.set_fused_sweeps(k); g.set_quench(2); g.set_temperature(1.1e-3)
+            g.sweep(5)
+            res[path] = (g.get_state(), g.counters())
+            g.close()
+        assert torch.equal(res["STRIP"][0], res["PLAIN"][0]) and res["STRIP"][1] == res["PLAIN"][1]
