@@ -112,3 +112,33 @@ def test_undefined_cases_and_limits(mpr):
     m0 = torch.zeros((L, L), dtype=torch.uint8, device=dev)
     got = mpr.sample_energy_static(z, m0, out).cpu().numpy()
     assert got[1] == 2 * L * (L - 1) and not math.isnan(got[0])
+
+
+def test_captured_in_a_cuda_graph(mpr, inputs):
+    """The reason the entry point exists: it can be recorded into a CUDA graph (no allocation, no synchronisation, no
+    host read-back inside the call) and replayed on new data in the same buffers."""
+    import torch
+    dev = torch.device("cuda:0")
+    assert mpr.lib().mpr_static_setup() == mpr.MPR_OK         # the symbol's address is taken before the capture
+    a = inputs.make_problem(200, 8.0, 61, 0.5)
+    b = inputs.make_problem(200, 8.0, 62, 0.7)
+    dv, dm = torch.from_numpy(a[0]).to(dev), torch.from_numpy(a[1]).to(dev)
+    out = torch.zeros(6, dtype=torch.float64, device=dev)
+    side = torch.cuda.Stream(device=dev)
+    side.wait_stream(torch.cuda.current_stream(dev))
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.stream(side):
+        mpr.sample_energy_static(dv, dm, out, stream=side)    # warm-up outside the capture (loads the kernels)
+        side.synchronize()
+        with torch.cuda.graph(graph, stream=side):
+            mpr.sample_energy_static(dv, dm, out, stream=side)
+    torch.cuda.current_stream(dev).wait_stream(side)
+    out.zero_()
+    graph.replay()
+    torch.cuda.synchronize(dev)
+    check(mpr, out, a[0], a[1])
+    dv.copy_(torch.from_numpy(b[0]))                           # new data in the same buffers, same graph
+    dm.copy_(torch.from_numpy(b[1]))
+    graph.replay()
+    torch.cuda.synchronize(dev)
+    check(mpr, out, b[0], b[1])
