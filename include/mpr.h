@@ -251,6 +251,10 @@ int mpr_predict_host_rect(int Lx, int Ly, const double* h_values, const uint8_t*
  *                  caller refreshes the halos (export from the owner, import into the neighbour) at least every
  *                  halo / 4 sweeps -- paper_1910_08448_b200/slabs.py does, in one process or one rank per slab.
  *                  (mpr_set_workspace on a slab context: call mpr_set_slab again afterwards.)
+ *   mpr_create_slab   mpr_create_rect for rows that are GOING TO BE a slab: the local sample may hold no measured site, or a
+ *                  single value (sparse data, thin slabs) -- what counts is the whole grid's range, which mpr_set_slab
+ *                  brings; until mpr_set_slab every compute call returns MPR_ERR_NOT_READY.  Non-finite measured values
+ *                  still fail.
  *   mpr_set_peers  PEER MODE: instead of export / import between launches, every STRIP launch of a slab stores the 4 own
  *                  rows next to each inner edge straight into the halo rows of the neighbour's destination buffer
  *                  (peer memory: on one GPU another pointer, between GPUs of one process a store over NVLink once peer
@@ -273,6 +277,8 @@ int mpr_predict_host_rect(int Lx, int Ly, const double* h_values, const uint8_t*
  *   mpr_fetch_series   the first n slots of that series -> HOST out (synchronises the stream).
  *   mpr_predict    the back-mapped average of phi accumulated since the last chain reset -> d_pred f64[Lx*Ly].
  *   mpr_debug_trial_lengths   the fixed sweep counts of one temperature trial of R6 (equilibration, measurement). */
+int mpr_create_slab(mpr_ctx** out, int Lx, int Ly, const double* d_values, const uint8_t* d_mask,
+                    void* d_workspace, size_t workspace_bytes, void* cuda_stream);
 int mpr_set_slab(mpr_ctx* ctx, int global_row0, int own_begin, int own_end, double z_min, double z_max,
                  double global_bonds);
 int mpr_set_peers(mpr_ctx* ctx, mpr_ctx* up, mpr_ctx* down);

@@ -119,6 +119,7 @@ struct mpr_ctx {
   double pair_sum = 0.0;         // sum of cos over the measured pairs behind e_sample (mpr_sample_energy_parts)
   double nb_norm = 0.0;          // bonds the energy is normalised by: bond_count(g), or the whole grid's for a slab
   bool slab = false;
+  bool expect_slab = false;    // created by mpr_create_slab: unusable until mpr_set_slab, local sample may be empty / constant
   // peer mode (mpr_set_peers): the neighbour slabs' contexts (same process) and the number of strip launches made so
   // far, by which a launch finds the buffer its neighbour's launch of the same number writes
   mpr_ctx* peer[2] = {nullptr, nullptr};
@@ -538,6 +539,7 @@ void mark_stale(mpr_ctx* c) {
 }
 int ensure_chain(mpr_ctx* c) {
   if (!c->ws) return fail(c, MPR_ERR_WORKSPACE, "no workspace attached (mpr_set_workspace)");
+  if (c->expect_slab && !c->slab) return fail(c, MPR_ERR_NOT_READY, "created by mpr_create_slab: mpr_set_slab first");
   return c->stale ? reset_chain(c, 0) : MPR_OK;
 }
 
@@ -648,9 +650,16 @@ int setup(mpr_ctx* c) {
   double h[4];
   CUDA_OK(c, cudaMemcpyAsync(h, c->scal(), sizeof(h), cudaMemcpyDeviceToHost, c->stream));
   CUDA_OK(c, cudaStreamSynchronize(c->stream));
-  if (h[2] == 0.0) return fail(c, MPR_ERR_NO_MEASURED, "no measured site");
   if (h[3] != 0.0) return fail(c, MPR_ERR_NONFINITE, "non-finite value at a measured site");
-  if (!(h[1] > h[0])) return fail(c, MPR_ERR_DEGENERATE_RANGE, "z_max == z_min over the measured sample");
+  if (c->expect_slab && (h[2] == 0.0 || !(h[1] > h[0]))) {
+    // the rows of a slab may hold no measured site, or one value only: the range that counts is the whole grid's,
+    // which mpr_set_slab brings (a placeholder until then)
+    h[0] = 0.0;
+    h[1] = 1.0;
+  } else {
+    if (h[2] == 0.0) return fail(c, MPR_ERR_NO_MEASURED, "no measured site");
+    if (!(h[1] > h[0])) return fail(c, MPR_ERR_DEGENERATE_RANGE, "z_max == z_min over the measured sample");
+  }
   c->zmin = h[0];
   c->zmax = h[1];
   // R6: sample energy
@@ -742,8 +751,18 @@ int mpr_create(mpr_ctx** out, int L, const double* d_values, const uint8_t* d_ma
   return mpr_create_rect(out, L, L, d_values, d_mask, d_workspace, workspace_bytes, cuda_stream);
 }
 
+static int create_impl(mpr_ctx** out, int Lx, int Ly, const double* d_values, const uint8_t* d_mask, void* d_workspace,
+                       size_t workspace_bytes, void* cuda_stream, bool expect_slab);
 int mpr_create_rect(mpr_ctx** out, int Lx, int Ly, const double* d_values, const uint8_t* d_mask, void* d_workspace,
                     size_t workspace_bytes, void* cuda_stream) {
+  return create_impl(out, Lx, Ly, d_values, d_mask, d_workspace, workspace_bytes, cuda_stream, false);
+}
+int mpr_create_slab(mpr_ctx** out, int Lx, int Ly, const double* d_values, const uint8_t* d_mask, void* d_workspace,
+                    size_t workspace_bytes, void* cuda_stream) {
+  return create_impl(out, Lx, Ly, d_values, d_mask, d_workspace, workspace_bytes, cuda_stream, true);
+}
+static int create_impl(mpr_ctx** out, int Lx, int Ly, const double* d_values, const uint8_t* d_mask, void* d_workspace,
+                       size_t workspace_bytes, void* cuda_stream, bool expect_slab) {
   if (!out) return MPR_ERR_INVALID_ARG;
   *out = nullptr;
   if (!valid_shape(Lx, Ly) || !d_values || !d_mask) return MPR_ERR_INVALID_ARG;
@@ -759,6 +778,7 @@ int mpr_create_rect(mpr_ctx** out, int Lx, int Ly, const double* d_values, const
   c->d_values = d_values;
   c->d_mask = d_mask;
   c->stream = static_cast<cudaStream_t>(cuda_stream);
+  c->expect_slab = expect_slab;
   // SURVEY 8(b) form: create(L, values, mask) first, mpr_set_workspace / mpr_set_stream afterwards
   if (with_ws) {
     const int st = mpr_set_workspace(c, d_workspace, workspace_bytes);

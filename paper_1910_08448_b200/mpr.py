@@ -35,7 +35,7 @@ SYMBOLS = [
     "mpr_get_info",
     "mpr_get_launch_stats", "mpr_workspace_bytes_host", "mpr_predict_host", "mpr_debug_philox",
     "mpr_workspace_bytes_rect", "mpr_create_rect", "mpr_workspace_bytes_host_rect", "mpr_predict_host_rect",
-    "mpr_set_slab", "mpr_set_peers", "mpr_sample_energy_parts", "mpr_rows_bytes", "mpr_export_rows", "mpr_import_rows", "mpr_advance",
+    "mpr_create_slab", "mpr_set_slab", "mpr_set_peers", "mpr_sample_energy_parts", "mpr_rows_bytes", "mpr_export_rows", "mpr_import_rows", "mpr_advance",
     "mpr_fetch_series", "mpr_predict", "mpr_debug_trial_lengths", "mpr_quench",
     "mpr_debug_accept",
     "mpr_static_setup", "mpr_static_max_sites", "mpr_static_last_error", "mpr_sample_energy_static",
@@ -115,6 +115,7 @@ def lib():
         "mpr_predict_host": (C.c_int, [C.c_int, vp, vp, C.c_int, C.c_uint64, C.c_double, C.c_int, C.c_int, vp,
                                        C.c_size_t, vp, vp, dp, dp, dp, u64p]),
         "mpr_debug_philox": (C.c_int, [vp, C.POINTER(C.c_uint32), vp, i64, vp]),
+        "mpr_create_slab": (C.c_int, [C.POINTER(vp), C.c_int, C.c_int, vp, vp, vp, C.c_size_t, vp]),
         "mpr_set_slab": (C.c_int, [vp, C.c_int, C.c_int, C.c_int, C.c_double, C.c_double, C.c_double]),
         "mpr_sample_energy_parts": (C.c_int, [vp, dp, i64p]),
         "mpr_set_peers": (C.c_int, [vp, vp, vp]),
@@ -169,7 +170,7 @@ class Mpr:
     mask:   uint8   [L, L], 1 = prediction site
     """
 
-    def __init__(self, values, mask, mode="DP", seed=None, device="cuda:0", stream=None):
+    def __init__(self, values, mask, mode="DP", seed=None, device="cuda:0", stream=None, slab=False):
         torch = _torch()
         self._torch = torch
         dev = torch.device(device)
@@ -191,7 +192,10 @@ class Mpr:
         # globals (lib, C) may already be cleared
         self._destroy, self._null = lib().mpr_destroy, C.c_void_p
         with torch.cuda.device(dev):
-            if self.L is not None:
+            if slab:        # rows that will become a slab (mpr_create_slab): set_slab must follow
+                st = lib().mpr_create_slab(C.byref(self.h), self.Lx, self.Ly, self.values.data_ptr(), self.mask.data_ptr(),
+                                           self._ws_ptr, self.ws.numel() - off, sptr)
+            elif self.L is not None:
                 st = lib().mpr_create(C.byref(self.h), self.L, self.values.data_ptr(), self.mask.data_ptr(),
                                       self._ws_ptr, self.ws.numel() - off, sptr)
             else:

@@ -175,7 +175,7 @@ class MprSlab:
         self.plan = plan
         v = np.ascontiguousarray(np.asarray(values)[plan.row0_g:plan.row1_g])
         m = np.ascontiguousarray(np.asarray(mask)[plan.row0_g:plan.row1_g])
-        self.ctx = mpr.Mpr(v, m, mode=mode, seed=seed, device=device)
+        self.ctx = mpr.Mpr(v, m, mode=mode, seed=seed, device=device, slab=True)
         self.ctx.set_quench(0)              # SlabSet runs the quench passes itself, with halo refreshes in between
         self.ctx.set_path(path)
         self.ctx.set_schedule(schedule)

@@ -170,3 +170,36 @@ def test_peer_mode_temperature_matching_and_checks(mpr, inputs, slabs):
     with pytest.raises(mpr.MprError):
         ss.slabs[0].ctx.set_peers(ss.slabs[1].ctx, None)       # slab 1 lies below slab 0, not above
     g.close()
+
+
+def test_slab_without_measured_sites_of_its_own(mpr, slabs):
+    """Sparse data on a thin grid: the rows of one slab hold no measured site at all, those of another a single value.
+    The slab contexts are created all the same (mpr_create_slab), the range comes from the whole grid, and the result is
+    the single context's."""
+    Ly, Lx = 80, 6
+    rng = np.random.default_rng(8)
+    values = np.full((Ly, Lx), np.nan)
+    mask = np.ones((Ly, Lx), dtype=np.uint8)
+    for (y, x) in [(1, 2), (3, 4), (4, 4), (45, 1), (70, 3), (71, 3), (72, 0)]:       # rows 20..39 empty, rows 40..59 one value
+        mask[y, x] = 0
+        values[y, x] = rng.normal(50.0, 10.0)
+    for mode, peer in (("DP", False), ("SP_INTRINSIC", True)):
+        g = mpr.Mpr(values, mask, mode=mode, seed=4)
+        g.set_path("STRIP"); g.set_temperature(0.3)
+        pred, e, se = g.run(6, 3)
+        st_w, acc_w = g.get_state().cpu().numpy(), g.counters()[0]
+        g.close()
+        ss = slabs.make_slab_set(values, mask, 4, halo=4, mode=mode, seed=4, path="STRIP", peer=peer)
+        ss.set_temperature(0.3)
+        ss.reset_chain(0)
+        series, e_s, se_s = ss.run(6, 3)
+        assert np.array_equal(ss.state(), st_w) and ss.accepted() == acc_w and abs(e_s - e) <= 2e-12
+    # a context created for a slab is not usable before it is told its place
+    h = mpr.Mpr(values[20:40], mask[20:40], slab=True)
+    with pytest.raises(mpr.MprError) as ei:
+        h.sweep(1)
+    assert ei.value.code == mpr.ERR_NOT_READY
+    # ... and the ordinary creation call still refuses such rows
+    with pytest.raises(mpr.MprError) as ei:
+        mpr.Mpr(values[20:40], mask[20:40])
+    assert ei.value.code == mpr.ERR_NO_MEASURED
