@@ -64,3 +64,49 @@ def test_random_configurations_agree_with_the_per_pass_kernels(seed):
                 assert np.array_equal(ss.state(), ref[0].numpy()) and ss.accepted() == ref[1][0], (what, count, peer)
                 assert np.array_equal(np.nan_to_num(ss.prediction(), nan=-1.0), ref[2].numpy()), (what, count, peer)
         done += 1
+
+
+@pytest.mark.parametrize("seed", [21, 22])
+def test_random_dp_configurations_match_the_oracle(oracle_mod, seed):
+    """The same idea against the oracle: DP on random shapes, masked fractions, temperatures, schedules, quench counts and
+    q in (0, 1/2], on a random path -- identical accepted-move counts, spins to 1e-9, energies to 1e-10, predictions to
+    1e-9 of the data range."""
+    import torch
+    from paper_1910_08448_b200 import mpr
+    rng = np.random.default_rng(seed)
+    done = 0
+    while done < 40:
+        Ly, Lx = int(rng.integers(1, 140)), int(rng.integers(1, 140))
+        if Ly * Lx < 2:
+            continue
+        f = float(rng.choice([0.05, 0.33, 0.66, 0.9, 0.99]))
+        values = rng.normal(50, 10, (Ly, Lx))
+        mask = (rng.uniform(size=(Ly, Lx)) < f).astype(np.uint8)
+        if int((mask == 0).sum()) < 2:
+            mask.reshape(-1)[:2] = 0
+        values[mask == 1] = np.nan
+        sched = str(rng.choice(["R4", "SITE_FUSED"]))
+        T = float(10 ** rng.uniform(-3.0, 0.5))
+        q = float(rng.choice([0.5, 0.5, 0.5, 0.37, 0.2]))
+        chain_seed, nq = int(rng.integers(0, 2 ** 40)), int(rng.choice([0, 1, 4, 32]))
+        n_sw, n_me = int(rng.integers(1, 7)), int(rng.integers(1, 4))
+        path = str(rng.choice(["AUTO", "PLAIN", "LIST", "STRIP"] + (["TILED"] if sched == "R4" else [])))
+        what = ((Ly, Lx), f, sched, T, q, chain_seed, nq, n_sw, n_me, path)
+        o = oracle_mod.Oracle(values=values, mask=mask, seed=chain_seed)
+        g = mpr.Mpr(values, mask, mode="DP", seed=chain_seed)
+        for h in (o, g):
+            h.set_quench(nq)
+            if q != 0.5:
+                h.set_q(q)
+            h.set_schedule(sched)
+            h.set_temperature(T)
+        g.set_path(path)
+        pred_o, e_o, se_o = o.run(n_sw, n_me)
+        pred_g, e_g, se_g = g.run(n_sw, n_me)
+        assert g.counters() == o.counters(), what
+        assert np.max(np.abs(g.get_state().cpu().numpy() - o.get_state())) <= 1e-9, what
+        assert abs(e_g - e_o) <= 1e-10 and abs(se_g - se_o) <= 1e-10, what
+        zr = o.zrange()
+        assert np.max(np.abs(np.nan_to_num(pred_g.cpu().numpy() - pred_o))) <= 1e-9 * (zr[1] - zr[0]), what
+        g.close()
+        done += 1
