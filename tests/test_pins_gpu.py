@@ -443,3 +443,37 @@ def test_maximum_size_runs_and_paths_agree(mpr):
             assert abs(e - ref[2]) <= 1e-9
         del st
         torch.cuda.empty_cache()
+
+
+def test_over_relaxation_tie_at_the_edge_of_the_range(mpr, oracle_mod):
+    """A degenerate case with two valid outcomes (found by fuzzing 1 x n grids): in a chain of free sites next to a
+    measured site at phi = 0 the quench passes leave exact relations such as phi_1 = phi_0 + phi_2, and the reflection
+    phi' = phi_0 + phi_2 - phi_1 of R5 then lands on the edge of [0, 2 pi] to within rounding.  The oracle, working on
+    angles, gets phi' = 0 and keeps it; the library, working on unit vectors, gets sin(q phi') = -1e-17 and leaves the
+    spin -- "unchanged if phi' is outside [0, 2 pi]".  Both follow R5; which one happens is decided by the last bit.
+    The test pins that this IS such a tie: up to the pass in question the two agree to rounding, the oracle's new angle
+    is 0 within 1e-15, the library's spin is the old one, and the sum rule that produced the tie holds to rounding."""
+    values = np.array([np.nan, np.nan, np.nan, 34.75851636, np.nan, 50.36306022, np.nan, np.nan]).reshape(8, 1)
+    mask = np.isnan(values).astype(np.uint8)
+    o = oracle_mod.Oracle(values=values, mask=mask, seed=5)
+    g = mpr.Mpr(values, mask, mode="DP", seed=5)
+    for h in (o, g):
+        h.set_quench(4)
+        h.set_temperature(0.3)
+    g.set_path("PLAIN")
+    for kind, c in [("MET", 0), ("MET", 1), ("OR", 0)]:
+        if kind == "MET":
+            o.met_pass(c, 1)
+        else:
+            o.or_pass(c)
+        g.pass_(kind, c, 1)
+    before_g, before_o = g.get_state().cpu().numpy().ravel(), o.get_state().ravel()
+    assert np.max(np.abs(before_g - before_o)) <= 1e-15
+    assert abs(before_o[0] + before_o[2] - before_o[1]) <= 1e-15          # the exact relation behind the tie
+    o.or_pass(1)
+    g.pass_("OR", 1, 1)
+    after_g, after_o = g.get_state().cpu().numpy().ravel(), o.get_state().ravel()
+    if abs(after_g[1] - after_o[1]) > 1e-12:                               # the tie went two ways (it does on B200 today)
+        assert abs(after_o[1]) <= 1e-15 and after_g[1] == before_g[1]
+    others = [i for i in range(8) if i != 1]
+    assert np.max(np.abs(after_g[others] - after_o[others])) <= 1e-15
