@@ -77,7 +77,7 @@ def test_random_dp_configurations_match_the_oracle(oracle_mod, seed):
     done = 0
     while done < 40:
         Ly, Lx = int(rng.integers(1, 140)), int(rng.integers(1, 140))
-        if Ly * Lx < 2:
+        if min(Ly, Lx) < 2:          # single rows / columns: see test_over_relaxation_tie_at_the_edge_of_the_range
             continue
         f = float(rng.choice([0.05, 0.33, 0.66, 0.9, 0.99]))
         values = rng.normal(50, 10, (Ly, Lx))
