@@ -20,7 +20,8 @@
  *   - Pointers named d_* are DEVICE pointers, h_* / plain scalars are HOST memory.
  *   - Grids are row-major, site index s = y*L + x, 0 <= x,y < L.
  *   - Ownership: the caller owns every buffer (inputs, outputs, workspace); the library
- *     allocates no device memory and creates no stream.  It borrows d_values, d_mask and
+ *     allocates no device memory (its only device storage of its own is the fixed 49 KB scratch array of
+ *     mpr_sample_energy_static) and creates no stream.  It borrows d_values, d_mask and
  *     the workspace for the life of the context and never writes d_values / d_mask.
  *   - Errors: every call returns 0 (MPR_OK) or a negative mpr_status.  Nothing is thrown,
  *     printed or aborted.  mpr_last_error() gives a text for the last failure of a context.
@@ -28,7 +29,8 @@
  *     host scalars (create, set_workspace, estimate_temperature, run, get_counters, get_energy_series,
  *     get_launch_stats) synchronise that stream before returning; the others are asynchronous.
  *   - Determinism: for fixed (inputs, seed, mode, T) the spin state after any number of
- *     sweeps is bit-identical for every kernel path, tile size and fused depth.
+ *     sweeps is bit-identical for every kernel path, tile size and fused depth, and for any cut of the grid into
+ *     slabs (mpr_set_slab).
  *   - There is no CPU fallback: without a CUDA device every compute call returns MPR_ERR_CUDA.
  */
 #ifndef MPR_H_
