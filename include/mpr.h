@@ -266,8 +266,11 @@ int mpr_predict_host_rect(int Lx, int Ly, const double* h_values, const uint8_t*
  *                  of exactly 4 rows, >= 8 own rows, q = 1/2; every slab makes the same sequence of calls, one launch
  *                  each in turn (a launch finds the neighbour's buffer by the number of launches both have made);
  *                  one sweep per launch, quench double passes two per launch.  Launch n + 1 of a slab must follow launch
- *                  n of its neighbours: this version requires all slabs on ONE stream, whose order gives exactly that
- *                  (slabs on several devices would need peer access and an event per launch: not built).  Resets the chain.
+ *                  n of its neighbours (it reads the halo rows they wrote and overwrites the buffer they read): on ONE
+ *                  stream the stream order gives that; with a stream per slab the caller records an event after every
+ *                  launch and makes the neighbours' streams wait for it before their next one (slabs.py does;
+ *                  tests/test_slabs_gpu.py runs it on one GPU).  Slabs on several devices of one process need peer
+ *                  access enabled besides: the same calls, not exercised here.  Resets the chain.
  *   mpr_sample_energy_parts   the sum of cos over, and the number of, measured nearest-neighbour pairs to the right
  *                  of and below the own rows: e_s of the whole grid = -2 J sum(parts) / sum(counts).  HOST outs.
  *   mpr_rows_bytes / mpr_export_rows / mpr_import_rows   n_rows rows of the chain state from row_begin on (both

@@ -1085,8 +1085,8 @@ int mpr_set_peers(mpr_ctx* c, mpr_ctx* up, mpr_ctx* down) {
   for (int d = 0; d < 2; ++d) {
     const mpr_ctx* p = ps[d];
     if (!p) continue;
-    if (p == c || !p->slab || p->lo.g.L != g.L || p->mode != c->mode || p->stream != c->stream)
-      return fail(c, MPR_ERR_INVALID_ARG, "peer mode: neighbours are slabs of the same grid, mode and stream");
+    if (p == c || !p->slab || p->lo.g.L != g.L || p->mode != c->mode)
+      return fail(c, MPR_ERR_INVALID_ARG, "peer mode: neighbours are slabs of the same grid and mode");
     // the neighbour's halo must be exactly the rows this slab sends: kPeerRows rows beyond its own rows, on my side
     const int my_first = c->slab_row0 + g.own0, my_last = c->slab_row0 + g.own1;         // global own rows [first, last)
     const int p_first = p->slab_row0 + p->lo.g.own0, p_last = p->slab_row0 + p->lo.g.own1;

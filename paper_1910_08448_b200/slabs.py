@@ -170,12 +170,13 @@ class MprSlab:
     """The rows plan.row0_g .. plan.row1_g of (values, mask) as an mpr.Mpr context in slab mode.  The interface SlabSet
     drives; tests/test_slabs_gloo.py drives the same SlabSet with a stand-in that needs no GPU."""
 
-    def __init__(self, plan, values, mask, mode="DP", seed=0, device="cuda:0", path="AUTO", schedule="R4"):
+    def __init__(self, plan, values, mask, mode="DP", seed=0, device="cuda:0", path="AUTO", schedule="R4", stream=None):
         from . import mpr
         self.plan = plan
+        self.stream = stream                 # a torch.cuda.Stream of this slab's own, or None (torch's current stream)
         v = np.ascontiguousarray(np.asarray(values)[plan.row0_g:plan.row1_g])
         m = np.ascontiguousarray(np.asarray(mask)[plan.row0_g:plan.row1_g])
-        self.ctx = mpr.Mpr(v, m, mode=mode, seed=seed, device=device, slab=True)
+        self.ctx = mpr.Mpr(v, m, mode=mode, seed=seed, device=device, slab=True, stream=stream)
         self.ctx.set_quench(0)              # SlabSet runs the quench passes itself, with halo refreshes in between
         self.ctx.set_path(path)
         self.ctx.set_schedule(schedule)
@@ -228,13 +229,18 @@ class MprSlab:
     def import_rows(self, row, n, buf):
         self.ctx.import_rows(row, n, buf)
 
+    def _done(self, t):
+        if self.stream is not None:          # the kernel ran on this slab's stream, the copy below runs on torch's
+            self.stream.synchronize()
+        return t
+
     def own_state(self):
         p = self.plan
-        return self.ctx.get_state()[p.own_begin:p.own_end].cpu().numpy()
+        return self._done(self.ctx.get_state())[p.own_begin:p.own_end].cpu().numpy()
 
     def own_prediction(self):
         p = self.plan
-        return self.ctx.predict()[p.own_begin:p.own_end].cpu().numpy()
+        return self._done(self.ctx.predict())[p.own_begin:p.own_end].cpu().numpy()
 
 
 # ---- the orchestrator ----------------------------------------------------------------------------------------------
@@ -281,6 +287,9 @@ class SlabSet:
         if self.peer:
             for i, s in slabs.items():
                 s.set_peers(slabs.get(i - 1), slabs.get(i + 1))
+        # peer mode with a stream per slab: launch n + 1 of a slab waits for launch n of its neighbours (an event each)
+        self._own_streams = self.peer and all(getattr(s, "stream", None) is not None for s in slabs.values())
+        self._events = {}
 
     def moves(self):
         """The rows that travel in one refresh: every slab sends the `halo` own rows next to each inner edge."""
@@ -297,6 +306,27 @@ class SlabSet:
             self.transport.transfer(self.slabs, self.moves())
             self.exchanges += 1
 
+    def _ordered(self, i, call):
+        """Runs one launch round of slab i; with a stream per slab, after the neighbours' latest rounds."""
+        if not self._own_streams:
+            return call()
+        import torch
+        st = self.slabs[i].stream
+        for j in (i - 1, i + 1):
+            if j in self._events:
+                st.wait_event(self._events[j])
+        out = call()
+        ev = torch.cuda.Event()
+        ev.record(st)
+        self._events[i] = ev
+        return out
+
+    def _barrier(self):
+        if self._own_streams:
+            import torch
+            torch.cuda.synchronize()
+            self._events = {}
+
     def set_temperature(self, T):
         self.T = float(T)
         for s in self.slabs.values():
@@ -305,13 +335,15 @@ class SlabSet:
     def reset_chain(self, trial=0):
         """R8: uniform spins (a function of the global site index and the trial: the halos agree without an exchange),
         then n_quench double passes; one double pass spoils 2 halo rows."""
+        self._barrier()                       # the initialisation rewrites whole buffers, halos included
         for s in self.slabs.values():
             s.reset_chain(trial)
+        self._barrier()
         per, done = self.halo // 2, 0
         while done < self.n_quench:
             m = min(per, self.n_quench - done)
-            for s in self.slabs.values():
-                s.quench(m)
+            for i, s in self.slabs.items():
+                self._ordered(i, lambda s=s: s.quench(m))
             self.exchange()
             done += m
         self.sweeps = 0
@@ -322,8 +354,8 @@ class SlabSet:
         done = 0
         while done < n:
             m = min(k, n - done)
-            for s in self.slabs.values():
-                s.advance(m, 0, 0)
+            for i, s in self.slabs.items():
+                self._ordered(i, lambda s=s: s.advance(m, 0, 0))
             self.exchange()
             done += m
         self.sweeps += n
@@ -335,8 +367,8 @@ class SlabSet:
         # colour-0 sites of that row -- the only halo sites an owned colour-1 site is bonded to -- go stale one pass later
         k = self.sweeps_per_exchange
         for i in range(n):
-            for s in self.slabs.values():
-                s.advance(1, 2 if accumulate else 1, i)
+            for j, s in self.slabs.items():
+                self._ordered(j, lambda s=s: s.advance(1, 2 if accumulate else 1, i))
             if (i + 1) % k == 0 or i + 1 == n:
                 self.exchange()
         self.sweeps += n
@@ -384,7 +416,7 @@ class SlabSet:
 
 
 def make_slab_set(values, mask, count, halo=8, mode="DP", seed=0, device="cuda:0", path="AUTO", schedule="R4",
-                  transport=None, n_quench=32, peer=False):
+                  transport=None, n_quench=32, peer=False, streams=False):
     """The CUDA path on `count` slabs.  transport None: all slabs in this process on `device`; a DistTransport: this rank
     builds slab number transport.rank only (count = world size)."""
     from . import mpr
@@ -392,6 +424,10 @@ def make_slab_set(values, mask, count, halo=8, mode="DP", seed=0, device="cuda:0
     plans = plan_slabs(int(mask.shape[0]), count, halo)
     transport = transport or LocalTransport()
     mine = [p for p in plans if transport.owner(p.index) == transport.rank]
-    slabs = {p.index: MprSlab(p, values, mask, mode=mode, seed=seed, device=device, path=path, schedule=schedule) for p in mine}
+    def own_stream():
+        import torch
+        return torch.cuda.Stream(device=device) if (peer and streams) else None
+    slabs = {p.index: MprSlab(p, values, mask, mode=mode, seed=seed, device=device, path=path, schedule=schedule,
+                              stream=own_stream()) for p in mine}
     return SlabSet(plans, slabs, int(mask.shape[1]), transport, n_quench=n_quench, trial_lengths=mpr.debug_trial_lengths(),
                    stats=mpr.debug_series_stats, match=mpr.debug_match_temperature, peer=peer)

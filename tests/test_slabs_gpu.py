@@ -203,3 +203,23 @@ def test_slab_without_measured_sites_of_its_own(mpr, slabs):
     with pytest.raises(mpr.MprError) as ei:
         mpr.Mpr(values[20:40], mask[20:40])
     assert ei.value.code == mpr.ERR_NO_MEASURED
+
+
+@pytest.mark.parametrize("mode,schedule,count", [("SP_INTRINSIC", "R4", 3), ("DP", "SITE_FUSED", 2), ("SP_INTRINSIC", "R4", 4)])
+def test_peer_mode_with_a_stream_per_slab(mpr, inputs, slabs, mode, schedule, count):
+    """Peer mode with every slab on a stream of its own: nothing but the events SlabSet records after each launch and
+    waits for before the neighbours' next one orders the kernels (on one stream the stream order would).  Same spins as
+    the single context, for runs long enough that unordered kernels would overlap."""
+    Ly, Lx = 1100, 700
+    values, mask, _ = inputs.make_rect_problem(Ly, Lx, 12.0, 57, 0.8)
+    T, n_eq, n_meas = 0.02, 25, 5
+    st_w, acc_w, series_w, pred_w, e_w, se_w, _, _ = whole(mpr, values, mask, mode, 79, "STRIP", schedule, T, n_eq, n_meas)
+    ss = slabs.make_slab_set(values, mask, count, halo=4, mode=mode, seed=79, path="STRIP", schedule=schedule, peer=True,
+                             streams=True)
+    assert ss._own_streams and len({s.stream.cuda_stream for s in ss.slabs.values()}) == count
+    ss.set_temperature(T)
+    ss.reset_chain(0)
+    series, e, se = ss.run(n_eq, n_meas)
+    assert np.array_equal(ss.state(), st_w) and ss.accepted() == acc_w
+    assert abs(e - e_w) <= 2e-12
+    assert np.array_equal(np.nan_to_num(ss.prediction(), nan=-1.0), np.nan_to_num(pred_w, nan=-1.0))
